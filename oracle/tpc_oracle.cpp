@@ -1,0 +1,707 @@
+// =============================================================================================
+// tpc_oracle.cpp -- plain, slow, single-threaded CPU ORACLE of the TPC tracking hot path.
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may build, load or call it.  It shares no
+// code, header, table or helper with the CUDA path under paper_2106_03636_b200/csrc/.
+//
+// What it computes (BASELINE.json north_star steps 1-4; PAPER.md is a system overview that
+// names TPC tracking as the dominant synchronous workload but does not
+// spell the algorithm out, so every rule is a *reading* fixed in SURVEY.md §8(c) R1-R23 and
+// restated in DESIGN.md "Readings"):
+//   orc_grid        R7      per-(sector,row) (y, zeta) grid: stable sort by bin, bin_first
+//   orc_neighbours  R9      cellular-automaton best (up,down) pair per cluster
+//   orc_links       R10     reciprocal-link cleaning, start hits
+//   orc_follow      R11-R18 Kalman following of every start hit (chain, up leg, down leg)
+//   orc_select      R20     one-shot arbitration by 64-bit key, exclusive assignment
+//   orc_fit         R21-R22 3-point seed + outward/inward Kalman refit
+//   orc_propagate / orc_update   the R12 / R13 primitives, exported for the pins (I7)
+//
+// Every function exists for real_t = float (suffix _f32: reproduces the GPU's arithmetic, one
+// IEEE operation per written operation, no contraction: build with -ffp-contract=off) and for
+// real_t = double (suffix _f64: analytic pins I1, I7, I8).  The step order and notation follow
+// R1-R23 so the file can be checked against DESIGN.md by eye; nothing is blocked, fused or
+// reordered.  The grid is only an acceleration structure (R8): every search is defined over all
+// clusters of a row, and `use_grid = 0` runs exactly that brute force.
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): I1-I10 of SURVEY.md §8(c).  Track count,
+// efficiency and fake rate themselves are "parity unpinned" by the paper (it publishes no number
+// for any synthetic workload); they are fixed only by oracle == GPU.
+// =============================================================================================
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+constexpr int kMaxRows = 152;
+
+// Host POD filled by oracle/tpc_oracle.py (its own definition; not the CUDA library's header).
+struct OrcParams {
+  int32_t n_sectors, n_rows;
+  double row_x[kMaxRows];
+  double tan_half, kB, sigma_y, sigma_z, z_lo, z_hi, cell_y, cell_z;
+  double ca_max_dydx, ca_max_dzdx, ca_cut;
+  double chi2_cut, chi2_chain_cut, win_max, max_sinphi, edge_margin;
+  int32_t max_gap, min_hits, n_fit_passes, reserved;
+  double cov0[5];
+};
+
+// ---------------------------------------------------------------------------------------------
+// Geometry tables (R1, R2, R7), all in real_t T so that float mode rounds exactly like the GPU.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+struct Geo {
+  int nsec, nrows, nz;
+  T X[kMaxRows], ymax[kMaxRows];
+  int ny[kMaxRows];
+  int64_t rowbase[kMaxRows + 1];  // first bin of row r inside a sector; rowbase[nrows] = bins per sector
+  T inv_cy, inv_cz, z_lo;
+  T kB, sy2, sz2;
+
+  explicit Geo(const OrcParams& P) {
+    nsec = P.n_sectors;
+    nrows = P.n_rows;
+    const T tan_half = (T)P.tan_half, cell_y = (T)P.cell_y, cell_z = (T)P.cell_z;
+    z_lo = (T)P.z_lo;
+    nz = std::max(1, (int)std::ceil(((T)P.z_hi - z_lo) / cell_z));
+    inv_cy = (T)1 / cell_y;
+    inv_cz = (T)1 / cell_z;
+    rowbase[0] = 0;
+    for (int r = 0; r < nrows; r++) {
+      X[r] = (T)P.row_x[r];
+      ymax[r] = X[r] * tan_half;                                         // R1: |y| <= X_r tan 10deg
+      ny[r] = std::max(1, (int)std::ceil(((T)2 * ymax[r]) / cell_y));     // R7
+      rowbase[r + 1] = rowbase[r] + (int64_t)ny[r] * nz;
+    }
+    kB = (T)P.kB;
+    sy2 = (T)P.sigma_y * (T)P.sigma_y;
+    sz2 = (T)P.sigma_z * (T)P.sigma_z;
+  }
+  // R2/R7: mirrored drift coordinate zeta = side*z, side = +1 for sectors 0..17, -1 for 18..35.
+  T side(int sector) const { return sector < 18 ? (T)1 : (T)-1; }
+  static int clampbin(T v, int n) {
+    if (!(v > (T)0)) return 0;
+    if (v >= (T)n) return n - 1;
+    return (int)v;
+  }
+  int ybin(int r, T y) const { return clampbin((y + ymax[r]) * inv_cy, ny[r]); }
+  int zbin(int sector, T z) const { return clampbin((side(sector) * z - z_lo) * inv_cz, nz); }
+  int64_t bins_per_sector() const { return rowbase[nrows]; }
+  int64_t bin_of(int sector, int r, T y, T z) const {
+    return (int64_t)sector * bins_per_sector() + rowbase[r] + (int64_t)zbin(sector, z) * ny[r] + ybin(r, y);
+  }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Cluster container + the two search back ends (R8): brute force over the row, or the R7 grid.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+struct Clusters {
+  int64_t n;
+  const T* y;
+  const T* z;
+  const int32_t* sector_row;
+  int nrows;
+  int sector(int64_t i) const { return sector_row[i] / nrows; }
+  int row(int64_t i) const { return sector_row[i] % nrows; }
+};
+
+template <class T>
+struct Index {
+  const Geo<T>& G;
+  const Clusters<T>& cl;
+  bool use_grid;
+  std::vector<int32_t> sorted;      // original indices in (sector,row,bin) order, ties by index (R7)
+  std::vector<int32_t> bin_first;   // exclusive prefix sum over all bins, +1 sentinel
+  std::vector<int64_t> row_first;   // first sorted position of every (sector,row), +1 sentinel
+
+  Index(const Geo<T>& g, const Clusters<T>& c, bool grid) : G(g), cl(c), use_grid(grid) {
+    const int64_t nb = (int64_t)G.nsec * G.bins_per_sector();
+    std::vector<int64_t> key(cl.n);
+    for (int64_t i = 0; i < cl.n; i++) key[i] = G.bin_of(cl.sector(i), cl.row(i), cl.y[i], cl.z[i]);
+    sorted.resize(cl.n);
+    for (int64_t i = 0; i < cl.n; i++) sorted[i] = (int32_t)i;
+    std::stable_sort(sorted.begin(), sorted.end(), [&](int32_t a, int32_t b) { return key[a] < key[b]; });
+    bin_first.assign(nb + 1, 0);
+    for (int64_t i = 0; i < cl.n; i++) bin_first[key[i] + 1]++;
+    for (int64_t b = 0; b < nb; b++) bin_first[b + 1] += bin_first[b];
+    row_first.assign((int64_t)G.nsec * G.nrows + 1, 0);
+    for (int s = 0; s < G.nsec; s++)
+      for (int r = 0; r < G.nrows; r++)
+        row_first[(int64_t)s * G.nrows + r] = bin_first[(int64_t)s * G.bins_per_sector() + G.rowbase[r]];
+    row_first[(int64_t)G.nsec * G.nrows] = cl.n;
+  }
+
+  // Visit every cluster of (sector,row) that could lie in [ya,yb] x [za,zb] (cm).  The visitor
+  // re-checks the exact window itself, so the grid only has to return a superset (R8).
+  template <class F>
+  void visit(int sector, int r, T ya, T yb, T za, T zb, F&& f) const {
+    const int64_t sr = (int64_t)sector * G.nrows + r;
+    if (!use_grid) {
+      for (int64_t k = row_first[sr]; k < row_first[sr + 1]; k++) f(sorted[k]);
+      return;
+    }
+    // widen by a few ulps of the largest |z| so rounding of window edges can never drop a bin
+    const T pz = (T)0.01 + ((T)4.8e-7) * std::max(std::fabs(za), std::fabs(zb));
+    const T py = (T)0.001;
+    const T s = G.side(sector);
+    T z0 = s > 0 ? za - pz : -(zb + pz);
+    T z1 = s > 0 ? zb + pz : -(za - pz);
+    const int zb0 = Geo<T>::clampbin((z0 - G.z_lo) * G.inv_cz, G.nz);
+    const int zb1 = Geo<T>::clampbin((z1 - G.z_lo) * G.inv_cz, G.nz);
+    const int yb0 = G.ybin(r, ya - py), yb1 = G.ybin(r, yb + py);
+    const int64_t base = (int64_t)sector * G.bins_per_sector() + G.rowbase[r];
+    for (int zb_ = zb0; zb_ <= zb1; zb_++) {
+      const int64_t b0 = base + (int64_t)zb_ * G.ny[r] + yb0, b1 = base + (int64_t)zb_ * G.ny[r] + yb1;
+      for (int64_t k = bin_first[b0]; k < bin_first[b1 + 1]; k++) f(sorted[k]);
+    }
+  }
+};
+
+// ---------------------------------------------------------------------------------------------
+// R11-R13: state p = (y, dz, sinphi, tanlambda, q/pT) at local x, full symmetric covariance.
+// ---------------------------------------------------------------------------------------------
+template <class T> struct Thr;
+template <> struct Thr<float>  { static constexpr float  asin_u = 0.05f, e_kdx = 1e-3f; };
+template <> struct Thr<double> { static constexpr double asin_u = 1e-3,  e_kdx = 1e-5;  };
+
+template <class T>
+struct State {
+  T p[5];
+  T C[5][5];
+};
+
+// asin(u)/u: series for small |u| (next term 35 u^8/1152), otherwise the double-precision library
+// asin rounded once to T (the GPU does the same, so float mode agrees to the last bit in practice).
+template <class T>
+T asin_ratio(T u) {
+  if (std::fabs(u) < Thr<T>::asin_u) {
+    const T u2 = u * u;
+    return (T)1 + u2 * ((T)0.16666667 + u2 * ((T)0.075 + u2 * (T)0.044642857));
+  }
+  const double ud = (double)u;
+  return (T)(std::asin(ud) / ud);
+}
+
+// R12: exact helix transport x -> x + dx.  Returns false (state untouched) if |sinphi'| > max_sinphi.
+// If F_out != nullptr the 5x5 Jacobian is written there.
+template <class T>
+bool propagate(State<T>& st, T dx, T kB, T max_sinphi, T (*F_out)[5] = nullptr) {
+  const T y = st.p[0], dz = st.p[1], s1 = st.p[2], tl = st.p[3], q = st.p[4];
+  const T kappa = -(kB * q);                       // R4: dphi/ds = -kB q/pT
+  const T s2 = s1 + kappa * dx;
+  if (!(std::fabs(s1) <= max_sinphi) || !(std::fabs(s2) <= max_sinphi)) return false;
+  const T c1 = std::sqrt((T)1 - s1 * s1), c2 = std::sqrt((T)1 - s2 * s2);
+  const T cc = c1 + c2;
+  const T t = (s1 + s2) / cc;                      // tan of the mean direction
+  const T L = dx * std::sqrt((T)1 + t * t);        // signed chord
+  const T u = (kappa * L) * (T)0.5;
+  const T arc = L * asin_ratio(u);                 // signed arc length in the bending plane
+  // Jacobian (non-trivial terms), g = 1 + c1 c2 + s1 s2
+  const T g = ((T)1 + c1 * c2) + s1 * s2;
+  const T c1c2 = c1 * c2;
+  const T f02 = (dx * g) / (cc * c1c2);                       // dy'/dsinphi
+  const T f04 = -((kB * (dx * dx)) * g) / (c2 * (cc * cc));   // dy'/dq
+  const T f12 = ((tl * dx) * t) / c1c2;                       // ddz'/dsinphi
+  const T f13 = arc;                                          // ddz'/dtanl
+  const T f24 = -(kB * dx);                                   // dsinphi'/dq
+  T E;                                                        // d(arc)/d(kappa)
+  if (std::fabs(kappa * dx) < Thr<T>::e_kdx) {
+    const T c1_2 = c1 * c1, c1_3 = c1_2 * c1, c1_5 = c1_3 * c1_2;
+    E = ((dx * dx) * s1) / ((T)2 * c1_3) + ((kappa * ((dx * dx) * dx)) * ((T)1 + (T)2 * (s1 * s1))) / ((T)3 * c1_5);
+  } else {
+    E = (dx / c2 - arc) / kappa;
+  }
+  const T f14 = -((kB * tl) * E);                             // ddz'/dq
+  T F[5][5] = {{1, 0, f02, 0, f04}, {0, 1, f12, f13, f14}, {0, 0, 1, 0, f24}, {0, 0, 0, 1, 0}, {0, 0, 0, 0, 1}};
+  // state
+  st.p[0] = y + dx * t;
+  st.p[1] = dz + tl * arc;
+  st.p[2] = s2;
+  // C' = F C F^T (Q = 0, R6): dense products, sums over k ascending; lower triangle kept, mirrored.
+  T M[5][5], N[5][5];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) {
+      T acc = 0;
+      for (int k = 0; k < 5; k++) acc += F[i][k] * st.C[k][j];
+      M[i][j] = acc;
+    }
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) {
+      T acc = 0;
+      for (int k = 0; k < 5; k++) acc += M[i][k] * F[j][k];
+      N[i][j] = acc;
+    }
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = N[i][j];
+  if (F_out)
+    for (int i = 0; i < 5; i++)
+      for (int j = 0; j < 5; j++) F_out[i][j] = F[i][j];
+  return true;
+}
+
+// R13: innovation covariance S = C[0:2,0:2] + R and its inverse (full 2x2).
+template <class T>
+struct Innov {
+  T S00, S01, S11, Si00, Si01, Si11;
+};
+template <class T>
+Innov<T> innovation(const State<T>& st, T sy2, T sz2) {
+  Innov<T> I;
+  I.S00 = st.C[0][0] + sy2;
+  I.S01 = st.C[1][0];
+  I.S11 = st.C[1][1] + sz2;
+  const T det = I.S00 * I.S11 - I.S01 * I.S01;
+  const T idet = (T)1 / det;
+  I.Si00 = I.S11 * idet;
+  I.Si01 = -(I.S01 * idet);
+  I.Si11 = I.S00 * idet;
+  return I;
+}
+template <class T>
+T chi2_of(const Innov<T>& I, T r0, T r1) {
+  return ((r0 * r0) * I.Si00 + (T)2 * ((r0 * r1) * I.Si01)) + (r1 * r1) * I.Si11;
+}
+// R13: Kalman update with measurement (ym, zm) (zm already relative to zRef); returns chi2.
+template <class T>
+T update(State<T>& st, T ym, T zm, T sy2, T sz2) {
+  const Innov<T> I = innovation(st, sy2, sz2);
+  const T r0 = ym - st.p[0], r1 = zm - st.p[1];
+  const T chi2 = chi2_of(I, r0, r1);
+  T K[5][2];
+  for (int i = 0; i < 5; i++) {
+    K[i][0] = st.C[i][0] * I.Si00 + st.C[i][1] * I.Si01;
+    K[i][1] = st.C[i][0] * I.Si01 + st.C[i][1] * I.Si11;
+  }
+  T N[5][5];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) N[i][j] = st.C[i][j] - (K[i][0] * st.C[0][j] + K[i][1] * st.C[1][j]);
+  for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K[i][0] * r0 + K[i][1] * r1);
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = N[i][j];
+  return chi2;
+}
+
+template <class T>
+void reset_cov(State<T>& st, const OrcParams& P) {
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) st.C[i][j] = (i == j) ? (T)P.cov0[i] : (T)0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 2 -- R9: cellular-automaton neighbour finder.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+void neighbours(const OrcParams& P, const Geo<T>& G, const Clusters<T>& cl, const Index<T>& ix,
+                int32_t* link_up, int32_t* link_dn) {
+  for (int64_t h = 0; h < cl.n; h++) {
+    link_up[h] = link_dn[h] = -1;
+    const int r = cl.row(h), s = cl.sector(h);
+    if (r < 1 || r > G.nrows - 2) continue;
+    const T dxu = G.X[r + 1] - G.X[r], dxd = G.X[r] - G.X[r - 1];
+    const T wu = dxd / (dxu + dxd), wd = (T)1 - wu;
+    const T den = ((T)1 + wu * wu) + wd * wd;
+    const T iy = (T)1 / (G.sy2 * den), iz = (T)1 / (G.sz2 * den);
+    const T wyu = (T)P.ca_max_dydx * dxu, wzu = (T)P.ca_max_dzdx * dxu;
+    const T wyd = (T)P.ca_max_dydx * dxd, wzd = (T)P.ca_max_dzdx * dxd;
+    const T yh = cl.y[h], zh = cl.z[h];
+    std::vector<int32_t> U, D;
+    ix.visit(s, r + 1, yh - wyu, yh + wyu, zh - wzu, zh + wzu, [&](int32_t u) {
+      if (std::fabs(cl.y[u] - yh) <= wyu && std::fabs(cl.z[u] - zh) <= wzu) U.push_back(u);
+    });
+    ix.visit(s, r - 1, yh - wyd, yh + wyd, zh - wzd, zh + wzd, [&](int32_t d) {
+      if (std::fabs(cl.y[d] - yh) <= wyd && std::fabs(cl.z[d] - zh) <= wzd) D.push_back(d);
+    });
+    std::sort(U.begin(), U.end());
+    std::sort(D.begin(), D.end());
+    bool have = false;
+    T best = 0;
+    int32_t bu = -1, bd = -1;
+    for (int32_t u : U)
+      for (int32_t d : D) {
+        const T ry = (yh - cl.y[d]) - wu * (cl.y[u] - cl.y[d]);
+        const T rz = (zh - cl.z[d]) - wu * (cl.z[u] - cl.z[d]);
+        const T D2 = (ry * ry) * iy + (rz * rz) * iz;
+        if (!have || D2 < best) { have = true; best = D2; bu = u; bd = d; }   // ties: lowest u, then lowest d
+      }
+    if (have && best < (T)P.ca_cut) { link_up[h] = bu; link_dn[h] = bd; }
+  }
+}
+
+// R10: keep reciprocal links only; start hit = cleaned up-link present and cleaned down-link absent.
+void clean_links(int64_t n, const int32_t* link_up, const int32_t* link_dn, int32_t* up_c, int32_t* dn_c,
+                 std::vector<int32_t>& starts) {
+  for (int64_t h = 0; h < n; h++) {
+    up_c[h] = (link_up[h] >= 0 && link_dn[link_up[h]] == (int32_t)h) ? link_up[h] : -1;
+    dn_c[h] = (link_dn[h] >= 0 && link_up[link_dn[h]] == (int32_t)h) ? link_dn[h] : -1;
+  }
+  starts.clear();
+  for (int64_t h = 0; h < n; h++)
+    if (up_c[h] >= 0 && dn_c[h] < 0) starts.push_back((int32_t)h);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 3a -- R14-R18: Kalman following of one start hit.
+// ---------------------------------------------------------------------------------------------
+struct TraceRec {   // one record per hit attached in an R16 search (pin I6)
+  int32_t tracklet, row, chosen, pad;
+  double y_pred, dz_pred, zref, S00, S01, S11, chi2;
+};
+
+template <class T>
+struct Follower {
+  const OrcParams& P;
+  const Geo<T>& G;
+  const Clusters<T>& cl;
+  const Index<T>& ix;
+  TraceRec* trace;
+  int64_t trace_cap, trace_n;
+
+  // R16: extrapolate row by row in direction dir (+1/-1) starting after row r_at (state is at X[r_at]).
+  // Returns the row the state is at when the leg ends.
+  int extrapolate(State<T>& st, T zref, int sector, int r_at, int r_first, int dir, int32_t* row_hit, int tracklet) {
+    int misses = 0;
+    for (int r = r_first; r >= 0 && r < G.nrows; r += dir) {
+      if (!propagate(st, G.X[r] - G.X[r_at], G.kB, (T)P.max_sinphi)) break;   // |sinphi'| > max: stop
+      r_at = r;
+      if (std::fabs(st.p[0]) > G.ymax[r] + (T)P.edge_margin) break;           // left the sector
+      const Innov<T> I = innovation(st, G.sy2, G.sz2);
+      const T wy = std::min(std::sqrt((T)P.chi2_cut * I.S00), (T)P.win_max);
+      const T wz = std::min(std::sqrt((T)P.chi2_cut * I.S11), (T)P.win_max);
+      const T yp = st.p[0], dzp = st.p[1];
+      const T zc = zref + dzp;
+      bool have = false;
+      T best = 0;
+      int32_t bi = -1;
+      ix.visit(sector, r, yp - wy, yp + wy, zc - wz, zc + wz, [&](int32_t c) {
+        const T r0 = cl.y[c] - yp, r1 = (cl.z[c] - zref) - dzp;
+        if (!(std::fabs(r0) <= wy && std::fabs(r1) <= wz)) return;
+        const T chi2 = chi2_of(I, r0, r1);
+        if (!have || chi2 < best || (chi2 == best && c < bi)) { have = true; best = chi2; bi = c; }
+      });
+      if (have && best < (T)P.chi2_cut) {
+        if (trace && trace_n < trace_cap) {
+          TraceRec& t = trace[trace_n++];
+          t.tracklet = tracklet; t.row = r; t.chosen = bi; t.pad = 0;
+          t.y_pred = yp; t.dz_pred = dzp; t.zref = zref; t.S00 = I.S00; t.S01 = I.S01; t.S11 = I.S11; t.chi2 = best;
+        }
+        update(st, cl.y[bi], cl.z[bi] - zref, G.sy2, G.sz2);
+        row_hit[r] = bi;
+        misses = 0;
+      } else {
+        misses++;
+        if (misses > P.max_gap) break;
+      }
+    }
+    return r_at;
+  }
+
+  // Follow start hit h0; row_hit[nrows] receives original indices (-1 = none).  Returns nHits.
+  int follow(int32_t h0, const int32_t* up_c, int32_t* row_hit, int tracklet, State<T>* final_state, T* zref_out) {
+    for (int r = 0; r < G.nrows; r++) row_hit[r] = -1;
+    const int sector = cl.sector(h0), r0 = cl.row(h0);
+    const int32_t h1 = up_c[h0];
+    // R14: initial state from the start hit and its up-neighbour
+    const T dx = G.X[cl.row(h1)] - G.X[r0], dy = cl.y[h1] - cl.y[h0];
+    const T ch = std::sqrt(dx * dx + dy * dy);
+    const T zref = cl.z[h0];
+    State<T> st;
+    st.p[0] = cl.y[h0];
+    st.p[1] = 0;
+    st.p[2] = dy / ch;
+    st.p[3] = (cl.z[h1] - cl.z[h0]) / ch;
+    st.p[4] = 0;
+    reset_cov(st, P);
+    update(st, cl.y[h0], (T)0, G.sy2, G.sz2);
+    row_hit[r0] = h0;
+    // R15: chain phase along the cleaned up-links
+    int r_at = r0;
+    for (int32_t h = h0; up_c[h] >= 0;) {
+      const int32_t hn = up_c[h];
+      const int rn = cl.row(hn);
+      State<T> trial = st;
+      if (!propagate(trial, G.X[rn] - G.X[r_at], G.kB, (T)P.max_sinphi)) break;
+      const Innov<T> I = innovation(trial, G.sy2, G.sz2);
+      const T chi2 = chi2_of(I, cl.y[hn] - trial.p[0], (cl.z[hn] - zref) - trial.p[1]);
+      if (chi2 > (T)P.chi2_chain_cut) break;       // discard the prediction; state stays at the previous hit
+      update(trial, cl.y[hn], cl.z[hn] - zref, G.sy2, G.sz2);
+      st = trial;
+      row_hit[rn] = hn;
+      r_at = rn;
+      h = hn;
+    }
+    // R16 upward from the last chain hit
+    r_at = extrapolate(st, zref, sector, r_at, r_at + 1, +1, row_hit, tracklet);
+    // R17: one step back to the start row (no update), then R16 downward
+    if (propagate(st, G.X[r0] - G.X[r_at], G.kB, (T)P.max_sinphi))
+      extrapolate(st, zref, sector, r0, r0 - 1, -1, row_hit, tracklet);
+    int nh = 0;
+    for (int r = 0; r < G.nrows; r++) nh += row_hit[r] >= 0;
+    if (final_state) *final_state = st;
+    if (zref_out) *zref_out = zref;
+    return nh;
+  }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Step 3b -- R21-R22: refit of one hit list (row-ascending original indices).
+// out: par[5], cov[15] (lower triangle row-major: 00,10,11,20,21,22,...), xref, zref, chi2, ndf
+// ---------------------------------------------------------------------------------------------
+template <class T>
+bool fit_one(const OrcParams& P, const Geo<T>& G, const Clusters<T>& cl, const int32_t* hits, int n, T* par, T* cov,
+             T* xref, T* zref_out, T* chi2_out, int32_t* ndf) {
+  const int32_t a = hits[0], b = hits[n / 2], c = hits[n - 1];
+  const T x1 = G.X[cl.row(a)], y1 = cl.y[a], x2 = G.X[cl.row(b)], y2 = cl.y[b], x3 = G.X[cl.row(c)], y3 = cl.y[c];
+  // R21: signed curvature of the circle through the three points, kappa = 2*cross/(d12 d23 d13)
+  const T cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+  const T d12 = std::sqrt((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+  const T d23 = std::sqrt((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+  const T d13 = std::sqrt((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+  const T kappa = ((T)2 * cross) / ((d12 * d23) * d13);
+  const int32_t h1 = hits[1];
+  const T dx = G.X[cl.row(h1)] - x1, dy = cl.y[h1] - y1;
+  const T ch = std::sqrt(dx * dx + dy * dy);
+  T sphi = dy / ch - ((kappa * ch) * (T)0.5) * (dx / ch);
+  const T ms = (T)P.max_sinphi;
+  if (sphi > ms) sphi = ms;
+  if (sphi < -ms) sphi = -ms;
+  const T zref = cl.z[a];
+  State<T> st;
+  st.p[0] = y1;
+  st.p[1] = 0;
+  st.p[2] = sphi;
+  st.p[3] = (cl.z[h1] - zref) / ch;
+  st.p[4] = -(kappa / G.kB);
+  // R22: pass 1 inner -> outer, pass 2 outer -> inner, ...; C reset at the start of every pass
+  T chi2 = 0;
+  int at = 0;   // index into hits[] of the hit the state sits at
+  bool ok = true;
+  for (int pass = 0; pass < P.n_fit_passes && ok; pass++) {
+    reset_cov(st, P);
+    chi2 = 0;
+    const int dir = (pass % 2 == 0) ? +1 : -1;
+    const int first = (dir > 0) ? 0 : n - 1;
+    for (int k = first; k >= 0 && k < n; k += dir) {
+      const int32_t h = hits[k];
+      if (k != at) {
+        if (!propagate(st, G.X[cl.row(h)] - G.X[cl.row(hits[at])], G.kB, (T)P.max_sinphi)) { ok = false; break; }
+        at = k;
+      }
+      chi2 += update(st, cl.y[h], cl.z[h] - zref, G.sy2, G.sz2);
+    }
+  }
+  for (int i = 0; i < 5; i++) par[i] = st.p[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) cov[m++] = st.C[i][j];
+  *xref = G.X[cl.row(hits[at])];
+  *zref_out = zref;
+  *chi2_out = ok ? chi2 : (T)-1;
+  *ndf = ok ? 2 * n - 5 : -1;
+  return ok;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Whole-stage drivers behind the extern "C" surface.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+struct Ctx {
+  OrcParams P;
+  Geo<T> G;
+  Clusters<T> cl;
+  Index<T> ix;
+  Ctx(const OrcParams& p, int64_t n, const T* y, const T* z, const int32_t* sr, int use_grid)
+      : P(p), G(p), cl{n, y, z, sr, p.n_rows}, ix(G, cl, use_grid != 0) {}
+};
+
+template <class T>
+int64_t grid_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int32_t* sorted_idx,
+                  int32_t* bin_first, int64_t bin_cap) {
+  Ctx<T> c(*P, n, y, z, sr, 1);
+  const int64_t nb = (int64_t)c.G.nsec * c.G.bins_per_sector();
+  if (sorted_idx) std::memcpy(sorted_idx, c.ix.sorted.data(), sizeof(int32_t) * n);
+  if (bin_first && bin_cap >= nb + 1) std::memcpy(bin_first, c.ix.bin_first.data(), sizeof(int32_t) * (nb + 1));
+  return nb;
+}
+
+template <class T>
+void neighbours_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int use_grid,
+                     int32_t* link_up, int32_t* link_dn) {
+  Ctx<T> c(*P, n, y, z, sr, use_grid);
+  neighbours(c.P, c.G, c.cl, c.ix, link_up, link_dn);
+}
+
+template <class T>
+int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int use_grid,
+                    const int32_t* up_c, int64_t n_starts, const int32_t* starts, int32_t* row_hit, int32_t* n_hits,
+                    T* state_out, TraceRec* trace, int64_t trace_cap) {
+  Ctx<T> c(*P, n, y, z, sr, use_grid);
+  Follower<T> f{c.P, c.G, c.cl, c.ix, trace, trace_cap, 0};
+  for (int64_t t = 0; t < n_starts; t++) {
+    State<T> fs;
+    T zref;
+    n_hits[t] = f.follow(starts[t], up_c, row_hit + t * c.G.nrows, (int)t, &fs, &zref);
+    if (state_out) {   // 5 params, 15 cov (lower), zref : 21 values per tracklet
+      T* o = state_out + t * 21;
+      for (int i = 0; i < 5; i++) o[i] = fs.p[i];
+      for (int i = 0, m = 5; i < 5; i++)
+        for (int j = 0; j <= i; j++) o[m++] = fs.C[i][j];
+      o[20] = zref;
+    }
+  }
+  return f.trace_n;
+}
+
+// R20: selection.  key(t) = nHits << 32 | (0xFFFFFFFF - start index); owner = max key per cluster.
+int64_t select_impl(int64_t n, int n_rows, int64_t n_starts, const int32_t* starts, const int32_t* row_hit,
+                    const int32_t* n_hits, int min_hits, int32_t* cluster_track, int32_t* trk_seed, int32_t* trk_nhits,
+                    int64_t* trk_first_hit, int32_t* trk_hits) {
+  std::vector<uint64_t> owner(n, 0);
+  auto key = [&](int64_t t) { return ((uint64_t)(uint32_t)n_hits[t] << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)starts[t]); };
+  for (int64_t t = 0; t < n_starts; t++)
+    for (int r = 0; r < n_rows; r++) {
+      const int32_t c = row_hit[t * n_rows + r];
+      if (c >= 0) owner[c] = std::max(owner[c], key(t));
+    }
+  for (int64_t i = 0; i < n; i++) cluster_track[i] = -1;
+  int64_t K = 0, nh = 0;
+  for (int64_t t = 0; t < n_starts; t++) {
+    int kept = 0;
+    for (int r = 0; r < n_rows; r++) {
+      const int32_t c = row_hit[t * n_rows + r];
+      if (c >= 0 && owner[c] == key(t)) kept++;
+    }
+    if (kept < min_hits) continue;
+    trk_seed[K] = starts[t];
+    trk_nhits[K] = kept;
+    trk_first_hit[K] = nh;
+    for (int r = 0; r < n_rows; r++) {
+      const int32_t c = row_hit[t * n_rows + r];
+      if (c >= 0 && owner[c] == key(t)) { trk_hits[nh++] = c; cluster_track[c] = (int32_t)K; }
+    }
+    K++;
+  }
+  return K;
+}
+
+template <class T>
+void fit_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int64_t K,
+              const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, T* par, T* cov, T* xref,
+              T* zref, T* chi2, int32_t* ndf) {
+  OrcParams Pp = *P;
+  Geo<T> G(Pp);
+  Clusters<T> cl{n, y, z, sr, Pp.n_rows};
+  for (int64_t k = 0; k < K; k++) {
+    T p5[5], c15[15];
+    fit_one(Pp, G, cl, trk_hits + trk_first_hit[k], trk_nhits[k], p5, c15, xref + k, zref + k, chi2 + k, ndf + k);
+    for (int i = 0; i < 5; i++) par[i * K + k] = p5[i];     // SoA [5][K]
+    for (int i = 0; i < 15; i++) cov[i * K + k] = c15[i];   // SoA [15][K]
+  }
+}
+
+template <class T>
+int propagate_impl(const OrcParams* P, T* p5, T* c15, T dx, T* F25) {
+  State<T> st;
+  for (int i = 0; i < 5; i++) st.p[i] = p5[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = c15[m++];
+  T F[5][5];
+  const bool ok = propagate(st, dx, (T)P->kB, (T)P->max_sinphi, F);
+  if (!ok) return 0;
+  for (int i = 0; i < 5; i++) p5[i] = st.p[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) c15[m++] = st.C[i][j];
+  if (F25)
+    for (int i = 0; i < 5; i++)
+      for (int j = 0; j < 5; j++) F25[i * 5 + j] = F[i][j];
+  return 1;
+}
+
+template <class T>
+T update_impl(const OrcParams* P, T* p5, T* c15, T ym, T zm) {
+  State<T> st;
+  for (int i = 0; i < 5; i++) st.p[i] = p5[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = c15[m++];
+  const T sy2 = (T)P->sigma_y * (T)P->sigma_y, sz2 = (T)P->sigma_z * (T)P->sigma_z;
+  const T chi2 = update(st, ym, zm, sy2, sz2);
+  for (int i = 0; i < 5; i++) p5[i] = st.p[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) c15[m++] = st.C[i][j];
+  return chi2;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C surface (loaded with ctypes by oracle/tpc_oracle.py)
+// =============================================================================================
+#define ORC_API extern "C" __attribute__((visibility("default")))
+
+ORC_API int64_t orc_sizeof_params() { return (int64_t)sizeof(OrcParams); }
+ORC_API int64_t orc_sizeof_trace() { return (int64_t)sizeof(TraceRec); }
+
+ORC_API int64_t orc_grid_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,
+                             int32_t* sorted_idx, int32_t* bin_first, int64_t bin_cap) {
+  return grid_impl<float>(P, n, y, z, sr, sorted_idx, bin_first, bin_cap);
+}
+ORC_API int64_t orc_grid_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr,
+                             int32_t* sorted_idx, int32_t* bin_first, int64_t bin_cap) {
+  return grid_impl<double>(P, n, y, z, sr, sorted_idx, bin_first, bin_cap);
+}
+ORC_API void orc_neighbours_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,
+                                int use_grid, int32_t* link_up, int32_t* link_dn) {
+  neighbours_impl<float>(P, n, y, z, sr, use_grid, link_up, link_dn);
+}
+ORC_API void orc_neighbours_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr,
+                                int use_grid, int32_t* link_up, int32_t* link_dn) {
+  neighbours_impl<double>(P, n, y, z, sr, use_grid, link_up, link_dn);
+}
+// returns the number of start hits written to starts[] (capacity n)
+ORC_API int64_t orc_links(int64_t n, const int32_t* link_up, const int32_t* link_dn, int32_t* up_c, int32_t* dn_c,
+                          int32_t* starts) {
+  std::vector<int32_t> s;
+  clean_links(n, link_up, link_dn, up_c, dn_c, s);
+  std::memcpy(starts, s.data(), sizeof(int32_t) * s.size());
+  return (int64_t)s.size();
+}
+ORC_API int64_t orc_follow_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,
+                               int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts,
+                               int32_t* row_hit, int32_t* n_hits, float* state_out, TraceRec* trace, int64_t trace_cap) {
+  return follow_impl<float>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap);
+}
+ORC_API int64_t orc_follow_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr,
+                               int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts,
+                               int32_t* row_hit, int32_t* n_hits, double* state_out, TraceRec* trace, int64_t trace_cap) {
+  return follow_impl<double>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap);
+}
+ORC_API int64_t orc_select(int64_t n, int n_rows, int64_t n_starts, const int32_t* starts, const int32_t* row_hit,
+                           const int32_t* n_hits, int min_hits, int32_t* cluster_track, int32_t* trk_seed,
+                           int32_t* trk_nhits, int64_t* trk_first_hit, int32_t* trk_hits) {
+  return select_impl(n, n_rows, n_starts, starts, row_hit, n_hits, min_hits, cluster_track, trk_seed, trk_nhits,
+                     trk_first_hit, trk_hits);
+}
+ORC_API void orc_fit_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr, int64_t K,
+                         const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, float* par,
+                         float* cov, float* xref, float* zref, float* chi2, int32_t* ndf) {
+  fit_impl<float>(P, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf);
+}
+ORC_API void orc_fit_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr, int64_t K,
+                         const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, double* par,
+                         double* cov, double* xref, double* zref, double* chi2, int32_t* ndf) {
+  fit_impl<double>(P, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf);
+}
+ORC_API int orc_propagate_f32(const OrcParams* P, float* p5, float* c15, float dx, float* F25) {
+  return propagate_impl<float>(P, p5, c15, dx, F25);
+}
+ORC_API int orc_propagate_f64(const OrcParams* P, double* p5, double* c15, double dx, double* F25) {
+  return propagate_impl<double>(P, p5, c15, dx, F25);
+}
+ORC_API float orc_update_f32(const OrcParams* P, float* p5, float* c15, float ym, float zm) {
+  return update_impl<float>(P, p5, c15, ym, zm);
+}
+ORC_API double orc_update_f64(const OrcParams* P, double* p5, double* c15, double ym, double zm) {
+  return update_impl<double>(P, p5, c15, ym, zm);
+}

@@ -1,0 +1,244 @@
+"""ctypes front end of the CPU ORACLE (oracle/tpc_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  Nothing under paper_2106_03636_b200/ imports it and it
+imports nothing from there (parameters arrive as any object with the TpcParams attribute names;
+clusters as numpy arrays).
+
+`build()` compiles the oracle with g++ (-O2 -ffp-contract=off: one IEEE operation per written
+operation, which is what makes float mode comparable with the GPU).  `run()` chains the stages
+R7 -> R9 -> R10 -> R14-R18 -> R20 -> R21-R22 and returns every intermediate
+so the parity tests can compare stage by stage.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import time
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_LIB = os.path.join(_HERE, "libtpc_oracle.so")
+_lib = None
+
+N_ROWS_MAX = 152
+
+
+class OrcParams(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.c_double * N_ROWS_MAX),
+                ("tan_half", C.c_double), ("kB", C.c_double), ("sigma_y", C.c_double), ("sigma_z", C.c_double),
+                ("z_lo", C.c_double), ("z_hi", C.c_double), ("cell_y", C.c_double), ("cell_z", C.c_double),
+                ("ca_max_dydx", C.c_double), ("ca_max_dzdx", C.c_double), ("ca_cut", C.c_double),
+                ("chi2_cut", C.c_double), ("chi2_chain_cut", C.c_double), ("win_max", C.c_double),
+                ("max_sinphi", C.c_double), ("edge_margin", C.c_double),
+                ("max_gap", C.c_int32), ("min_hits", C.c_int32), ("n_fit_passes", C.c_int32), ("reserved", C.c_int32),
+                ("cov0", C.c_double * 5)]
+
+
+class TraceRec(C.Structure):
+    _fields_ = [("tracklet", C.c_int32), ("row", C.c_int32), ("chosen", C.c_int32), ("pad", C.c_int32),
+                ("y_pred", C.c_double), ("dz_pred", C.c_double), ("zref", C.c_double),
+                ("S00", C.c_double), ("S01", C.c_double), ("S11", C.c_double), ("chi2", C.c_double)]
+
+
+TRACE_DTYPE = np.dtype([("tracklet", "i4"), ("row", "i4"), ("chosen", "i4"), ("pad", "i4"), ("y_pred", "f8"),
+                        ("dz_pred", "f8"), ("zref", "f8"), ("S00", "f8"), ("S01", "f8"), ("S11", "f8"), ("chi2", "f8")])
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/tpc_oracle.cpp -> oracle/libtpc_oracle.so (no-op if up to date)."""
+    if (not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + f".tmp{os.getpid()}"
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+           "-fvisibility=hidden", "-o", tmp, _SRC]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        L.orc_sizeof_params.restype = C.c_int64
+        L.orc_sizeof_trace.restype = C.c_int64
+        assert L.orc_sizeof_params() == C.sizeof(OrcParams), "OrcParams layout mismatch"
+        assert L.orc_sizeof_trace() == C.sizeof(TraceRec) == TRACE_DTYPE.itemsize, "TraceRec layout mismatch"
+        for sfx in ("f32", "f64"):
+            getattr(L, f"orc_grid_{sfx}").restype = C.c_int64
+            getattr(L, f"orc_follow_{sfx}").restype = C.c_int64
+            getattr(L, f"orc_neighbours_{sfx}").restype = None
+            getattr(L, f"orc_fit_{sfx}").restype = None
+            getattr(L, f"orc_propagate_{sfx}").restype = C.c_int
+        L.orc_update_f32.restype = C.c_float
+        L.orc_update_f64.restype = C.c_double
+        L.orc_links.restype = C.c_int64
+        L.orc_select.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def make_params(p, precision: str = "f32") -> OrcParams:
+    """Marshal a TpcParams-like object.  In f32 mode every real is first rounded to float32."""
+    rnd = (lambda v: float(np.float32(v))) if precision == "f32" else float
+    P = OrcParams()
+    P.n_sectors, P.n_rows = int(p.n_sectors), int(p.n_rows)
+    rx = np.asarray(p.row_x, dtype=np.float64)
+    for i in range(P.n_rows):
+        P.row_x[i] = rnd(rx[i])
+    for name in ("tan_half", "kB", "sigma_y", "sigma_z", "z_lo", "z_hi", "cell_y", "cell_z", "ca_max_dydx",
+                 "ca_max_dzdx", "ca_cut", "chi2_cut", "chi2_chain_cut", "win_max", "max_sinphi", "edge_margin"):
+        setattr(P, name, rnd(getattr(p, name)))
+    P.max_gap, P.min_hits, P.n_fit_passes = int(p.max_gap), int(p.min_hits), int(p.n_fit_passes)
+    for i in range(5):
+        P.cov0[i] = rnd(p.cov0[i])
+    return P
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _real(precision):
+    return (np.float32, "f32") if precision == "f32" else (np.float64, "f64")
+
+
+def n_bins(p, precision="f32") -> int:
+    P = make_params(p, precision)
+    e = np.zeros(0, _real(precision)[0]); s = np.zeros(0, np.int32)
+    return int(getattr(lib(), f"orc_grid_{_real(precision)[1]}")(C.byref(P), C.c_int64(0), _ptr(e), _ptr(e), _ptr(s),
+                                                                   None, None, C.c_int64(0)))
+
+
+def grid(p, y, z, sector_row, precision="f32"):
+    """R7: returns (sorted_idx[n], bin_first[n_bins+1])."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    nb = n_bins(p, precision)
+    sorted_idx = np.empty(y.size, np.int32); bin_first = np.empty(nb + 1, np.int32)
+    getattr(lib(), f"orc_grid_{sfx}")(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), _ptr(sorted_idx),
+                                      _ptr(bin_first), C.c_int64(nb + 1))
+    return sorted_idx, bin_first
+
+
+def neighbours(p, y, z, sector_row, precision="f32", use_grid=True):
+    """R9: returns (link_up[n], link_dn[n]) in original indices, -1 = none."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    up = np.empty(y.size, np.int32); dn = np.empty(y.size, np.int32)
+    getattr(lib(), f"orc_neighbours_{sfx}")(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr),
+                                            C.c_int(int(use_grid)), _ptr(up), _ptr(dn))
+    return up, dn
+
+
+def links(link_up, link_dn):
+    """R10: returns (up_c, dn_c, starts)."""
+    n = link_up.size
+    up_c = np.empty(n, np.int32); dn_c = np.empty(n, np.int32); starts = np.empty(n, np.int32)
+    ns = lib().orc_links(C.c_int64(n), _ptr(np.ascontiguousarray(link_up, np.int32)),
+                         _ptr(np.ascontiguousarray(link_dn, np.int32)), _ptr(up_c), _ptr(dn_c), _ptr(starts))
+    return up_c, dn_c, starts[:ns].copy()
+
+
+def follow(p, y, z, sector_row, up_c, starts, precision="f32", use_grid=True, want_state=False, trace_cap=0):
+    """R14-R18: returns dict(row_hit[S, n_rows], n_hits[S], state[S,21]?, trace?)."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    starts = np.ascontiguousarray(starts, np.int32); up_c = np.ascontiguousarray(up_c, np.int32)
+    S = starts.size
+    row_hit = np.empty((S, P.n_rows), np.int32); n_hits = np.empty(S, np.int32)
+    state = np.empty((S, 21), rt) if want_state else None
+    trace = np.zeros(trace_cap, TRACE_DTYPE) if trace_cap else None
+    nt = getattr(lib(), f"orc_follow_{sfx}")(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr),
+                                             C.c_int(int(use_grid)), _ptr(up_c), C.c_int64(S), _ptr(starts),
+                                             _ptr(row_hit), _ptr(n_hits), _ptr(state), _ptr(trace), C.c_int64(trace_cap))
+    out = dict(row_hit=row_hit, n_hits=n_hits)
+    if want_state:
+        out["state"] = state
+    if trace_cap:
+        out["trace"] = trace[:nt]
+    return out
+
+
+def select(n, n_rows, starts, row_hit, n_hits, min_hits):
+    """R20: returns dict(cluster_track[n], trk_seed, trk_nhits, trk_first_hit, trk_hits)."""
+    starts = np.ascontiguousarray(starts, np.int32); row_hit = np.ascontiguousarray(row_hit, np.int32)
+    n_hits = np.ascontiguousarray(n_hits, np.int32)
+    S = starts.size
+    cluster_track = np.empty(n, np.int32)
+    trk_seed = np.empty(S, np.int32); trk_nhits = np.empty(S, np.int32); trk_first = np.empty(S, np.int64)
+    trk_hits = np.empty(max(n, 1), np.int32)
+    K = lib().orc_select(C.c_int64(n), C.c_int(n_rows), C.c_int64(S), _ptr(starts), _ptr(row_hit), _ptr(n_hits),
+                         C.c_int(int(min_hits)), _ptr(cluster_track), _ptr(trk_seed), _ptr(trk_nhits), _ptr(trk_first),
+                         _ptr(trk_hits))
+    nh = int(trk_nhits[:K].sum())
+    return dict(cluster_track=cluster_track, trk_seed=trk_seed[:K].copy(), trk_nhits=trk_nhits[:K].copy(),
+                trk_first_hit=trk_first[:K].copy(), trk_hits=trk_hits[:nh].copy())
+
+
+def fit(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, precision="f32"):
+    """R21-R22: returns dict(par[5,K], cov[15,K], xref, zref, chi2, ndf)."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    nh = np.ascontiguousarray(trk_nhits, np.int32); fh = np.ascontiguousarray(trk_first_hit, np.int64)
+    th = np.ascontiguousarray(trk_hits, np.int32)
+    K = nh.size
+    par = np.empty((5, K), rt); cov = np.empty((15, K), rt)
+    xref = np.empty(K, rt); zref = np.empty(K, rt); chi2 = np.empty(K, rt); ndf = np.empty(K, np.int32)
+    getattr(lib(), f"orc_fit_{sfx}")(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int64(K), _ptr(nh),
+                                     _ptr(fh), _ptr(th), _ptr(par), _ptr(cov), _ptr(xref), _ptr(zref), _ptr(chi2),
+                                     _ptr(ndf))
+    return dict(par=par, cov=cov, xref=xref, zref=zref, chi2=chi2, ndf=ndf)
+
+
+def propagate(p, par5, cov15, dx, precision="f64"):
+    """R12 primitive: returns (ok, par5', cov15', F[5,5])."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    a = np.array(par5, rt); c = np.array(cov15, rt); F = np.zeros(25, rt)
+    ct = C.c_float if sfx == "f32" else C.c_double
+    ok = getattr(lib(), f"orc_propagate_{sfx}")(C.byref(P), _ptr(a), _ptr(c), ct(dx), _ptr(F))
+    return bool(ok), a, c, F.reshape(5, 5)
+
+
+def update(p, par5, cov15, ym, zm, precision="f64"):
+    """R13 primitive: returns (chi2, par5', cov15')."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    a = np.array(par5, rt); c = np.array(cov15, rt)
+    ct = C.c_float if sfx == "f32" else C.c_double
+    chi2 = getattr(lib(), f"orc_update_{sfx}")(C.byref(P), _ptr(a), _ptr(c), ct(ym), ct(zm))
+    return float(chi2), a, c
+
+
+def run(p, y, z, sector_row, precision="f32", use_grid=True, want_state=False, trace_cap=0, timings=None):
+    """Whole hot path a1..a6.  Returns every stage's output (original cluster indices everywhere)."""
+    t0 = time.perf_counter()
+    out = {}
+    if use_grid:
+        out["sorted_idx"], out["bin_first"] = grid(p, y, z, sector_row, precision)
+    t1 = time.perf_counter()
+    up, dn = neighbours(p, y, z, sector_row, precision, use_grid)
+    t2 = time.perf_counter()
+    up_c, dn_c, starts = links(up, dn)
+    t3 = time.perf_counter()
+    fo = follow(p, y, z, sector_row, up_c, starts, precision, use_grid, want_state, trace_cap)
+    t4 = time.perf_counter()
+    se = select(int(np.asarray(y).size), int(p.n_rows), starts, fo["row_hit"], fo["n_hits"], p.min_hits)
+    t5 = time.perf_counter()
+    fi = fit(p, y, z, sector_row, se["trk_nhits"], se["trk_first_hit"], se["trk_hits"], precision)
+    t6 = time.perf_counter()
+    out.update(link_up=up, link_dn=dn, up_c=up_c, dn_c=dn_c, starts=starts, **fo, **se, **fi)
+    if timings is not None:
+        timings.update(grid=t1 - t0, neighbours=t2 - t1, links=t3 - t2, follow=t4 - t3, select=t5 - t4, fit=t6 - t5,
+                       total=t6 - t0)
+    return out
