@@ -1,0 +1,179 @@
+/* =============================================================================================
+ * tpc_b200.h -- C ABI of the B200-native TPC track-reconstruction hot path.
+ *
+ * What it is.  The data-parallel hot path of ALICE's Run-3 synchronous GPU processing: TPC track
+ * reconstruction on a continuous-readout Time Frame (TF = 128 orbits, no event
+ * boundaries; l.37, l.47: TPC tracking dominates the synchronous workload and has no a-priori
+ * absolute z; l.102: cost grows with tracks x attached clusters).  The paper names the step but
+ * never spells the algorithm out, so the operations are the four steps of BASELINE.json
+ * `north_star` made concrete by the readings R1-R23 of SURVEY.md §8(c) (restated in DESIGN.md):
+ *
+ *   tpc_grid_build   step 1  (R7)        per-(sector,row) (y, zeta) search grid: stable counting
+ *                                        sort by bin, bin start offsets
+ *   tpc_find_tracks  steps 2,3a,4        cellular-automaton neighbours (R9), reciprocal links and
+ *                    (R9-R20)            start hits (R10), Kalman following (R11-R18), one-shot
+ *                                        selection with exclusive cluster assignment (R20)
+ *   tpc_fit_tracks   step 3b (R21-R22)   3-point seed + outward/inward Kalman refit, fp32
+ *
+ * Conventions.
+ *  - Every pointer is a DEVICE pointer unless its name ends in `_host`.  Every call only enqueues
+ *    work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and
+ *    returns without synchronising.  The library never allocates or frees device memory: the
+ *    caller owns every buffer, including the workspace.
+ *  - Return value: TPC_OK (0) or a negative tpc_status_t.  Host-detectable misuse (NULL pointer,
+ *    workspace too small, sizes out of range) is a return code and nothing is enqueued.  Problems
+ *    found on the device (tracklet / track capacity overflow, cluster outside the grid's z range)
+ *    set bits in counters[TPC_CNT_STATUS]; outputs are truncated, never written out of bounds.
+ *  - Layout: external cluster data is SoA fp32 (one array per field) + int32 sector_row =
+ *    sector*n_rows + row, in arbitrary order.  The workspace holds the library's internal state
+ *    (sorted 16-byte cluster records, bin offsets, links, tracklet tables) and is laid out as a
+ *    pure function of (params, n_clusters, max_tracklets): the same three values must be passed
+ *    to tpc_workspace_bytes, tpc_grid_build and tpc_find_tracks.  The grid inside it is valid
+ *    until the next tpc_grid_build on the same workspace.
+ *  - All cluster indices in outputs are ORIGINAL indices (positions in the caller's arrays).
+ *  - Arithmetic: IEEE fp32, one rounding per written operation (compiled without FMA
+ *    contraction) so that results are reproducible bit for bit; integer work is exact and every
+ *    arg-min/arg-max breaks ties by original cluster index, so the output is deterministic.
+ * ============================================================================================= */
+#ifndef TPC_B200_H_
+#define TPC_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPC_MAX_ROWS 152
+
+typedef enum {
+  TPC_OK = 0,
+  TPC_EINVAL = -1,     /* NULL pointer, negative size, n_rows/n_sectors out of range, bins >= 2^31 */
+  TPC_ENOMEM_WS = -2,  /* ws_bytes smaller than tpc_workspace_bytes() for these sizes */
+  TPC_ECUDA = -3       /* a CUDA runtime call failed at enqueue time (see tpc_last_cuda_error) */
+} tpc_status_t;
+
+/* indices into the int32 counters[8] device array written by tpc_find_tracks */
+enum {
+  TPC_CNT_TRACKS = 0,     /* K  = number of accepted tracks (clamped to max_tracks)            */
+  TPC_CNT_TRACKLETS = 1,  /* S  = number of start hits followed (clamped to max_tracklets)      */
+  TPC_CNT_HITS = 2,       /* sum of trk_nhits over the K tracks = entries used in trk_hits      */
+  TPC_CNT_STATUS = 3,     /* bit mask of TPC_ST_*                                               */
+  TPC_CNT_STARTS_FOUND = 4, /* start hits found before clamping                                 */
+  TPC_CNT_TRACKS_FOUND = 5, /* accepted tracks before clamping                                  */
+  TPC_CNT_RESERVED6 = 6,
+  TPC_CNT_RESERVED7 = 7,
+  TPC_N_COUNTERS = 8
+};
+#define TPC_ST_TRACKLET_OVERFLOW 1 /* more start hits than max_tracklets: the excess was dropped */
+#define TPC_ST_TRACK_OVERFLOW 2    /* more accepted tracks than max_tracks: the excess was dropped */
+#define TPC_ST_Z_CLAMPED 4         /* a cluster lay outside [z_lo,z_hi] and was put in an edge bin */
+
+/* Host POD, passed by pointer and copied during the call.  Every field is an input of the method
+ * (SURVEY.md §8(b),(c)): geometry R1-R2, field constant R4, measurement errors R6, grid cell R7,
+ * cuts R9-R22.  Defaults in parentheses. */
+typedef struct {
+  int32_t n_sectors;             /* 36 (18 per side; sectors >= 18 have side = -1), or 1         */
+  int32_t n_rows;                /* <= TPC_MAX_ROWS (152)                                         */
+  float row_x[TPC_MAX_ROWS];     /* sector-local x of pad row r, cm, strictly increasing (R1)     */
+  float tan_half;                /* tan(10 deg): row r spans |y| <= row_x[r]*tan_half (R1)        */
+  float kB;                      /* 0.299792458e-2 * B[T]; dphi/ds = -kB*q/pT (R4)                */
+  float sigma_y, sigma_z;        /* cluster errors, cm (0.08, 0.10) (R6)                          */
+  float z_lo, z_hi;              /* range of zeta = side*z covered by the grid, cm (R7)           */
+  float cell_y, cell_z;          /* grid cell, cm (R7)                                            */
+  float ca_max_dydx, ca_max_dzdx, ca_cut;                 /* R9  (2.0, 2.5, 20)                   */
+  float chi2_cut, chi2_chain_cut, win_max;                /* R15-R16 (16, 30, 5 cm)               */
+  float max_sinphi, edge_margin;                          /* R12, R16 (0.95, 1 cm)                */
+  int32_t max_gap, min_hits, n_fit_passes;                /* R16, R20, R22 (4, 10, 2)             */
+  float cov0[5];                 /* initial covariance diagonal (1,1,1,10,100) (R14, R22)         */
+} tpc_params_t;
+
+/* Human-readable text for a tpc_status_t (static storage). */
+const char* tpc_strerror(int status);
+/* Text of the last CUDA runtime error seen by this thread's last failing call (static storage). */
+const char* tpc_last_cuda_error(void);
+/* Library version, e.g. "0.1.0". */
+const char* tpc_version(void);
+
+/* Number of grid bins for these parameters: n_sectors * sum_r ny_r * nz (R7).  Host only.
+ * Returns TPC_EINVAL if params are inconsistent or the count does not fit in int32. */
+int tpc_grid_bins(const tpc_params_t* params_host, int64_t* n_bins_host);
+
+/* Bytes of workspace needed for n_clusters clusters and at most max_tracklets start hits. */
+int tpc_workspace_bytes(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                        size_t* bytes_host);
+
+/* Step 1 (R7).  Sorts the n clusters into the grid held in `workspace`.
+ *   y, z, sector_row : [n] inputs, arbitrary order; must stay alive and unmodified until the last
+ *                      call that uses this grid has completed on `stream`.
+ *   x, q             : [n] pad-row x and cluster charge; carried by the interface (BASELINE.json
+ *                      "fp32 (x,y,z,row,charge) clusters") but not read: x == row_x[row] by
+ *                      construction and the tracker does not use charge.  May be NULL.
+ * n == 0 is legal.  Clusters outside [z_lo,z_hi] are clamped into the edge bins (status bit is
+ * raised later by tpc_find_tracks' counters; results stay exact because searches re-check cm). */
+int tpc_grid_build(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                   const float* x, const float* y, const float* z, const float* q,
+                   const int32_t* sector_row, void* workspace, size_t ws_bytes, void* stream);
+
+/* Debug/parity view of the grid (R7): original indices in sorted order and bin offsets.
+ * sorted_idx [n] and/or bin_first [n_bins+1] may be NULL.  Enqueues device-to-device copies. */
+int tpc_grid_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                    const void* workspace, size_t ws_bytes, int32_t* sorted_idx, int32_t* bin_first,
+                    void* stream);
+
+/* Steps 2, 3a, 4 (R9-R20) on the grid built by tpc_grid_build in the same workspace.
+ *   cluster_track [n]           : track index (0..K-1) owning each cluster, -1 = none (R20)
+ *   trk_seed      [max_tracks]  : original index of the track's start hit (unique per track)
+ *   trk_sector    [max_tracks]  : sector of the track
+ *   trk_nhits     [max_tracks]  : hits kept after arbitration (>= min_hits)
+ *   trk_first_hit [max_tracks]  : offset of the track's first hit in trk_hits
+ *   trk_hits      [n]           : original cluster indices, row-ascending per track
+ *   counters      [TPC_N_COUNTERS] int32, see TPC_CNT_*
+ * Track order is deterministic (ascending grid position of the start hit) but carries no meaning:
+ * match tracks by trk_seed. */
+int tpc_find_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                    void* workspace, size_t ws_bytes, int32_t* cluster_track, int64_t max_tracks,
+                    int32_t* trk_seed, int32_t* trk_sector, int32_t* trk_nhits,
+                    int64_t* trk_first_hit, int32_t* trk_hits, int32_t* counters, void* stream);
+
+/* Debug/parity view of the intermediate stages of the last tpc_find_tracks on this workspace,
+ * all in ORIGINAL cluster indices (-1 = none).  Any output pointer may be NULL.
+ *   link_up, link_dn [n]  : R9 raw links;  up_c, dn_c [n] : R10 cleaned links
+ *   starts [max_tracklets]: start hit of tracklet t;  tl_nhits [max_tracklets]: hits recorded
+ *   row_hit [max_tracklets * n_rows] : row_hit[t*n_rows + r] (R18), row-major per tracklet
+ * Entries for t >= counters[TPC_CNT_TRACKLETS] are left untouched. */
+int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                    const void* workspace, size_t ws_bytes, int32_t* link_up, int32_t* link_dn,
+                    int32_t* up_c, int32_t* dn_c, int32_t* starts, int32_t* tl_nhits,
+                    int32_t* row_hit, void* stream);
+
+/* Step 3b (R21-R22).  Refit of K = counters[TPC_CNT_TRACKS] hit lists (read on the device; the
+ * call never synchronises).  Self-contained: reads cluster coordinates through y, z, sector_row
+ * (the caller's arrays, original order) so it can be fed any hit lists, e.g. truth hits.
+ *   par [5][max_tracks]  : y, dz = z - zref, sinphi, tanlambda, q/pT at x = xref   (SoA)
+ *   cov [15][max_tracks] : lower triangle, row-major (00,10,11,20,21,22,...)       (SoA)
+ *   xref, zref, chi2 [max_tracks], ndf [max_tracks] (= 2*nhits-5; chi2 = -1, ndf = -1 if the
+ *   propagation left |sinphi| <= max_sinphi). */
+int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, const float* y,
+                   const float* z, const int32_t* sector_row, const int32_t* counters,
+                   int64_t max_tracks, const int32_t* trk_nhits, const int64_t* trk_first_hit,
+                   const int32_t* trk_hits, float* par, float* cov, float* xref, float* zref,
+                   float* chi2, int32_t* ndf, void* stream);
+
+/* Host-buffer convenience for end-to-end measurement (bench.py `e2e`): copies the five input
+ * arrays host->device into caller-provided device staging buffers, runs the three steps, and
+ * copies counters + track parameters back.  All on `stream`; synchronises before returning. */
+int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                   int64_t max_tracks, const float* y_host, const float* z_host,
+                   const int32_t* sector_row_host, float* y_dev, float* z_dev, int32_t* sector_row_dev,
+                   void* workspace, size_t ws_bytes, int32_t* cluster_track_dev, int32_t* trk_seed_dev,
+                   int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
+                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev,
+                   float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
+                   int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_B200_H_ */

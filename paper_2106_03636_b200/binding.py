@@ -1,0 +1,274 @@
+"""Thin Python binding of libtpc_b200.so (include/tpc_b200.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; PyTorch is used for device memory and
+streams.  There is no CPU fallback: loading fails loudly when the library is missing or cannot be built,
+and every compute entry point refuses non-CUDA tensors.
+
+    lib = binding.load()
+    trk = binding.Tracker(params, n_clusters)          # allocates workspace + outputs once
+    res = trk.run(y, z, sector_row)                     # tpc_grid_build -> tpc_find_tracks -> tpc_fit_tracks
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+TPC_MAX_ROWS = 152
+TPC_N_COUNTERS = 8
+CNT_TRACKS, CNT_TRACKLETS, CNT_HITS, CNT_STATUS, CNT_STARTS_FOUND, CNT_TRACKS_FOUND = 0, 1, 2, 3, 4, 5
+ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
+
+#: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
+SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
+           "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
+           "tpc_track_host")
+
+
+class tpc_params_t(C.Structure):
+    """Mirror of the host POD in include/tpc_b200.h."""
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.c_float * TPC_MAX_ROWS),
+                ("tan_half", C.c_float), ("kB", C.c_float), ("sigma_y", C.c_float), ("sigma_z", C.c_float),
+                ("z_lo", C.c_float), ("z_hi", C.c_float), ("cell_y", C.c_float), ("cell_z", C.c_float),
+                ("ca_max_dydx", C.c_float), ("ca_max_dzdx", C.c_float), ("ca_cut", C.c_float),
+                ("chi2_cut", C.c_float), ("chi2_chain_cut", C.c_float), ("win_max", C.c_float),
+                ("max_sinphi", C.c_float), ("edge_margin", C.c_float),
+                ("max_gap", C.c_int32), ("min_hits", C.c_int32), ("n_fit_passes", C.c_int32),
+                ("cov0", C.c_float * 5)]
+
+
+class TpcError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load(rebuild: bool = False):
+    """Load (building in-tree first if needed) libtpc_b200.so.  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None and not rebuild:
+        return _lib
+    path = _build.LIB
+    if rebuild or not _build.up_to_date():
+        try:
+            path = _build.build_library(force=rebuild)
+        except Exception as e:  # no nvcc on this machine: use the shipped binary if there is one
+            if not os.path.exists(path):
+                raise TpcError(f"libtpc_b200.so is missing and cannot be built ({e}); there is no CPU fallback") from e
+    L = C.CDLL(path)
+    for name in SYMBOLS:
+        if not hasattr(L, name):
+            raise TpcError(f"libtpc_b200.so does not export {name}")
+    for name in ("tpc_strerror", "tpc_last_cuda_error", "tpc_version"):
+        getattr(L, name).restype = C.c_char_p
+    for name in SYMBOLS[3:]:
+        getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def make_params(p) -> tpc_params_t:
+    """Marshal a TpcParams-like object (attribute names of tpc_params_t) into the C struct."""
+    P = tpc_params_t()
+    P.n_sectors, P.n_rows = int(p.n_sectors), int(p.n_rows)
+    rx = np.asarray(p.row_x, dtype=np.float32)
+    for i in range(P.n_rows):
+        P.row_x[i] = float(rx[i])
+    for name in ("tan_half", "kB", "sigma_y", "sigma_z", "z_lo", "z_hi", "cell_y", "cell_z", "ca_max_dydx",
+                 "ca_max_dzdx", "ca_cut", "chi2_cut", "chi2_chain_cut", "win_max", "max_sinphi", "edge_margin"):
+        setattr(P, name, float(getattr(p, name)))
+    P.max_gap, P.min_hits, P.n_fit_passes = int(p.max_gap), int(p.min_hits), int(p.n_fit_passes)
+    for i in range(5):
+        P.cov0[i] = float(p.cov0[i])
+    return P
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        L = load()
+        msg = L.tpc_strerror(rc).decode()
+        if rc == -3:
+            msg += " (" + L.tpc_last_cuda_error().decode() + ")"
+        raise TpcError(f"{what}: {msg}")
+
+
+def _dp(t):
+    """Device pointer of a CUDA tensor (None -> NULL)."""
+    if t is None:
+        return C.c_void_p(0)
+    if not t.is_cuda:
+        raise TpcError("expected a CUDA tensor: the hot path has no CPU implementation")
+    if not t.is_contiguous():
+        raise TpcError("expected a contiguous tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def grid_bins(params) -> int:
+    out = C.c_int64(0)
+    _check(load().tpc_grid_bins(C.byref(make_params(params)), C.byref(out)), "tpc_grid_bins")
+    return int(out.value)
+
+
+def workspace_bytes(params, n_clusters: int, max_tracklets: int) -> int:
+    out = C.c_size_t(0)
+    _check(load().tpc_workspace_bytes(C.byref(make_params(params)), C.c_int64(n_clusters), C.c_int64(max_tracklets),
+                                      C.byref(out)), "tpc_workspace_bytes")
+    return int(out.value)
+
+
+def default_max_tracklets(n_clusters: int) -> int:
+    """Start hits are ~4-7 % of the clusters on the BASELINE.json configs; n/8 + 1024 leaves headroom."""
+    return int(n_clusters) // 8 + 1024
+
+
+def default_max_tracks(n_clusters: int) -> int:
+    """Accepted tracks need >= min_hits (10) exclusive clusters each; n/16 + 1024 is never reached in practice."""
+    return int(n_clusters) // 16 + 1024
+
+
+class Tracker:
+    """Owns the device buffers for events of up to `n_clusters` clusters and calls the three C entry points."""
+
+    def __init__(self, params, n_clusters: int, max_tracklets: int | None = None, max_tracks: int | None = None,
+                 device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.lib = load()
+        self.params = params
+        self.P = make_params(params)
+        self.n = int(n_clusters)
+        self.max_tracklets = int(max_tracklets) if max_tracklets is not None else default_max_tracklets(self.n)
+        self.max_tracks = int(max_tracks) if max_tracks is not None else default_max_tracks(self.n)
+        self.device = torch.device(device)
+        self.ws_bytes = workspace_bytes(params, self.n, self.max_tracklets)
+        i32, i64, f32 = torch.int32, torch.int64, torch.float32
+        dev = self.device
+        # torch allocations are >= 512-byte aligned, which satisfies the 256-byte requirement of the workspace
+        self.workspace = torch.empty(self.ws_bytes, dtype=torch.uint8, device=dev)
+        n1, K = max(self.n, 1), self.max_tracks
+        self.cluster_track = torch.empty(n1, dtype=i32, device=dev)
+        self.trk_seed = torch.empty(K, dtype=i32, device=dev)
+        self.trk_sector = torch.empty(K, dtype=i32, device=dev)
+        self.trk_nhits = torch.empty(K, dtype=i32, device=dev)
+        self.trk_first_hit = torch.empty(K, dtype=i64, device=dev)
+        self.trk_hits = torch.empty(n1, dtype=i32, device=dev)
+        self.counters = torch.zeros(TPC_N_COUNTERS, dtype=i32, device=dev)
+        self.par = torch.empty((5, K), dtype=f32, device=dev)
+        self.cov = torch.empty((15, K), dtype=f32, device=dev)
+        self.xref = torch.empty(K, dtype=f32, device=dev)
+        self.zref = torch.empty(K, dtype=f32, device=dev)
+        self.chi2 = torch.empty(K, dtype=f32, device=dev)
+        self.ndf = torch.empty(K, dtype=i32, device=dev)
+        self._inputs = None
+
+    # ---- the three calls of the boundary -----------------------------------------------------
+    def grid_build(self, y, z, sector_row, x=None, q=None):
+        assert y.numel() == self.n and z.numel() == self.n and sector_row.numel() == self.n
+        assert y.dtype == self.torch.float32 and z.dtype == self.torch.float32 and sector_row.dtype == self.torch.int32
+        self._inputs = (y, z, sector_row)   # keep alive: the fit reads them
+        _check(self.lib.tpc_grid_build(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), _dp(x), _dp(y),
+                                       _dp(z), _dp(q), _dp(sector_row), _dp(self.workspace), C.c_size_t(self.ws_bytes),
+                                       _stream()), "tpc_grid_build")
+
+    def find_tracks(self):
+        _check(self.lib.tpc_find_tracks(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets),
+                                        _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(self.cluster_track),
+                                        C.c_int64(self.max_tracks), _dp(self.trk_seed), _dp(self.trk_sector),
+                                        _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits),
+                                        _dp(self.counters), _stream()), "tpc_find_tracks")
+
+    def fit_tracks(self):
+        y, z, sr = self._inputs
+        _check(self.lib.tpc_fit_tracks(C.byref(self.P), C.c_int64(self.n), _dp(y), _dp(z), _dp(sr), _dp(self.counters),
+                                       C.c_int64(self.max_tracks), _dp(self.trk_nhits), _dp(self.trk_first_hit),
+                                       _dp(self.trk_hits), _dp(self.par), _dp(self.cov), _dp(self.xref), _dp(self.zref),
+                                       _dp(self.chi2), _dp(self.ndf), _stream()), "tpc_fit_tracks")
+
+    def step(self, y, z, sector_row):
+        """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""
+        self.grid_build(y, z, sector_row)
+        self.find_tracks()
+        self.fit_tracks()
+
+    # ---- parity / debug views -----------------------------------------------------------------
+    def grid_export(self):
+        t = self.torch
+        nb = grid_bins(self.params)
+        sorted_idx = t.empty(max(self.n, 1), dtype=t.int32, device=self.device)
+        bin_first = t.empty(nb + 1, dtype=t.int32, device=self.device)
+        _check(self.lib.tpc_grid_export(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets),
+                                        _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(sorted_idx), _dp(bin_first),
+                                        _stream()), "tpc_grid_export")
+        return sorted_idx[:self.n].cpu().numpy(), bin_first.cpu().numpy()
+
+    def find_export(self, want_row_hit=True):
+        t = self.torch
+        n1 = max(self.n, 1)
+        S = int(self.counters[CNT_TRACKLETS].item())
+        mk = lambda m: t.full((max(m, 1),), -1, dtype=t.int32, device=self.device)
+        up, dn, upc, dnc = mk(n1), mk(n1), mk(n1), mk(n1)
+        starts, nh = mk(self.max_tracklets), mk(self.max_tracklets)
+        nrows = int(self.params.n_rows)
+        rh = t.full((max(S, 1) * nrows,), -1, dtype=t.int32, device=self.device) if want_row_hit else None
+        _check(self.lib.tpc_find_export(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets),
+                                        _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(up), _dp(dn), _dp(upc),
+                                        _dp(dnc), _dp(starts), _dp(nh), _dp(rh), _stream()), "tpc_find_export")
+        out = dict(link_up=up[:self.n].cpu().numpy(), link_dn=dn[:self.n].cpu().numpy(), up_c=upc[:self.n].cpu().numpy(),
+                   dn_c=dnc[:self.n].cpu().numpy(), starts=starts[:S].cpu().numpy(), n_hits=nh[:S].cpu().numpy())
+        if want_row_hit:
+            out["row_hit"] = rh[:S * nrows].cpu().numpy().reshape(S, nrows)
+        return out
+
+    def results(self):
+        """Synchronise and copy the outputs of the last step to numpy (original cluster indices)."""
+        cnt = self.counters.cpu().numpy()
+        K, H = int(cnt[CNT_TRACKS]), int(cnt[CNT_HITS])
+        return dict(counters=cnt, status=int(cnt[CNT_STATUS]),
+                    cluster_track=self.cluster_track[:self.n].cpu().numpy(),
+                    trk_seed=self.trk_seed[:K].cpu().numpy(), trk_sector=self.trk_sector[:K].cpu().numpy(),
+                    trk_nhits=self.trk_nhits[:K].cpu().numpy(), trk_first_hit=self.trk_first_hit[:K].cpu().numpy(),
+                    trk_hits=self.trk_hits[:H].cpu().numpy(), par=self.par[:, :K].cpu().numpy(),
+                    cov=self.cov[:, :K].cpu().numpy(), xref=self.xref[:K].cpu().numpy(), zref=self.zref[:K].cpu().numpy(),
+                    chi2=self.chi2[:K].cpu().numpy(), ndf=self.ndf[:K].cpu().numpy())
+
+    def run(self, y, z, sector_row):
+        self.step(y, z, sector_row)
+        return self.results()
+
+    # ---- host-buffer path (bench.py e2e) ------------------------------------------------------
+    def make_host_staging(self):
+        """Device staging buffers + pinned host outputs for `track_host`."""
+        t = self.torch
+        n1 = max(self.n, 1)
+        self._y_dev = t.empty(n1, dtype=t.float32, device=self.device)
+        self._z_dev = t.empty(n1, dtype=t.float32, device=self.device)
+        self._sr_dev = t.empty(n1, dtype=t.int32, device=self.device)
+        self.counters_host = t.zeros(TPC_N_COUNTERS, dtype=t.int32).pin_memory()
+        self.cluster_track_host = t.empty(n1, dtype=t.int32).pin_memory()
+        self.par_host = t.empty((5, self.max_tracks), dtype=t.float32).pin_memory()
+
+    def track_host(self, y_host, z_host, sr_host):
+        """tpc_track_host: H2D of the inputs, a1..a6, D2H of counters + cluster_track + track parameters; synchronous."""
+        for a in (y_host, z_host, sr_host):
+            assert not a.is_cuda and a.is_contiguous() and a.numel() == self.n
+        hp = lambda a: C.c_void_p(a.data_ptr())
+        self._inputs = (self._y_dev, self._z_dev, self._sr_dev)
+        _check(self.lib.tpc_track_host(
+            C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), C.c_int64(self.max_tracks),
+            hp(y_host), hp(z_host), hp(sr_host), _dp(self._y_dev), _dp(self._z_dev), _dp(self._sr_dev),
+            _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(self.cluster_track), _dp(self.trk_seed),
+            _dp(self.trk_sector), _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits), _dp(self.counters),
+            _dp(self.par), _dp(self.cov), _dp(self.xref), _dp(self.zref), _dp(self.chi2), _dp(self.ndf),
+            hp(self.counters_host), hp(self.cluster_track_host), hp(self.par_host), _stream()), "tpc_track_host")
+        h2d = 12 * self.n
+        d2h = 4 * TPC_N_COUNTERS + 4 * self.n + 4 * 5 * self.max_tracks
+        return h2d, d2h

@@ -1,0 +1,244 @@
+// =============================================================================================
+// tpc_api.cu -- the extern "C" surface declared in include/tpc_b200.h: argument checks, geometry
+// tables (R1, R7, R9 per-row constants, computed once per call on the host in fp32 with one
+// rounding per operation), workspace layout, and the launch sequence.  No torch types, no device
+// allocation, no synchronisation (except tpc_track_host, which is the host-buffer convenience).
+// =============================================================================================
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "tpc_common.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return TPC_ECUDA;
+}
+
+// Builds the device geometry from the host POD.  Returns false if the parameters are unusable.
+bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
+  if (!P) return false;
+  if (P->n_sectors < 1 || P->n_sectors > 36 || P->n_rows < 3 || P->n_rows > TPC_MAX_ROWS) return false;
+  if (!(P->cell_y > 0.0f) || !(P->cell_z > 0.0f) || !(P->z_hi > P->z_lo)) return false;
+  if (!(P->sigma_y > 0.0f) || !(P->sigma_z > 0.0f) || !(P->tan_half > 0.0f)) return false;
+  if (P->n_fit_passes < 1 || P->min_hits < 1 || P->max_gap < 0) return false;
+  for (int r = 1; r < P->n_rows; r++)
+    if (!(P->row_x[r] > P->row_x[r - 1])) return false;
+  memset(G, 0, sizeof(*G));
+  tpc::Scalars& s = G->s;
+  s.nsec = P->n_sectors;
+  s.nrows = P->n_rows;
+  const float zspan = (P->z_hi - P->z_lo) / P->cell_z;
+  if (!(zspan < 2.0e9f)) return false;
+  s.nz = (int)ceilf(zspan);
+  if (s.nz < 1) s.nz = 1;
+  s.inv_cy = 1.0f / P->cell_y;
+  s.inv_cz = 1.0f / P->cell_z;
+  s.z_lo = P->z_lo;
+  s.z_hi = P->z_hi;
+  s.kB = P->kB;
+  s.sy2 = P->sigma_y * P->sigma_y;
+  s.sz2 = P->sigma_z * P->sigma_z;
+  s.ca_cut = P->ca_cut;
+  s.chi2_cut = P->chi2_cut;
+  s.chi2_chain_cut = P->chi2_chain_cut;
+  s.win_max = P->win_max;
+  s.max_sinphi = P->max_sinphi;
+  s.edge_margin = P->edge_margin;
+  s.max_gap = P->max_gap;
+  s.min_hits = P->min_hits;
+  s.n_fit_passes = P->n_fit_passes;
+  for (int i = 0; i < 5; i++) s.cov0[i] = P->cov0[i];
+  int64_t base = 0;
+  for (int r = 0; r < s.nrows; r++) {
+    const float X = P->row_x[r];
+    const float ymax = X * P->tan_half;                   // R1
+    const float yspan = (2.0f * ymax) / P->cell_y;        // R7
+    if (!(yspan < 2.0e9f)) return false;
+    int ny = (int)ceilf(yspan);
+    if (ny < 1) ny = 1;
+    G->row.X[r] = X;
+    G->row.ymax[r] = ymax;
+    G->row.ny[r] = ny;
+    G->row.rowbase[r] = (int32_t)base;
+    base += (int64_t)ny * s.nz;
+    if (base * s.nsec >= 2147483000ll) return false;      // bin ids are int32
+  }
+  G->row.rowbase[s.nrows] = (int32_t)base;
+  s.bins_per_sector = (int32_t)base;
+  *n_bins = base * s.nsec;
+  // R9 per-row constants of the neighbour finder (rows 1..n_rows-2)
+  for (int r = 1; r + 1 < s.nrows; r++) {
+    const float dxu = G->row.X[r + 1] - G->row.X[r], dxd = G->row.X[r] - G->row.X[r - 1];
+    const float wu = dxd / (dxu + dxd), wd = 1.0f - wu;
+    const float den = (1.0f + wu * wu) + wd * wd;
+    G->ca.wu[r] = wu;
+    G->ca.iy[r] = 1.0f / (s.sy2 * den);
+    G->ca.iz[r] = 1.0f / (s.sz2 * den);
+    G->ca.wyu[r] = P->ca_max_dydx * dxu;
+    G->ca.wzu[r] = P->ca_max_dzdx * dxu;
+    G->ca.wyd[r] = P->ca_max_dydx * dxd;
+    G->ca.wzd[r] = P->ca_max_dzdx * dxd;
+  }
+  return true;
+}
+
+struct Prep {
+  tpc::Geo G;
+  tpc::Layout L;
+  tpc::Ws W;
+};
+
+// Shared argument handling of the workspace-taking entry points.
+int prepare(const tpc_params_t* P, int64_t n, int64_t max_tracklets, const void* ws, size_t ws_bytes, Prep* out) {
+  int64_t nb = 0;
+  if (!make_geo(P, &out->G, &nb)) return TPC_EINVAL;
+  if (n < 0 || n > 2147483000ll || max_tracklets < 1 || max_tracklets > 2147483000ll || !ws) return TPC_EINVAL;
+  out->L = tpc::make_layout(n, max_tracklets, nb, P->n_rows);
+  if (ws_bytes < out->L.total) return TPC_ENOMEM_WS;
+  if (((uintptr_t)ws & 255) != 0) return TPC_EINVAL;
+  out->W = tpc::bind_ws(out->L, const_cast<void*>(ws));
+  return TPC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tpc_strerror(int status) {
+  switch (status) {
+    case TPC_OK: return "ok";
+    case TPC_EINVAL: return "invalid argument";
+    case TPC_ENOMEM_WS: return "workspace too small";
+    case TPC_ECUDA: return "CUDA runtime error";
+    default: return "unknown status";
+  }
+}
+
+const char* tpc_last_cuda_error(void) { return g_cuda_err; }
+
+const char* tpc_version(void) { return "0.1.0"; }
+
+int tpc_grid_bins(const tpc_params_t* params_host, int64_t* n_bins_host) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!n_bins_host || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  *n_bins_host = nb;
+  return TPC_OK;
+}
+
+int tpc_workspace_bytes(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, size_t* bytes_host) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!bytes_host || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (n_clusters < 0 || n_clusters > 2147483000ll || max_tracklets < 1 || max_tracklets > 2147483000ll) return TPC_EINVAL;
+  *bytes_host = tpc::make_layout(n_clusters, max_tracklets, nb, params_host->n_rows).total;
+  return TPC_OK;
+}
+
+int tpc_grid_build(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, const float* x,
+                   const float* y, const float* z, const float* q, const int32_t* sector_row, void* workspace,
+                   size_t ws_bytes, void* stream) {
+  (void)x;
+  (void)q;
+  Prep pr;
+  const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+  if (rc != TPC_OK) return rc;
+  if (n_clusters > 0 && (!y || !z || !sector_row)) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_grid_build(pr.G, pr.W, y, z, sector_row, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_grid_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, const void* workspace,
+                    size_t ws_bytes, int32_t* sorted_idx, int32_t* bin_first, void* stream) {
+  Prep pr;
+  const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+  if (rc != TPC_OK) return rc;
+  const cudaError_t e = tpc::launch_grid_export(pr.W, sorted_idx, bin_first, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_find_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, void* workspace,
+                    size_t ws_bytes, int32_t* cluster_track, int64_t max_tracks, int32_t* trk_seed, int32_t* trk_sector,
+                    int32_t* trk_nhits, int64_t* trk_first_hit, int32_t* trk_hits, int32_t* counters, void* stream) {
+  Prep pr;
+  const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+  if (rc != TPC_OK) return rc;
+  if (max_tracks < 1 || !trk_seed || !trk_sector || !trk_nhits || !trk_first_hit || !counters) return TPC_EINVAL;
+  if (n_clusters > 0 && (!cluster_track || !trk_hits)) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_find(pr.G, pr.W, cluster_track, max_tracks, trk_seed, trk_sector, trk_nhits,
+                                         trk_first_hit, trk_hits, counters, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, const void* workspace,
+                    size_t ws_bytes, int32_t* link_up, int32_t* link_dn, int32_t* up_c, int32_t* dn_c, int32_t* starts,
+                    int32_t* tl_nhits, int32_t* row_hit, void* stream) {
+  Prep pr;
+  const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+  if (rc != TPC_OK) return rc;
+  const cudaError_t e = tpc::launch_find_export(pr.G, pr.W, link_up, link_dn, up_c, dn_c, starts, tl_nhits, row_hit,
+                                                (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
+                   const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                   const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
+                   float* zref, float* chi2, int32_t* ndf, void* stream) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (n_clusters < 0 || max_tracks < 1 || !counters || !trk_nhits || !trk_first_hit || !par || !cov || !xref || !zref ||
+      !chi2 || !ndf)
+    return TPC_EINVAL;
+  if (n_clusters > 0 && (!y || !z || !sector_row || !trk_hits)) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_fit(G, n_clusters, y, z, sector_row, counters, max_tracks, trk_nhits, trk_first_hit,
+                                        trk_hits, par, cov, xref, zref, chi2, ndf, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
+                   const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
+                   int32_t* sector_row_dev, void* workspace, size_t ws_bytes, int32_t* cluster_track_dev,
+                   int32_t* trk_seed_dev, int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
+                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev, float* xref_dev,
+                   float* zref_dev, float* chi2_dev, int32_t* ndf_dev, int32_t* counters_host,
+                   int32_t* cluster_track_host, float* par_host, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e;
+  const size_t n = (size_t)(n_clusters > 0 ? n_clusters : 0);
+  if (n > 0 && (!y_host || !z_host || !sector_row_host || !y_dev || !z_dev || !sector_row_dev)) return TPC_EINVAL;
+  if (!counters_host) return TPC_EINVAL;
+  if (n > 0) {
+    if ((e = cudaMemcpyAsync(y_dev, y_host, n * sizeof(float), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(z_dev, z_host, n * sizeof(float), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(sector_row_dev, sector_row_host, n * sizeof(int32_t), cudaMemcpyHostToDevice, st)) != cudaSuccess)
+      return cuda_fail(e);
+  }
+  int rc = tpc_grid_build(params_host, n_clusters, max_tracklets, nullptr, y_dev, z_dev, nullptr, sector_row_dev, workspace,
+                          ws_bytes, stream);
+  if (rc != TPC_OK) return rc;
+  rc = tpc_find_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, cluster_track_dev, max_tracks,
+                       trk_seed_dev, trk_sector_dev, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, counters_dev, stream);
+  if (rc != TPC_OK) return rc;
+  rc = tpc_fit_tracks(params_host, n_clusters, y_dev, z_dev, sector_row_dev, counters_dev, max_tracks, trk_nhits_dev,
+                      trk_first_hit_dev, trk_hits_dev, par_dev, cov_dev, xref_dev, zref_dev, chi2_dev, ndf_dev, stream);
+  if (rc != TPC_OK) return rc;
+  if ((e = cudaMemcpyAsync(counters_host, counters_dev, sizeof(int32_t) * TPC_N_COUNTERS, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    return cuda_fail(e);
+  if (cluster_track_host && n > 0)
+    if ((e = cudaMemcpyAsync(cluster_track_host, cluster_track_dev, n * sizeof(int32_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+      return cuda_fail(e);
+  if (par_host)
+    if ((e = cudaMemcpyAsync(par_host, par_dev, sizeof(float) * 5 * (size_t)max_tracks, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+      return cuda_fail(e);
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+  return TPC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,176 @@
+// =============================================================================================
+// tpc_common.cuh -- device-side geometry tables, workspace layout and small helpers shared by the
+// kernels of libtpc_b200.so (grid, find, fit).  Product code: shares nothing with oracle/.
+//
+// Geometry and conventions follow SURVEY.md §8(c) R1-R7 (restated in DESIGN.md "Readings"):
+//   R1 rows at sector-local x = row_x[r], |y| <= row_x[r]*tan_half
+//   R2 sectors 0..17 side +1, 18..35 side -1; the grid's drift axis is zeta = side*z
+//   R7 per (sector,row): ny_r = max(1, ceil(2 ymax_r / cell_y)), nz = ceil((z_hi-z_lo)/cell_z),
+//      bin = zbin*ny_r + ybin (z-major), all fp32, one rounding per operation
+// =============================================================================================
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_b200.h"
+
+namespace tpc {
+
+constexpr int kMaxRows = TPC_MAX_ROWS;
+
+// Per-row geometry needed by every search (R1, R7).  Passed to kernels by value (__grid_constant__)
+// and staged into shared memory by each block, because rows differ across the lanes of a warp.
+struct RowGeo {
+  float X[kMaxRows];       // pad-row x
+  float ymax[kMaxRows];    // X*tan_half
+  int32_t ny[kMaxRows];    // y bins of the row
+  int32_t rowbase[kMaxRows + 1];  // first bin of row r inside a sector; [n_rows] = bins per sector
+};
+
+// Per-row constants of the cellular-automaton neighbour finder (R9).
+struct CaGeo {
+  float wu[kMaxRows];    // weight of the upper neighbour in the 3-point interpolation
+  float iy[kMaxRows];    // 1/(sigma_y^2 (1+wu^2+wd^2))
+  float iz[kMaxRows];    // 1/(sigma_z^2 (1+wu^2+wd^2))
+  float wyu[kMaxRows], wzu[kMaxRows];  // search half-window towards row r+1
+  float wyd[kMaxRows], wzd[kMaxRows];  // search half-window towards row r-1
+};
+
+// Scalars (R4, R6, R7, R9-R22).
+struct Scalars {
+  int32_t nsec, nrows, nz, bins_per_sector;
+  float inv_cy, inv_cz, z_lo, z_hi;
+  float kB, sy2, sz2;
+  float ca_cut, chi2_cut, chi2_chain_cut, win_max, max_sinphi, edge_margin;
+  int32_t max_gap, min_hits, n_fit_passes;
+  float cov0[5];
+};
+
+struct Geo {
+  Scalars s;
+  RowGeo row;
+  CaGeo ca;
+};
+
+// Internal device counters (int32) at the head of the workspace.
+enum {
+  WC_N_STARTS = 0,     // tracklets to follow (clamped)
+  WC_QUEUE = 1,        // work-queue head of the follower
+  WC_STATUS = 2,       // TPC_ST_* bits
+  WC_STARTS_FOUND = 3, // before clamping
+  WC_QUEUE2 = 4,
+  WC_N = 16
+};
+
+// Sorted 16-byte cluster record: one LDG.128 brings everything a candidate test needs.
+//   .x = y, .y = z (raw, not mirrored), .z = original index (int bits), .w = sector_row (int bits)
+using Rec = float4;
+
+// Workspace layout: a pure function of (n, max_tracklets, n_bins).  All offsets 256-byte aligned.
+struct Layout {
+  int64_t n, scap, scap_pad, nb;
+  int64_t scan_tiles;  // capacity (elements) of the scan scratch
+  size_t off_counters, off_rec, off_key, off_rank, off_bin_first, off_link_up, off_link_dn, off_up_c,
+      off_owner, off_starts, off_tl_info, off_tl_scan, off_row_hit, off_scan_tmp, total;
+};
+
+constexpr int kScanTile = 4096;  // elements per scan tile (256 threads x 16)
+
+inline size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows) {
+  Layout L{};
+  L.n = n;
+  L.scap = scap;
+  L.scap_pad = (scap + 31) & ~(int64_t)31;
+  L.nb = nb;
+  int64_t longest = nb + 1;
+  if (n + 1 > longest) longest = n + 1;
+  if (scap + 1 > longest) longest = scap + 1;
+  L.scan_tiles = (longest + kScanTile - 1) / kScanTile + 2;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = align256(o + bytes);
+    return at;
+  };
+  L.off_counters = take(sizeof(int32_t) * WC_N);
+  L.off_rec = take(sizeof(Rec) * (size_t)(n + 1));
+  L.off_key = take(sizeof(int32_t) * (size_t)(n + 1));      // bin id per cluster; later start-flag scan
+  L.off_rank = take(sizeof(int32_t) * (size_t)(n + 1));     // rank in bin; later unused
+  L.off_bin_first = take(sizeof(int32_t) * (size_t)(nb + 2));
+  L.off_link_up = take(sizeof(int32_t) * (size_t)(n + 1));
+  L.off_link_dn = take(sizeof(int32_t) * (size_t)(n + 1));
+  L.off_up_c = take(sizeof(int32_t) * (size_t)(n + 1));
+  L.off_owner = take(sizeof(uint64_t) * (size_t)(n + 1));
+  L.off_starts = take(sizeof(int32_t) * (size_t)(L.scap_pad + 1));
+  L.off_tl_info = take(sizeof(int32_t) * (size_t)(L.scap_pad + 1));
+  L.off_tl_scan = take(sizeof(int64_t) * (size_t)(L.scap_pad + 2));
+  L.off_row_hit = take(sizeof(int32_t) * (size_t)L.scap_pad * (size_t)nrows);
+  L.off_scan_tmp = take(sizeof(int64_t) * (size_t)L.scan_tiles);
+  L.total = o;
+  return L;
+}
+
+
+// Typed view of a workspace.
+struct Ws {
+  Layout L;
+  int32_t* counters;
+  Rec* rec;
+  int32_t *key, *rank, *bin_first, *link_up, *link_dn, *up_c;
+  unsigned long long* owner;
+  int32_t *starts, *tl_info;
+  long long* tl_scan;
+  int32_t* row_hit;
+  long long* scan_tmp;
+};
+
+inline Ws bind_ws(const Layout& L, void* workspace) {
+  char* b = (char*)workspace;
+  Ws w;
+  w.L = L;
+  w.counters = (int32_t*)(b + L.off_counters);
+  w.rec = (Rec*)(b + L.off_rec);
+  w.key = (int32_t*)(b + L.off_key);
+  w.rank = (int32_t*)(b + L.off_rank);
+  w.bin_first = (int32_t*)(b + L.off_bin_first);
+  w.link_up = (int32_t*)(b + L.off_link_up);
+  w.link_dn = (int32_t*)(b + L.off_link_dn);
+  w.up_c = (int32_t*)(b + L.off_up_c);
+  w.owner = (unsigned long long*)(b + L.off_owner);
+  w.starts = (int32_t*)(b + L.off_starts);
+  w.tl_info = (int32_t*)(b + L.off_tl_info);
+  w.tl_scan = (long long*)(b + L.off_tl_scan);
+  w.row_hit = (int32_t*)(b + L.off_row_hit);
+  w.scan_tmp = (long long*)(b + L.off_scan_tmp);
+  return w;
+}
+
+// Host launchers implemented in tpc_grid.cu / tpc_find.cu / tpc_fit.cu (each only enqueues).
+cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const float* z, const int32_t* sector_row,
+                              cudaStream_t st);
+cudaError_t launch_grid_export(const Ws& w, int32_t* sorted_idx, int32_t* bin_first, cudaStream_t st);
+cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64_t max_tracks, int32_t* trk_seed,
+                        int32_t* trk_sector, int32_t* trk_nhits, int64_t* trk_first_hit, int32_t* trk_hits,
+                        int32_t* counters, cudaStream_t st);
+cudaError_t launch_find_export(const Geo& g, const Ws& w, int32_t* link_up, int32_t* link_dn, int32_t* up_c,
+                               int32_t* dn_c, int32_t* starts, int32_t* tl_nhits, int32_t* row_hit, cudaStream_t st);
+cudaError_t launch_fit(const Geo& g, int64_t n, const float* y, const float* z, const int32_t* sector_row,
+                       const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                       const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
+                       float* zref, float* chi2, int32_t* ndf, cudaStream_t st);
+
+// ---- device helpers -------------------------------------------------------------------------
+// R7: clamp-to-range binning; NaN and negatives go to bin 0.
+__device__ __forceinline__ int clampbin(float v, int n) {
+  if (!(v > 0.0f)) return 0;
+  if (v >= (float)n) return n - 1;
+  return (int)v;
+}
+
+__device__ __forceinline__ Rec ld_rec(const Rec* __restrict__ recs, int k) { return __ldg(recs + k); }
+__device__ __forceinline__ int rec_idx(const Rec& r) { return __float_as_int(r.z); }
+__device__ __forceinline__ int rec_sr(const Rec& r) { return __float_as_int(r.w); }
+
+}  // namespace tpc

@@ -1,0 +1,107 @@
+// =============================================================================================
+// tpc_fit.cu -- step 3b of the hot path (BASELINE.json north_star (3) "refit of helices ... with
+// the time offset left free"): per accepted track, a 3-point circle seed
+// followed by an outward and an inward fp32 Kalman pass over its hit list.
+//
+//   k_fit   one thread per track; 5-parameter state + 15 covariance elements in registers;
+//           hits are gathered through the caller's y / z / sector_row arrays (original indices),
+//           so the kernel is self-contained and can refit any hit lists (e.g. truth hits).
+// The track count K is read from counters[TPC_CNT_TRACKS] on the device (no host sync).
+// =============================================================================================
+#include "tpc_common.cuh"
+#include "tpc_kalman.cuh"
+
+namespace tpc {
+
+namespace {
+
+constexpr int kFitThreads = 128;
+
+__global__ void __launch_bounds__(kFitThreads)
+k_fit(const __grid_constant__ Geo g, const float* __restrict__ y, const float* __restrict__ z,
+      const int32_t* __restrict__ sector_row, const int32_t* __restrict__ counters, int64_t max_tracks,
+      const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+      const int32_t* __restrict__ trk_hits, float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref,
+      float* __restrict__ zref_out, float* __restrict__ chi2_out, int32_t* __restrict__ ndf) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  const int nrows = sc.nrows;
+  for (int r = threadIdx.x; r < nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
+  for (int64_t k = (int64_t)blockIdx.x * kFitThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kFitThreads) {
+    const int n = trk_nhits[k];
+    const int32_t* hits = trk_hits + trk_first_hit[k];
+    auto rowx = [&](int h) { return sX[__ldg(sector_row + h) % nrows]; };
+    // R21: seed from the first, middle and last hit
+    const int a = hits[0], b = hits[n / 2], c = hits[n - 1], h1 = hits[1];
+    const float x1 = rowx(a), y1 = __ldg(y + a), x2 = rowx(b), y2 = __ldg(y + b), x3 = rowx(c), y3 = __ldg(y + c);
+    const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+    const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+    const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+    const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+    const float kappa = (2.0f * cross) / ((d12 * d23) * d13);  // signed curvature of the circumcircle
+    const float dx = rowx(h1) - x1, dy = __ldg(y + h1) - y1;
+    const float ch = sqrtf(dx * dx + dy * dy);
+    float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);  // chord direction rotated back by half the turn
+    if (sphi > ms) sphi = ms;
+    if (sphi < -ms) sphi = -ms;
+    const float zref = __ldg(z + a);
+    KState st;
+    st.p[0] = y1;
+    st.p[1] = 0.0f;
+    st.p[2] = sphi;
+    st.p[3] = (__ldg(z + h1) - zref) / ch;
+    st.p[4] = -(kappa / kB);
+    // R22: pass 1 inner -> outer, pass 2 outer -> inner, ...; covariance reset at the start of every pass
+    float chi2 = 0.0f;
+    float x_at = x1;
+    bool ok = true;
+    for (int pass = 0; pass < sc.n_fit_passes && ok; pass++) {
+      reset_cov(st, sc.cov0);
+      chi2 = 0.0f;
+      const int dir = (pass & 1) ? -1 : 1;
+      int i = dir > 0 ? 0 : n - 1;
+      for (int cnt = 0; cnt < n; cnt++, i += dir) {
+        const int h = hits[i];
+        const float xh = rowx(h);
+        if (cnt > 0) {  // the first hit of a pass is the one the state already sits at (no transport)
+          if (!propagate(st, xh - x_at, kB, ms)) {
+            ok = false;
+            break;
+          }
+          x_at = xh;
+        }
+        const Innov I = innovation(st, sy2, sz2);
+        chi2 = chi2 + update(st, I, __ldg(y + h), __ldg(z + h) - zref);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 5; i++) par[(int64_t)i * max_tracks + k] = st.p[i];
+#pragma unroll
+    for (int i = 0; i < 15; i++) cov[(int64_t)i * max_tracks + k] = st.C[i];
+    xref[k] = x_at;
+    zref_out[k] = zref;
+    chi2_out[k] = ok ? chi2 : -1.0f;
+    ndf[k] = ok ? 2 * n - 5 : -1;
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_fit(const Geo& g, int64_t n, const float* y, const float* z, const int32_t* sector_row,
+                       const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                       const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
+                       float* zref, float* chi2, int32_t* ndf, cudaStream_t st) {
+  (void)n;
+  if (max_tracks <= 0) return cudaSuccess;
+  int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits, trk_first_hit,
+                                                  trk_hits, par, cov, xref, zref, chi2, ndf);
+  return cudaGetLastError();
+}
+
+}  // namespace tpc

@@ -1,0 +1,162 @@
+// =============================================================================================
+// tpc_kalman.cuh -- fp32 5-parameter Kalman state in registers: helix transport (R12),
+// measurement update (R13).  SURVEY.md §8(c) R11-R13; DESIGN.md "Kernels / follower".
+//
+//   state p = (y, dz = z - zRef, sinphi, tanlambda, q/pT) at sector-local x, cosphi > 0   (R11)
+//   covariance: 15 lower-triangle elements C(i,j), j <= i, index i*(i+1)/2 + j
+//
+// Every expression is written as one IEEE operation per operator and the library is compiled
+// with -fmad=false, so the rounding sequence is fixed by the source text (DESIGN.md "Arithmetic
+// contract").  The sparse F C F^T below adds the non-zero terms of the dense product in
+// ascending-k order, which gives the same fp32 result as the dense triple loop.
+// =============================================================================================
+#pragma once
+#include "tpc_common.cuh"
+
+namespace tpc {
+
+#define TPC_CI(i, j) ((i) * ((i) + 1) / 2 + (j))
+
+struct KState {
+  float p[5];
+  float C[15];
+};
+
+// symmetric read: element (i,j) of the full matrix
+__device__ __forceinline__ float csym(const float (&C)[15], int i, int j) {
+  return (j <= i) ? C[TPC_CI(i, j)] : C[TPC_CI(j, i)];
+}
+
+__device__ __forceinline__ void reset_cov(KState& st, const float (&cov0)[5]) {
+#pragma unroll
+  for (int k = 0; k < 15; k++) st.C[k] = 0.0f;
+  st.C[TPC_CI(0, 0)] = cov0[0];
+  st.C[TPC_CI(1, 1)] = cov0[1];
+  st.C[TPC_CI(2, 2)] = cov0[2];
+  st.C[TPC_CI(3, 3)] = cov0[3];
+  st.C[TPC_CI(4, 4)] = cov0[4];
+}
+
+// asin(u)/u.  Series below |u| = 0.05 (row-to-row steps always land here); the long R17 jump
+// back to the start row can exceed it and takes the double-precision asin rounded once to fp32.
+__device__ __forceinline__ float asin_ratio(float u) {
+  if (fabsf(u) < 0.05f) {
+    const float u2 = u * u;
+    return 1.0f + u2 * (0.16666667f + u2 * (0.075f + u2 * 0.044642857f));
+  }
+  const double ud = (double)u;
+  return (float)(asin(ud) / ud);
+}
+
+// R12: exact helix transport x -> x + dx with Jacobian; C' = F C F^T (no process noise, R6).
+// Returns false and leaves the state untouched when |sinphi| would exceed max_sinphi.
+__device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float max_sinphi) {
+  const float y = st.p[0], dz = st.p[1], s1 = st.p[2], tl = st.p[3], q = st.p[4];
+  const float kappa = -(kB * q);  // R4
+  const float s2 = s1 + kappa * dx;
+  if (!(fabsf(s1) <= max_sinphi) || !(fabsf(s2) <= max_sinphi)) return false;
+  const float c1 = sqrtf(1.0f - s1 * s1), c2 = sqrtf(1.0f - s2 * s2);
+  const float cc = c1 + c2;
+  const float t = (s1 + s2) / cc;             // tangent of the mean direction
+  const float L = dx * sqrtf(1.0f + t * t);   // signed chord
+  const float u = (kappa * L) * 0.5f;
+  const float arc = L * asin_ratio(u);        // signed arc length in the bending plane
+  const float g = (1.0f + c1 * c2) + s1 * s2;
+  const float c1c2 = c1 * c2;
+  const float f02 = (dx * g) / (cc * c1c2);                    // dy'/dsinphi
+  const float f04 = -((kB * (dx * dx)) * g) / (c2 * (cc * cc));  // dy'/dq
+  const float f12 = ((tl * dx) * t) / c1c2;                    // ddz'/dsinphi
+  const float f13 = arc;                                       // ddz'/dtanl
+  const float f24 = -(kB * dx);                                // dsinphi'/dq
+  float E;                                                     // d(arc)/d(kappa), series near 0
+  if (fabsf(kappa * dx) < 1e-3f) {
+    const float c1_2 = c1 * c1, c1_3 = c1_2 * c1, c1_5 = c1_3 * c1_2;
+    E = ((dx * dx) * s1) / (2.0f * c1_3) +
+        ((kappa * ((dx * dx) * dx)) * (1.0f + 2.0f * (s1 * s1))) / (3.0f * c1_5);
+  } else {
+    E = (dx / c2 - arc) / kappa;
+  }
+  const float f14 = -((kB * tl) * E);  // ddz'/dq
+  st.p[0] = y + dx * t;
+  st.p[1] = dz + tl * arc;
+  st.p[2] = s2;
+  // M = F C (rows 0,1,2 differ from C), then N = M F^T, lower triangle.
+  float M0[5], M1[5], M2[5];
+#pragma unroll
+  for (int j = 0; j < 5; j++) {
+    const float C0j = csym(st.C, 0, j), C1j = csym(st.C, 1, j), C2j = csym(st.C, 2, j), C3j = csym(st.C, 3, j),
+                C4j = csym(st.C, 4, j);
+    M0[j] = (C0j + f02 * C2j) + f04 * C4j;
+    M1[j] = ((C1j + f12 * C2j) + f13 * C3j) + f14 * C4j;
+    M2[j] = C2j + f24 * C4j;
+  }
+  // rows 3 and 4 of M are rows 3 and 4 of C
+  const float M30 = st.C[TPC_CI(3, 0)], M31 = st.C[TPC_CI(3, 1)], M32 = st.C[TPC_CI(3, 2)], M33 = st.C[TPC_CI(3, 3)],
+              M34 = st.C[TPC_CI(4, 3)];
+  const float M40 = st.C[TPC_CI(4, 0)], M41 = st.C[TPC_CI(4, 1)], M42 = st.C[TPC_CI(4, 2)], M43 = st.C[TPC_CI(4, 3)],
+              M44 = st.C[TPC_CI(4, 4)];
+  st.C[TPC_CI(0, 0)] = (M0[0] + M0[2] * f02) + M0[4] * f04;
+  st.C[TPC_CI(1, 0)] = (M1[0] + M1[2] * f02) + M1[4] * f04;
+  st.C[TPC_CI(1, 1)] = ((M1[1] + M1[2] * f12) + M1[3] * f13) + M1[4] * f14;
+  st.C[TPC_CI(2, 0)] = (M2[0] + M2[2] * f02) + M2[4] * f04;
+  st.C[TPC_CI(2, 1)] = ((M2[1] + M2[2] * f12) + M2[3] * f13) + M2[4] * f14;
+  st.C[TPC_CI(2, 2)] = M2[2] + M2[4] * f24;
+  st.C[TPC_CI(3, 0)] = (M30 + M32 * f02) + M34 * f04;
+  st.C[TPC_CI(3, 1)] = ((M31 + M32 * f12) + M33 * f13) + M34 * f14;
+  st.C[TPC_CI(3, 2)] = M32 + M34 * f24;
+  st.C[TPC_CI(3, 3)] = M33;
+  st.C[TPC_CI(4, 0)] = (M40 + M42 * f02) + M44 * f04;
+  st.C[TPC_CI(4, 1)] = ((M41 + M42 * f12) + M43 * f13) + M44 * f14;
+  st.C[TPC_CI(4, 2)] = M42 + M44 * f24;
+  st.C[TPC_CI(4, 3)] = M43;
+  st.C[TPC_CI(4, 4)] = M44;
+  return true;
+}
+
+// R13: innovation covariance S = C[0:2,0:2] + diag(sigma_y^2, sigma_z^2) and its inverse.
+struct Innov {
+  float S00, S01, S11, Si00, Si01, Si11;
+};
+
+__device__ __forceinline__ Innov innovation(const KState& st, float sy2, float sz2) {
+  Innov I;
+  I.S00 = st.C[TPC_CI(0, 0)] + sy2;
+  I.S01 = st.C[TPC_CI(1, 0)];
+  I.S11 = st.C[TPC_CI(1, 1)] + sz2;
+  const float det = I.S00 * I.S11 - I.S01 * I.S01;
+  const float idet = 1.0f / det;
+  I.Si00 = I.S11 * idet;
+  I.Si01 = -(I.S01 * idet);
+  I.Si11 = I.S00 * idet;
+  return I;
+}
+
+__device__ __forceinline__ float chi2_of(const Innov& I, float r0, float r1) {
+  return ((r0 * r0) * I.Si00 + 2.0f * ((r0 * r1) * I.Si01)) + (r1 * r1) * I.Si11;
+}
+
+// R13: Kalman update with measurement (ym, zm) (zm relative to zRef), gain K = C H^T S^-1.
+__device__ __forceinline__ float update(KState& st, const Innov& I, float ym, float zm) {
+  const float r0 = ym - st.p[0], r1 = zm - st.p[1];
+  const float chi2 = chi2_of(I, r0, r1);
+  float K0[5], K1[5];
+#pragma unroll
+  for (int i = 0; i < 5; i++) {
+    const float Ci0 = csym(st.C, i, 0), Ci1 = csym(st.C, i, 1);
+    K0[i] = Ci0 * I.Si00 + Ci1 * I.Si01;
+    K1[i] = Ci0 * I.Si01 + Ci1 * I.Si11;
+  }
+  float N[15];
+#pragma unroll
+  for (int i = 0; i < 5; i++)
+#pragma unroll
+    for (int j = 0; j <= i; j++)
+      N[TPC_CI(i, j)] = st.C[TPC_CI(i, j)] - (K0[i] * csym(st.C, 0, j) + K1[i] * csym(st.C, 1, j));
+#pragma unroll
+  for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K0[i] * r0 + K1[i] * r1);
+#pragma unroll
+  for (int k = 0; k < 15; k++) st.C[k] = N[k];
+  return chi2;
+}
+
+}  // namespace tpc

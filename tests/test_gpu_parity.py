@@ -1,0 +1,191 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, same seeded inputs.
+
+configs[0..3] of BASELINE.json whole; configs[4] (the bench workload) on sampled sectors in
+test_gpu_config4.py.  Edge cases: empty input, one cluster, clusters outside the z range, capacity overflow,
+determinism (two runs bit-identical).
+"""
+import numpy as np
+import pytest
+
+import parity
+from paper_2106_03636_b200.synth import make_config, config0
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: -m gpu tests must run on the B200 box")
+    return torch
+
+
+def _dev(torch, ev):
+    return (torch.from_numpy(ev.y).cuda(), torch.from_numpy(ev.z).cuda(), torch.from_numpy(ev.sector_row).cuda())
+
+
+def _run_both(torch, orc, ev, stages=True):
+    from paper_2106_03636_b200 import binding
+    o = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)
+    trk = binding.Tracker(ev.params, ev.n)
+    y, z, sr = _dev(torch, ev)
+    res = trk.run(y, z, sr)
+    torch.cuda.synchronize()
+    assert res["status"] == 0, f"device status bits {res['status']}"
+    if stages:
+        sidx, bfirst = trk.grid_export()
+        parity.compare_grid(o, sidx, bfirst)
+        fe = trk.find_export()
+        parity.compare_links(o, fe)
+        nd, nt = parity.compare_tracklets(o, fe)
+        assert nd == 0, f"{nd} of {nt} tracklets differ from the oracle's row_hit tables"
+    st = parity.compare_tracks(o, res, ev.n)
+    print(ev.name, st)
+    return o, res, st
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_config_matches_oracle(torch_cuda, orc, cfg):
+    ev = make_config(cfg)
+    o, res, st = _run_both(torch_cuda, orc, ev)
+    parity.assert_contract(st, exact_count=True)
+    # the CUDA arithmetic restates the oracle's rounding sequence: expect identity, not just tolerance
+    assert st["assign_identical"] == ev.n
+    assert st["tracks_same_hits"] == st["tracks_oracle"]
+    assert st["par_bit_identical"] and st["cov_bit_identical"]
+
+
+def test_config0_golden_counts(torch_cuda, orc):
+    """tests/golden/config0_oracle_summary.txt (written from the oracle alone) against the CUDA path."""
+    import os
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "config0_oracle_summary.txt")) as f:
+        for line in f:
+            if not line.startswith("#"):
+                k, v = line.split()
+                gold[k] = v
+    from paper_2106_03636_b200 import binding
+    ev = config0()
+    trk = binding.Tracker(ev.params, ev.n)
+    res = trk.run(*_dev(torch_cuda, ev))
+    assert ev.n == int(gold["n_clusters"])
+    assert int(res["counters"][binding.CNT_TRACKLETS]) == int(gold["n_start_hits"])
+    assert res["trk_seed"].size == int(gold["n_tracks"])
+    assert int(np.count_nonzero(res["cluster_track"] >= 0)) == int(gold["n_assigned"])
+    import hashlib
+    cs = parity.cluster_seed(res["cluster_track"], res["trk_seed"]).astype(np.int32)
+    assert hashlib.sha256(cs.tobytes()).hexdigest() == gold["sha256_cluster_seed"]
+
+
+def test_deterministic_two_runs(torch_cuda):
+    from paper_2106_03636_b200 import binding
+    ev = make_config(1)
+    trk = binding.Tracker(ev.params, ev.n)
+    d = _dev(torch_cuda, ev)
+    a = trk.run(*d)
+    ga = trk.grid_export()
+    b = trk.run(*d)
+    gb = trk.grid_export()
+    assert np.array_equal(ga[0], gb[0]) and np.array_equal(ga[1], gb[1])
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_empty_and_tiny_inputs(torch_cuda, orc):
+    from paper_2106_03636_b200 import binding
+    torch = torch_cuda
+    p = config0().params
+    # n = 0
+    trk = binding.Tracker(p, 0)
+    e = torch.empty(0, dtype=torch.float32, device="cuda")
+    res = trk.run(e, e, torch.empty(0, dtype=torch.int32, device="cuda"))
+    assert res["counters"][binding.CNT_TRACKS] == 0 and res["counters"][binding.CNT_TRACKLETS] == 0
+    assert res["status"] == 0
+    # n = 1, n = 2 on the same row
+    for n in (1, 2):
+        trk = binding.Tracker(p, n)
+        y = torch.zeros(n, dtype=torch.float32, device="cuda")
+        z = torch.full((n,), 10.0, dtype=torch.float32, device="cuda")
+        sr = torch.full((n,), 70, dtype=torch.int32, device="cuda")
+        res = trk.run(y, z, sr)
+        assert res["counters"][binding.CNT_TRACKS] == 0
+        assert np.all(res["cluster_track"] == -1)
+
+
+def test_short_tracks_below_min_hits(torch_cuda, orc):
+    """A 6-row stub (< min_hits) is followed but rejected; a 30-row track is kept: ragged tail of the track list."""
+    from paper_2106_03636_b200 import binding
+    from paper_2106_03636_b200.synth import single_helix
+    ev = single_helix(0.8, np.radians(9.0), 0.3)
+    keep = (ev.sector_row % 152 < 30)
+    stub = (ev.sector_row % 152 >= 100) & (ev.sector_row % 152 < 106)
+    sel = keep | stub
+    y, z, sr = ev.y[sel], ev.z[sel], ev.sector_row[sel]
+    o = orc.run(ev.params, y, z, sr, "f32", True)
+    trk = binding.Tracker(ev.params, y.size)
+    res = trk.run(torch_cuda.from_numpy(y).cuda(), torch_cuda.from_numpy(z).cuda(), torch_cuda.from_numpy(sr).cuda())
+    st = parity.compare_tracks(o, res, y.size)
+    parity.assert_contract(st, exact_count=True)
+    assert st["tracks_cuda"] == 1 and res["counters"][binding.CNT_TRACKLETS] == 2
+
+
+def test_clusters_outside_z_range_are_clamped_not_lost(torch_cuda, orc):
+    """z_lo/z_hi tighter than the data: edge bins absorb the outliers (status bit set), results stay exact (R8)."""
+    from paper_2106_03636_b200 import binding
+    ev = config0()
+    p = ev.params.with_(z_lo=20.0, z_hi=180.0)
+    o = orc.run(p, ev.y, ev.z, ev.sector_row, "f32", True)
+    trk = binding.Tracker(p, ev.n)
+    res = trk.run(*_dev(torch_cuda, ev))
+    assert res["status"] & binding.ST_Z_CLAMPED
+    sidx, bfirst = trk.grid_export()
+    parity.compare_grid(o, sidx, bfirst)
+    st = parity.compare_tracks(o, res, ev.n)
+    parity.assert_contract(st, exact_count=True)
+    assert st["assign_identical"] == ev.n
+
+
+def test_capacity_overflow_is_flagged_and_bounded(torch_cuda):
+    from paper_2106_03636_b200 import binding
+    ev = config0()
+    trk = binding.Tracker(ev.params, ev.n, max_tracklets=40, max_tracks=8)
+    res = trk.run(*_dev(torch_cuda, ev))
+    assert res["status"] & binding.ST_TRACKLET_OVERFLOW
+    assert res["counters"][binding.CNT_TRACKLETS] == 40
+    assert res["counters"][binding.CNT_STARTS_FOUND] > 40
+    assert res["status"] & binding.ST_TRACK_OVERFLOW
+    assert res["trk_seed"].size == 8 and res["trk_hits"].size == int(res["trk_nhits"].sum())
+    assert np.all(res["cluster_track"] < 8)
+
+
+@pytest.mark.parametrize("cell", [1.0, 3.25])
+def test_grid_cell_independence(torch_cuda, orc, cell):
+    """R8 / pin I4 on the CUDA side: another cell size changes the grid, not the tracks."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(1, n_tracks=600)
+    p = ev.params.with_(cell_y=cell, cell_z=cell)
+    o = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)     # oracle at the default cell
+    trk = binding.Tracker(p, ev.n)
+    res = trk.run(*_dev(torch_cuda, ev))
+    st = parity.compare_tracks(o, res, ev.n)
+    parity.assert_contract(st, exact_count=True)
+    assert st["assign_identical"] == ev.n
+
+
+def test_host_buffer_entry_point(torch_cuda, orc):
+    """tpc_track_host (the e2e call of bench.py) gives the same answer as the device-pointer calls."""
+    from paper_2106_03636_b200 import binding
+    torch = torch_cuda
+    ev = make_config(1, n_tracks=400)
+    trk = binding.Tracker(ev.params, ev.n)
+    ref = trk.run(*_dev(torch, ev))
+    trk2 = binding.Tracker(ev.params, ev.n)
+    trk2.make_host_staging()
+    hy, hz, hs = (torch.from_numpy(a).pin_memory() for a in (ev.y, ev.z, ev.sector_row))
+    h2d, d2h = trk2.track_host(hy, hz, hs)
+    assert h2d == 12 * ev.n
+    K = int(trk2.counters_host[binding.CNT_TRACKS])
+    assert K == ref["trk_seed"].size
+    assert np.array_equal(trk2.cluster_track_host.numpy()[:ev.n], ref["cluster_track"])
+    assert np.array_equal(trk2.par_host.numpy()[:, :K], ref["par"])
