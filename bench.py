@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- TPC tracking throughput on B200 (BASELINE.json metric: clusters/s and Time Frames/s).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (tpc_grid_build -> tpc_find_tracks -> tpc_fit_tracks, SURVEY.md
+§8(a) rows a1..a6) over one synthetic event.  The default workload is BASELINE.json configs[4]: one 128-orbit
+50 kHz min-bias Pb-Pb Time Frame (~1.4e8 clusters, seeded synthetic).
+
+ value        clusters/s with the clusters resident in HBM (CUDA events, max over ranks)
+ e2e          same metric through tpc_track_host: pinned host buffers, H2D + D2H inside the timed region
+ roofline     the dominant kernel (by CUDA-event time measured live on the launching stream, tpc_profile_*)
+ cpu_baseline the CPU oracle, as it stands, on a bounded sample of the same event (rank 0, N = 1 only)
+ --impl reference : times the oracle alone on the host cores (this tier's reference arm)
+
+N > 1 (torchrun): every rank tracks its OWN Time Frame (TF-level replicas: GPUs process
+independent TFs); no data-path collective; "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "tpc_clusters_tracked_per_s"
+UNIT = "clusters/s"
+L2_BYTES = 126e6
+
+# Algorithmic HBM bytes per unit and fp32 operations per unit of every kernel (DESIGN.md "Kernels and
+# rooflines").  unit: "cluster" = per input cluster, "bin" = per grid bin,
+# "step" = per follower row step (propagate + search + update), "hit" = per refitted hit.
+KERNEL_MODEL = {
+    # name: (bound, bytes per cluster, bytes per bin, flop per unit [for alu-bound], unit)
+    "k_bin_count": ("hbm", 12 + 8 + 8, 0, 0, "cluster"),       # y,z,sr in; key,rank out; count RMW (4+4)
+    "k_scan_*": ("hbm", 0, 8, 0, "bin"),                        # read + write per scanned element (int32)
+    "k_scatter": ("hbm", 12 + 8 + 4 + 16, 0, 0, "cluster"),     # y,z,sr,key,rank,bin_first in; 16 B record out
+    "k_canon": ("hbm", 0, 4, 0, "bin"),
+    "k_neighbours": ("hbm", 16 + 8, 0, 0, "cluster"),           # own record in, two links out (neighbours from L2)
+    "k_clean": ("hbm", 8 + 8, 0, 0, "cluster"),
+    "k_compact_starts": ("hbm", 4, 0, 0, "cluster"),
+    "k_follow": ("alu", 0, 0, 0, "step"),
+    "k_count_kept": ("hbm", 0, 0, 0, "cluster"),
+    "k_write_tracks": ("hbm", 8, 0, 0, "cluster"),
+    "k_fit": ("alu", 0, 0, 0, "hit"),
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: one Time Frame)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def make_event(cfg: int, rank: int, world: int):
+    from paper_2106_03636_b200.synth import make_config
+    kw = {}
+    if cfg >= 2:
+        kw["workers"] = max(1, min(32, (os.cpu_count() or 1) // max(world, 1)))
+    seed = cfg + 1 + 100 * rank            # A7: seed = config index + 1; other ranks get their own Time Frame
+    return make_config(cfg, seed=seed, **kw)
+
+
+def workload_name(cfg: int) -> str:
+    return {0: "configs[0]: tiny single sector, 200 helices",
+            1: "configs[1]: one central Pb-Pb collision, full TPC",
+            2: "configs[2]: pp-like continuous slice, 200 collisions over 1 ms",
+            3: "configs[3]: pileup stress, 5 central Pb-Pb + loopers + 20% noise",
+            4: "configs[4]: one 128-orbit 50 kHz min-bias Pb-Pb Time Frame"}[cfg]
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks DURING the timed region")
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._pump, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons, power = [], None, set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for r in self.rows if t0 <= r[0] <= t1] or self.rows[-3:]
+        for _, line in rows:
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); smax = float(f[1])
+                for nm, v in zip(names, f[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+                power.append(float(f[6]))
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(power) if power else None}
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): bounded sample of the same workload
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(ev, max_clusters: int):
+    """Clusters of sector 0 (sectors are independent through the whole hot path), cut to the lowest-zeta slab
+    holding <= max_clusters clusters.  Returns (y, z, sector_row, description)."""
+    nrows = int(ev.params.n_rows)
+    sel = np.nonzero(ev.sector_row < nrows)[0]
+    desc = f"sector 0 of {ev.params.n_sectors}"
+    if sel.size > max_clusters:
+        zs = ev.z[sel]
+        cut = np.partition(zs, max_clusters)[max_clusters]
+        sel = sel[zs < cut]
+        desc += f", z < {float(cut):.1f} cm slab"
+    return ev.y[sel].copy(), ev.z[sel].copy(), ev.sector_row[sel].copy(), f"{desc}: {sel.size} clusters"
+
+
+def time_oracle(ev, y, z, sr, steps: int, warmup: int):
+    from oracle import tpc_oracle as orc
+    orc.build()
+    p1 = ev.params.with_(n_sectors=1) if int(ev.params.n_sectors) > 1 else ev.params
+    times, ntr = [], 0
+    for i in range(warmup + steps):
+        tm = {}
+        t0 = time.perf_counter()
+        o = orc.run(p1, y, z, sr, "f32", True, timings=tm)
+        dt = time.perf_counter() - t0
+        ntr = int(o["trk_seed"].size)
+        if i >= warmup:
+            times.append(dt)
+    return float(np.mean(times)), ntr
+
+
+def run_reference(args, rank: int):
+    """This tier's reference arm: the CPU oracle, as it stands, on a bounded sample per step."""
+    if rank != 0:
+        return
+    ev = make_event(args.config, 0, 1)
+    per_step_s = min(12.0, 200.0 / max(args.steps + args.warmup, 1))
+    y, z, sr, desc = oracle_sample(ev, int(per_step_s * 1.2e5))
+    dt, ntr = time_oracle(ev, y, z, sr, args.steps, args.warmup)
+    val = y.size / dt
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": workload_name(args.config), "n_clusters": int(y.size), "sample": desc},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "tracks_found": ntr}
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def run_ours(args, rank: int, local_rank: int, world: int):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU implementation")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2106_03636_b200 import binding
+
+    t_gen = time.perf_counter()
+    ev = make_event(args.config, rank, world)
+    t_gen = time.perf_counter() - t_gen
+    n = ev.n
+    hy, hz, hs = (torch.from_numpy(a).pin_memory() for a in (ev.y, ev.z, ev.sector_row))
+    y, z, sr = (a.to(dev, non_blocking=True) for a in (hy, hz, hs))
+    trk = binding.Tracker(ev.params, n, device=dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        trk.step(y, z, sr)
+    torch.cuda.synchronize()
+    cnt = trk.counters.cpu().numpy()
+    if int(cnt[binding.CNT_STATUS]) & (binding.ST_TRACKLET_OVERFLOW | binding.ST_TRACK_OVERFLOW):
+        raise RuntimeError(f"capacity overflow, status bits {int(cnt[binding.CNT_STATUS])}: the run would skip work")
+
+    # ---- timed region: K steps, inputs resident in HBM, CUDA events on the launching stream -----
+    binding.profile_collect(reset=True)
+    binding.profile_enable(True)
+    sampler = ClockSampler(local_rank)
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(); torch.cuda.synchronize()
+    w0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        trk.step(y, z, sr)
+    e1.record()
+    torch.cuda.synchronize(); barrier()
+    w1 = time.perf_counter()
+    clocks = sampler.stop(w0, w1)
+    ms_total = e0.elapsed_time(e1)
+    prof = binding.profile_collect(reset=True)
+    binding.profile_enable(False)
+    res = trk.results()
+    K_tracks = int(res["trk_seed"].size)
+    n_tracklets = int(res["counters"][binding.CNT_TRACKLETS])
+    n_hits = int(res["counters"][binding.CNT_HITS])
+
+    # ---- end to end through the host-buffer entry point -----------------------------------------
+    t_e2e, h2d, d2h = 0.0, 0, 0
+    if not args.no_e2e:
+        trk.make_host_staging()
+        trk.track_host(hy, hz, hs)                       # warm-up (first-touch of the staging buffers)
+        barrier(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            h2d, d2h = trk.track_host(hy, hz, hs)        # synchronises before returning
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) / args.steps
+        assert int(trk.counters_host[binding.CNT_TRACKS]) == K_tracks
+
+    # ---- max over ranks ----------------------------------------------------------------------------
+    ms_step = ms_total / args.steps
+    tot_clusters = float(n)
+    if world > 1:
+        t = torch.tensor([ms_step, t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, t_e2e = float(t[0]), float(t[1])
+        c = torch.tensor([float(n)], dtype=torch.float64, device=dev)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        tot_clusters = float(c[0])
+    if rank != 0:
+        return
+
+    hbm_peak, sm_max_mhz, peak_src = load_peaks()
+    value = tot_clusters / (ms_step * 1e-3)
+    # ---- per-kernel table and roofline of the dominant kernel -----------------------------------
+    kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps}
+            for k, v in prof.items() if v[1] > 0}
+    launches = int(sum(v[1] for v in prof.values()))
+    top = max(kern, key=lambda k: kern[k]["ms_per_step"])
+    top_ms = kern[top]["ms_per_step"] / max(kern[top]["launches_per_step"], 1)
+    nb = binding.grid_bins(ev.params)
+    work = binding.work_counts(res["counters"])
+    roofline = kernel_roofline(top, top_ms, n, nb, work, n_hits, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz,
+                               peak_src)
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+           "data": "synthetic",
+           "config": {"workload": workload_name(args.config), "n_clusters": n, "n_bins": nb,
+                      "time_frames_per_step_per_gpu": 1 if args.config == 4 else None,
+                      "l2": f"inputs ({12 * n / 1e6:.0f} MB/step) and workspace exceed the 126 MB L2; no explicit flush",
+                      "parallelism": f"tf-replicas x{world}", "gen_seconds": round(t_gen, 1)},
+           "time_frames_per_s": (world / (ms_step * 1e-3)) if args.config == 4 else None,
+           "tracks_found": K_tracks, "tracklets_followed": n_tracklets, "clusters_assigned": n_hits,
+           "follower_work": work,
+           "clocks": clocks, "gpu_launches": launches, "kernels": kern, "roofline": roofline}
+    if not args.no_e2e:
+        out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
+                      "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3}
+    if world == 1 and not args.no_cpu_baseline:
+        ys, zs, ss, desc = oracle_sample(ev, 1_500_000)
+        dt, ntr = time_oracle(ev, ys, zs, ss, 1, 0)
+        out["cpu_baseline"] = {"value": ys.size / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+                               "seconds": dt, "host_cores_available": os.cpu_count()}
+    print(json.dumps(out), flush=True)
+
+
+def kernel_roofline(name, ms, n, nb, work, n_hits, n_passes, hbm_peak, sm_max_mhz, peak_src):
+    bound, b_cl, b_bin, _, unit = KERNEL_MODEL.get(name, ("hbm", 0, 0, 0, "cluster"))
+    if bound == "hbm":
+        by = b_cl * n + b_bin * nb
+        ach = by / (ms * 1e-3) / 1e9
+        return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "traffic": None, "algorithmic_bytes_per_launch": by, "ms_per_launch": ms, "peak_source": peak_src}
+    # alu-bound kernels: fp32 operations actually required per unit
+    from paper_2106_03636_b200 import flops
+    if name == "k_follow":
+        units, fl = work["propagations"], flops.follow_flop(work)
+    else:
+        units, fl = n_hits * n_passes, flops.fit_flop(n_hits, n_passes)
+    peak = 148 * 128 * sm_max_mhz * 1e6 / 1e12      # fp32 lanes x clock, non-FMA (one op per lane per cycle), TFLOP/s
+    ach = fl / (ms * 1e-3) / 1e12
+    return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+            "traffic": None, "algorithmic_flop_per_launch": fl, "units": units, "unit_kind": unit, "ms_per_launch": ms,
+            "peak_source": f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz, 1 op/lane/cycle (no FMA contraction by contract)"}
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, local_rank, world)
+    if world > 1:
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -54,7 +54,7 @@ typedef enum {
   TPC_ECUDA = -3       /* a CUDA runtime call failed at enqueue time (see tpc_last_cuda_error) */
 } tpc_status_t;
 
-/* indices into the int32 counters[8] device array written by tpc_find_tracks */
+/* indices into the int32 counters[TPC_N_COUNTERS] device array written by tpc_find_tracks */
 enum {
   TPC_CNT_TRACKS = 0,     /* K  = number of accepted tracks (clamped to max_tracks)            */
   TPC_CNT_TRACKLETS = 1,  /* S  = number of start hits followed (clamped to max_tracklets)      */
@@ -64,7 +64,13 @@ enum {
   TPC_CNT_TRACKS_FOUND = 5, /* accepted tracks before clamping                                  */
   TPC_CNT_RESERVED6 = 6,
   TPC_CNT_RESERVED7 = 7,
-  TPC_N_COUNTERS = 8
+  TPC_CNT_PROP_LO = 8,    /* follower work (time ~ tracks x attached clusters):      */
+  TPC_CNT_PROP_HI = 9,    /*   64-bit count of helix transports (R12) done by the follower, lo/hi    */
+  TPC_CNT_UPD_LO = 10,    /*   64-bit count of Kalman updates (R13) done by the follower, lo/hi      */
+  TPC_CNT_UPD_HI = 11,
+  TPC_CNT_CAND_LO = 12,   /*   64-bit count of candidate clusters chi2-tested in R16 searches, lo/hi */
+  TPC_CNT_CAND_HI = 13,
+  TPC_N_COUNTERS = 16
 };
 #define TPC_ST_TRACKLET_OVERFLOW 1 /* more start hits than max_tracklets: the excess was dropped */
 #define TPC_ST_TRACK_OVERFLOW 2    /* more accepted tracks than max_tracks: the excess was dropped */
@@ -172,6 +178,21 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
                    int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev,
                    float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
                    int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
+
+/* ---- measurement support (bench.py `roofline`, `gpu_launches`) --------------------------------
+ * The library counts every kernel it launches, per kernel id, and can bracket each launch with a
+ * cudaEvent pair recorded on the launching stream.  Host-side state, one driving thread per GPU
+ * (PAPER.md l.72).  Event timing is off by default and costs nothing on the device when off.
+ *   tpc_profile_enable(on)   : switch event timing on/off and drop pending records
+ *   tpc_profile_kernels()    : number of kernel ids;  tpc_profile_name(id): its name (static storage)
+ *   tpc_profile_collect(n_ids, ms_host[n_ids] or NULL, launches_host[n_ids] or NULL, reset):
+ *       waits for the recorded events, writes the summed elapsed ms and the launch counts per
+ *       kernel id since the last reset; reset != 0 clears both.  At most 8192 timed launches are
+ *       kept between collects (later ones are counted but not timed). */
+int tpc_profile_enable(int on);
+int tpc_profile_kernels(void);
+const char* tpc_profile_name(int kernel_id);
+int tpc_profile_collect(int n_ids, double* ms_host, int64_t* launches_host, int reset);
 
 #ifdef __cplusplus
 }

@@ -18,14 +18,15 @@ import numpy as np
 from . import build as _build
 
 TPC_MAX_ROWS = 152
-TPC_N_COUNTERS = 8
+TPC_N_COUNTERS = 16
 CNT_TRACKS, CNT_TRACKLETS, CNT_HITS, CNT_STATUS, CNT_STARTS_FOUND, CNT_TRACKS_FOUND = 0, 1, 2, 3, 4, 5
+CNT_PROP_LO, CNT_UPD_LO, CNT_CAND_LO = 8, 10, 12
 ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_host")
+           "tpc_track_host", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
 
 
 class tpc_params_t(C.Structure):
@@ -67,6 +68,7 @@ def load(rebuild: bool = False):
         getattr(L, name).restype = C.c_char_p
     for name in SYMBOLS[3:]:
         getattr(L, name).restype = C.c_int
+    L.tpc_profile_name.restype = C.c_char_p
     _lib = L
     return L
 
@@ -76,6 +78,8 @@ def make_params(p) -> tpc_params_t:
     P = tpc_params_t()
     P.n_sectors, P.n_rows = int(p.n_sectors), int(p.n_rows)
     rx = np.asarray(p.row_x, dtype=np.float32)
+    if not (0 < P.n_rows <= TPC_MAX_ROWS) or rx.size < P.n_rows:
+        raise TpcError(f"n_rows = {P.n_rows} outside 1..{TPC_MAX_ROWS} or row_x too short")
     for i in range(P.n_rows):
         P.row_x[i] = float(rx[i])
     for name in ("tan_half", "kB", "sigma_y", "sigma_z", "z_lo", "z_hi", "cell_y", "cell_z", "ca_max_dydx",
@@ -110,6 +114,29 @@ def _dp(t):
 def _stream():
     import torch
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def profile_enable(on: bool):
+    """tpc_profile_enable: per-kernel CUDA-event timing on the launching stream."""
+    _check(load().tpc_profile_enable(C.c_int(int(on))), "tpc_profile_enable")
+
+
+def profile_collect(reset: bool = True) -> dict:
+    """tpc_profile_collect: {kernel name: (summed ms, launches)} since the last reset (synchronises)."""
+    L = load()
+    k = L.tpc_profile_kernels()
+    ms = (C.c_double * k)()
+    cnt = (C.c_int64 * k)()
+    _check(L.tpc_profile_collect(C.c_int(k), ms, cnt, C.c_int(int(reset))), "tpc_profile_collect")
+    return {L.tpc_profile_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
+
+
+def work_counts(counters) -> dict:
+    """Follower work from the counters array: transports (R12), updates (R13), candidates tested (R16)."""
+    c = np.asarray(counters).astype(np.int64) & 0xFFFFFFFF
+    return {"propagations": int(c[CNT_PROP_LO] | (c[CNT_PROP_LO + 1] << 32)),
+            "updates": int(c[CNT_UPD_LO] | (c[CNT_UPD_LO + 1] << 32)),
+            "candidates": int(c[CNT_CAND_LO] | (c[CNT_CAND_LO + 1] << 32))}
 
 
 def grid_bins(params) -> int:

@@ -9,6 +9,46 @@
 #include <string.h>
 
 #include "tpc_common.cuh"
+#include "tpc_prof.cuh"
+
+// ---- launch accounting / per-kernel event timing (tpc_prof.cuh) --------------------------------
+namespace tpc {
+namespace {
+constexpr int kMaxRec = 8192;
+bool g_prof_on = false;
+int64_t g_launches[KID_N] = {0};
+struct Rec2 {
+  int id;
+  cudaEvent_t a, b;
+};
+Rec2 g_rec[kMaxRec];
+int g_nrec = 0, g_nrec_created = 0;
+const char* const kKernelNames[KID_N] = {"k_bin_count", "k_scan_*", "k_scatter", "k_canon", "k_neighbours", "k_clean",
+                                         "k_compact_starts", "k_follow", "k_count_kept", "k_write_tracks", "k_fit",
+                                         "k_export_*"};
+}  // namespace
+
+void prof_begin(int id, cudaStream_t st) {
+  g_launches[id]++;
+  if (!g_prof_on || g_nrec >= kMaxRec) return;
+  if (g_nrec == g_nrec_created) {
+    if (cudaEventCreate(&g_rec[g_nrec].a) != cudaSuccess || cudaEventCreate(&g_rec[g_nrec].b) != cudaSuccess) {
+      g_prof_on = false;
+      return;
+    }
+    g_nrec_created++;
+  }
+  g_rec[g_nrec].id = id;
+  cudaEventRecord(g_rec[g_nrec].a, st);
+}
+
+void prof_end(int id, cudaStream_t st) {
+  (void)id;
+  if (!g_prof_on || g_nrec >= kMaxRec) return;
+  cudaEventRecord(g_rec[g_nrec].b, st);
+  g_nrec++;
+}
+}  // namespace tpc
 
 namespace {
 
@@ -122,6 +162,39 @@ const char* tpc_strerror(int status) {
 const char* tpc_last_cuda_error(void) { return g_cuda_err; }
 
 const char* tpc_version(void) { return "0.1.0"; }
+
+int tpc_profile_enable(int on) {
+  tpc::g_prof_on = on != 0;
+  tpc::g_nrec = 0;
+  return TPC_OK;
+}
+
+int tpc_profile_kernels(void) { return tpc::KID_N; }
+
+const char* tpc_profile_name(int kernel_id) {
+  return (kernel_id >= 0 && kernel_id < tpc::KID_N) ? tpc::kKernelNames[kernel_id] : "";
+}
+
+int tpc_profile_collect(int n_ids, double* ms_host, int64_t* launches_host, int reset) {
+  if (n_ids < 0 || n_ids > tpc::KID_N) return TPC_EINVAL;
+  if (ms_host) {
+    for (int i = 0; i < n_ids; i++) ms_host[i] = 0.0;
+    for (int k = 0; k < tpc::g_nrec; k++) {
+      cudaError_t e = cudaEventSynchronize(tpc::g_rec[k].b);
+      float ms = 0.0f;
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, tpc::g_rec[k].a, tpc::g_rec[k].b);
+      if (e != cudaSuccess) return cuda_fail(e);
+      if (tpc::g_rec[k].id < n_ids) ms_host[tpc::g_rec[k].id] += (double)ms;
+    }
+  }
+  if (launches_host)
+    for (int i = 0; i < n_ids; i++) launches_host[i] = tpc::g_launches[i];
+  if (reset) {
+    tpc::g_nrec = 0;
+    for (int i = 0; i < tpc::KID_N; i++) tpc::g_launches[i] = 0;
+  }
+  return TPC_OK;
+}
 
 int tpc_grid_bins(const tpc_params_t* params_host, int64_t* n_bins_host) {
   tpc::Geo G;

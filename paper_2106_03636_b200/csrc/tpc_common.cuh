@@ -59,6 +59,9 @@ enum {
   WC_STATUS = 2,       // TPC_ST_* bits
   WC_STARTS_FOUND = 3, // before clamping
   WC_QUEUE2 = 4,
+  WC_PROP64 = 8,       // unsigned long long at [8,9]: follower transports
+  WC_UPD64 = 10,       // unsigned long long at [10,11]: follower updates
+  WC_CAND64 = 12,      // unsigned long long at [12,13]: candidates tested
   WC_N = 16
 };
 

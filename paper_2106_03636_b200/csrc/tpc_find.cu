@@ -201,6 +201,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   const int n_starts = ws_counters[WC_N_STARTS];
   const int lane = threadIdx.x & 31;
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
+  unsigned long long work[3] = {0ull, 0ull, 0ull};
   for (;;) {
     int base = 0;
     if (lane == 0) base = atomicAdd(ws_counters + WC_QUEUE, 32);
@@ -233,16 +234,19 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     }
     my_hits[(int64_t)r0 * scap_pad] = p0;
     int nh = 1, lo = r0, hi = r0, r_at = r0;
+    unsigned nprop = 0, nupd = 1, ncand = 0;  // work counters (TPC_CNT_PROP/UPD/CAND)
     // R15: chain phase along the cleaned up-links
     for (int hn = p1; hn >= 0;) {
       const Rec c = ld_rec(rec, hn);
       const int rn = rec_sr(c) - s * nrows;
       KState trial = st;
       if (!propagate(trial, sm.X[rn] - sm.X[r_at], kB, ms)) break;
+      nprop++;
       const Innov I = innovation(trial, sy2, sz2);
       const float chi2 = chi2_of(I, c.x - trial.p[0], (c.y - zref) - trial.p[1]);
       if (chi2 > sc.chi2_chain_cut) break;  // discard the prediction: state stays at the previous hit
       update(trial, I, c.x, c.y - zref);
+      nupd++;
       st = trial;
       my_hits[(int64_t)rn * scap_pad] = hn;
       nh++;
@@ -256,11 +260,13 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
       int r = leg == 0 ? r_at + 1 : r0 - 1;
       if (leg == 1) {
         if (!propagate(st, sm.X[r0] - sm.X[r_at], kB, ms)) break;
+        nprop++;
         r_at = r0;
       }
       int misses = 0;
       for (; r >= 0 && r < nrows; r += dir) {
         if (!propagate(st, sm.X[r] - sm.X[r_at], kB, ms)) break;
+        nprop++;
         r_at = r;
         if (fabsf(st.p[0]) > sm.ymax[r] + sc.edge_margin) break;  // left the sector
         const Innov I = innovation(st, sy2, sz2);
@@ -280,6 +286,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
             const float q0 = c.x - yp, q1 = (c.y - zref) - dzp;
             if (!(fabsf(q0) <= wy && fabsf(q1) <= wz)) continue;
             const float chi2 = chi2_of(I, q0, q1);
+            ncand++;
             const int ci = rec_idx(c);
             if (!have || chi2 < best || (chi2 == best && ci < bi)) {  // ties: lowest original index
               have = true;
@@ -293,6 +300,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
         }
         if (have && best < sc.chi2_cut) {
           update(st, I, by, bz - zref);
+          nupd++;
           my_hits[(int64_t)r * scap_pad] = bk;
           nh++;
           lo = min(lo, r);
@@ -312,6 +320,17 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
       const int c = my_hits[(int64_t)r * scap_pad];
       if (c >= 0) atomicMax(owner + c, key);
     }
+    work[0] += nprop;
+    work[1] += nupd;
+    work[2] += ncand;
+  }
+  // one 64-bit atomic per warp and counter
+#pragma unroll
+  for (int k = 0; k < 3; k++) {
+    unsigned long long v = work[k];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if (lane == 0 && v) atomicAdd((unsigned long long*)(ws_counters + WC_PROP64) + k, v);
   }
 }
 
@@ -361,6 +380,9 @@ k_write_tracks(int nrows, const Rec* __restrict__ rec, const int32_t* __restrict
       counters[TPC_CNT_STATUS] = ws_counters[WC_STATUS] | (K > max_tracks ? TPC_ST_TRACK_OVERFLOW : 0);
       counters[TPC_CNT_RESERVED6] = 0;
       counters[TPC_CNT_RESERVED7] = 0;
+      for (int k = 0; k < 6; k++) counters[TPC_CNT_PROP_LO + k] = ws_counters[WC_PROP64 + k];
+      counters[14] = 0;
+      counters[15] = 0;
     }
     if (t >= n_starts) continue;
     const long long ex = tl_scan[t], nx = tl_scan[t + 1];
@@ -450,24 +472,30 @@ cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64
   // queue heads restart; status bits from the grid build are kept
   if ((e = cudaMemsetAsync(w.counters + WC_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.counters + WC_N_STARTS, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(w.counters + WC_PROP64, 0, sizeof(int32_t) * 6, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.owner, 0, sizeof(uint64_t) * (size_t)(n + 1), st)) != cudaSuccess) return e;
   if (n > 0 && (e = cudaMemsetAsync(cluster_track, 0xFF, sizeof(int32_t) * (size_t)n, st)) != cudaSuccess) return e;
   int32_t* flag = w.key;  // the bin ids of the grid build are dead by now
-  if (n > 0) k_neighbours<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, w.rec, w.bin_first, w.link_up, w.link_dn);
-  k_clean<<<blocks_for(n + 1, kThreads), kThreads, 0, st>>>(n, w.link_up, w.link_dn, w.up_c, flag);
+  if (n > 0)
+    TPC_LAUNCH(KID_NEIGHBOURS, st,
+               (k_neighbours<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, w.rec, w.bin_first, w.link_up, w.link_dn)));
+  TPC_LAUNCH(KID_CLEAN, st, (k_clean<<<blocks_for(n + 1, kThreads), kThreads, 0, st>>>(n, w.link_up, w.link_dn, w.up_c, flag)));
   if ((e = exclusive_scan<int32_t>(flag, flag, n + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
   if (n > 0) {
-    k_compact_starts<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, scap, flag, w.starts, w.counters);
-    k_follow<<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.starts, scap_pad, w.row_hit,
-                                                         w.tl_info, w.owner, w.counters);
+    TPC_LAUNCH(KID_COMPACT_STARTS, st,
+               (k_compact_starts<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, scap, flag, w.starts, w.counters)));
+    TPC_LAUNCH(KID_FOLLOW, st,
+               (k_follow<<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.starts, scap_pad,
+                                                                    w.row_hit, w.tl_info, w.owner, w.counters)));
   }
-  k_count_kept<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(g.s.min_hits, w.rec, w.starts, scap_pad,
-                                                                        w.row_hit, w.tl_info, w.owner, w.tl_scan,
-                                                                        w.counters);
+  TPC_LAUNCH(KID_COUNT_KEPT, st,
+             (k_count_kept<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(
+                 g.s.min_hits, w.rec, w.starts, scap_pad, w.row_hit, w.tl_info, w.owner, w.tl_scan, w.counters)));
   if ((e = exclusive_scan<long long>(w.tl_scan, w.tl_scan, scap_pad + 1, w.scan_tmp, st)) != cudaSuccess) return e;
-  k_write_tracks<<<blocks_for(scap_pad > 0 ? scap_pad : 1, kThreads), kThreads, 0, st>>>(
-      g.s.nrows, w.rec, w.starts, scap_pad, w.row_hit, w.tl_info, w.owner, w.tl_scan, max_tracks, cluster_track,
-      trk_seed, trk_sector, trk_nhits, trk_first_hit, trk_hits, counters, w.counters);
+  TPC_LAUNCH(KID_WRITE_TRACKS, st,
+             (k_write_tracks<<<blocks_for(scap_pad > 0 ? scap_pad : 1, kThreads), kThreads, 0, st>>>(
+                 g.s.nrows, w.rec, w.starts, scap_pad, w.row_hit, w.tl_info, w.owner, w.tl_scan, max_tracks,
+                 cluster_track, trk_seed, trk_sector, trk_nhits, trk_first_hit, trk_hits, counters, w.counters)));
   return cudaGetLastError();
 }
 
@@ -475,12 +503,13 @@ cudaError_t launch_find_export(const Geo& g, const Ws& w, int32_t* link_up, int3
                                int32_t* dn_c, int32_t* starts, int32_t* tl_nhits, int32_t* row_hit, cudaStream_t st) {
   const int64_t n = w.L.n;
   if (n > 0 && (link_up || link_dn || up_c || dn_c))
-    k_export_links<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, w.rec, w.link_up, w.link_dn, w.up_c, link_up, link_dn,
-                                                                 up_c, dn_c);
+    TPC_LAUNCH(KID_EXPORT, st,
+               (k_export_links<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, w.rec, w.link_up, w.link_dn, w.up_c,
+                                                                            link_up, link_dn, up_c, dn_c)));
   if (w.L.scap > 0 && (starts || tl_nhits || row_hit))
-    k_export_tracklets<<<blocks_for(w.L.scap, kThreads), kThreads, 0, st>>>(g.s.nrows, w.rec, w.starts, w.L.scap_pad,
-                                                                            w.row_hit, w.tl_info, starts, tl_nhits,
-                                                                            row_hit, w.counters);
+    TPC_LAUNCH(KID_EXPORT, st,
+               (k_export_tracklets<<<blocks_for(w.L.scap, kThreads), kThreads, 0, st>>>(
+                   g.s.nrows, w.rec, w.starts, w.L.scap_pad, w.row_hit, w.tl_info, starts, tl_nhits, row_hit, w.counters)));
   return cudaGetLastError();
 }
 

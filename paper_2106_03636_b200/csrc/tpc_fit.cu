@@ -10,6 +10,7 @@
 // =============================================================================================
 #include "tpc_common.cuh"
 #include "tpc_kalman.cuh"
+#include "tpc_prof.cuh"
 
 namespace tpc {
 
@@ -99,8 +100,9 @@ cudaError_t launch_fit(const Geo& g, int64_t n, const float* y, const float* z, 
   if (max_tracks <= 0) return cudaSuccess;
   int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
   if (blocks > 148 * 16) blocks = 148 * 16;
-  k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits, trk_first_hit,
-                                                  trk_hits, par, cov, xref, zref, chi2, ndf);
+  TPC_LAUNCH(KID_FIT, st,
+             (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits,
+                                                             trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf)));
   return cudaGetLastError();
 }
 

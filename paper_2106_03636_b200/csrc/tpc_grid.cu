@@ -110,13 +110,16 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
   if ((e = cudaMemsetAsync(w.counters, 0, sizeof(int32_t) * WC_N, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.bin_first, 0, sizeof(int32_t) * (size_t)(nb + 2), st)) != cudaSuccess) return e;
   if (n > 0) {
-    k_bin_count<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, y, z, sector_row, w.key, w.rank, w.bin_first,
-                                                              w.counters);
+    TPC_LAUNCH(KID_BIN_COUNT, st,
+               (k_bin_count<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, y, z, sector_row, w.key, w.rank,
+                                                                         w.bin_first, w.counters)));
   }
   if ((e = exclusive_scan<int32_t>(w.bin_first, w.bin_first, nb + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
   if (n > 0) {
-    k_scatter<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, y, z, sector_row, w.key, w.rank, w.bin_first, w.rec);
-    k_canon<<<blocks_for(nb, kThreads), kThreads, 0, st>>>(nb, w.bin_first, w.rec);
+    TPC_LAUNCH(KID_SCATTER, st,
+               (k_scatter<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, y, z, sector_row, w.key, w.rank, w.bin_first,
+                                                                       w.rec)));
+    TPC_LAUNCH(KID_CANON, st, (k_canon<<<blocks_for(nb, kThreads), kThreads, 0, st>>>(nb, w.bin_first, w.rec)));
   }
   return cudaGetLastError();
 }
@@ -124,7 +127,8 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
 cudaError_t launch_grid_export(const Ws& w, int32_t* sorted_idx, int32_t* bin_first, cudaStream_t st) {
   cudaError_t e;
   if (sorted_idx && w.L.n > 0)
-    k_export_sorted<<<blocks_for(w.L.n, kThreads), kThreads, 0, st>>>(w.L.n, w.rec, sorted_idx);
+    TPC_LAUNCH(KID_EXPORT, st,
+               (k_export_sorted<<<blocks_for(w.L.n, kThreads), kThreads, 0, st>>>(w.L.n, w.rec, sorted_idx)));
   if (bin_first)
     if ((e = cudaMemcpyAsync(bin_first, w.bin_first, sizeof(int32_t) * (size_t)(w.L.nb + 1), cudaMemcpyDeviceToDevice,
                              st)) != cudaSuccess)

@@ -1,0 +1,50 @@
+// =============================================================================================
+// tpc_prof.cuh -- launch accounting and optional per-kernel CUDA-event timing on the LAUNCHING
+// stream (bench.py's `roofline` and `gpu_launches`; include/tpc_b200.h tpc_profile_*).
+//
+// Every kernel launch of the library goes through TPC_LAUNCH(id, stream, kernel<<<...>>>(...)):
+//   - the per-kernel launch counter is always incremented (host side, a few ns);
+//   - when profiling is enabled, a cudaEvent pair is recorded around the launch on the same
+//     stream; tpc_profile_collect() later synchronises those events and sums the elapsed times
+//     per kernel id.  Disabled (the default) it costs nothing on the device.
+// Not thread-safe: one host thread drives one GPU ("one CPU core per GPU").
+// =============================================================================================
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tpc {
+
+enum KernelId {
+  KID_BIN_COUNT = 0,
+  KID_SCAN,
+  KID_SCATTER,
+  KID_CANON,
+  KID_NEIGHBOURS,
+  KID_CLEAN,
+  KID_COMPACT_STARTS,
+  KID_FOLLOW,
+  KID_COUNT_KEPT,
+  KID_WRITE_TRACKS,
+  KID_FIT,
+  KID_EXPORT,
+  KID_N
+};
+
+void prof_begin(int id, cudaStream_t st);
+void prof_end(int id, cudaStream_t st);
+
+struct ProfScope {
+  int id;
+  cudaStream_t st;
+  ProfScope(int i, cudaStream_t s) : id(i), st(s) { prof_begin(id, st); }
+  ~ProfScope() { prof_end(id, st); }
+};
+
+}  // namespace tpc
+
+#define TPC_LAUNCH(id, st, ...)       \
+  do {                                \
+    ::tpc::ProfScope _ps((id), (st)); \
+    __VA_ARGS__;                      \
+  } while (0)

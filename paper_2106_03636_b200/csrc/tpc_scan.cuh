@@ -9,6 +9,7 @@
 // =============================================================================================
 #pragma once
 #include "tpc_common.cuh"
+#include "tpc_prof.cuh"
 
 namespace tpc {
 
@@ -119,9 +120,9 @@ template <class T>
 inline cudaError_t exclusive_scan(const T* in, T* out, int64_t n, T* tmp, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
   const int64_t ntiles = (n + kScanTile - 1) / kScanTile;
-  k_scan_reduce<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(in, n, tmp);
-  k_scan_tiles<T><<<1, 1024, 0, st>>>(tmp, ntiles);
-  k_scan_apply<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(in, out, n, tmp);
+  TPC_LAUNCH(KID_SCAN, st, (k_scan_reduce<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(in, n, tmp)));
+  TPC_LAUNCH(KID_SCAN, st, (k_scan_tiles<T><<<1, 1024, 0, st>>>(tmp, ntiles)));
+  TPC_LAUNCH(KID_SCAN, st, (k_scan_apply<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(in, out, n, tmp)));
   return cudaGetLastError();
 }
 

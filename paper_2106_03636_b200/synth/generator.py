@@ -15,6 +15,7 @@ No item of any public dataset is reproduced: the paper's inputs were ALICE raw T
 from __future__ import annotations
 
 import math
+import os
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -203,11 +204,11 @@ def choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi, lo=1.0, hi=8.0):
     return float(np.float32(round(c * 4.0) / 4.0))      # quarter-cm steps: exact in fp32
 
 
-def _assemble(name, rng, t, t_us, sigma_y, sigma_z, dropout, noise_frac, single_sector, params_kw=None,
-              smear=True, shuffle=True):
-    """Trace all tracks, apply drift-time shift (R5), smear, drop, add noise (A5), shuffle."""
-    row_x = default_row_x()
-    rx64 = row_x.astype(np.float64)
+def _trace_signal(rng, t, t_us, sigma_y, sigma_z, dropout, single_sector, smear=True):
+    """Trace tracks `t`, apply dropout (A5), the drift-time shift (R5) and smearing.
+
+    Returns (track index, sector, row, y_local, z_meas) of every signal cluster; float64 y/z."""
+    rx64 = default_row_x().astype(np.float64)
     tan_half = math.tan(math.radians(10.0))
     t = dict(t)
     t["kappa"] = -KB * t["qpt"]
@@ -227,10 +228,19 @@ def _assemble(name, rng, t, t_us, sigma_y, sigma_z, dropout, noise_frac, single_
     sector = a_s + np.where(side > 0, 0, SECTORS_PER_SIDE)
     if single_sector:
         sector = np.zeros_like(a_s)
-    zm = a_z - side * V_DRIFT * t_us[a_t]                 # R5
+    zm = a_z - side * V_DRIFT * np.asarray(t_us)[a_t]     # R5
     if smear:
         a_y = a_y + rng.normal(0.0, sigma_y, a_t.size)
         zm = zm + rng.normal(0.0, sigma_z, a_t.size)
+    return a_t, sector, a_r, a_y, zm
+
+
+def _finish(name, rng, t, t_us, sig, noise_frac, single_sector, params_kw=None, shuffle=True):
+    """Add noise (A5) and charge (A6), shuffle, choose the grid range/cell and build the Event."""
+    a_t, sector, a_r, a_y, zm = sig
+    row_x = default_row_x()
+    rx64 = row_x.astype(np.float64)
+    tan_half = math.tan(math.radians(10.0))
     n_sig = a_t.size
     n_sectors = 1 if single_sector else 2 * SECTORS_PER_SIDE
     # noise (A5): uniform over (sector,row), y across the row, z over that side's occupied range
@@ -239,8 +249,10 @@ def _assemble(name, rng, t, t_us, sigma_y, sigma_z, dropout, noise_frac, single_
         ns = rng.integers(0, n_sectors, n_noise)
         nr = rng.integers(0, N_ROWS, n_noise)
         ny = rng.uniform(-1.0, 1.0, n_noise) * rx64[nr] * tan_half
+        side = np.where(sector < SECTORS_PER_SIDE, 1.0, -1.0) if not single_sector else np.ones(n_sig)
         zeta = side * zm                                   # mirrored drift coordinate
         zl, zh = (float(zeta.min()), float(zeta.max())) if n_sig else (0.0, Z_MAX)
+        del zeta, side
         nside = np.where(ns < SECTORS_PER_SIDE, 1.0, -1.0)
         nz = nside * rng.uniform(zl, zh, n_noise)
         sector = np.concatenate([sector, ns]); a_r = np.concatenate([a_r, nr])
@@ -248,23 +260,36 @@ def _assemble(name, rng, t, t_us, sigma_y, sigma_z, dropout, noise_frac, single_
         a_t = np.concatenate([a_t, np.full(n_noise, -1)])
     n = a_t.size
     q = 20.0 + rng.exponential(30.0, n)                    # A6
-    perm = rng.permutation(n) if shuffle else np.arange(n)
-    sector, a_r, a_y, zm, a_t, q = sector[perm], a_r[perm], a_y[perm], zm[perm], a_t[perm], q[perm]
     y32 = a_y.astype(np.float32); z32 = zm.astype(np.float32)
     sr = (sector * N_ROWS + a_r).astype(np.int32)
-    sgn = np.where(sector < SECTORS_PER_SIDE, 1.0, -1.0) if not single_sector else np.ones(n)
-    zeta = sgn * z32.astype(np.float64)
+    tt = a_t.astype(np.int32); q32 = q.astype(np.float32)
+    del a_y, zm, a_t, q
+    if shuffle:
+        perm = rng.permutation(n)
+        y32, z32, sr, tt, q32 = y32[perm], z32[perm], sr[perm], tt[perm], q32[perm]
+        del perm
+    sgn = np.where(sr < SECTORS_PER_SIDE * N_ROWS, np.float32(1.0), np.float32(-1.0)) if not single_sector \
+        else np.ones(n, np.float32)
+    zeta = (sgn * z32).astype(np.float64)
     z_lo = float(np.floor(zeta.min() - 1.0)) if n else -1.0
     z_hi = float(np.ceil(zeta.max() + 1.0)) if n else Z_MAX + 1.0
+    del zeta, sgn
     cell = choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi)
     kw = dict(n_sectors=n_sectors, z_lo=z_lo, z_hi=z_hi, cell_y=cell, cell_z=cell)
     kw.update(params_kw or {})
     p = TpcParams(**kw)
     trk = {k: np.asarray(v) for k, v in t.items()}
     trk["t_us"] = np.asarray(t_us)
-    return Event(name=name, params=p, x=row_x[a_r].astype(np.float32), y=y32, z=z32, q=q.astype(np.float32),
-                 sector_row=sr, true_track=a_t.astype(np.int32), trk=trk,
+    return Event(name=name, params=p, x=row_x[sr % N_ROWS], y=y32, z=z32, q=q32,
+                 sector_row=sr, true_track=tt, trk=trk,
                  meta=dict(n_signal=int(n_sig), n_noise=int(n_noise)))
+
+
+def _assemble(name, rng, t, t_us, sigma_y, sigma_z, dropout, noise_frac, single_sector, params_kw=None,
+              smear=True, shuffle=True):
+    """Trace all tracks, apply drift-time shift (R5), smear, drop, add noise (A5), shuffle."""
+    sig = _trace_signal(rng, t, t_us, sigma_y, sigma_z, dropout, single_sector, smear)
+    return _finish(name, rng, t, t_us, sig, noise_frac, single_sector, params_kw, shuffle)
 
 
 def config0(seed=1, n_tracks=200, **kw):
@@ -287,18 +312,45 @@ def config1(seed=2, n_tracks=5000, **kw):
     return _assemble("c1", rng, t, np.zeros(n_tracks), 0.08, 0.10, 0.02, 0.05, False, **kw)
 
 
-def _pileup(name, seed, t_coll_us, mult, dropout, noise, looper_frac=0.0, **kw):
-    rng = np.random.Generator(np.random.PCG64(seed))
-    parts, times, coll = [], [], []
-    for ic, (tc, m) in enumerate(zip(t_coll_us, mult)):
-        if m <= 0:
-            continue
-        vz0 = rng.normal(0.0, 5.0)
-        parts.append(_sample_tracks_pbpb(rng, int(m), looper_frac=looper_frac, vz0=vz0))
-        times.append(np.full(int(m), tc)); coll.append(np.full(int(m), ic))
+def _one_collision(args):
+    """Tracks + signal clusters of one collision from its own counter-seeded stream (order-free, so the
+    collisions can be generated by a process pool and the event is identical for any worker count)."""
+    seed, ic, tc, m, dropout, looper_frac = args
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([int(seed), int(ic)])))
+    vz0 = rng.normal(0.0, 5.0)
+    t = _sample_tracks_pbpb(rng, int(m), looper_frac=looper_frac, vz0=vz0)
+    a_t, sector, a_r, a_y, zm = _trace_signal(rng, t, np.full(int(m), tc), 0.08, 0.10, dropout, False)
+    return t, (a_t.astype(np.int32), sector.astype(np.int8), a_r.astype(np.int16), a_y.astype(np.float32), zm)
+
+
+def _pileup(name, seed, t_coll_us, mult, dropout, noise, looper_frac=0.0, workers=None, **kw):
+    jobs = [(seed, ic, float(tc), int(m), dropout, looper_frac)
+            for ic, (tc, m) in enumerate(zip(t_coll_us, mult)) if m > 0]
+    total = sum(j[3] for j in jobs)
+    if workers is None:
+        workers = min(os.cpu_count() or 1, 32) if total > 100000 else 1
+    if workers > 1:
+        import multiprocessing as mp
+        order = sorted(range(len(jobs)), key=lambda i: -jobs[i][3])       # big collisions first
+        with mp.get_context("fork").Pool(workers) as pool:
+            res = pool.map(_one_collision, [jobs[i] for i in order], chunksize=1)
+        out = [None] * len(jobs)
+        for i, r in zip(order, res):
+            out[i] = r
+    else:
+        out = [_one_collision(j) for j in jobs]
+    parts = [o[0] for o in out]
     t = {k: np.concatenate([p[k] for p in parts]) for k in parts[0]}
-    t["collision"] = np.concatenate(coll)
-    return _assemble(name, rng, t, np.concatenate(times), 0.08, 0.10, dropout, noise, False, **kw), rng
+    t["collision"] = np.concatenate([np.full(j[3], j[1]) for j in jobs])
+    t_us = np.concatenate([np.full(j[3], j[2]) for j in jobs])
+    off = np.cumsum([0] + [j[3] for j in jobs])
+    a_t = np.concatenate([o[1][0].astype(np.int64) + off[i] for i, o in enumerate(out)])
+    sig = (a_t, np.concatenate([o[1][1] for o in out]).astype(np.int64),
+           np.concatenate([o[1][2] for o in out]).astype(np.int64),
+           np.concatenate([o[1][3] for o in out]), np.concatenate([o[1][4] for o in out]))
+    del out, parts
+    rng = np.random.Generator(np.random.PCG64(seed))
+    return _finish(name, rng, t, t_us, sig, noise, False, kw.pop("params_kw", None), **kw), rng
 
 
 def config2(seed=3, n_coll=200, mean_mult=30.0, window_us=1000.0, **kw):
