@@ -107,3 +107,52 @@ def assert_contract(st, exact_count=False):
         assert st["tracks_oracle"] == st["tracks_cuda"], (st["tracks_oracle"], st["tracks_cuda"])
     assert st.get("par_max_rel", 0.0) <= REL_TOL, f"track parameters differ by {st['par_max_rel']:.3e} relative"
     assert st.get("cov_max_rel", 0.0) <= REL_TOL, f"covariance diagonals differ by {st['cov_max_rel']:.3e} relative"
+
+
+def restrict_to_sector(res, sector_row, n_rows, sector):
+    """View of a whole-event CUDA result restricted to one sector, re-indexed to the sector's own cluster
+    numbering (position in `sel`, which is ascending in original index, so every index tie-break is preserved).
+    Sectors are independent through the whole hot path (R2, R9-R22 are sector-local), so the oracle run on the
+    sector's clusters alone must reproduce this view.  Returns (sel, res_sector)."""
+    sel = np.nonzero(np.asarray(sector_row) // n_rows == sector)[0]
+    tk = np.nonzero(res["trk_sector"] == sector)[0]
+    new_of_old = np.full(res["trk_seed"].size, -1, np.int64)
+    new_of_old[tk] = np.arange(tk.size)
+    ct = res["cluster_track"][sel]
+    ct_new = np.where(ct >= 0, new_of_old[np.maximum(ct, 0)], -1)
+    assert np.all((ct < 0) | (ct_new >= 0)), "a cluster of this sector is owned by a track of another sector"
+    nh = res["trk_nhits"][tk]
+    first = np.concatenate([[0], np.cumsum(nh)[:-1]]).astype(np.int64) if tk.size else np.zeros(0, np.int64)
+    hits = np.concatenate([res["trk_hits"][res["trk_first_hit"][k]:res["trk_first_hit"][k] + res["trk_nhits"][k]]
+                           for k in tk]) if tk.size else np.zeros(0, np.int32)
+    pos = np.searchsorted(sel, hits)
+    assert np.array_equal(sel[np.minimum(pos, sel.size - 1)], hits), "a track holds a cluster of another sector"
+    out = dict(cluster_track=ct_new.astype(np.int32), trk_seed=np.searchsorted(sel, res["trk_seed"][tk]).astype(np.int32),
+               trk_sector=res["trk_sector"][tk], trk_nhits=nh, trk_first_hit=first, trk_hits=pos.astype(np.int32))
+    for k in ("par", "cov"):
+        out[k] = res[k][:, tk]
+    for k in ("xref", "zref", "chi2", "ndf"):
+        out[k] = res[k][tk]
+    return sel, out
+
+
+def check_output_invariants(res, sector_row, n_rows, min_hits):
+    """Properties of a valid output that hold at any size (used at the full bench size, where the oracle can only
+    be afforded on sampled sectors): exclusivity, list/flag consistency, one sector and strictly ascending rows per
+    track, >= min_hits, ndf = 2 nHits - 5, unique seeds (a seed may be owned by a longer rival, R20)."""
+    ct, hits, nh, first = res["cluster_track"], res["trk_hits"], res["trk_nhits"], res["trk_first_hit"]
+    K = res["trk_seed"].size
+    assert int(nh.sum()) == hits.size
+    assert np.array_equal(first, np.concatenate([[0], np.cumsum(nh)[:-1]])), "hit lists are not packed in track order"
+    assert np.all(nh >= min_hits)
+    owner = np.repeat(np.arange(K, dtype=np.int32), nh)
+    assert np.array_equal(ct[hits], owner), "cluster_track disagrees with the hit lists"
+    assert int(np.count_nonzero(ct >= 0)) == hits.size, "a cluster is flagged assigned but is in no hit list (or twice)"
+    sr = np.asarray(sector_row)[hits]
+    assert np.array_equal(sr // n_rows, np.repeat(res["trk_sector"], nh)), "a track mixes sectors"
+    inner = np.ones(hits.size, bool)
+    inner[first] = False
+    assert np.all(np.diff(sr % n_rows)[inner[1:]] > 0), "rows of a track are not strictly ascending"
+    assert np.unique(res["trk_seed"]).size == K
+    ok = res["ndf"] >= 0
+    assert np.array_equal(res["ndf"][ok], 2 * nh[ok] - 5)

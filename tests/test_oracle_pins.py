@@ -605,3 +605,22 @@ def test_config0_efficiency_and_purity(orc):
     findable = nclu >= 20
     assert np.all(found[findable] == 1)
     assert (o["cluster_track"] >= 0).mean() > 0.98
+
+
+def test_sector_independence_whole_event_vs_single_sector(orc):
+    """R2/R9-R22 are sector-local: the whole-event result restricted to one sector equals the oracle run on that
+    sector's clusters alone (same 36-sector geometry).  This is what lets tests/test_gpu_config4.py check the
+    1.4e8-cluster bench workload on sampled sectors; it also exercises parity.restrict_to_sector itself."""
+    import parity
+    ev = config1(n_tracks=1500)
+    nrows = int(ev.params.n_rows)
+    whole = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)
+    whole["trk_sector"] = ev.sector_row[whole["trk_seed"]] // nrows
+    parity.check_output_invariants(whole, ev.sector_row, nrows, int(ev.params.min_hits))
+    for sector in (4, 22):
+        sel, rs = parity.restrict_to_sector(whole, ev.sector_row, nrows, sector)
+        alone = orc.run(ev.params, ev.y[sel], ev.z[sel], ev.sector_row[sel], "f32", True)
+        st = parity.compare_tracks(alone, rs, sel.size)
+        assert st["tracks_oracle"] == st["tracks_cuda"] == st["tracks_same_hits"] > 10
+        assert st["assign_identical"] == sel.size
+        assert st["par_bit_identical"] and st["cov_bit_identical"]
