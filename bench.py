@@ -40,18 +40,23 @@ L2_BYTES = 126e6
 # rooflines").  unit: "cluster" = per input cluster, "bin" = per grid bin,
 # "step" = per follower row step (propagate + search + update), "hit" = per refitted hit.
 KERNEL_MODEL = {
-    # name: (bound, bytes per cluster, bytes per bin, flop per unit [for alu-bound], unit)
-    "k_bin_count": ("hbm", 12 + 8 + 8, 0, 0, "cluster"),       # y,z,sr in; key,rank out; count RMW (4+4)
-    "k_scan_*": ("hbm", 0, 8, 0, "bin"),                        # read + write per scanned element (int32)
-    "k_scatter": ("hbm", 12 + 8 + 4 + 16, 0, 0, "cluster"),     # y,z,sr,key,rank,bin_first in; 16 B record out
-    "k_canon": ("hbm", 0, 4, 0, "bin"),
-    "k_neighbours": ("hbm", 16 + 8, 0, 0, "cluster"),           # own record in, two links out (neighbours from L2)
-    "k_clean": ("hbm", 8 + 8, 0, 0, "cluster"),
-    "k_compact_starts": ("hbm", 4, 0, 0, "cluster"),
-    "k_follow": ("alu", 0, 0, 0, "step"),
-    "k_count_kept": ("hbm", 0, 0, 0, "cluster"),
-    "k_write_tracks": ("hbm", 8, 0, 0, "cluster"),
-    "k_fit": ("alu", 0, 0, 0, "hit"),
+    # name: (bound, {unit: algorithmic HBM bytes per unit}, unit the alu-bound kernels are counted in)
+    # units: cluster = input cluster, bin = grid bin, tracklet = followed start hit, claim = (tracklet,row) hit
+    # recorded by the follower, hit = hit of an accepted track
+    "k_bin_count": ("hbm", {"cluster": 12 + 8 + 8}, None),       # y,z,sr in; key,rank out; count RMW (4+4)
+    "k_scan_*": ("hbm", {"bin": 12, "cluster": 12, "tracklet": 24}, None),  # all scans of a step: 2 reads + 1 write per element
+    "k_scatter": ("hbm", {"cluster": 12 + 8 + 4 + 16}, None),     # y,z,sr,key,rank,bin_first in; 16 B record out
+    "k_canon": ("hbm", {"bin": 4}, None),
+    "k_neighbours": ("hbm", {"cluster": 16 + 8}, None),           # own record in, two links out (neighbours from L2)
+    "k_clean": ("hbm", {"cluster": 8 + 8}, None),
+    "k_compact_starts": ("hbm", {"cluster": 4, "tracklet": 32}, None),
+    "k_follow": ("alu", {}, "step"),
+    "k_push_keys": ("hbm", {"claim": 4 + 8 + 8, "tracklet": 12}, None),   # row_hit in, 8-byte atomicMax RMW
+    "k_mark": ("hbm", {"cluster": 8 + 16 + 4 + 4}, None),         # owner, record in; 4-byte atomicOr RMW
+    "k_count_kept": ("hbm", {"tracklet": 32 + 8}, None),
+    "k_assign": ("hbm", {"cluster": 16 + 8 + 4, "hit": 32 + 16 + 4 + 16}, None),  # + mask, scan in; trk_hits, hit_rec out
+    "k_track_info": ("hbm", {"tracklet": 16}, None),
+    "k_fit": ("alu", {}, "hit"),
 }
 
 
@@ -284,8 +289,14 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     top_ms = kern[top]["ms_per_step"] / max(kern[top]["launches_per_step"], 1)
     nb = binding.grid_bins(ev.params)
     work = binding.work_counts(res["counters"])
-    roofline = kernel_roofline(top, top_ms, n, nb, work, n_hits, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz,
-                               peak_src)
+    units = {"cluster": n, "bin": nb, "tracklet": int(res["counters"][binding.CNT_TRACKLETS]), "claim": work["updates"],
+             "hit": n_hits}
+    roofline = kernel_roofline(top, top_ms, units, work, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
+    for k in kern:       # every kernel's own fraction of its roof, so that the table can be read without DESIGN.md
+        r = kernel_roofline(k, kern[k]["ms_per_step"] / max(kern[k]["launches_per_step"], 1) *
+                            (kern[k]["launches_per_step"] if k == "k_scan_*" else 1), units, work,
+                            int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
+        kern[k]["bound"], kern[k]["frac"] = r["bound"], round(r["frac"], 4)
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic",
@@ -308,23 +319,24 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     print(json.dumps(out), flush=True)
 
 
-def kernel_roofline(name, ms, n, nb, work, n_hits, n_passes, hbm_peak, sm_max_mhz, peak_src):
-    bound, b_cl, b_bin, _, unit = KERNEL_MODEL.get(name, ("hbm", 0, 0, 0, "cluster"))
+def kernel_roofline(name, ms, units, work, n_passes, hbm_peak, sm_max_mhz, peak_src):
+    """units: {"cluster": N, "bin": B, "tracklet": S, "claim": follower updates, "hit": hits of accepted tracks}."""
+    bound, per_unit, unit = KERNEL_MODEL.get(name, ("hbm", {}, None))
     if bound == "hbm":
-        by = b_cl * n + b_bin * nb
+        by = sum(b * units[u] for u, b in per_unit.items())
         ach = by / (ms * 1e-3) / 1e9
         return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                 "traffic": None, "algorithmic_bytes_per_launch": by, "ms_per_launch": ms, "peak_source": peak_src}
     # alu-bound kernels: fp32 operations actually required per unit (DESIGN.md "Kernels / follower")
     from paper_2106_03636_b200 import flops
     if name == "k_follow":
-        units, fl = work["propagations"], flops.follow_flop(work)
+        n_units, fl = work["propagations"], flops.follow_flop(work)
     else:
-        units, fl = n_hits * n_passes, flops.fit_flop(n_hits, n_passes)
+        n_units, fl = units["hit"] * n_passes, flops.fit_flop(units["hit"], n_passes)
     peak = 148 * 128 * sm_max_mhz * 1e6 / 1e12      # fp32 lanes x clock, non-FMA (one op per lane per cycle), TFLOP/s
     ach = fl / (ms * 1e-3) / 1e12
     return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-            "traffic": None, "algorithmic_flop_per_launch": fl, "units": units, "unit_kind": unit, "ms_per_launch": ms,
+            "traffic": None, "algorithmic_flop_per_launch": fl, "units": n_units, "unit_kind": unit, "ms_per_launch": ms,
             "peak_source": f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz, 1 op/lane/cycle (no FMA contraction by contract)"}
 
 

@@ -46,6 +46,7 @@ extern "C" {
 #endif
 
 #define TPC_MAX_ROWS 152
+#define TPC_MAX_TRACKLETS 33554432 /* 2^25 */
 
 typedef enum {
   TPC_OK = 0,
@@ -106,7 +107,9 @@ const char* tpc_version(void);
  * Returns TPC_EINVAL if params are inconsistent or the count does not fit in int32. */
 int tpc_grid_bins(const tpc_params_t* params_host, int64_t* n_bins_host);
 
-/* Bytes of workspace needed for n_clusters clusters and at most max_tracklets start hits. */
+/* Bytes of workspace needed for n_clusters clusters and at most max_tracklets start hits.
+ * max_tracklets <= TPC_MAX_TRACKLETS (the tracklet number shares the 64-bit R20 selection key
+ * with nHits and the start index); larger values are TPC_EINVAL in every workspace-taking call. */
 int tpc_workspace_bytes(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
                         size_t* bytes_host);
 
@@ -147,7 +150,7 @@ int tpc_find_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t
  * all in ORIGINAL cluster indices (-1 = none).  Any output pointer may be NULL.
  *   link_up, link_dn [n]  : R9 raw links;  up_c, dn_c [n] : R10 cleaned links
  *   starts [max_tracklets]: start hit of tracklet t;  tl_nhits [max_tracklets]: hits recorded
- *   row_hit [max_tracklets * n_rows] : row_hit[t*n_rows + r] (R18), row-major per tracklet
+ *   row_hit [TPC_CNT_TRACKLETS * n_rows] : row_hit[t*n_rows + r] (R18), row-major per tracklet
  * Entries for t >= counters[TPC_CNT_TRACKLETS] are left untouched. */
 int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
                     const void* workspace, size_t ws_bytes, int32_t* link_up, int32_t* link_dn,
@@ -155,17 +158,26 @@ int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t
                     int32_t* row_hit, void* stream);
 
 /* Step 3b (R21-R22).  Refit of K = counters[TPC_CNT_TRACKS] hit lists (read on the device; the
- * call never synchronises).  Self-contained: reads cluster coordinates through y, z, sector_row
- * (the caller's arrays, original order) so it can be fed any hit lists, e.g. truth hits.
+ * call never synchronises).
+ *   workspace != NULL : must be the workspace on which tpc_find_tracks produced exactly these
+ *                       trk_nhits / trk_first_hit / trk_hits (same n_clusters, max_tracklets).
+ *                       tpc_find_tracks stored the (y, z, row) of every hit in hit-list order
+ *                       there; the fit streams those records instead of gathering, and y, z,
+ *                       sector_row, trk_hits are not read (may be NULL).
+ *   workspace == NULL : self-contained gather through y, z, sector_row (the caller's arrays,
+ *                       original order) and trk_hits, so any hit lists can be refitted, e.g.
+ *                       truth hits; max_tracklets and ws_bytes are ignored.
+ * Both paths run the same arithmetic and give bit-identical results.
  *   par [5][max_tracks]  : y, dz = z - zref, sinphi, tanlambda, q/pT at x = xref   (SoA)
  *   cov [15][max_tracks] : lower triangle, row-major (00,10,11,20,21,22,...)       (SoA)
  *   xref, zref, chi2 [max_tracks], ndf [max_tracks] (= 2*nhits-5; chi2 = -1, ndf = -1 if the
  *   propagation left |sinphi| <= max_sinphi). */
-int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, const float* y,
-                   const float* z, const int32_t* sector_row, const int32_t* counters,
-                   int64_t max_tracks, const int32_t* trk_nhits, const int64_t* trk_first_hit,
-                   const int32_t* trk_hits, float* par, float* cov, float* xref, float* zref,
-                   float* chi2, int32_t* ndf, void* stream);
+int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                   void* workspace, size_t ws_bytes, const float* y, const float* z,
+                   const int32_t* sector_row, const int32_t* counters, int64_t max_tracks,
+                   const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
+                   float* par, float* cov, float* xref, float* zref, float* chi2, int32_t* ndf,
+                   void* stream);
 
 /* Host-buffer convenience for end-to-end measurement (bench.py `e2e`): copies the five input
  * arrays host->device into caller-provided device staging buffers, runs the three steps, and

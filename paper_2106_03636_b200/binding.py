@@ -19,6 +19,7 @@ from . import build as _build
 
 TPC_MAX_ROWS = 152
 TPC_N_COUNTERS = 16
+TPC_MAX_TRACKLETS = 1 << 25
 CNT_TRACKS, CNT_TRACKLETS, CNT_HITS, CNT_STATUS, CNT_STARTS_FOUND, CNT_TRACKS_FOUND = 0, 1, 2, 3, 4, 5
 CNT_PROP_LO, CNT_UPD_LO, CNT_CAND_LO = 8, 10, 12
 ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
@@ -154,7 +155,7 @@ def workspace_bytes(params, n_clusters: int, max_tracklets: int) -> int:
 
 def default_max_tracklets(n_clusters: int) -> int:
     """Start hits are ~4-7 % of the clusters on the BASELINE.json configs; n/8 + 1024 leaves headroom."""
-    return int(n_clusters) // 8 + 1024
+    return min(int(n_clusters) // 8 + 1024, TPC_MAX_TRACKLETS)
 
 
 def default_max_tracks(n_clusters: int) -> int:
@@ -213,9 +214,12 @@ class Tracker:
                                         _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits),
                                         _dp(self.counters), _stream()), "tpc_find_tracks")
 
-    def fit_tracks(self):
+    def fit_tracks(self, gather: bool = False):
+        """tpc_fit_tracks; gather=True passes workspace = NULL (self-contained gather through y/z/sector_row)."""
         y, z, sr = self._inputs
-        _check(self.lib.tpc_fit_tracks(C.byref(self.P), C.c_int64(self.n), _dp(y), _dp(z), _dp(sr), _dp(self.counters),
+        ws = C.c_void_p(0) if gather else _dp(self.workspace)
+        _check(self.lib.tpc_fit_tracks(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), ws,
+                                       C.c_size_t(self.ws_bytes), _dp(y), _dp(z), _dp(sr), _dp(self.counters),
                                        C.c_int64(self.max_tracks), _dp(self.trk_nhits), _dp(self.trk_first_hit),
                                        _dp(self.trk_hits), _dp(self.par), _dp(self.cov), _dp(self.xref), _dp(self.zref),
                                        _dp(self.chi2), _dp(self.ndf), _stream()), "tpc_fit_tracks")

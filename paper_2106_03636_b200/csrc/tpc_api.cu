@@ -24,8 +24,8 @@ struct Rec2 {
 Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bin_count", "k_scan_*", "k_scatter", "k_canon", "k_neighbours", "k_clean",
-                                         "k_compact_starts", "k_follow", "k_count_kept", "k_write_tracks", "k_fit",
-                                         "k_export_*"};
+                                         "k_compact_starts", "k_follow", "k_push_keys", "k_mark", "k_count_kept",
+                                         "k_assign", "k_track_info", "k_fit", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -137,7 +137,7 @@ struct Prep {
 int prepare(const tpc_params_t* P, int64_t n, int64_t max_tracklets, const void* ws, size_t ws_bytes, Prep* out) {
   int64_t nb = 0;
   if (!make_geo(P, &out->G, &nb)) return TPC_EINVAL;
-  if (n < 0 || n > 2147483000ll || max_tracklets < 1 || max_tracklets > 2147483000ll || !ws) return TPC_EINVAL;
+  if (n < 0 || n > 2147483000ll || max_tracklets < 1 || max_tracklets > tpc::kMaxTracklets || !ws) return TPC_EINVAL;
   out->L = tpc::make_layout(n, max_tracklets, nb, P->n_rows);
   if (ws_bytes < out->L.total) return TPC_ENOMEM_WS;
   if (((uintptr_t)ws & 255) != 0) return TPC_EINVAL;
@@ -208,7 +208,7 @@ int tpc_workspace_bytes(const tpc_params_t* params_host, int64_t n_clusters, int
   tpc::Geo G;
   int64_t nb = 0;
   if (!bytes_host || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
-  if (n_clusters < 0 || n_clusters > 2147483000ll || max_tracklets < 1 || max_tracklets > 2147483000ll) return TPC_EINVAL;
+  if (n_clusters < 0 || n_clusters > 2147483000ll || max_tracklets < 1 || max_tracklets > tpc::kMaxTracklets) return TPC_EINVAL;
   *bytes_host = tpc::make_layout(n_clusters, max_tracklets, nb, params_host->n_rows).total;
   return TPC_OK;
 }
@@ -259,19 +259,25 @@ int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
-int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
-                   const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
-                   const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
-                   float* zref, float* chi2, int32_t* ndf, void* stream) {
-  tpc::Geo G;
-  int64_t nb = 0;
-  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, void* workspace,
+                   size_t ws_bytes, const float* y, const float* z, const int32_t* sector_row, const int32_t* counters,
+                   int64_t max_tracks, const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
+                   float* par, float* cov, float* xref, float* zref, float* chi2, int32_t* ndf, void* stream) {
+  Prep pr;
+  if (workspace) {
+    const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+    if (rc != TPC_OK) return rc;
+  } else {
+    int64_t nb = 0;
+    if (!make_geo(params_host, &pr.G, &nb)) return TPC_EINVAL;
+  }
   if (n_clusters < 0 || max_tracks < 1 || !counters || !trk_nhits || !trk_first_hit || !par || !cov || !xref || !zref ||
       !chi2 || !ndf)
     return TPC_EINVAL;
-  if (n_clusters > 0 && (!y || !z || !sector_row || !trk_hits)) return TPC_EINVAL;
-  const cudaError_t e = tpc::launch_fit(G, n_clusters, y, z, sector_row, counters, max_tracks, trk_nhits, trk_first_hit,
-                                        trk_hits, par, cov, xref, zref, chi2, ndf, (cudaStream_t)stream);
+  if (!workspace && n_clusters > 0 && (!y || !z || !sector_row || !trk_hits)) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_fit(pr.G, workspace ? &pr.W : nullptr, n_clusters, y, z, sector_row, counters, max_tracks,
+                                        trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf,
+                                        (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
@@ -299,8 +305,9 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
   rc = tpc_find_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, cluster_track_dev, max_tracks,
                        trk_seed_dev, trk_sector_dev, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, counters_dev, stream);
   if (rc != TPC_OK) return rc;
-  rc = tpc_fit_tracks(params_host, n_clusters, y_dev, z_dev, sector_row_dev, counters_dev, max_tracks, trk_nhits_dev,
-                      trk_first_hit_dev, trk_hits_dev, par_dev, cov_dev, xref_dev, zref_dev, chi2_dev, ndf_dev, stream);
+  rc = tpc_fit_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, y_dev, z_dev, sector_row_dev, counters_dev,
+                      max_tracks, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, par_dev, cov_dev, xref_dev, zref_dev, chi2_dev,
+                      ndf_dev, stream);
   if (rc != TPC_OK) return rc;
   if ((e = cudaMemcpyAsync(counters_host, counters_dev, sizeof(int32_t) * TPC_N_COUNTERS, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
     return cuda_fail(e);

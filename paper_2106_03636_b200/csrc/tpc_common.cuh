@@ -58,7 +58,7 @@ enum {
   WC_QUEUE = 1,        // work-queue head of the follower
   WC_STATUS = 2,       // TPC_ST_* bits
   WC_STARTS_FOUND = 3, // before clamping
-  WC_QUEUE2 = 4,
+  WC_FIT_QUEUE = 4,    // work-queue head of the cached refit
   WC_PROP64 = 8,       // unsigned long long at [8,9]: follower transports
   WC_UPD64 = 10,       // unsigned long long at [10,11]: follower updates
   WC_CAND64 = 12,      // unsigned long long at [12,13]: candidates tested
@@ -74,7 +74,22 @@ struct Layout {
   int64_t n, scap, scap_pad, nb;
   int64_t scan_tiles;  // capacity (elements) of the scan scratch
   size_t off_counters, off_rec, off_key, off_rank, off_bin_first, off_link_up, off_link_dn, off_up_c,
-      off_owner, off_starts, off_tl_info, off_tl_scan, off_row_hit, off_scan_tmp, total;
+      off_owner, off_hit_rec, off_tl_init, off_tl_info, off_tl_key, off_tl_mask, off_tl_scan, off_row_hit,
+      off_scan_tmp, total;
+};
+
+// R20 selection key, 64 bits: [63:56] nHits | [55:25] 0x7FFFFFFF - original index of the start hit |
+// [24:0] tracklet number t.  (nHits, start index) is unique per tracklet, so the low field never
+// decides a comparison: max(key) = most hits, ties to the lowest original start index, as R20 asks;
+// carrying t lets the per-cluster passes find the owning tracklet without a search.
+constexpr int kKeyTBits = 25;
+constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
+constexpr int kMaskWords = 8;  // 32-byte row mask per tracklet (rows 0..159 in words 0..4)
+
+// Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.
+struct TlInit {
+  float y0, z0, y1, z1;       // start hit and its cleaned up-neighbour
+  int32_t p0, p1, sr0, orig0; // grid positions, sector_row and original index of the start hit
 };
 
 constexpr int kScanTile = 4096;  // elements per scan tile (256 threads x 16)
@@ -106,10 +121,13 @@ inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows) {
   L.off_link_dn = take(sizeof(int32_t) * (size_t)(n + 1));
   L.off_up_c = take(sizeof(int32_t) * (size_t)(n + 1));
   L.off_owner = take(sizeof(uint64_t) * (size_t)(n + 1));
-  L.off_starts = take(sizeof(int32_t) * (size_t)(L.scap_pad + 1));
+  L.off_hit_rec = take(sizeof(float4) * (size_t)(n + 1));   // (y, z, row, orig) in hit-list order for the refit
+  L.off_tl_init = take(sizeof(TlInit) * (size_t)(L.scap_pad + 1));
   L.off_tl_info = take(sizeof(int32_t) * (size_t)(L.scap_pad + 1));
+  L.off_tl_key = take(sizeof(uint64_t) * (size_t)(L.scap_pad + 1));
+  L.off_tl_mask = take(sizeof(uint32_t) * kMaskWords * (size_t)(L.scap_pad + 1));
   L.off_tl_scan = take(sizeof(int64_t) * (size_t)(L.scap_pad + 2));
-  L.off_row_hit = take(sizeof(int32_t) * (size_t)L.scap_pad * (size_t)nrows);
+  L.off_row_hit = take(sizeof(int32_t) * (size_t)L.scap_pad * (size_t)nrows);  // [t][row], tracklet-major
   L.off_scan_tmp = take(sizeof(int64_t) * (size_t)L.scan_tiles);
   L.total = o;
   return L;
@@ -123,7 +141,11 @@ struct Ws {
   Rec* rec;
   int32_t *key, *rank, *bin_first, *link_up, *link_dn, *up_c;
   unsigned long long* owner;
-  int32_t *starts, *tl_info;
+  float4* hit_rec;
+  TlInit* tl_init;
+  int32_t* tl_info;
+  unsigned long long* tl_key;
+  uint32_t* tl_mask;
   long long* tl_scan;
   int32_t* row_hit;
   long long* scan_tmp;
@@ -142,8 +164,11 @@ inline Ws bind_ws(const Layout& L, void* workspace) {
   w.link_dn = (int32_t*)(b + L.off_link_dn);
   w.up_c = (int32_t*)(b + L.off_up_c);
   w.owner = (unsigned long long*)(b + L.off_owner);
-  w.starts = (int32_t*)(b + L.off_starts);
+  w.hit_rec = (float4*)(b + L.off_hit_rec);
+  w.tl_init = (TlInit*)(b + L.off_tl_init);
   w.tl_info = (int32_t*)(b + L.off_tl_info);
+  w.tl_key = (unsigned long long*)(b + L.off_tl_key);
+  w.tl_mask = (uint32_t*)(b + L.off_tl_mask);
   w.tl_scan = (long long*)(b + L.off_tl_scan);
   w.row_hit = (int32_t*)(b + L.off_row_hit);
   w.scan_tmp = (long long*)(b + L.off_scan_tmp);
@@ -159,7 +184,13 @@ cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64
                         int32_t* counters, cudaStream_t st);
 cudaError_t launch_find_export(const Geo& g, const Ws& w, int32_t* link_up, int32_t* link_dn, int32_t* up_c,
                                int32_t* dn_c, int32_t* starts, int32_t* tl_nhits, int32_t* row_hit, cudaStream_t st);
-cudaError_t launch_fit(const Geo& g, int64_t n, const float* y, const float* z, const int32_t* sector_row,
+// follower (tpc_follow.cu) and selection (tpc_select.cu) stages of launch_find
+cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st);
+cudaError_t launch_select(const Geo& g, const Ws& w, int32_t* cluster_track, int64_t max_tracks, int32_t* trk_seed,
+                          int32_t* trk_sector, int32_t* trk_nhits, int64_t* trk_first_hit, int32_t* trk_hits,
+                          int32_t* counters, cudaStream_t st);
+// w == nullptr: gather the hits through y / z / sector_row; else read the records tpc_find_tracks cached in w
+cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, const float* z, const int32_t* sector_row,
                        const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
                        const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
                        float* zref, float* chi2, int32_t* ndf, cudaStream_t st);
@@ -175,5 +206,19 @@ __device__ __forceinline__ int clampbin(float v, int n) {
 __device__ __forceinline__ Rec ld_rec(const Rec* __restrict__ recs, int k) { return __ldg(recs + k); }
 __device__ __forceinline__ int rec_idx(const Rec& r) { return __float_as_int(r.z); }
 __device__ __forceinline__ int rec_sr(const Rec& r) { return __float_as_int(r.w); }
+
+// R20 selection key (layout above)
+__device__ __forceinline__ unsigned long long sel_key(int nh, int start_orig, int t) {
+  return ((unsigned long long)(unsigned)nh << 56) | ((unsigned long long)(0x7FFFFFFFu - (unsigned)start_orig) << kKeyTBits) |
+         (unsigned long long)(unsigned)t;
+}
+__device__ __forceinline__ int key_tracklet(unsigned long long key) { return (int)(key & (unsigned long long)(kMaxTracklets - 1)); }
+
+inline unsigned blocks_for(int64_t n, int threads, int64_t cap = 148 * 64) {
+  int64_t b = (n + threads - 1) / threads;
+  if (b > cap) b = cap;
+  if (b < 1) b = 1;
+  return (unsigned)b;
+}
 
 }  // namespace tpc

@@ -3,9 +3,13 @@
 // the time offset left free"): per accepted track, a 3-point circle seed
 // followed by an outward and an inward fp32 Kalman pass over its hit list.
 //
-//   k_fit   one thread per track; 5-parameter state + 15 covariance elements in registers;
-//           hits are gathered through the caller's y / z / sector_row arrays (original indices),
-//           so the kernel is self-contained and can refit any hit lists (e.g. truth hits).
+//   k_fit         one LANE per track, 5-parameter state + 15 covariance elements in registers.  Reads
+//                 the (y, z, row) records that tpc_find_tracks stored in hit-list order (one
+//                 sequential 16-byte stream per track).  Like the follower it is one loop with a
+//                 single copy of transport + update; a lane that finishes its track pulls the next
+//                 one from a queue, so the lanes of a warp stay busy whatever the track lengths.
+//   k_fit_gather  same arithmetic, hits gathered through the caller's y / z / sector_row arrays
+//                 (original indices): self-contained, refits any hit lists (e.g. truth hits).
 // The track count K is read from counters[TPC_CNT_TRACKS] on the device (no host sync).
 // =============================================================================================
 #include "tpc_common.cuh"
@@ -19,7 +23,7 @@ namespace {
 constexpr int kFitThreads = 128;
 
 __global__ void __launch_bounds__(kFitThreads)
-k_fit(const __grid_constant__ Geo g, const float* __restrict__ y, const float* __restrict__ z,
+k_fit_gather(const __grid_constant__ Geo g, const float* __restrict__ y, const float* __restrict__ z,
       const int32_t* __restrict__ sector_row, const int32_t* __restrict__ counters, int64_t max_tracks,
       const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
       const int32_t* __restrict__ trk_hits, float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref,
@@ -90,19 +94,163 @@ k_fit(const __grid_constant__ Geo g, const float* __restrict__ y, const float* _
   }
 }
 
+constexpr unsigned kFull = 0xffffffffu;
+enum FitPhase { F_FETCH = 0, F_RUN, F_DONE };
+
+__global__ void __launch_bounds__(kFitThreads)
+k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const int32_t* __restrict__ counters,
+      int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+      float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref, float* __restrict__ zref_out,
+      float* __restrict__ chi2_out, int32_t* __restrict__ ndf, int32_t* __restrict__ ws_counters) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t K64 = counters[TPC_CNT_TRACKS];
+  if (K64 > max_tracks) K64 = max_tracks;
+  const int K = (int)K64;
+  const int lane = threadIdx.x & 31;
+  const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
+  const int npass = sc.n_fit_passes;
+
+  int phase = F_FETCH;
+  KState st;
+#pragma unroll
+  for (int k = 0; k < 5; k++) st.p[k] = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 15; k++) st.C[k] = 0.0f;
+  const float4* hits = hit_rec;
+  float4 pre = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  int k = 0, n = 0, i = 0, cnt = 0, pass = 0, dir = 1;
+  float x_at = 0.0f, chi2 = 0.0f, zref = 0.0f;
+
+  for (;;) {
+    const unsigned need = __ballot_sync(kFull, phase == F_FETCH);
+    if (need) {
+      const int leader = __ffs(need) - 1;
+      int base = 0;
+      if (lane == leader) base = atomicAdd(ws_counters + WC_FIT_QUEUE, __popc(need));
+      base = __shfl_sync(kFull, base, leader);
+      if (phase == F_FETCH) {
+        k = base + __popc(need & ((1u << lane) - 1u));
+        if (k >= K) {
+          phase = F_DONE;
+        } else {
+          n = trk_nhits[k];
+          hits = hit_rec + trk_first_hit[k];
+          // R21: seed from the first, middle and last hit
+          const float4 a = __ldg(hits), b = __ldg(hits + n / 2), c = __ldg(hits + (n - 1)), h1 = __ldg(hits + (n > 1 ? 1 : 0));
+          const float x1 = sX[__float_as_int(a.z)], y1 = a.x, x2 = sX[__float_as_int(b.z)], y2 = b.x,
+                      x3 = sX[__float_as_int(c.z)], y3 = c.x;
+          const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+          const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+          const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+          const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+          const float kappa = (2.0f * cross) / ((d12 * d23) * d13);  // signed curvature of the circumcircle
+          const float dx = sX[__float_as_int(h1.z)] - x1, dy = h1.x - y1;
+          const float ch = sqrtf(dx * dx + dy * dy);
+          float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);  // chord direction rotated back by half the turn
+          if (sphi > ms) sphi = ms;
+          if (sphi < -ms) sphi = -ms;
+          zref = a.y;
+          st.p[0] = y1;
+          st.p[1] = 0.0f;
+          st.p[2] = sphi;
+          st.p[3] = (h1.y - zref) / ch;
+          st.p[4] = -(kappa / kB);
+          reset_cov(st, sc.cov0);  // R22: covariance reset at the start of every pass
+          x_at = x1;
+          chi2 = 0.0f;
+          pass = 0;
+          dir = 1;
+          i = 0;
+          cnt = 0;
+          pre = a;
+          phase = F_RUN;
+        }
+      }
+    }
+    if (__all_sync(kFull, phase == F_DONE)) break;
+    const bool run = phase == F_RUN;
+    // this step's hit was loaded one step ahead; issue the next one now
+    const float4 h = pre;
+    int i_next = i + dir;
+    if (cnt + 1 >= n) i_next = ((pass + 1) & 1) ? n - 1 : 0;  // first hit of the next pass
+    if (run) pre = __ldg(hits + i_next);
+    const float xh = sX[__float_as_int(h.z)];
+    bool ok = true;
+    if (run && cnt > 0) {  // the first hit of a pass is the one the state already sits at (no transport)
+      ok = propagate(st, xh - x_at, kB, ms);
+      if (ok) x_at = xh;
+    }
+    if (run && ok) {
+      const Innov I = innovation(st, sy2, sz2);
+      chi2 = chi2 + update(st, I, h.x, h.y - zref);
+    }
+    if (run) {
+      bool finish = !ok;
+      if (ok) {
+        cnt++;
+        i = i_next;
+        if (cnt >= n) {  // end of a pass: R22 pass 1 inner -> outer, pass 2 outer -> inner, ...
+          pass++;
+          if (pass >= npass) {
+            finish = true;
+          } else {
+            reset_cov(st, sc.cov0);
+            chi2 = 0.0f;
+            dir = (pass & 1) ? -1 : 1;
+            cnt = 0;
+          }
+        }
+      }
+      if (finish) {
+#pragma unroll
+        for (int q = 0; q < 5; q++) par[(int64_t)q * max_tracks + k] = st.p[q];
+#pragma unroll
+        for (int q = 0; q < 15; q++) cov[(int64_t)q * max_tracks + k] = st.C[q];
+        xref[k] = x_at;
+        zref_out[k] = zref;
+        chi2_out[k] = ok ? chi2 : -1.0f;
+        ndf[k] = ok ? 2 * n - 5 : -1;
+        phase = F_FETCH;
+      }
+    }
+  }
+}
+
+int g_fit_blocks = 0;
+
 }  // namespace
 
-cudaError_t launch_fit(const Geo& g, int64_t n, const float* y, const float* z, const int32_t* sector_row,
+cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, const float* z, const int32_t* sector_row,
                        const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
                        const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
                        float* zref, float* chi2, int32_t* ndf, cudaStream_t st) {
   (void)n;
   if (max_tracks <= 0) return cudaSuccess;
+  cudaError_t e;
+  if (w) {
+    if (g_fit_blocks == 0) {
+      int dev = 0, sms = 0, per_sm = 0;
+      if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+      if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+      if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit, kFitThreads, 0)) != cudaSuccess) return e;
+      g_fit_blocks = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
+    if (blocks > g_fit_blocks) blocks = g_fit_blocks;
+    if ((e = cudaMemsetAsync(w->counters + WC_FIT_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
+    TPC_LAUNCH(KID_FIT, st,
+               (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, w->hit_rec, counters, max_tracks, trk_nhits, trk_first_hit,
+                                                               par, cov, xref, zref, chi2, ndf, w->counters)));
+    return cudaGetLastError();
+  }
   int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
   if (blocks > 148 * 16) blocks = 148 * 16;
   TPC_LAUNCH(KID_FIT, st,
-             (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits,
-                                                             trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf)));
+             (k_fit_gather<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits,
+                                                                    trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf)));
   return cudaGetLastError();
 }
 

@@ -94,13 +94,6 @@ k_export_sorted(int64_t n, const Rec* __restrict__ rec, int32_t* __restrict__ so
     sorted_idx[i] = rec_idx(rec[i]);
 }
 
-inline unsigned blocks_for(int64_t n, int threads, int64_t cap = 148 * 64) {
-  int64_t b = (n + threads - 1) / threads;
-  if (b > cap) b = cap;
-  if (b < 1) b = 1;
-  return (unsigned)b;
-}
-
 }  // namespace
 
 cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const float* z, const int32_t* sector_row,

@@ -56,6 +56,23 @@ def test_config_matches_oracle(torch_cuda, orc, cfg):
     assert st["par_bit_identical"] and st["cov_bit_identical"]
 
 
+def test_fit_gather_path_is_bit_identical(torch_cuda):
+    """tpc_fit_tracks with workspace = NULL (self-contained gather through y/z/sector_row, any hit lists) runs the
+    same arithmetic as the cached-record path tpc_find_tracks feeds: every output bit-identical."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(3, n_coll=2, n_tracks=1000)
+    trk = binding.Tracker(ev.params, ev.n)
+    a = trk.run(*_dev(torch_cuda, ev))
+    for t in (trk.par, trk.cov, trk.xref, trk.zref, trk.chi2):
+        t.fill_(float("nan"))
+    trk.ndf.fill_(-7)
+    trk.fit_tracks(gather=True)
+    b = trk.results()
+    assert a["trk_seed"].size > 100
+    for k in ("par", "cov", "xref", "zref", "chi2", "ndf"):
+        assert np.array_equal(a[k], b[k]), k
+
+
 def test_config0_golden_counts(torch_cuda, orc):
     """tests/golden/config0_oracle_summary.txt (written from the oracle alone) against the CUDA path."""
     import os
