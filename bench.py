@@ -52,10 +52,8 @@ KERNEL_MODEL = {
     "k_compact_starts": ("hbm", {"cluster": 4, "tracklet": 32}, None),
     "k_follow": ("alu", {}, "step"),
     "k_push_keys": ("hbm", {"claim": 4 + 8 + 8, "tracklet": 12}, None),   # row_hit in, 8-byte atomicMax RMW
-    "k_mark": ("hbm", {"cluster": 8 + 16 + 4 + 4}, None),         # owner, record in; 4-byte atomicOr RMW
-    "k_count_kept": ("hbm", {"tracklet": 32 + 8}, None),
-    "k_assign": ("hbm", {"cluster": 16 + 8 + 4, "hit": 32 + 16 + 4 + 16}, None),  # + mask, scan in; trk_hits, hit_rec out
-    "k_track_info": ("hbm", {"tracklet": 16}, None),
+    "k_count_kept": ("hbm", {"claim": 4 + 8, "tracklet": 12 + 20 + 8}, None),   # row_hit, owner in; mask, value out
+    "k_write_tracks": ("hbm", {"hit": 4 + 16 + 4 + 16 + 8, "tracklet": 16 + 20}, None),  # rec in; trk_hits, hit_rec, cluster_track out
     "k_fit": ("alu", {}, "hit"),
 }
 

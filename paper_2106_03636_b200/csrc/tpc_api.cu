@@ -24,8 +24,8 @@ struct Rec2 {
 Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bin_count", "k_scan_*", "k_scatter", "k_canon", "k_neighbours", "k_clean",
-                                         "k_compact_starts", "k_follow", "k_push_keys", "k_mark", "k_count_kept",
-                                         "k_assign", "k_track_info", "k_fit", "k_export_*"};
+                                         "k_compact_starts", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
+                                         "k_fit", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -110,6 +110,15 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
   }
   G->row.rowbase[s.nrows] = (int32_t)base;
   s.bins_per_sector = (int32_t)base;
+  // tracklet ordering (tpc_find.cu): z slabs of about one drift length, at most 1024 of them
+  {
+    int w = (int)ceilf(256.0f / P->cell_z);
+    if (w < 1) w = 1;
+    const int wmin = (s.nz + 1023) / 1024;
+    if (w < wmin) w = wmin;
+    s.slab_w = w;
+    s.nslab = (s.nz + w - 1) / w;
+  }
   *n_bins = base * s.nsec;
   // R9 per-row constants of the neighbour finder (rows 1..n_rows-2)
   for (int r = 1; r + 1 < s.nrows; r++) {
@@ -138,7 +147,7 @@ int prepare(const tpc_params_t* P, int64_t n, int64_t max_tracklets, const void*
   int64_t nb = 0;
   if (!make_geo(P, &out->G, &nb)) return TPC_EINVAL;
   if (n < 0 || n > 2147483000ll || max_tracklets < 1 || max_tracklets > tpc::kMaxTracklets || !ws) return TPC_EINVAL;
-  out->L = tpc::make_layout(n, max_tracklets, nb, P->n_rows);
+  out->L = tpc::make_layout(n, max_tracklets, nb, P->n_rows, (int64_t)out->G.s.nsec * out->G.s.nslab * out->G.s.nrows);
   if (ws_bytes < out->L.total) return TPC_ENOMEM_WS;
   if (((uintptr_t)ws & 255) != 0) return TPC_EINVAL;
   out->W = tpc::bind_ws(out->L, const_cast<void*>(ws));
@@ -209,7 +218,7 @@ int tpc_workspace_bytes(const tpc_params_t* params_host, int64_t n_clusters, int
   int64_t nb = 0;
   if (!bytes_host || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
   if (n_clusters < 0 || n_clusters > 2147483000ll || max_tracklets < 1 || max_tracklets > tpc::kMaxTracklets) return TPC_EINVAL;
-  *bytes_host = tpc::make_layout(n_clusters, max_tracklets, nb, params_host->n_rows).total;
+  *bytes_host = tpc::make_layout(n_clusters, max_tracklets, nb, params_host->n_rows, (int64_t)G.s.nsec * G.s.nslab * G.s.nrows).total;
   return TPC_OK;
 }
 

@@ -39,6 +39,7 @@ struct CaGeo {
 // Scalars (R4, R6, R7, R9-R22).
 struct Scalars {
   int32_t nsec, nrows, nz, bins_per_sector;
+  int32_t slab_w, nslab;  // tracklet ordering: z slabs of slab_w bins, nslab = ceil(nz / slab_w)
   float inv_cy, inv_cz, z_lo, z_hi;
   float kB, sy2, sz2;
   float ca_cut, chi2_cut, chi2_chain_cut, win_max, max_sinphi, edge_margin;
@@ -71,11 +72,11 @@ using Rec = float4;
 
 // Workspace layout: a pure function of (n, max_tracklets, n_bins).  All offsets 256-byte aligned.
 struct Layout {
-  int64_t n, scap, scap_pad, nb;
+  int64_t n, scap, scap_pad, nb, nchunks;
   int64_t scan_tiles;  // capacity (elements) of the scan scratch
   size_t off_counters, off_rec, off_key, off_rank, off_bin_first, off_link_up, off_link_dn, off_up_c,
       off_owner, off_hit_rec, off_tl_init, off_tl_info, off_tl_key, off_tl_mask, off_tl_scan, off_row_hit,
-      off_scan_tmp, total;
+      off_chunk_base, off_chunk_scan0, off_scan_tmp, total;
 };
 
 // R20 selection key, 64 bits: [63:56] nHits | [55:25] 0x7FFFFFFF - original index of the start hit |
@@ -84,7 +85,7 @@ struct Layout {
 // carrying t lets the per-cluster passes find the owning tracklet without a search.
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
-constexpr int kMaskWords = 8;  // 32-byte row mask per tracklet (rows 0..159 in words 0..4)
+constexpr int kMaskWords = 5;  // kept-row mask per tracklet (rows 0..159)
 
 // Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.
 struct TlInit {
@@ -96,13 +97,15 @@ constexpr int kScanTile = 4096;  // elements per scan tile (256 threads x 16)
 
 inline size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows) {
+inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows, int64_t nchunks) {
   Layout L{};
   L.n = n;
   L.scap = scap;
   L.scap_pad = (scap + 31) & ~(int64_t)31;
   L.nb = nb;
+  L.nchunks = nchunks;
   int64_t longest = nb + 1;
+  if (nchunks + 1 > longest) longest = nchunks + 1;
   if (n + 1 > longest) longest = n + 1;
   if (scap + 1 > longest) longest = scap + 1;
   L.scan_tiles = (longest + kScanTile - 1) / kScanTile + 2;
@@ -128,6 +131,8 @@ inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows) {
   L.off_tl_mask = take(sizeof(uint32_t) * kMaskWords * (size_t)(L.scap_pad + 1));
   L.off_tl_scan = take(sizeof(int64_t) * (size_t)(L.scap_pad + 2));
   L.off_row_hit = take(sizeof(int32_t) * (size_t)L.scap_pad * (size_t)nrows);  // [t][row], tracklet-major
+  L.off_chunk_base = take(sizeof(int32_t) * (size_t)(nchunks + 2));   // tracklets before chunk (sector, slab, row)
+  L.off_chunk_scan0 = take(sizeof(int32_t) * (size_t)(nchunks + 2));  // grid-order start count at the chunk's first cluster
   L.off_scan_tmp = take(sizeof(int64_t) * (size_t)L.scan_tiles);
   L.total = o;
   return L;
@@ -148,6 +153,7 @@ struct Ws {
   uint32_t* tl_mask;
   long long* tl_scan;
   int32_t* row_hit;
+  int32_t *chunk_base, *chunk_scan0;
   long long* scan_tmp;
 };
 
@@ -171,6 +177,8 @@ inline Ws bind_ws(const Layout& L, void* workspace) {
   w.tl_mask = (uint32_t*)(b + L.off_tl_mask);
   w.tl_scan = (long long*)(b + L.off_tl_scan);
   w.row_hit = (int32_t*)(b + L.off_row_hit);
+  w.chunk_base = (int32_t*)(b + L.off_chunk_base);
+  w.chunk_scan0 = (int32_t*)(b + L.off_chunk_scan0);
   w.scan_tmp = (long long*)(b + L.off_scan_tmp);
   return w;
 }

@@ -171,29 +171,59 @@ k_clean(int64_t n, const int32_t* __restrict__ link_up, const int32_t* __restric
   }
 }
 
-// Start list in grid order.  Everything R14 needs from memory goes into one 32-byte record per tracklet,
-// gathered here with full memory-level parallelism instead of as a dependent chain inside the follower.
+// Tracklet order.  Tracklets are numbered by (sector, z slab, row, grid order inside): a slab is slab_w z-bins
+// (about one drift length), so tracklets with neighbouring numbers are tracks of the same few collisions
+// and touch the same few percent of a sector.  The passes that run one WARP per tracklet (selection) then
+// have a working set far below the L2 size.  The numbering needs no sort: a chunk (sector, slab, row) is a
+// contiguous range of grid positions, its number of start hits is a difference of the grid-order flag scan,
+// and an exclusive scan over the chunks in (sector, slab, row) order gives each chunk's first tracklet.
 __global__ void __launch_bounds__(kThreads)
-k_compact_starts(int64_t n, int64_t scap, const int32_t* __restrict__ scan, const Rec* __restrict__ rec,
-                 const int32_t* __restrict__ up_c, TlInit* __restrict__ tl_init, int32_t* __restrict__ ws_counters) {
+k_chunk_counts(const __grid_constant__ Geo g, int64_t nchunks, const int32_t* __restrict__ bin_first,
+               const int32_t* __restrict__ scan, int32_t* __restrict__ chunk_cnt, int32_t* __restrict__ chunk_scan0) {
+  const Scalars& sc = g.s;
+  for (int64_t q = (int64_t)blockIdx.x * kThreads + threadIdx.x; q <= nchunks; q += (int64_t)gridDim.x * kThreads) {
+    if (q == nchunks) {
+      chunk_cnt[q] = 0;  // sentinel: the exclusive scan leaves the total here
+      continue;
+    }
+    const int r = (int)(q % sc.nrows);
+    const int sj = (int)(q / sc.nrows);
+    const int j = sj % sc.nslab, s = sj / sc.nslab;
+    const int ny = g.row.ny[r];
+    const int base = s * sc.bins_per_sector + g.row.rowbase[r];
+    const int zb0 = j * sc.slab_w;
+    int zb1 = zb0 + sc.slab_w;
+    if (zb1 > sc.nz) zb1 = sc.nz;
+    const int s0 = scan[bin_first[base + zb0 * ny]], s1 = scan[bin_first[base + zb1 * ny]];
+    chunk_cnt[q] = s1 - s0;
+    chunk_scan0[q] = s0;
+  }
+}
+
+// Start list.  Everything R14 needs from memory goes into one 32-byte record per tracklet, gathered here
+// with full memory-level parallelism instead of as a dependent chain inside the follower.
+__global__ void __launch_bounds__(kThreads)
+k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const int32_t* __restrict__ scan,
+                 const Rec* __restrict__ rec, const int32_t* __restrict__ up_c, const int32_t* __restrict__ chunk_base,
+                 const int32_t* __restrict__ chunk_scan0, TlInit* __restrict__ tl_init, int32_t* __restrict__ ws_counters) {
+  const Scalars& sc = g.s;
   for (int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x; p < n; p += (int64_t)gridDim.x * kThreads) {
-    const int t = scan[p];
-    if (scan[p + 1] != t && t < scap) {
+    const int ex = scan[p];
+    if (scan[p + 1] != ex) {
       const Rec h0 = ld_rec(rec, (int)p);
-      const int p1 = up_c[p];
-      const Rec h1 = ld_rec(rec, p1);
-      TlInit I;
-      I.y0 = h0.x;
-      I.z0 = h0.y;
-      I.y1 = h1.x;
-      I.z1 = h1.y;
-      I.p0 = (int)p;
-      I.p1 = p1;
-      I.sr0 = rec_sr(h0);
-      I.orig0 = rec_idx(h0);
-      float4* o = reinterpret_cast<float4*>(tl_init + t);
-      o[0] = make_float4(I.y0, I.z0, I.y1, I.z1);
-      o[1] = make_float4(__int_as_float(I.p0), __int_as_float(I.p1), __int_as_float(I.sr0), __int_as_float(I.orig0));
+      const int sr0 = rec_sr(h0);
+      const int s = sr0 / sc.nrows, r = sr0 - s * sc.nrows;
+      const float zeta = (s < 18) ? h0.y : -h0.y;  // R2/R7, the same expression the grid build bins with
+      const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
+      const int64_t q = ((int64_t)s * sc.nslab + zb / sc.slab_w) * sc.nrows + r;
+      const int t = chunk_base[q] + (ex - chunk_scan0[q]);
+      if (t < scap) {
+        const int p1 = up_c[p];
+        const Rec h1 = ld_rec(rec, p1);
+        float4* o = reinterpret_cast<float4*>(tl_init + t);
+        o[0] = make_float4(h0.x, h0.y, h1.x, h1.y);
+        o[1] = make_float4(__int_as_float((int)p), __int_as_float(p1), __int_as_float(sr0), h0.z);
+      }
     }
     if (p == 0) {
       const int total = scan[n];
@@ -257,9 +287,15 @@ cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64
   TPC_LAUNCH(KID_CLEAN, st, (k_clean<<<blocks_for(n + 1, kThreads), kThreads, 0, st>>>(n, w.link_up, w.link_dn, w.up_c, flag)));
   if ((e = exclusive_scan<int32_t>(flag, flag, n + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
   if (n > 0) {
+    const int64_t nchunks = w.L.nchunks;
     TPC_LAUNCH(KID_COMPACT_STARTS, st,
-               (k_compact_starts<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, scap, flag, w.rec, w.up_c, w.tl_init,
-                                                                              w.counters)));
+               (k_chunk_counts<<<blocks_for(nchunks + 1, kThreads), kThreads, 0, st>>>(g, nchunks, w.bin_first, flag,
+                                                                                      w.chunk_base, w.chunk_scan0)));
+    if ((e = exclusive_scan<int32_t>(w.chunk_base, w.chunk_base, nchunks + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess)
+      return e;
+    TPC_LAUNCH(KID_COMPACT_STARTS, st,
+               (k_compact_starts<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, scap, flag, w.rec, w.up_c, w.chunk_base,
+                                                                              w.chunk_scan0, w.tl_init, w.counters)));
     if ((e = launch_follow(g, w, st)) != cudaSuccess) return e;
   }
   return launch_select(g, w, cluster_track, max_tracks, trk_seed, trk_sector, trk_nhits, trk_first_hit, trk_hits, counters,

@@ -179,6 +179,7 @@ k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const i
     if (run) pre = __ldg(hits + i_next);
     const float xh = sX[__float_as_int(h.z)];
     bool ok = true;
+    __syncwarp();  // one copy of transport + update for all lanes (see tpc_follow.cu)
     if (run && cnt > 0) {  // the first hit of a pass is the one the state already sits at (no transport)
       ok = propagate(st, xh - x_at, kB, ms);
       if (ok) x_at = xh;

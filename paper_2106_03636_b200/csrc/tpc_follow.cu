@@ -98,158 +98,153 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     }
     if (__all_sync(kFull, phase == PH_DONE)) break;
 
-    // ---- target row of this step; chain steps prefetch their cluster and the next link ---------
-    const bool chain = phase == PH_CHAIN;
+    // ---- target row of this step; chain steps prefetch their next link --------------------------
+    const bool isI = phase == PH_INIT, chain = phase == PH_CHAIN, isJ = phase == PH_JUMP;
     const bool leg = phase == PH_UP || phase == PH_DOWN;
     int rn = r0;                      // PH_INIT, PH_JUMP
     if (chain) rn = r_at + 1;         // links join adjacent rows (R9)
     if (leg) rn = r;
-    Rec cpre = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     int nxt = -1;
-    if (chain) {
-      cpre = ld_rec(rec, hn);
-      nxt = __ldg(up_c + hn);
-    }
-    // ---- R12 transport (one copy for every phase) -----------------------------------------------
+    if (chain) nxt = __ldg(up_c + hn);
+    // ---- R12 transport (one copy for every phase; __syncwarp keeps the compiler from cloning it
+    //      into the phase branches, which would serialise the lanes again) --------------------------
+    __syncwarp();
     KState nx = st;
     bool ok = phase != PH_DONE;
-    if (ok && phase != PH_INIT) {
+    if (ok && !isI) {
       ok = propagate(nx, sm.X[rn] - sm.X[r_at], kB, ms);
       if (ok) nprop++;
     }
     const Innov I = innovation(nx, sy2, sz2);
-    // ---- measurement for this step ----------------------------------------------------------------
-    bool upd = false, edge_out = false;
-    float my = 0.0f, mz = 0.0f;
-    int mk = -1;
-    if (phase == PH_INIT) {  // R14: update with the start hit itself
-      upd = true;
-      my = nx.p[0];
-      mz = 0.0f;
-      mk = p0;
-    } else if (chain && ok) {  // R15: the linked cluster, no window; a bad chi2 discards the prediction
-      const float chi2 = chi2_of(I, cpre.x - nx.p[0], (cpre.y - zref) - nx.p[1]);
-      if (chi2 > sc.chi2_chain_cut) {
-        ok = false;
-      } else {
-        upd = true;
-        my = cpre.x;
-        mz = cpre.y - zref;
-        mk = hn;
-      }
-    } else if (leg && ok) {  // R16: windowed arg-min chi2 over the row
-      edge_out = fabsf(nx.p[0]) > sm.ymax[rn] + sc.edge_margin;
+    // ---- candidates of this step: up to two contiguous ranges of grid positions -------------------
+    //   chain step (R15): the linked cluster alone, no window;  leg step (R16): the bins covering the
+    //   chi2 window (a superset, every candidate is re-tested in cm);  init / jump: none.
+    const float yp = nx.p[0], dzp = nx.p[1];
+    float wy = 3.0e38f, wz = 3.0e38f;
+    int ka0 = 0, n0 = 0, ka1 = 0, n1 = 0;
+    bool edge_out = false, many = false;
+    BinWin W;
+    W.first = W.ny = W.ybspan = W.nzb = 0;
+    if (chain && ok) {
+      ka0 = hn;
+      n0 = 1;
+    } else if (leg && ok) {
+      edge_out = fabsf(yp) > sm.ymax[rn] + sc.edge_margin;
       if (!edge_out) {
-        const float wy = fminf(sqrtf(sc.chi2_cut * I.S00), sc.win_max);
-        const float wz = fminf(sqrtf(sc.chi2_cut * I.S11), sc.win_max);
-        const float yp = nx.p[0], dzp = nx.p[1];
+        wy = fminf(sqrtf(sc.chi2_cut * I.S00), sc.win_max);
+        wz = fminf(sqrtf(sc.chi2_cut * I.S11), sc.win_max);
         const float zc = zref + dzp;
-        const BinWin W = bin_window(sm, sc, s, rn, yp - wy, yp + wy, zc - wz, zc + wz);
-        bool have = false;
-        float best = 0.0f, by = 0.0f, bz = 0.0f;
-        int bi = 0, bk = -1;
-        for (int zi = 0; zi < W.nzb; zi++) {
-          const int b0 = W.first + zi * W.ny;
-          const int ka = __ldg(bin_first + b0), ke = __ldg(bin_first + b0 + W.ybspan);
-          for (int k = ka; k < ke; k++) {
-            const Rec c = ld_rec(rec, k);
-            const float q0 = c.x - yp, q1 = (c.y - zref) - dzp;
-            if (!(fabsf(q0) <= wy && fabsf(q1) <= wz)) continue;
-            const float chi2 = chi2_of(I, q0, q1);
-            ncand++;
-            const int ci = rec_idx(c);
-            if (!have || chi2 < best || (chi2 == best && ci < bi)) {  // ties: lowest original index
-              have = true;
-              best = chi2;
-              bi = ci;
-              bk = k;
-              by = c.x;
-              bz = c.y;
-            }
-          }
+        W = bin_window(sm, sc, s, rn, yp - wy, yp + wy, zc - wz, zc + wz);
+        const int e0 = __ldg(bin_first + W.first + W.ybspan);
+        ka0 = __ldg(bin_first + W.first);
+        if (W.nzb > 1) {
+          const int e1 = __ldg(bin_first + W.first + W.ny + W.ybspan);
+          ka1 = __ldg(bin_first + W.first + W.ny);
+          n1 = e1 - ka1;
         }
-        if (have && best < sc.chi2_cut) {
-          upd = true;
-          my = by;
-          mz = bz - zref;
-          mk = bk;
+        n0 = e0 - ka0;
+        many = W.nzb > 2;
+      }
+    }
+    // ---- arg-min chi2 over the candidates (ties: lowest original index) ----------------------------
+    __syncwarp();
+    bool have = false;
+    float best = 0.0f, by = 0.0f, bz = 0.0f;
+    int bi = 0, bk = -1;
+    const int ntot = n0 + n1;
+    for (int i = 0; i < ntot; i++) {
+      const int k = i < n0 ? ka0 + i : ka1 + (i - n0);
+      const Rec c = ld_rec(rec, k);
+      const float q0 = c.x - yp, q1 = (c.y - zref) - dzp;
+      if (!(fabsf(q0) <= wy && fabsf(q1) <= wz)) continue;
+      const float chi2 = chi2_of(I, q0, q1);
+      if (leg) ncand++;
+      const int ci = rec_idx(c);
+      if (!have || chi2 < best || (chi2 == best && ci < bi)) {
+        have = true;
+        best = chi2;
+        bi = ci;
+        bk = k;
+        by = c.x;
+        bz = c.y;
+      }
+    }
+    if (many) {  // windows of more than two z-bin rows (cells much smaller than the window): generic loop
+      for (int zi = 2; zi < W.nzb; zi++) {
+        const int b0 = W.first + zi * W.ny;
+        const int ka = __ldg(bin_first + b0), ke = __ldg(bin_first + b0 + W.ybspan);
+        for (int k = ka; k < ke; k++) {
+          const Rec c = ld_rec(rec, k);
+          const float q0 = c.x - yp, q1 = (c.y - zref) - dzp;
+          if (!(fabsf(q0) <= wy && fabsf(q1) <= wz)) continue;
+          const float chi2 = chi2_of(I, q0, q1);
+          ncand++;
+          const int ci = rec_idx(c);
+          if (!have || chi2 < best || (chi2 == best && ci < bi)) {
+            have = true;
+            best = chi2;
+            bi = ci;
+            bk = k;
+            by = c.x;
+            bz = c.y;
+          }
         }
       }
     }
-    // commit the transport (a failed one leaves the state where it was, R15)
-    if (ok) st = nx;
-    // ---- R13 update (one copy for every phase) -----------------------------------------------------
+    // ---- decision: R14 start hit / R15 chain cut (a bad chi2 discards the prediction) / R16 cut ----
+    bool upd = isI;
+    float my = yp, mz = 0.0f;  // R14: update with the start hit itself (yp == y0, dz == 0)
+    int mk = p0;
+    if (chain && ok) {
+      if (!have || best > sc.chi2_chain_cut) ok = false;
+      else upd = true;
+    }
+    if (leg && have && best < sc.chi2_cut) upd = true;
+    if (!isI && upd) {
+      my = by;
+      mz = bz - zref;
+      mk = bk;
+    }
+    // ---- commit the transport, R13 update (one copy for every phase) --------------------------------
+    __syncwarp();
+    if (ok) {
+      st = nx;
+      r_at = rn;
+    }
     if (upd) {
       update(st, I, my, mz);
       nupd++;
+      nh++;
+      lo = min(lo, rn);
+      hi = max(hi, rn);
     }
-    // ---- bookkeeping and phase transitions ------------------------------------------------------------
-    bool finish = false, end_leg = false;
-    switch (phase) {
-      case PH_INIT:
-        my_hits[r0] = p0;
-        nh = 1;
-        phase = PH_CHAIN;
-        break;
-      case PH_CHAIN:
-        if (upd) {
-          my_hits[rn] = mk;
-          nh++;
-          hi = rn;
-          r_at = rn;
-          hn = nxt;
-        }
-        if (!upd || hn < 0) {  // end of the chain phase: R16 upward from the last chain hit
-          phase = PH_UP;
-          r = r_at + 1;
-          misses = 0;
-          if (r >= nrows) phase = PH_JUMP;
-        }
-        break;
-      case PH_UP:
-      case PH_DOWN:
-        if (!ok) {
-          end_leg = true;
-        } else {
-          r_at = rn;
-          if (edge_out) {
-            end_leg = true;  // left the sector
-          } else {
-            if (upd) {
-              my_hits[rn] = mk;
-              nh++;
-              lo = min(lo, rn);
-              hi = max(hi, rn);
-              misses = 0;
-            } else {
-              my_hits[rn] = -1;
-              misses++;
-              if (misses > sc.max_gap) end_leg = true;
-            }
-            if (!end_leg) {
-              r += (phase == PH_UP) ? 1 : -1;
-              if (r < 0 || r >= nrows) end_leg = true;
-            }
-          }
-        }
-        if (end_leg) {
-          if (phase == PH_UP) phase = PH_JUMP;  // R17
-          else finish = true;
-        }
-        break;
-      case PH_JUMP:
-        if (!ok) {
-          finish = true;
-        } else {
-          r_at = r0;
-          phase = PH_DOWN;
-          r = r0 - 1;
-          misses = 0;
-          if (r < 0) finish = true;
-        }
-        break;
-      default:
-        break;
+    // ---- bookkeeping and phase transitions ---------------------------------------------------------------
+    __syncwarp();
+    const bool searched = leg && ok && !edge_out;
+    if (upd || searched) my_hits[rn] = upd ? mk : -1;
+    bool finish = false;
+    if (isI) {
+      phase = PH_CHAIN;
+    } else if (chain) {
+      if (upd) hn = nxt;
+      if (!upd || hn < 0) {  // end of the chain phase: R16 upward from the last chain hit
+        phase = PH_UP;
+        r = r_at + 1;
+        misses = 0;
+        if (r >= nrows) phase = PH_JUMP;
+      }
+    } else if (leg) {
+      misses = upd ? 0 : misses + 1;
+      r += (phase == PH_UP) ? 1 : -1;
+      if (!searched || misses > sc.max_gap || r < 0 || r >= nrows) {  // end of the leg
+        if (phase == PH_UP) phase = PH_JUMP;  // R17
+        else finish = true;
+      }
+    } else if (isJ) {
+      phase = PH_DOWN;
+      r = r0 - 1;
+      misses = 0;
+      if (!ok || r < 0) finish = true;
     }
     if (finish) {  // R18 record; the R20 key is pushed by k_push_keys
       tl_info[t] = nh | (lo << 8) | (hi << 16);

@@ -25,10 +25,8 @@ enum KernelId {
   KID_COMPACT_STARTS,
   KID_FOLLOW,
   KID_PUSH_KEYS,
-  KID_MARK,
   KID_COUNT_KEPT,
-  KID_ASSIGN,
-  KID_TRACK_INFO,
+  KID_WRITE_TRACKS,
   KID_FIT,
   KID_EXPORT,
   KID_N
