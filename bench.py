@@ -43,10 +43,10 @@ KERNEL_MODEL = {
     # name: (bound, {unit: algorithmic HBM bytes per unit}, unit the alu-bound kernels are counted in)
     # units: cluster = input cluster, bin = grid bin, tracklet = followed start hit, claim = (tracklet,row) hit
     # recorded by the follower, hit = hit of an accepted track
-    "k_bin_count": ("hbm", {"cluster": 12 + 8 + 8}, None),       # y,z,sr in; key,rank out; count RMW (4+4)
-    "k_scan_*": ("hbm", {"bin": 12, "cluster": 12, "tracklet": 24}, None),  # all scans of a step: 2 reads + 1 write per element
-    "k_scatter": ("hbm", {"cluster": 12 + 8 + 4 + 16}, None),     # y,z,sr,key,rank,bin_first in; 16 B record out
-    "k_canon": ("hbm", {"bin": 4}, None),
+    "k_bucket_hist": ("hbm", {"cluster": 12}, None),                # y, z, sector_row in
+    "k_scan_*": ("hbm", {"cluster": 12, "tracklet": 24}, None),     # all scans of a step: 2 reads + 1 write per element
+    "k_bucket_scatter": ("hbm", {"cluster": 12 + 16}, None),        # inputs in, 16 B record out
+    "k_bucket_sort": ("hbm", {"cluster": 16 + 16, "bin": 4}, None), # records in (second read from L2), records + bin_first out
     "k_neighbours": ("hbm", {"cluster": 16 + 8}, None),           # own record in, two links out (neighbours from L2)
     "k_clean": ("hbm", {"cluster": 8 + 8}, None),
     "k_compact_starts": ("hbm", {"cluster": 4, "tracklet": 32}, None),

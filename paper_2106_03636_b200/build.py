@@ -33,23 +33,25 @@ def up_to_date() -> bool:
     return all(os.path.getmtime(d) <= t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/*.cu -> paper_2106_03636_b200/libtpc_b200.so for sm_100a."""
-    if not force and up_to_date():
+def build_library(force: bool = False, verbose: bool = False, out: str | None = None) -> str:
+    """Compile csrc/*.cu -> paper_2106_03636_b200/libtpc_b200.so (or `out`) for sm_100a."""
+    if out is None and not force and up_to_date():
         return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
+    target = out or LIB
+    tmp = target + f".tmp{os.getpid()}"
     cmd = [_nvcc(), "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
            "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared", "-o", tmp]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("TPC_B200_NVCC_FLAGS", "").split()     # tuning macros (-DTPC_FOLLOW_BATCH=...), optional
     cmd += [os.path.join(CSRC, s) for s in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed building libtpc_b200.so")
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, target)
+    return target
 
 
 if __name__ == "__main__":

@@ -23,7 +23,7 @@ struct Rec2 {
 };
 Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
-const char* const kKernelNames[KID_N] = {"k_bin_count", "k_scan_*", "k_scatter", "k_canon", "k_neighbours", "k_clean",
+const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
                                          "k_fit", "k_export_*"};
 }  // namespace
@@ -106,7 +106,7 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
     G->row.ny[r] = ny;
     G->row.rowbase[r] = (int32_t)base;
     base += (int64_t)ny * s.nz;
-    if (base * s.nsec >= 2147483000ll) return false;      // bin ids are int32
+    if (base * s.nsec > 1073741824ll) return false;       // bin ids: int32, and <= 32768 buckets of <= 32768 bins
   }
   G->row.rowbase[s.nrows] = (int32_t)base;
   s.bins_per_sector = (int32_t)base;

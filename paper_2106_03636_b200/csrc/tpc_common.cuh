@@ -74,7 +74,7 @@ using Rec = float4;
 struct Layout {
   int64_t n, scap, scap_pad, nb, nchunks;
   int64_t scan_tiles;  // capacity (elements) of the scan scratch
-  size_t off_counters, off_rec, off_key, off_rank, off_bin_first, off_link_up, off_link_dn, off_up_c,
+  size_t off_counters, off_rec, off_key, off_bucket_first, off_bucket_cursor, off_bin_first, off_link_up, off_link_dn, off_up_c,
       off_owner, off_hit_rec, off_tl_init, off_tl_info, off_tl_key, off_tl_mask, off_tl_scan, off_row_hit,
       off_chunk_base, off_chunk_scan0, off_scan_tmp, total;
 };
@@ -85,6 +85,7 @@ struct Layout {
 // carrying t lets the per-cluster passes find the owning tracklet without a search.
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
+constexpr int kMaxBuckets = 32768;  // grid build: first-level buckets of the counting sort
 constexpr int kMaskWords = 5;  // kept-row mask per tracklet (rows 0..159)
 
 // Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.
@@ -117,8 +118,9 @@ inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows, int64_
   };
   L.off_counters = take(sizeof(int32_t) * WC_N);
   L.off_rec = take(sizeof(Rec) * (size_t)(n + 1));
-  L.off_key = take(sizeof(int32_t) * (size_t)(n + 1));      // bin id per cluster; later start-flag scan
-  L.off_rank = take(sizeof(int32_t) * (size_t)(n + 1));     // rank in bin; later unused
+  L.off_key = take(sizeof(int32_t) * (size_t)(n + 1));      // start-hit flags and their scan (R10)
+  L.off_bucket_first = take(sizeof(int32_t) * (size_t)(kMaxBuckets + 2));
+  L.off_bucket_cursor = take(sizeof(int32_t) * (size_t)(kMaxBuckets + 2));
   L.off_bin_first = take(sizeof(int32_t) * (size_t)(nb + 2));
   L.off_link_up = take(sizeof(int32_t) * (size_t)(n + 1));
   L.off_link_dn = take(sizeof(int32_t) * (size_t)(n + 1));
@@ -144,7 +146,7 @@ struct Ws {
   Layout L;
   int32_t* counters;
   Rec* rec;
-  int32_t *key, *rank, *bin_first, *link_up, *link_dn, *up_c;
+  int32_t *key, *bucket_first, *bucket_cursor, *bin_first, *link_up, *link_dn, *up_c;
   unsigned long long* owner;
   float4* hit_rec;
   TlInit* tl_init;
@@ -164,7 +166,8 @@ inline Ws bind_ws(const Layout& L, void* workspace) {
   w.counters = (int32_t*)(b + L.off_counters);
   w.rec = (Rec*)(b + L.off_rec);
   w.key = (int32_t*)(b + L.off_key);
-  w.rank = (int32_t*)(b + L.off_rank);
+  w.bucket_first = (int32_t*)(b + L.off_bucket_first);
+  w.bucket_cursor = (int32_t*)(b + L.off_bucket_cursor);
   w.bin_first = (int32_t*)(b + L.off_bin_first);
   w.link_up = (int32_t*)(b + L.off_link_up);
   w.link_dn = (int32_t*)(b + L.off_link_dn);

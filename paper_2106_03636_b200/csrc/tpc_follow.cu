@@ -27,10 +27,17 @@ namespace {
 
 constexpr int kFollowThreads = 128;
 constexpr unsigned kFull = 0xffffffffu;
+#ifndef TPC_FOLLOW_BATCH
+#define TPC_FOLLOW_BATCH 4
+#endif
+#ifndef TPC_FOLLOW_MIN_BLOCKS
+#define TPC_FOLLOW_MIN_BLOCKS 4
+#endif
+constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
 
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
-__global__ void __launch_bounds__(kFollowThreads)
+__global__ void __launch_bounds__(kFollowThreads, TPC_FOLLOW_MIN_BLOCKS)
 k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32_t* __restrict__ bin_first,
          const int32_t* __restrict__ up_c, const TlInit* __restrict__ tl_init, int32_t* __restrict__ row_hit,
          int32_t* __restrict__ tl_info, unsigned long long* __restrict__ tl_key, int32_t* __restrict__ ws_counters) {
@@ -152,21 +159,32 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     float best = 0.0f, by = 0.0f, bz = 0.0f;
     int bi = 0, bk = -1;
     const int ntot = n0 + n1;
-    for (int i = 0; i < ntot; i++) {
-      const int k = i < n0 ? ka0 + i : ka1 + (i - n0);
-      const Rec c = ld_rec(rec, k);
-      const float q0 = c.x - yp, q1 = (c.y - zref) - dzp;
-      if (!(fabsf(q0) <= wy && fabsf(q1) <= wz)) continue;
-      const float chi2 = chi2_of(I, q0, q1);
-      if (leg) ncand++;
-      const int ci = rec_idx(c);
-      if (!have || chi2 < best || (chi2 == best && ci < bi)) {
-        have = true;
-        best = chi2;
-        bi = ci;
-        bk = k;
-        by = c.x;
-        bz = c.y;
+    // kBatch records are requested together (one memory round trip per batch instead of one per candidate)
+    // and tested branch-free; slots past the end re-read the last candidate and are masked out.
+    for (int i0 = 0; i0 < ntot; i0 += kBatch) {
+      Rec c[kBatch];
+      int kk[kBatch];
+#pragma unroll
+      for (int j = 0; j < kBatch; j++) {
+        const int i = min(i0 + j, ntot - 1);
+        kk[j] = i < n0 ? ka0 + i : ka1 + (i - n0);
+        c[j] = ld_rec(rec, kk[j]);
+      }
+#pragma unroll
+      for (int j = 0; j < kBatch; j++) {
+        const float q0 = c[j].x - yp, q1 = (c[j].y - zref) - dzp;
+        const bool in = (i0 + j < ntot) && fabsf(q0) <= wy && fabsf(q1) <= wz;
+        const float chi2 = chi2_of(I, q0, q1);
+        const int ci = rec_idx(c[j]);
+        if (in && leg) ncand++;
+        if (in && (!have || chi2 < best || (chi2 == best && ci < bi))) {
+          have = true;
+          best = chi2;
+          bi = ci;
+          bk = kk[j];
+          by = c[j].x;
+          bz = c[j].y;
+        }
       }
     }
     if (many) {  // windows of more than two z-bin rows (cells much smaller than the window): generic loop

@@ -2,15 +2,22 @@
 // tpc_grid.cu -- step 1 of the hot path (BASELINE.json north_star (1)):
 // sort the clusters of every (sector, pad row) into a (y, zeta) grid.
 //
-//   k_bin_count   one thread per cluster: bin id (R7 formula, fp32), rank = atomicAdd(count[bin])
-//   exclusive scan of the counts -> bin_first   (tpc_scan.cuh)
-//   k_scatter     cluster -> 16-byte record at bin_first[bin] + rank
-//   k_canon       bins holding >= 2 clusters are re-ordered by original index, which turns the
-//                 arrival-order ranks of the atomics into the STABLE order R7 asks for, so the
-//                 grid is bit-identical from run to run and equal to a stable sort by bin.
+// A two-level counting sort whose random accesses all stay inside the L2:
+//   k_bucket_hist     bin id of every cluster (R7 formula, fp32); a BUCKET is kBucketBins...
+//                     consecutive bins (a few thousand clusters).  Per-block shared-memory
+//                     histogram over the buckets, flushed with one atomic per non-empty bucket.
+//   scan              bucket offsets.
+//   k_bucket_scatter  cluster -> 16-byte record appended to its bucket's range of a temporary
+//                     array (warp-aggregated cursor atomics; the ~2e4 append frontiers are L2
+//                     resident, so DRAM sees whole lines).
+//   k_bucket_sort     one block per bucket: counts the bucket's bins in shared memory, scans them
+//                     (-> bin_first), places the records, and re-orders every bin holding >= 2
+//                     clusters by original index, which turns the arrival order of the atomics
+//                     into the STABLE order R7 asks for: the grid is bit-identical from run to
+//                     run and equal to a stable sort by bin.  The bucket (~100 KB) stays in L2
+//                     between the passes.
 //
-// Roofline: HBM-bound streaming + one random 4-byte atomic and one random 16-byte store per
-// cluster.
+// Roofline: HBM streaming, 72 B per cluster + 4 B per bin.
 // =============================================================================================
 #include "tpc_common.cuh"
 #include "tpc_scan.cuh"
@@ -20,6 +27,7 @@ namespace tpc {
 namespace {
 
 constexpr int kThreads = 256;
+constexpr unsigned kFull = 0xffffffffu;
 
 struct GridSmem {
   float ymax[kMaxRows];
@@ -27,63 +35,143 @@ struct GridSmem {
   int32_t rowbase[kMaxRows];
 };
 
-__global__ void __launch_bounds__(kThreads)
-k_bin_count(const __grid_constant__ Geo g, int64_t n, const float* __restrict__ y, const float* __restrict__ z,
-            const int32_t* __restrict__ sector_row, int32_t* __restrict__ key, int32_t* __restrict__ rank,
-            int32_t* __restrict__ count, int32_t* __restrict__ ws_counters) {
-  __shared__ GridSmem sm;
-  for (int r = threadIdx.x; r < g.s.nrows; r += kThreads) {
+__device__ __forceinline__ void load_grid_rows(GridSmem& sm, const Geo& g) {
+  for (int r = threadIdx.x; r < g.s.nrows; r += blockDim.x) {
     sm.ymax[r] = g.row.ymax[r];
     sm.ny[r] = g.row.ny[r];
     sm.rowbase[r] = g.row.rowbase[r];
   }
+}
+
+// R7 bin id, fp32, one rounding per operation; *clamped is raised for zeta outside [z_lo, z_hi].
+__device__ __forceinline__ int bin_of(const GridSmem& sm, const Scalars& sc, int sr, float yy, float zz, bool* clamped) {
+  const int s = sr / sc.nrows, r = sr - s * sc.nrows;
+  const float zeta = (s < 18) ? zz : -zz;  // R2/R7: mirrored drift coordinate
+  const int yb = clampbin((yy + sm.ymax[r]) * sc.inv_cy, sm.ny[r]);
+  const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
+  if (clamped) *clamped |= !(zeta >= sc.z_lo && zeta <= sc.z_hi);
+  return s * sc.bins_per_sector + sm.rowbase[r] + zb * sm.ny[r] + yb;
+}
+
+// shared-memory index with one pad word per 32: conflict-free both for t*32+k and for random access
+__device__ __forceinline__ int pad32(int j) { return j + (j >> 5); }
+
+__global__ void __launch_bounds__(kThreads)
+k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nbuckets, const float* __restrict__ y,
+              const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ bucket_cnt,
+              int32_t* __restrict__ ws_counters) {
+  extern __shared__ int32_t hist[];  // [nbuckets]
+  __shared__ GridSmem sm;
+  load_grid_rows(sm, g);
+  for (int j = threadIdx.x; j < nbuckets; j += kThreads) hist[j] = 0;
   __syncthreads();
-  const int nrows = g.s.nrows;
-  const float inv_cy = g.s.inv_cy, inv_cz = g.s.inv_cz, z_lo = g.s.z_lo, z_hi = g.s.z_hi;
-  const int nz = g.s.nz, bps = g.s.bins_per_sector;
+  const Scalars& sc = g.s;
   bool clamped = false;
-  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
-    const int sr = sector_row[i];
-    const int s = sr / nrows, r = sr - s * nrows;
-    const float yy = y[i];
-    const float zeta = (s < 18) ? z[i] : -z[i];  // R2/R7: mirrored drift coordinate
-    const int yb = clampbin((yy + sm.ymax[r]) * inv_cy, sm.ny[r]);
-    const int zb = clampbin((zeta - z_lo) * inv_cz, nz);
-    clamped |= !(zeta >= z_lo && zeta <= z_hi);
-    const int b = s * bps + sm.rowbase[r] + zb * sm.ny[r] + yb;
-    key[i] = b;
-    rank[i] = atomicAdd(count + b, 1);
+  // every block takes one contiguous slice of the input (the tail of the loop keeps the warp whole for match_any)
+  const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kThreads - 1) / kThreads * kThreads;
+  const int64_t lo = (int64_t)blockIdx.x * per, hi = lo + per < n ? lo + per : n;
+  for (int64_t i0 = lo + (threadIdx.x & ~31); i0 < hi; i0 += kThreads) {
+    const int64_t i = i0 + (threadIdx.x & 31);
+    int bk = -1;
+    if (i < hi) bk = bin_of(sm, sc, __ldcs(sector_row + i), __ldcs(y + i), __ldcs(z + i), &clamped) >> bucket_shift;
+    const unsigned peers = __match_any_sync(kFull, bk);  // inputs ordered by row put a whole warp in one bucket
+    if (bk >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + bk, __popc(peers));
   }
-  if (__any_sync(0xffffffffu, clamped) && (threadIdx.x & 31) == 0) atomicOr(ws_counters + WC_STATUS, TPC_ST_Z_CLAMPED);
+  __syncthreads();
+  for (int j = threadIdx.x; j < nbuckets; j += kThreads) {
+    const int c = hist[j];
+    if (c) atomicAdd(bucket_cnt + j, c);
+  }
+  if (__any_sync(kFull, clamped) && (threadIdx.x & 31) == 0) atomicOr(ws_counters + WC_STATUS, TPC_ST_Z_CLAMPED);
 }
 
 __global__ void __launch_bounds__(kThreads)
-k_scatter(int64_t n, const float* __restrict__ y, const float* __restrict__ z, const int32_t* __restrict__ sector_row,
-          const int32_t* __restrict__ key, const int32_t* __restrict__ rank, const int32_t* __restrict__ bin_first,
-          Rec* __restrict__ rec) {
-  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
-    const int pos = __ldg(bin_first + key[i]) + rank[i];
-    rec[pos] = make_float4(y[i], z[i], __int_as_float((int)i), __int_as_float(sector_row[i]));
+k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, const float* __restrict__ y,
+                 const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ cursor,
+                 Rec* __restrict__ tmp) {
+  __shared__ GridSmem sm;
+  load_grid_rows(sm, g);
+  __syncthreads();
+  const Scalars& sc = g.s;
+  const int lane = threadIdx.x & 31;
+  const int64_t nround = (n + 31) & ~(int64_t)31;
+  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < nround; i += (int64_t)gridDim.x * kThreads) {
+    int bk = -1, sr = 0;
+    float yy = 0.0f, zz = 0.0f;
+    if (i < n) {
+      sr = __ldcs(sector_row + i);
+      yy = __ldcs(y + i);
+      zz = __ldcs(z + i);
+      bk = bin_of(sm, sc, sr, yy, zz, nullptr) >> bucket_shift;
+    }
+    const unsigned peers = __match_any_sync(kFull, bk);
+    const int leader = __ffs(peers) - 1;
+    int base = 0;
+    if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
+    base = __shfl_sync(kFull, base, leader);
+    if (bk >= 0) tmp[base + __popc(peers & ((1u << lane) - 1u))] = make_float4(yy, zz, __int_as_float((int)i), __int_as_float(sr));
   }
 }
 
-// One thread per bin; bins with fewer than two clusters (the vast majority, mean occupancy ~1) cost two
-// coalesced loads.  Insertion sort by original index (max occupancy seen on the configs: 17).
+// One block per bucket (grid-stride).  cnt[] holds, in turn: bin counts, exclusive offsets, running cursors
+// (= end offsets once every record is placed).
 __global__ void __launch_bounds__(kThreads)
-k_canon(int64_t nb, const int32_t* __restrict__ bin_first, Rec* __restrict__ rec) {
-  for (int64_t b = (int64_t)blockIdx.x * kThreads + threadIdx.x; b < nb; b += (int64_t)gridDim.x * kThreads) {
-    const int a = bin_first[b], e = bin_first[b + 1];
-    for (int i = a + 1; i < e; i++) {
-      const Rec v = rec[i];
-      const int vi = rec_idx(v);
-      int j = i - 1;
-      while (j >= a) {
-        const Rec u = rec[j];
-        if (rec_idx(u) <= vi) break;
-        rec[j + 1] = u;
-        j--;
+k_bucket_sort(const __grid_constant__ Geo g, int64_t n, int64_t nb, int bucket_shift, int nbuckets,
+              const int32_t* __restrict__ bucket_first, const Rec* __restrict__ tmp, Rec* rec, int32_t* __restrict__ bin_first) {
+  extern __shared__ int32_t cnt[];  // [pad32(bucket bins)]
+  __shared__ GridSmem sm;
+  __shared__ int32_t scan_sm[kThreads / 32 + 1];
+  load_grid_rows(sm, g);
+  const Scalars& sc = g.s;
+  const int bbins = 1 << bucket_shift;
+  const int per_thread = bbins / kThreads;  // bucket bins are a multiple of 32 * kThreads... (>= 8192)
+  for (int b = blockIdx.x; b < nbuckets; b += gridDim.x) {
+    const int start = bucket_first[b], end = bucket_first[b + 1];
+    const int64_t bin0 = (int64_t)b << bucket_shift;
+    const int nbins = (int)((nb - bin0) < bbins ? (nb - bin0) : bbins);
+    __syncthreads();  // previous bucket's canon pass is done with cnt[]
+    for (int j = threadIdx.x; j < bbins; j += kThreads) cnt[pad32(j)] = 0;
+    __syncthreads();
+    for (int i = start + threadIdx.x; i < end; i += kThreads) {
+      const Rec r = tmp[i];
+      atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r), r.x, r.y, nullptr) - (int)bin0), 1);
+    }
+    __syncthreads();
+    // exclusive scan over the bucket's bins, thread t owns bins [t*per_thread, (t+1)*per_thread)
+    int acc = 0;
+    for (int k = 0; k < per_thread; k++) acc += cnt[pad32(threadIdx.x * per_thread + k)];
+    int total;
+    int ex = block_excl_scan<int, kThreads>(acc, &total, scan_sm);
+    for (int k = 0; k < per_thread; k++) {
+      const int j = threadIdx.x * per_thread + k;
+      const int c = cnt[pad32(j)];
+      cnt[pad32(j)] = ex;
+      if (j < nbins) bin_first[bin0 + j] = start + ex;
+      ex += c;
+    }
+    if (b == nbuckets - 1 && threadIdx.x == 0) bin_first[nb] = (int)n;
+    __syncthreads();
+    for (int i = start + threadIdx.x; i < end; i += kThreads) {
+      const Rec r = tmp[i];
+      const int pos = atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r), r.x, r.y, nullptr) - (int)bin0), 1);
+      rec[start + pos] = r;
+    }
+    __syncthreads();  // the block's own global writes are visible to it from here on
+    // bins with >= 2 clusters: insertion sort by original index (max occupancy seen on the configs: 17)
+    for (int j = threadIdx.x; j < nbins; j += kThreads) {
+      const int a = start + (j ? cnt[pad32(j - 1)] : 0), e = start + cnt[pad32(j)];
+      for (int i = a + 1; i < e; i++) {
+        const Rec v = rec[i];
+        const int vi = rec_idx(v);
+        int q = i - 1;
+        while (q >= a) {
+          const Rec u = rec[q];
+          if (rec_idx(u) <= vi) break;
+          rec[q + 1] = u;
+          q--;
+        }
+        rec[q + 1] = v;
       }
-      rec[j + 1] = v;
     }
   }
 }
@@ -96,24 +184,45 @@ k_export_sorted(int64_t n, const Rec* __restrict__ rec, int32_t* __restrict__ so
 
 }  // namespace
 
+// bucket geometry: 8192 bins per bucket, doubled until at most 32768 buckets remain (nb <= 2^30)
+static inline int bucket_shift_for(int64_t nb) {
+  int sh = 13;
+  while (((nb + ((int64_t)1 << sh) - 1) >> sh) > kMaxBuckets) sh++;
+  return sh;
+}
+
 cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const float* z, const int32_t* sector_row,
                               cudaStream_t st) {
   const int64_t n = w.L.n, nb = w.L.nb;
   cudaError_t e;
+  const int sh = bucket_shift_for(nb);
+  const int nbuckets = (int)((nb + ((int64_t)1 << sh) - 1) >> sh);
+  const size_t hist_smem = sizeof(int32_t) * (size_t)nbuckets;
+  const size_t sort_smem = sizeof(int32_t) * (size_t)(((size_t)1 << sh) + ((size_t)1 << (sh - 5)) + 32);
+  static bool attr_done = false;
+  if (!attr_done) {
+    if ((e = cudaFuncSetAttribute(k_bucket_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBuckets * 4)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_bucket_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (32768 + 1024 + 32) * 4)) != cudaSuccess)
+      return e;
+    attr_done = true;
+  }
   if ((e = cudaMemsetAsync(w.counters, 0, sizeof(int32_t) * WC_N, st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(w.bin_first, 0, sizeof(int32_t) * (size_t)(nb + 2), st)) != cudaSuccess) return e;
-  if (n > 0) {
-    TPC_LAUNCH(KID_BIN_COUNT, st,
-               (k_bin_count<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, y, z, sector_row, w.key, w.rank,
-                                                                         w.bin_first, w.counters)));
-  }
-  if ((e = exclusive_scan<int32_t>(w.bin_first, w.bin_first, nb + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
-  if (n > 0) {
-    TPC_LAUNCH(KID_SCATTER, st,
-               (k_scatter<<<blocks_for(n, kThreads), kThreads, 0, st>>>(n, y, z, sector_row, w.key, w.rank, w.bin_first,
-                                                                       w.rec)));
-    TPC_LAUNCH(KID_CANON, st, (k_canon<<<blocks_for(nb, kThreads), kThreads, 0, st>>>(nb, w.bin_first, w.rec)));
-  }
+  if ((e = cudaMemsetAsync(w.bucket_first, 0, sizeof(int32_t) * (size_t)(kMaxBuckets + 2), st)) != cudaSuccess) return e;
+  if (n > 0)
+    TPC_LAUNCH(KID_BUCKET_HIST, st,
+               (k_bucket_hist<<<blocks_for(n, kThreads * 64, 148 * 4), kThreads, hist_smem, st>>>(
+                   g, n, sh, nbuckets, y, z, sector_row, w.bucket_first, w.counters)));
+  if ((e = exclusive_scan<int32_t>(w.bucket_first, w.bucket_first, nbuckets + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
+  if ((e = cudaMemcpyAsync(w.bucket_cursor, w.bucket_first, sizeof(int32_t) * (size_t)(nbuckets + 1), cudaMemcpyDeviceToDevice,
+                           st)) != cudaSuccess)
+    return e;
+  if (n > 0)
+    TPC_LAUNCH(KID_BUCKET_SCATTER, st,
+               (k_bucket_scatter<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, sh, y, z, sector_row, w.bucket_cursor,
+                                                                              (Rec*)w.hit_rec)));
+  TPC_LAUNCH(KID_BUCKET_SORT, st,
+             (k_bucket_sort<<<blocks_for(nbuckets, 1, 148 * 8), kThreads, sort_smem, st>>>(
+                 g, n, nb, sh, nbuckets, w.bucket_first, (const Rec*)w.hit_rec, w.rec, w.bin_first)));
   return cudaGetLastError();
 }
 

@@ -16,10 +16,10 @@
 namespace tpc {
 
 enum KernelId {
-  KID_BIN_COUNT = 0,
+  KID_BUCKET_HIST = 0,
   KID_SCAN,
-  KID_SCATTER,
-  KID_CANON,
+  KID_BUCKET_SCATTER,
+  KID_BUCKET_SORT,
   KID_NEIGHBOURS,
   KID_CLEAN,
   KID_COMPACT_STARTS,
