@@ -73,12 +73,35 @@ __device__ __noinline__ void neighbours_nested(const Rec* __restrict__ rec, cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// R9: cellular-automaton neighbour finder.  The up-window candidates are staged once in shared
-// memory (slot-major, so a warp's 16-byte accesses are conflict-free); every down-window
-// candidate is then paired with the staged ones.  The arg-min is order-independent because the
-// tie-break is explicit.
+// R9: cellular-automaton neighbour finder.  A window covers at most two z-bin rows when the cell is
+// not smaller than the window (the normal case), so both sides' bin ranges are fetched up front in one
+// round trip; candidates are then requested kCaBatch at a time and tested branch-free.  The up-window
+// candidates are staged in shared memory (slot-major: a warp's 16-byte accesses are conflict-free) and
+// every down-window candidate is paired with the staged ones.  The arg-min is order-independent because
+// the tie-break is explicit.  Windows over more than two z-bin rows, or more than kMaxCand staged
+// candidates, take the plain nested loops.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads)
+constexpr int kCaBatch = 4;
+
+struct Ranges {
+  int ka0, n0, ka1, n1;
+};
+
+__device__ __forceinline__ Ranges load_ranges(const int32_t* __restrict__ bin_first, const BinWin& W) {
+  Ranges R;
+  R.ka1 = R.n1 = 0;
+  const int e0 = __ldg(bin_first + W.first + W.ybspan);
+  R.ka0 = __ldg(bin_first + W.first);
+  if (W.nzb > 1) {
+    const int e1 = __ldg(bin_first + W.first + W.ny + W.ybspan);
+    R.ka1 = __ldg(bin_first + W.first + W.ny);
+    R.n1 = e1 - R.ka1;
+  }
+  R.n0 = e0 - R.ka0;
+  return R;
+}
+
+__global__ void __launch_bounds__(kThreads, 4)
 k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ rec, const int32_t* __restrict__ bin_first,
              int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
   __shared__ SmRow sm;
@@ -114,33 +137,55 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
       B.best = 0.0f;
       B.bui = B.bdi = 0;
       B.bu = B.bd = -1;
-      int nu = 0;
-      for (int zu = 0; zu < WU.nzb; zu++) {
-        const int b0 = WU.first + zu * WU.ny;
-        const int ka = __ldg(bin_first + b0), ke = __ldg(bin_first + b0 + WU.ybspan);
-        for (int k = ka; k < ke; k++) {
-          const Rec u = ld_rec(rec, k);
-          if (!(fabsf(u.x - yh) <= wyu && fabsf(u.y - zh) <= wzu)) continue;
-          if (nu < kMaxCand) cand[nu][tid] = make_float4(u.x, u.y, u.z, __int_as_float(k));
-          nu++;
-        }
-      }
-      if (nu > kMaxCand) {
-        neighbours_nested(rec, bin_first, WU, WD, yh, zh, wu, iy, iz, wyu, wzu, wyd, wzd, B);
-      } else if (nu > 0) {
-        for (int zd = 0; zd < WD.nzb; zd++) {
-          const int c0 = WD.first + zd * WD.ny;
-          const int ja = __ldg(bin_first + c0), je = __ldg(bin_first + c0 + WD.ybspan);
-          for (int j = ja; j < je; j++) {
-            const Rec d = ld_rec(rec, j);
-            if (!(fabsf(d.x - yh) <= wyd && fabsf(d.y - zh) <= wzd)) continue;
-            const int di = rec_idx(d);
-            for (int a = 0; a < nu; a++) {
-              const float4 u = cand[a][tid];
-              B.offer(pair_d2(yh, zh, wu, iy, iz, u.x, u.y, d.x, d.y), __float_as_int(u.z), di, __float_as_int(u.w), j);
+      bool slow = WU.nzb > 2 || WD.nzb > 2;
+      if (!slow) {
+        const Ranges RU = load_ranges(bin_first, WU), RD = load_ranges(bin_first, WD);
+        int nu = 0;
+        const int ntu = RU.n0 + RU.n1;
+        for (int i0 = 0; i0 < ntu; i0 += kCaBatch) {
+          Rec c[kCaBatch];
+          int kk[kCaBatch];
+#pragma unroll
+          for (int j = 0; j < kCaBatch; j++) {
+            const int i = min(i0 + j, ntu - 1);
+            kk[j] = i < RU.n0 ? RU.ka0 + i : RU.ka1 + (i - RU.n0);
+            c[j] = ld_rec(rec, kk[j]);
+          }
+#pragma unroll
+          for (int j = 0; j < kCaBatch; j++) {
+            if (i0 + j < ntu && fabsf(c[j].x - yh) <= wyu && fabsf(c[j].y - zh) <= wzu) {
+              if (nu < kMaxCand) cand[nu][tid] = make_float4(c[j].x, c[j].y, c[j].z, __int_as_float(kk[j]));
+              nu++;
             }
           }
         }
+        slow = nu > kMaxCand;
+        const int ntd = (nu > 0 && !slow) ? RD.n0 + RD.n1 : 0;
+        for (int i0 = 0; i0 < ntd; i0 += kCaBatch) {
+          Rec c[kCaBatch];
+          int kk[kCaBatch];
+#pragma unroll
+          for (int j = 0; j < kCaBatch; j++) {
+            const int i = min(i0 + j, ntd - 1);
+            kk[j] = i < RD.n0 ? RD.ka0 + i : RD.ka1 + (i - RD.n0);
+            c[j] = ld_rec(rec, kk[j]);
+          }
+#pragma unroll
+          for (int j = 0; j < kCaBatch; j++) {
+            if (i0 + j < ntd && fabsf(c[j].x - yh) <= wyd && fabsf(c[j].y - zh) <= wzd) {
+              const int di = rec_idx(c[j]);
+              for (int a = 0; a < nu; a++) {
+                const float4 u = cand[a][tid];
+                B.offer(pair_d2(yh, zh, wu, iy, iz, u.x, u.y, c[j].x, c[j].y), __float_as_int(u.z), di, __float_as_int(u.w),
+                        kk[j]);
+              }
+            }
+          }
+        }
+      }
+      if (slow) {
+        B.have = false;
+        neighbours_nested(rec, bin_first, WU, WD, yh, zh, wu, iy, iz, wyu, wzu, wyd, wzd, B);
       }
       if (B.have && B.best < sc.ca_cut) {
         bu = B.bu;

@@ -28,6 +28,7 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kUnroll = 4;  // independent loads in flight per thread in the streaming passes
 
 struct GridSmem {
   float ymax[kMaxRows];
@@ -68,14 +69,26 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
   const Scalars& sc = g.s;
   bool clamped = false;
   // every block takes one contiguous slice of the input (the tail of the loop keeps the warp whole for match_any)
-  const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kThreads - 1) / kThreads * kThreads;
+  const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kThreads * kUnroll - 1) / (kThreads * kUnroll) * (kThreads * kUnroll);
   const int64_t lo = (int64_t)blockIdx.x * per, hi = lo + per < n ? lo + per : n;
-  for (int64_t i0 = lo + (threadIdx.x & ~31); i0 < hi; i0 += kThreads) {
-    const int64_t i = i0 + (threadIdx.x & 31);
-    int bk = -1;
-    if (i < hi) bk = bin_of(sm, sc, __ldcs(sector_row + i), __ldcs(y + i), __ldcs(z + i), &clamped) >> bucket_shift;
-    const unsigned peers = __match_any_sync(kFull, bk);  // inputs ordered by row put a whole warp in one bucket
-    if (bk >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + bk, __popc(peers));
+  // a warp takes kUnroll x 32 consecutive clusters per iteration: all loads are issued before the first use
+  for (int64_t i0 = lo + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < hi; i0 += (int64_t)kThreads * kUnroll) {
+    int srv[kUnroll];
+    float yv[kUnroll], zv[kUnroll];
+#pragma unroll
+    for (int j = 0; j < kUnroll; j++) {
+      const int64_t i = i0 + j * 32 + (threadIdx.x & 31);
+      srv[j] = i < hi ? __ldcs(sector_row + i) : -1;
+      yv[j] = i < hi ? __ldcs(y + i) : 0.0f;
+      zv[j] = i < hi ? __ldcs(z + i) : 0.0f;
+    }
+#pragma unroll
+    for (int j = 0; j < kUnroll; j++) {
+      int bk = -1;
+      if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], &clamped) >> bucket_shift;
+      const unsigned peers = __match_any_sync(kFull, bk);  // inputs ordered by row put a whole warp in one bucket
+      if (bk >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + bk, __popc(peers));
+    }
   }
   __syncthreads();
   for (int j = threadIdx.x; j < nbuckets; j += kThreads) {
@@ -94,71 +107,101 @@ k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, con
   __syncthreads();
   const Scalars& sc = g.s;
   const int lane = threadIdx.x & 31;
-  const int64_t nround = (n + 31) & ~(int64_t)31;
-  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < nround; i += (int64_t)gridDim.x * kThreads) {
-    int bk = -1, sr = 0;
-    float yy = 0.0f, zz = 0.0f;
-    if (i < n) {
-      sr = __ldcs(sector_row + i);
-      yy = __ldcs(y + i);
-      zz = __ldcs(z + i);
-      bk = bin_of(sm, sc, sr, yy, zz, nullptr) >> bucket_shift;
+  const int64_t span = (int64_t)kThreads * kUnroll;
+  for (int64_t i0 = (int64_t)blockIdx.x * span + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < n;
+       i0 += (int64_t)gridDim.x * span) {
+    int srv[kUnroll];
+    float yv[kUnroll], zv[kUnroll];
+#pragma unroll
+    for (int j = 0; j < kUnroll; j++) {
+      const int64_t i = i0 + j * 32 + lane;
+      srv[j] = i < n ? __ldcs(sector_row + i) : -1;
+      yv[j] = i < n ? __ldcs(y + i) : 0.0f;
+      zv[j] = i < n ? __ldcs(z + i) : 0.0f;
     }
-    const unsigned peers = __match_any_sync(kFull, bk);
-    const int leader = __ffs(peers) - 1;
-    int base = 0;
-    if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
-    base = __shfl_sync(kFull, base, leader);
-    if (bk >= 0) tmp[base + __popc(peers & ((1u << lane) - 1u))] = make_float4(yy, zz, __int_as_float((int)i), __int_as_float(sr));
+#pragma unroll
+    for (int j = 0; j < kUnroll; j++) {
+      const int64_t i = i0 + j * 32 + lane;
+      int bk = -1;
+      if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift;
+      const unsigned peers = __match_any_sync(kFull, bk);
+      const int leader = __ffs(peers) - 1;
+      int base = 0;
+      if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
+      base = __shfl_sync(kFull, base, leader);
+      if (bk >= 0)
+        tmp[base + __popc(peers & ((1u << lane) - 1u))] = make_float4(yv[j], zv[j], __int_as_float((int)i), __int_as_float(srv[j]));
+    }
   }
 }
 
 // One block per bucket (grid-stride).  cnt[] holds, in turn: bin counts, exclusive offsets, running cursors
 // (= end offsets once every record is placed).
-__global__ void __launch_bounds__(kThreads)
+constexpr int kSortThreads = 512;
+
+__global__ void __launch_bounds__(kSortThreads)
 k_bucket_sort(const __grid_constant__ Geo g, int64_t n, int64_t nb, int bucket_shift, int nbuckets,
               const int32_t* __restrict__ bucket_first, const Rec* __restrict__ tmp, Rec* rec, int32_t* __restrict__ bin_first) {
   extern __shared__ int32_t cnt[];  // [pad32(bucket bins)]
   __shared__ GridSmem sm;
-  __shared__ int32_t scan_sm[kThreads / 32 + 1];
+  __shared__ int32_t scan_sm[kSortThreads / 32 + 1];
   load_grid_rows(sm, g);
   const Scalars& sc = g.s;
   const int bbins = 1 << bucket_shift;
-  const int per_thread = bbins / kThreads;  // bucket bins are a multiple of 32 * kThreads... (>= 8192)
+  const int per_thread = bbins / kSortThreads;  // bucket bins are a power of two >= 8192
+  const int tid = threadIdx.x;
   for (int b = blockIdx.x; b < nbuckets; b += gridDim.x) {
     const int start = bucket_first[b], end = bucket_first[b + 1];
     const int64_t bin0 = (int64_t)b << bucket_shift;
     const int nbins = (int)((nb - bin0) < bbins ? (nb - bin0) : bbins);
-    __syncthreads();  // previous bucket's canon pass is done with cnt[]
-    for (int j = threadIdx.x; j < bbins; j += kThreads) cnt[pad32(j)] = 0;
+    __syncthreads();  // previous bucket's re-ordering pass is done with cnt[]
+    for (int j = tid; j < bbins; j += kSortThreads) cnt[pad32(j)] = 0;
     __syncthreads();
-    for (int i = start + threadIdx.x; i < end; i += kThreads) {
-      const Rec r = tmp[i];
-      atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r), r.x, r.y, nullptr) - (int)bin0), 1);
+    for (int i0 = start + tid; i0 < end; i0 += kSortThreads * kUnroll) {
+      Rec r[kUnroll];
+#pragma unroll
+      for (int j = 0; j < kUnroll; j++) {
+        const int i = i0 + j * kSortThreads;
+        r[j] = tmp[i < end ? i : end - 1];
+      }
+#pragma unroll
+      for (int j = 0; j < kUnroll; j++)
+        if (i0 + j * kSortThreads < end)
+          atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r[j]), r[j].x, r[j].y, nullptr) - (int)bin0), 1);
     }
     __syncthreads();
     // exclusive scan over the bucket's bins, thread t owns bins [t*per_thread, (t+1)*per_thread)
     int acc = 0;
-    for (int k = 0; k < per_thread; k++) acc += cnt[pad32(threadIdx.x * per_thread + k)];
+    for (int k = 0; k < per_thread; k++) acc += cnt[pad32(tid * per_thread + k)];
     int total;
-    int ex = block_excl_scan<int, kThreads>(acc, &total, scan_sm);
+    int ex = block_excl_scan<int, kSortThreads>(acc, &total, scan_sm);
     for (int k = 0; k < per_thread; k++) {
-      const int j = threadIdx.x * per_thread + k;
+      const int j = tid * per_thread + k;
       const int c = cnt[pad32(j)];
       cnt[pad32(j)] = ex;
-      if (j < nbins) bin_first[bin0 + j] = start + ex;
       ex += c;
     }
-    if (b == nbuckets - 1 && threadIdx.x == 0) bin_first[nb] = (int)n;
     __syncthreads();
-    for (int i = start + threadIdx.x; i < end; i += kThreads) {
-      const Rec r = tmp[i];
-      const int pos = atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r), r.x, r.y, nullptr) - (int)bin0), 1);
-      rec[start + pos] = r;
+    for (int j = tid; j < nbins; j += kSortThreads) bin_first[bin0 + j] = start + cnt[pad32(j)];  // coalesced
+    if (b == nbuckets - 1 && tid == 0) bin_first[nb] = (int)n;
+    __syncthreads();
+    for (int i0 = start + tid; i0 < end; i0 += kSortThreads * kUnroll) {
+      Rec r[kUnroll];
+#pragma unroll
+      for (int j = 0; j < kUnroll; j++) {
+        const int i = i0 + j * kSortThreads;
+        r[j] = tmp[i < end ? i : end - 1];
+      }
+#pragma unroll
+      for (int j = 0; j < kUnroll; j++)
+        if (i0 + j * kSortThreads < end) {
+          const int pos = atomicAdd(cnt + pad32(bin_of(sm, sc, rec_sr(r[j]), r[j].x, r[j].y, nullptr) - (int)bin0), 1);
+          rec[start + pos] = r[j];
+        }
     }
     __syncthreads();  // the block's own global writes are visible to it from here on
     // bins with >= 2 clusters: insertion sort by original index (max occupancy seen on the configs: 17)
-    for (int j = threadIdx.x; j < nbins; j += kThreads) {
+    for (int j = tid; j < nbins; j += kSortThreads) {
       const int a = start + (j ? cnt[pad32(j - 1)] : 0), e = start + cnt[pad32(j)];
       for (int i = a + 1; i < e; i++) {
         const Rec v = rec[i];
@@ -218,10 +261,10 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
     return e;
   if (n > 0)
     TPC_LAUNCH(KID_BUCKET_SCATTER, st,
-               (k_bucket_scatter<<<blocks_for(n, kThreads), kThreads, 0, st>>>(g, n, sh, y, z, sector_row, w.bucket_cursor,
+               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll), kThreads, 0, st>>>(g, n, sh, y, z, sector_row, w.bucket_cursor,
                                                                               (Rec*)w.hit_rec)));
   TPC_LAUNCH(KID_BUCKET_SORT, st,
-             (k_bucket_sort<<<blocks_for(nbuckets, 1, 148 * 8), kThreads, sort_smem, st>>>(
+             (k_bucket_sort<<<blocks_for(nbuckets, 1, 148 * 4), kSortThreads, sort_smem, st>>>(
                  g, n, nb, sh, nbuckets, w.bucket_first, (const Rec*)w.hit_rec, w.rec, w.bin_first)));
   return cudaGetLastError();
 }
