@@ -35,6 +35,9 @@ constexpr unsigned kFull = 0xffffffffu;
 #endif
 constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
 
+// L1 prefetch of one line: the follower knows one step ahead roughly where it will look.
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
 __global__ void __launch_bounds__(kFollowThreads, TPC_FOLLOW_MIN_BLOCKS)
@@ -59,6 +62,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   int misses = 0, nh = 0, lo = 0, hi = 0;
   unsigned nprop = 0, nupd = 0, ncand = 0;
   int32_t* my_hits = row_hit;
+  int pf_ka = -1;  // first grid position of the bin the NEXT step is expected to search (-1: no prediction)
 #pragma unroll
   for (int k = 0; k < 5; k++) st.p[k] = 0.0f;
 #pragma unroll
@@ -81,6 +85,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
           const float4 a = __ldg(ip), b = __ldg(ip + 1);
           p0 = __float_as_int(b.x);
           hn = __float_as_int(b.y);
+          prefetch_l1(rec + hn);
           const int sr0 = __float_as_int(b.z);
           orig0 = __float_as_int(b.w);
           s = sr0 / nrows;
@@ -113,46 +118,62 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     if (leg) rn = r;
     int nxt = -1;
     if (chain) nxt = __ldg(up_c + hn);
+    // the bin offset requested during the previous step has arrived by now: pull the records it points to
+    // into L1 while the transport below is computed
+    if (pf_ka >= 0) prefetch_l1(rec + pf_ka);
+    pf_ka = -1;
     // ---- R12 transport (one copy for every phase; __syncwarp keeps the compiler from cloning it
     //      into the phase branches, which would serialise the lanes again) --------------------------
     __syncwarp();
-    KState nx = st;
     bool ok = phase != PH_DONE;
-    if (ok && !isI) {
-      ok = propagate(nx, sm.X[rn] - sm.X[r_at], kB, ms);
-      if (ok) nprop++;
+    const bool moved = ok && !isI;
+    Transport T;
+    float yp = st.p[0], dzp = st.p[1];
+    float C00n = st.C[TPC_CI(0, 0)], C10n = st.C[TPC_CI(1, 0)], C11n = st.C[TPC_CI(1, 1)];
+    if (moved) {
+      ok = transport_state(st, sm.X[rn] - sm.X[r_at], kB, ms, T);
+      if (ok) {
+        nprop++;
+        yp = T.y;
+        dzp = T.dz;
+        transport_cov_diag(st, T, C00n, C11n);
+        C10n = transport_cov_10(st, T);
+      }
     }
-    const Innov I = innovation(nx, sy2, sz2);
     // ---- candidates of this step: up to two contiguous ranges of grid positions -------------------
     //   chain step (R15): the linked cluster alone, no window;  leg step (R16): the bins covering the
     //   chi2 window (a superset, every candidate is re-tested in cm);  init / jump: none.
-    const float yp = nx.p[0], dzp = nx.p[1];
+    // The bin offsets are requested here, as soon as the predicted position and its two variances are
+    // known; the rest of F C F^T below runs while they are in flight.
     float wy = 3.0e38f, wz = 3.0e38f;
-    int ka0 = 0, n0 = 0, ka1 = 0, n1 = 0;
+    int ka0 = 0, e0 = 0, ka1 = 0, e1 = 0;  // [ka, e) per range; the differences are taken after the covariance math
     bool edge_out = false, many = false;
     BinWin W;
     W.first = W.ny = W.ybspan = W.nzb = 0;
     if (chain && ok) {
       ka0 = hn;
-      n0 = 1;
+      e0 = hn + 1;
     } else if (leg && ok) {
       edge_out = fabsf(yp) > sm.ymax[rn] + sc.edge_margin;
       if (!edge_out) {
-        wy = fminf(sqrtf(sc.chi2_cut * I.S00), sc.win_max);
-        wz = fminf(sqrtf(sc.chi2_cut * I.S11), sc.win_max);
+        wy = fminf(sqrtf(sc.chi2_cut * (C00n + sy2)), sc.win_max);
+        wz = fminf(sqrtf(sc.chi2_cut * (C11n + sz2)), sc.win_max);
         const float zc = zref + dzp;
         W = bin_window(sm, sc, s, rn, yp - wy, yp + wy, zc - wz, zc + wz);
-        const int e0 = __ldg(bin_first + W.first + W.ybspan);
+        e0 = __ldg(bin_first + W.first + W.ybspan);
         ka0 = __ldg(bin_first + W.first);
         if (W.nzb > 1) {
-          const int e1 = __ldg(bin_first + W.first + W.ny + W.ybspan);
+          e1 = __ldg(bin_first + W.first + W.ny + W.ybspan);
           ka1 = __ldg(bin_first + W.first + W.ny);
-          n1 = e1 - ka1;
         }
-        n0 = e0 - ka0;
         many = W.nzb > 2;
       }
     }
+    // innovation covariance of the PREDICTED state from the three elements of C' it depends on: the search
+    // and the chain cut are decided before the transport is committed, so a rejected chain step (R15) simply
+    // never commits and no copy of the state is kept
+    const Innov I = innovation3(C00n, C10n, C11n, sy2, sz2);
+    const int n0 = e0 - ka0, n1 = e1 - ka1;
     // ---- arg-min chi2 over the candidates (ties: lowest original index) ----------------------------
     __syncwarp();
     bool have = false;
@@ -170,20 +191,54 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
         kk[j] = i < n0 ? ka0 + i : ka1 + (i - n0);
         c[j] = ld_rec(rec, kk[j]);
       }
+      // window test per slot (cheap); the chi2 arithmetic runs once, on the first slot inside the window --
+      // nearly always the only one -- and a rare second round takes the others.
+      unsigned inmask = 0u;
+      int first_in = kBatch;
 #pragma unroll
-      for (int j = 0; j < kBatch; j++) {
+      for (int j = kBatch - 1; j >= 0; j--) {
         const float q0 = c[j].x - yp, q1 = (c[j].y - zref) - dzp;
-        const bool in = (i0 + j < ntot) && fabsf(q0) <= wy && fabsf(q1) <= wz;
-        const float chi2 = chi2_of(I, q0, q1);
-        const int ci = rec_idx(c[j]);
-        if (in && leg) ncand++;
-        if (in && (!have || chi2 < best || (chi2 == best && ci < bi))) {
+        if ((i0 + j < ntot) && fabsf(q0) <= wy && fabsf(q1) <= wz) {
+          inmask |= 1u << j;
+          first_in = j;
+        }
+      }
+      if (leg) ncand += __popc(inmask);
+      Rec cs = c[0];
+      int ks = kk[0];
+#pragma unroll
+      for (int j = 1; j < kBatch; j++)
+        if (first_in == j) {
+          cs = c[j];
+          ks = kk[j];
+        }
+      if (inmask) {
+        const float chi2 = chi2_of(I, cs.x - yp, (cs.y - zref) - dzp);
+        const int ci = rec_idx(cs);
+        if (!have || chi2 < best || (chi2 == best && ci < bi)) {
           have = true;
           best = chi2;
           bi = ci;
-          bk = kk[j];
-          by = c[j].x;
-          bz = c[j].y;
+          bk = ks;
+          by = cs.x;
+          bz = cs.y;
+        }
+      }
+      if (inmask & (inmask - 1u)) {  // more than one slot inside the window
+#pragma unroll
+        for (int j = 1; j < kBatch; j++) {
+          if (((inmask >> j) & 1u) && j != first_in) {
+            const float chi2 = chi2_of(I, c[j].x - yp, (c[j].y - zref) - dzp);
+            const int ci = rec_idx(c[j]);
+            if (!have || chi2 < best || (chi2 == best && ci < bi)) {
+              have = true;
+              best = chi2;
+              bi = ci;
+              bk = kk[j];
+              by = c[j].x;
+              bz = c[j].y;
+            }
+          }
         }
       }
     }
@@ -223,12 +278,28 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
       mz = bz - zref;
       mk = bk;
     }
+    // ---- look one step ahead (prefetch only: nothing below depends on it) ---------------------------
+    //   next chain cluster: its record;  next row of a leg (or the first row after the chain): the bin at the
+    //   linearly extrapolated position -- its offset is loaded now (in flight during the update) and the
+    //   records behind it are prefetched at the top of the next iteration.  st still holds the state at the
+    //   previous row here, so the slope costs two subtractions.
+    if (chain && upd && nxt >= 0) prefetch_l1(rec + nxt);
+    if (moved && ok && !isJ) {
+      const int r2 = rn + ((phase == PH_DOWN) ? -1 : 1);
+      if (r2 >= 0 && r2 < nrows) {
+        const float y2 = yp + (yp - st.p[0]);
+        const float z2 = zref + (dzp + (dzp - st.p[1]));
+        const float zeta = (s < 18) ? z2 : -z2;
+        const int ny2 = sm.ny[r2];
+        const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
+        const int yb = clampbin((y2 + sm.ymax[r2]) * sc.inv_cy, ny2);
+        pf_ka = __ldg(bin_first + (s * sc.bins_per_sector + sm.rowbase[r2] + zb * ny2 + yb));
+      }
+    }
     // ---- commit the transport, R13 update (one copy for every phase) --------------------------------
     __syncwarp();
-    if (ok) {
-      st = nx;
-      r_at = rn;
-    }
+    if (moved && ok) transport_apply(st, T);
+    if (ok) r_at = rn;
     if (upd) {
       update(st, I, my, mz);
       nupd++;

@@ -48,9 +48,20 @@ __device__ __forceinline__ float asin_ratio(float u) {
   return (float)(asin(ud) / ud);
 }
 
-// R12: exact helix transport x -> x + dx with Jacobian; C' = F C F^T (no process noise, R6).
-// Returns false and leaves the state untouched when |sinphi| would exceed max_sinphi.
-__device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float max_sinphi) {
+// R12: exact helix transport x -> x + dx, in three pieces so that a caller can start its memory lookups
+// as soon as the predicted position and its variances are known and do the rest of F C F^T while they fly:
+//   transport_state     new (y, dz, sinphi) and the non-trivial Jacobian terms; false (nothing usable) when
+//                       |sinphi| would exceed max_sinphi
+//   transport_cov_diag  the (0,0) and (1,1) elements of C' = F C F^T (what the R16 search window needs)
+//   transport_apply     commits the state and the full C' (no process noise, R6)
+// propagate() = the three in sequence.  The expressions are the same in every piece, so a value computed
+// twice is the same value (and the compiler merges them).
+struct Transport {
+  float y, dz, s2;
+  float f02, f04, f12, f13, f14, f24;
+};
+
+__device__ __forceinline__ bool transport_state(const KState& st, float dx, float kB, float max_sinphi, Transport& T) {
   const float y = st.p[0], dz = st.p[1], s1 = st.p[2], tl = st.p[3], q = st.p[4];
   const float kappa = -(kB * q);  // R4
   const float s2 = s1 + kappa * dx;
@@ -63,12 +74,12 @@ __device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float 
   const float arc = L * asin_ratio(u);        // signed arc length in the bending plane
   const float g = (1.0f + c1 * c2) + s1 * s2;
   const float c1c2 = c1 * c2;
-  const float f02 = (dx * g) / (cc * c1c2);                    // dy'/dsinphi
-  const float f04 = -((kB * (dx * dx)) * g) / (c2 * (cc * cc));  // dy'/dq
-  const float f12 = ((tl * dx) * t) / c1c2;                    // ddz'/dsinphi
-  const float f13 = arc;                                       // ddz'/dtanl
-  const float f24 = -(kB * dx);                                // dsinphi'/dq
-  float E;                                                     // d(arc)/d(kappa), series near 0
+  T.f02 = (dx * g) / (cc * c1c2);                    // dy'/dsinphi
+  T.f04 = -((kB * (dx * dx)) * g) / (c2 * (cc * cc));  // dy'/dq
+  T.f12 = ((tl * dx) * t) / c1c2;                    // ddz'/dsinphi
+  T.f13 = arc;                                       // ddz'/dtanl
+  T.f24 = -(kB * dx);                                // dsinphi'/dq
+  float E;                                           // d(arc)/d(kappa), series near 0
   if (fabsf(kappa * dx) < 1e-3f) {
     const float c1_2 = c1 * c1, c1_3 = c1_2 * c1, c1_5 = c1_3 * c1_2;
     E = ((dx * dx) * s1) / (2.0f * c1_3) +
@@ -76,25 +87,48 @@ __device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float 
   } else {
     E = (dx / c2 - arc) / kappa;
   }
-  const float f14 = -((kB * tl) * E);  // ddz'/dq
-  st.p[0] = y + dx * t;
-  st.p[1] = dz + tl * arc;
-  st.p[2] = s2;
+  T.f14 = -((kB * tl) * E);  // ddz'/dq
+  T.y = y + dx * t;
+  T.dz = dz + tl * arc;
+  T.s2 = s2;
+  return true;
+}
+
+// row 0 and row 1 of M = F C
+__device__ __forceinline__ float tr_m0(const KState& st, const Transport& T, int j) {
+  return (csym(st.C, 0, j) + T.f02 * csym(st.C, 2, j)) + T.f04 * csym(st.C, 4, j);
+}
+__device__ __forceinline__ float tr_m1(const KState& st, const Transport& T, int j) {
+  return ((csym(st.C, 1, j) + T.f12 * csym(st.C, 2, j)) + T.f13 * csym(st.C, 3, j)) + T.f14 * csym(st.C, 4, j);
+}
+
+__device__ __forceinline__ void transport_cov_diag(const KState& st, const Transport& T, float& C00, float& C11) {
+  C00 = (tr_m0(st, T, 0) + tr_m0(st, T, 2) * T.f02) + tr_m0(st, T, 4) * T.f04;
+  C11 = ((tr_m1(st, T, 1) + tr_m1(st, T, 2) * T.f12) + tr_m1(st, T, 3) * T.f13) + tr_m1(st, T, 4) * T.f14;
+}
+// ... and the (1,0) element: with the two above, everything the innovation covariance S (R13) needs
+__device__ __forceinline__ float transport_cov_10(const KState& st, const Transport& T) {
+  return (tr_m1(st, T, 0) + tr_m1(st, T, 2) * T.f02) + tr_m1(st, T, 4) * T.f04;
+}
+
+__device__ __forceinline__ void transport_apply(KState& st, const Transport& T) {
+  const float f02 = T.f02, f04 = T.f04, f12 = T.f12, f13 = T.f13, f14 = T.f14, f24 = T.f24;
   // M = F C (rows 0,1,2 differ from C), then N = M F^T, lower triangle.
   float M0[5], M1[5], M2[5];
 #pragma unroll
   for (int j = 0; j < 5; j++) {
-    const float C0j = csym(st.C, 0, j), C1j = csym(st.C, 1, j), C2j = csym(st.C, 2, j), C3j = csym(st.C, 3, j),
-                C4j = csym(st.C, 4, j);
-    M0[j] = (C0j + f02 * C2j) + f04 * C4j;
-    M1[j] = ((C1j + f12 * C2j) + f13 * C3j) + f14 * C4j;
-    M2[j] = C2j + f24 * C4j;
+    M0[j] = tr_m0(st, T, j);
+    M1[j] = tr_m1(st, T, j);
+    M2[j] = csym(st.C, 2, j) + f24 * csym(st.C, 4, j);
   }
   // rows 3 and 4 of M are rows 3 and 4 of C
   const float M30 = st.C[TPC_CI(3, 0)], M31 = st.C[TPC_CI(3, 1)], M32 = st.C[TPC_CI(3, 2)], M33 = st.C[TPC_CI(3, 3)],
               M34 = st.C[TPC_CI(4, 3)];
   const float M40 = st.C[TPC_CI(4, 0)], M41 = st.C[TPC_CI(4, 1)], M42 = st.C[TPC_CI(4, 2)], M43 = st.C[TPC_CI(4, 3)],
               M44 = st.C[TPC_CI(4, 4)];
+  st.p[0] = T.y;
+  st.p[1] = T.dz;
+  st.p[2] = T.s2;
   st.C[TPC_CI(0, 0)] = (M0[0] + M0[2] * f02) + M0[4] * f04;
   st.C[TPC_CI(1, 0)] = (M1[0] + M1[2] * f02) + M1[4] * f04;
   st.C[TPC_CI(1, 1)] = ((M1[1] + M1[2] * f12) + M1[3] * f13) + M1[4] * f14;
@@ -110,6 +144,13 @@ __device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float 
   st.C[TPC_CI(4, 2)] = M42 + M44 * f24;
   st.C[TPC_CI(4, 3)] = M43;
   st.C[TPC_CI(4, 4)] = M44;
+}
+
+// Returns false and leaves the state untouched when |sinphi| would exceed max_sinphi.
+__device__ __forceinline__ bool propagate(KState& st, float dx, float kB, float max_sinphi) {
+  Transport T;
+  if (!transport_state(st, dx, kB, max_sinphi, T)) return false;
+  transport_apply(st, T);
   return true;
 }
 
@@ -118,17 +159,22 @@ struct Innov {
   float S00, S01, S11, Si00, Si01, Si11;
 };
 
-__device__ __forceinline__ Innov innovation(const KState& st, float sy2, float sz2) {
+// from the three covariance elements it depends on (so that it can be formed before C' is committed)
+__device__ __forceinline__ Innov innovation3(float C00, float C10, float C11, float sy2, float sz2) {
   Innov I;
-  I.S00 = st.C[TPC_CI(0, 0)] + sy2;
-  I.S01 = st.C[TPC_CI(1, 0)];
-  I.S11 = st.C[TPC_CI(1, 1)] + sz2;
+  I.S00 = C00 + sy2;
+  I.S01 = C10;
+  I.S11 = C11 + sz2;
   const float det = I.S00 * I.S11 - I.S01 * I.S01;
   const float idet = 1.0f / det;
   I.Si00 = I.S11 * idet;
   I.Si01 = -(I.S01 * idet);
   I.Si11 = I.S00 * idet;
   return I;
+}
+
+__device__ __forceinline__ Innov innovation(const KState& st, float sy2, float sz2) {
+  return innovation3(st.C[TPC_CI(0, 0)], st.C[TPC_CI(1, 0)], st.C[TPC_CI(1, 1)], sy2, sz2);
 }
 
 __device__ __forceinline__ float chi2_of(const Innov& I, float r0, float r1) {
