@@ -58,6 +58,13 @@ KERNEL_MODEL = {
 }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
+# launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
+NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 3.92, "k_bucket_sort": 6.86, "k_neighbours": 6.55,
+                     "k_clean": 2.25, "k_compact_starts": 2.06, "k_follow": 11.56, "k_push_keys": 6.24,
+                     "k_count_kept": 6.16, "k_write_tracks": 23.92, "k_fit": 4.89}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -197,6 +204,21 @@ def load_peaks():
         return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
+def reduce_over_ranks(ms_step: float, t_e2e: float, n_clusters: int, world: int, device):
+    """TF-level replicas: the job's step time is the MAX over ranks, its work the SUM of the ranks'
+    clusters.  The only collectives of a multi-GPU run; `device` is the tensor device of the process group's
+    backend (cuda for nccl, cpu for the gloo test in tests/test_multirank_gloo.py)."""
+    if world <= 1:
+        return ms_step, t_e2e, float(n_clusters)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_step, t_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([float(n_clusters)], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(c[0])
+
+
 def run_ours(args, rank: int, local_rank: int, world: int):
     import torch
     import torch.distributed as dist
@@ -265,15 +287,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         assert int(trk.counters_host[binding.CNT_TRACKS]) == K_tracks
 
     # ---- max over ranks ----------------------------------------------------------------------------
-    ms_step = ms_total / args.steps
-    tot_clusters = float(n)
-    if world > 1:
-        t = torch.tensor([ms_step, t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step, t_e2e = float(t[0]), float(t[1])
-        c = torch.tensor([float(n)], dtype=torch.float64, device=dev)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        tot_clusters = float(c[0])
+    ms_step, t_e2e, tot_clusters = reduce_over_ranks(ms_total / args.steps, t_e2e, n, world, dev)
     if rank != 0:
         return
 
@@ -290,6 +304,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     units = {"cluster": n, "bin": nb, "tracklet": int(res["counters"][binding.CNT_TRACKLETS]), "claim": work["updates"],
              "hit": n_hits}
     roofline = kernel_roofline(top, top_ms, units, work, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
+    if args.config == 4 and top in NCU_TRAFFIC_GB_C4:
+        roofline["traffic"] = NCU_TRAFFIC_GB_C4[top] * 1e9
+        roofline["traffic_source"] = "profiles/r01_ncu_summary.md (ncu dram__bytes_read.sum + dram__bytes_write.sum)"
     for k in kern:       # every kernel's own fraction of its roof, so that the table can be read without DESIGN.md
         r = kernel_roofline(k, kern[k]["ms_per_step"] / max(kern[k]["launches_per_step"], 1) *
                             (kern[k]["launches_per_step"] if k == "k_scan_*" else 1), units, work,
