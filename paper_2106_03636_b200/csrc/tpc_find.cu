@@ -170,14 +170,42 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
             kk[j] = i < RD.n0 ? RD.ka0 + i : RD.ka1 + (i - RD.n0);
             c[j] = ld_rec(rec, kk[j]);
           }
+          // window test per slot; the pair arithmetic runs once, for the first slot inside the window (nearly
+          // always the only one), and a rare second round takes the others
+          unsigned inmask = 0u;
+          int first_in = kCaBatch;
 #pragma unroll
-          for (int j = 0; j < kCaBatch; j++) {
+          for (int j = kCaBatch - 1; j >= 0; j--) {
             if (i0 + j < ntd && fabsf(c[j].x - yh) <= wyd && fabsf(c[j].y - zh) <= wzd) {
-              const int di = rec_idx(c[j]);
-              for (int a = 0; a < nu; a++) {
-                const float4 u = cand[a][tid];
-                B.offer(pair_d2(yh, zh, wu, iy, iz, u.x, u.y, c[j].x, c[j].y), __float_as_int(u.z), di, __float_as_int(u.w),
-                        kk[j]);
+              inmask |= 1u << j;
+              first_in = j;
+            }
+          }
+          Rec ds = c[0];
+          int ks = kk[0];
+#pragma unroll
+          for (int j = 1; j < kCaBatch; j++)
+            if (first_in == j) {
+              ds = c[j];
+              ks = kk[j];
+            }
+          if (inmask) {
+            const int di = rec_idx(ds);
+            for (int a = 0; a < nu; a++) {
+              const float4 u = cand[a][tid];
+              B.offer(pair_d2(yh, zh, wu, iy, iz, u.x, u.y, ds.x, ds.y), __float_as_int(u.z), di, __float_as_int(u.w), ks);
+            }
+          }
+          if (inmask & (inmask - 1u)) {
+#pragma unroll
+            for (int j = 1; j < kCaBatch; j++) {
+              if (((inmask >> j) & 1u) && j != first_in) {
+                const int di = rec_idx(c[j]);
+                for (int a = 0; a < nu; a++) {
+                  const float4 u = cand[a][tid];
+                  B.offer(pair_d2(yh, zh, wu, iy, iz, u.x, u.y, c[j].x, c[j].y), __float_as_int(u.z), di,
+                          __float_as_int(u.w), kk[j]);
+                }
               }
             }
           }

@@ -73,6 +73,30 @@ def test_fit_gather_path_is_bit_identical(torch_cuda):
         assert np.array_equal(a[k], b[k]), k
 
 
+def test_row_ordered_input_matches_oracle(torch_cuda, orc):
+    """Inputs ordered by (sector, row) -- the order a clusterizer delivers -- put whole warps into one grid bucket
+    (the warp-aggregated atomics of the grid build); the result must equal the oracle's on the same ordering."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(1, n_tracks=1500)
+    order = np.argsort(ev.sector_row, kind="stable")
+    y, z, sr = ev.y[order].copy(), ev.z[order].copy(), ev.sector_row[order].copy()
+    o = orc.run(ev.params, y, z, sr, "f32", True)
+    trk = binding.Tracker(ev.params, y.size)
+    res = trk.run(torch_cuda.from_numpy(y).cuda(), torch_cuda.from_numpy(z).cuda(), torch_cuda.from_numpy(sr).cuda())
+    sidx, bfirst = trk.grid_export()
+    parity.compare_grid(o, sidx, bfirst)
+    st = parity.compare_tracks(o, res, y.size)
+    parity.assert_contract(st, exact_count=True)
+    assert st["assign_identical"] == y.size and st["par_bit_identical"] and st["cov_bit_identical"]
+
+
+def test_max_tracklets_limit_is_an_argument_error(torch_cuda):
+    from paper_2106_03636_b200 import binding
+    ev = config0()
+    with pytest.raises(binding.TpcError):
+        binding.workspace_bytes(ev.params, ev.n, binding.TPC_MAX_TRACKLETS + 1)
+
+
 def test_config0_golden_counts(torch_cuda, orc):
     """tests/golden/config0_oracle_summary.txt (written from the oracle alone) against the CUDA path."""
     import os
