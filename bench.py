@@ -274,17 +274,29 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     n_hits = int(res["counters"][binding.CNT_HITS])
 
     # ---- end to end through the host-buffer entry point -----------------------------------------
+    # Two Time Frames in flight (two Tracker contexts, own workspace / staging / pinned outputs, one stream each):
+    # the H2D copy of one TF overlaps the tracking of the previous one and the D2H of the one before -- the
+    # steady state of a continuous TF stream.  Every step still copies its inputs from
+    # pinned host memory and reads counters + cluster_track + parameters back inside the timed region.
     t_e2e, h2d, d2h = 0.0, 0, 0
     if not args.no_e2e:
-        trk.make_host_staging()
-        trk.track_host(hy, hz, hs)                       # warm-up (first-touch of the staging buffers)
+        ctx = [trk, binding.Tracker(ev.params, n, device=dev)]
+        streams = [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
+        for c, st in zip(ctx, streams):
+            c.make_host_staging()
+            with torch.cuda.stream(st):
+                c.track_host(hy, hz, hs)                 # warm-up (first-touch of the staging buffers), synchronous
         barrier(); torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
-            h2d, d2h = trk.track_host(hy, hz, hs)        # synchronises before returning
-        torch.cuda.synchronize()
+        for i in range(args.steps):
+            with torch.cuda.stream(streams[i % 2]):
+                h2d, d2h = ctx[i % 2].track_host(hy, hz, hs, sync=False)
+        for st in streams:
+            st.synchronize()
         t_e2e = (time.perf_counter() - t0) / args.steps
-        assert int(trk.counters_host[binding.CNT_TRACKS]) == K_tracks
+        for c in ctx[:min(args.steps, 2)]:
+            assert int(c.counters_host[binding.CNT_TRACKS]) == K_tracks
+        del ctx
 
     # ---- max over ranks ----------------------------------------------------------------------------
     ms_step, t_e2e, tot_clusters = reduce_over_ranks(ms_total / args.steps, t_e2e, n, world, dev)
@@ -325,7 +337,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "clocks": clocks, "gpu_launches": launches, "kernels": kern, "roofline": roofline}
     if not args.no_e2e:
         out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
-                      "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3}
+                      "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3,
+                      "pipeline": "tpc_track_host_async, 2 Time Frames in flight on 2 streams (own workspace, staging and "
+                                  "pinned outputs each); wall clock over the K steps incl. pipeline fill"}
     if world == 1 and not args.no_cpu_baseline:
         ys, zs, ss, desc = oracle_sample(ev, 1_500_000)
         dt, ntr = time_oracle(ev, ys, zs, ss, 1, 0)

@@ -191,6 +191,20 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
                    float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
                    int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
 
+/* Same work as tpc_track_host, enqueue only: returns without synchronising, so that a caller with two sets of
+ * buffers on two streams can overlap the host->device copy of one Time Frame with the tracking of the previous
+ * one and the device->host copy of the one before (the TF stream is continuous and GPU
+ * memory is reused between steps).  The host buffers must be pinned and stay untouched until `stream` has
+ * passed this call's work (cudaStreamSynchronize / an event). */
+int tpc_track_host_async(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                         int64_t max_tracks, const float* y_host, const float* z_host,
+                         const int32_t* sector_row_host, float* y_dev, float* z_dev, int32_t* sector_row_dev,
+                         void* workspace, size_t ws_bytes, int32_t* cluster_track_dev, int32_t* trk_seed_dev,
+                         int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
+                         int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev,
+                         float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
+                         int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
+
 /* ---- measurement support (bench.py `roofline`, `gpu_launches`) --------------------------------
  * The library counts every kernel it launches, per kernel id, and can bracket each launch with a
  * cudaEvent pair recorded on the launching stream.  Host-side state, one driving thread per GPU

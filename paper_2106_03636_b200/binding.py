@@ -27,7 +27,7 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_host", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
+           "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
 
 
 class tpc_params_t(C.Structure):
@@ -287,13 +287,15 @@ class Tracker:
         self.cluster_track_host = t.empty(n1, dtype=t.int32).pin_memory()
         self.par_host = t.empty((5, self.max_tracks), dtype=t.float32).pin_memory()
 
-    def track_host(self, y_host, z_host, sr_host):
-        """tpc_track_host: H2D of the inputs, a1..a6, D2H of counters + cluster_track + track parameters; synchronous."""
+    def track_host(self, y_host, z_host, sr_host, sync: bool = True):
+        """tpc_track_host: H2D of the inputs, a1..a6, D2H of counters + cluster_track + track parameters.
+        sync=False calls tpc_track_host_async (enqueue only on the current stream)."""
         for a in (y_host, z_host, sr_host):
             assert not a.is_cuda and a.is_contiguous() and a.numel() == self.n
         hp = lambda a: C.c_void_p(a.data_ptr())
         self._inputs = (self._y_dev, self._z_dev, self._sr_dev)
-        _check(self.lib.tpc_track_host(
+        fn = self.lib.tpc_track_host if sync else self.lib.tpc_track_host_async
+        _check(fn(
             C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), C.c_int64(self.max_tracks),
             hp(y_host), hp(z_host), hp(sr_host), _dp(self._y_dev), _dp(self._z_dev), _dp(self._sr_dev),
             _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(self.cluster_track), _dp(self.trk_seed),

@@ -290,7 +290,7 @@ int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
-int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
+int tpc_track_host_async(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
                    const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
                    int32_t* sector_row_dev, void* workspace, size_t ws_bytes, int32_t* cluster_track_dev,
                    int32_t* trk_seed_dev, int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
@@ -326,8 +326,24 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
   if (par_host)
     if ((e = cudaMemcpyAsync(par_host, par_dev, sizeof(float) * 5 * (size_t)max_tracks, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
       return cuda_fail(e);
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
   return TPC_OK;
+}
+
+int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
+                   const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
+                   int32_t* sector_row_dev, void* workspace, size_t ws_bytes, int32_t* cluster_track_dev,
+                   int32_t* trk_seed_dev, int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
+                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev, float* xref_dev,
+                   float* zref_dev, float* chi2_dev, int32_t* ndf_dev, int32_t* counters_host,
+                   int32_t* cluster_track_host, float* par_host, void* stream) {
+  const int rc = tpc_track_host_async(params_host, n_clusters, max_tracklets, max_tracks, y_host, z_host, sector_row_host, y_dev,
+                                      z_dev, sector_row_dev, workspace, ws_bytes, cluster_track_dev, trk_seed_dev,
+                                      trk_sector_dev, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, counters_dev, par_dev,
+                                      cov_dev, xref_dev, zref_dev, chi2_dev, ndf_dev, counters_host, cluster_track_host,
+                                      par_host, stream);
+  if (rc != TPC_OK) return rc;
+  const cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
 }  // extern "C"

@@ -230,3 +230,16 @@ def test_host_buffer_entry_point(torch_cuda, orc):
     assert K == ref["trk_seed"].size
     assert np.array_equal(trk2.cluster_track_host.numpy()[:ev.n], ref["cluster_track"])
     assert np.array_equal(trk2.par_host.numpy()[:, :K], ref["par"])
+    # enqueue-only variant on a side stream, two contexts in flight (bench.py's e2e pipeline)
+    trk3 = binding.Tracker(ev.params, ev.n)
+    trk3.make_host_staging()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for i, t in enumerate((trk2, trk3, trk2, trk3)):
+        with torch.cuda.stream(streams[i % 2]):
+            t.track_host(hy, hz, hs, sync=False)
+    for st in streams:
+        st.synchronize()
+    for t in (trk2, trk3):
+        assert int(t.counters_host[binding.CNT_TRACKS]) == K
+        assert np.array_equal(t.cluster_track_host.numpy()[:ev.n], ref["cluster_track"])
+        assert np.array_equal(t.par_host.numpy()[:, :K], ref["par"])
