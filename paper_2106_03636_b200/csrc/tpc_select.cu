@@ -36,11 +36,19 @@ k_push_keys(int nrows, const int32_t* __restrict__ row_hit, const int32_t* __res
     const int lo = (info >> 8) & 0xff, hi = (info >> 16) & 0xff;
     const unsigned long long key = __ldg(tl_key + t);
     const int32_t* hits = row_hit + t * nrows;
-    for (int r = lo + lane; r <= hi; r += 32) {
-      const int c = __ldg(hits + r);
-      // a plain read first: a claim that already lost (on average about half of them) needs no atomic
-      if (c >= 0 && __ldcg(owner + c) < key) atomicMax(owner + c, key);
+    int c[kMaskWords];
+    unsigned long long own[kMaskWords];
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) {
+      const int r = 32 * w + lane;
+      c[w] = (r >= lo && r <= hi) ? __ldg(hits + r) : -1;
     }
+    // a plain read first: a claim that already lost (on average about half of them) needs no atomic
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) own[w] = c[w] >= 0 ? __ldcg(owner + c[w]) : ~0ull;
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++)
+      if (own[w] < key) atomicMax(owner + c[w], key);
   }
 }
 
@@ -56,20 +64,22 @@ k_count_kept(int nrows, int min_hits, const int32_t* __restrict__ row_hit, const
     const int lo = (info >> 8) & 0xff, hi = (info >> 16) & 0xff;
     const unsigned long long key = __ldg(tl_key + t);
     const int32_t* hits = row_hit + t * nrows;
+    // all of the tracklet's rows are requested before the first use, then all owner gathers (5 loads in flight per
+    // lane instead of 1: these kernels are latency-bound, not bandwidth-bound)
+    int c[kMaskWords];
+    unsigned long long own[kMaskWords];
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) {
+      const int r = 32 * w + lane;
+      c[w] = (r >= lo && r <= hi) ? __ldg(hits + r) : -1;
+    }
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) own[w] = c[w] >= 0 ? __ldcg(owner + c[w]) : 0ull;
     int kept = 0;
     unsigned mine = 0u;  // lane w keeps mask word w
 #pragma unroll
     for (int w = 0; w < kMaskWords; w++) {
-      unsigned m = 0u;
-      if (32 * w <= hi && 32 * w + 31 >= lo) {  // warp-uniform
-        const int r = 32 * w + lane;
-        bool k = false;
-        if (r >= lo && r <= hi) {
-          const int c = __ldg(hits + r);
-          k = c >= 0 && owner[c] == key;
-        }
-        m = __ballot_sync(0xffffffffu, k);
-      }
+      const unsigned m = __ballot_sync(0xffffffffu, c[w] >= 0 && own[w] == key);
       kept += __popc(m);
       if (lane == w) mine = m;
     }
@@ -118,20 +128,25 @@ k_write_tracks(int nrows, const Rec* __restrict__ rec, const TlInit* __restrict_
       trk_first_hit[k] = first;
     }
     const int32_t* hits = row_hit + t * nrows;
+    unsigned m[kMaskWords];
+    int c[kMaskWords];
+    Rec h[kMaskWords];
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) m[w] = __ldg(tl_mask + t * kMaskWords + w);
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) c[w] = ((m[w] >> lane) & 1u) ? __ldg(hits + 32 * w + lane) : -1;
+#pragma unroll
+    for (int w = 0; w < kMaskWords; w++) h[w] = c[w] >= 0 ? ld_rec(rec, c[w]) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     long long at = first;
 #pragma unroll
     for (int w = 0; w < kMaskWords; w++) {
-      const unsigned m = __ldg(tl_mask + t * kMaskWords + w);
-      if (m == 0u) continue;  // warp-uniform
-      if ((m >> lane) & 1u) {
-        const int r = 32 * w + lane;
-        const Rec h = ld_rec(rec, __ldg(hits + r));
-        const long long o = at + __popc(m & ((1u << lane) - 1u));
-        trk_hits[o] = rec_idx(h);
-        hit_rec[o] = make_float4(h.x, h.y, __int_as_float(r), h.z);
-        cluster_track[rec_idx(h)] = (int)k;
+      if (c[w] >= 0) {
+        const long long o = at + __popc(m[w] & ((1u << lane) - 1u));
+        trk_hits[o] = rec_idx(h[w]);
+        hit_rec[o] = make_float4(h[w].x, h[w].y, __int_as_float(32 * w + lane), h[w].z);
+        cluster_track[rec_idx(h[w])] = (int)k;
       }
-      at += __popc(m);
+      at += __popc(m[w]);
     }
   }
 }
