@@ -14,6 +14,7 @@
  *                    (R9-R20)            start hits (R10), Kalman following (R11-R18), one-shot
  *                                        selection with exclusive cluster assignment (R20)
  *   tpc_fit_tracks   step 3b (R21-R22)   3-point seed + outward/inward Kalman refit, fp32
+ *   tpc_track_time   next     (R24)       per-track closest approach to the beam line, z0, time offset
  *
  * Conventions.
  *  - Every pointer is a DEVICE pointer unless its name ends in `_host`.  Every call only enqueues
@@ -178,6 +179,19 @@ int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
                    const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
                    float* par, float* cov, float* xref, float* zref, float* chi2, int32_t* ndf,
                    void* stream);
+
+/* After the hot path (R24; tracks are assigned to collisions only
+ * after the reconstruction).  For each of the K = counters[TPC_CNT_TRACKS] fitted tracks: the point of closest
+ * approach of its helix to the beam line (origin of the sector-local frames), in fp64 from the fp32 state:
+ *   phi0 [max_tracks] : global azimuth of the direction of flight there, [0, 2 pi)
+ *   z0   [max_tracks] : z there (same frame as the input z: includes the drift-time shift), cm
+ *   dca  [max_tracks] : distance of closest approach in the bending plane, cm (>= 0)
+ *   t0   [max_tracks] : time offset -side*z0/v_drift in microseconds for v_drift in cm/us (R5): the collision
+ *                       time of a primary from a vertex at z = 0
+ * par, xref, zref, trk_sector are the outputs of tpc_fit_tracks / tpc_find_tracks.  Enqueue only. */
+int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int64_t max_tracks,
+                   const int32_t* trk_sector, const float* par, const float* xref, const float* zref,
+                   float v_drift, float* phi0, float* z0, float* dca, float* t0, void* stream);
 
 /* Host-buffer convenience for end-to-end measurement (bench.py `e2e`): copies the five input
  * arrays host->device into caller-provided device staging buffers, runs the three steps, and

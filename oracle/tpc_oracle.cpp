@@ -705,3 +705,56 @@ ORC_API float orc_update_f32(const OrcParams* P, float* p5, float* c15, float ym
 ORC_API double orc_update_f64(const OrcParams* P, double* p5, double* c15, double ym, double zm) {
   return update_impl<double>(P, p5, c15, ym, zm);
 }
+
+// ---------------------------------------------------------------------------------------------
+// R24 ("assignment of tracks to collisions happens only after
+// the track reconstruction"): point of closest approach of a fitted helix to the beam line -- the origin of
+// every sector-local frame -- the z there, and the time offset it implies.  Plain double arithmetic on the
+// fp32 track state; textbook circle geometry:
+//   curvature kappa = -kB q/pT, cos(phi) = sqrt(1 - sin^2), circle centre C = (x - sin/kappa, y + cos/kappa),
+//   r_C = |C|, R = 1/|kappa|;  dca = |r_C - R|;  closest point P = C (1 - R/r_C);
+//   direction at P: phi_P = atan2(-(C_x - P_x) kappa, (C_y - P_y) kappa);
+//   turning angle P -> state: dphi = asin(sin phi) - phi_P wrapped to (-pi, pi];  z0 = z - tanl dphi / kappa;
+//   straight line (|kappa| < 1e-9 / cm): path t* = -(x cos + y sin), P = (x, y) + t* (cos, sin), z0 = z + tanl t*.
+//   global azimuth phi0 = phi_P + alpha_sector (R2) in [0, 2 pi);  time offset t0 = -side z0 / v_drift (R5: a
+//   primary from a vertex at z = 0 is measured at z = -side v_d t at the beam line).
+// ---------------------------------------------------------------------------------------------
+ORC_API void orc_beamline(const OrcParams* P, int64_t K, const float* par, int64_t ldp, const float* xref,
+                          const float* zref, const int32_t* sector, double v_drift, float* phi0, float* z0, float* dca,
+                          float* t0) {
+  const double kPi = 3.14159265358979323846;
+  for (int64_t k = 0; k < K; k++) {
+    const double x = xref[k], y = par[0 * ldp + k], dz = par[1 * ldp + k], s = par[2 * ldp + k], tl = par[3 * ldp + k],
+                 q = par[4 * ldp + k];
+    const double c = std::sqrt(1.0 - s * s);
+    const double kap = -(P->kB * q);
+    const double zabs = (double)zref[k] + dz;
+    double phip, zb, d;
+    if (std::fabs(kap) < 1e-9) {
+      const double ts = -(x * c + y * s);
+      const double px = x + ts * c, py = y + ts * s;
+      d = std::sqrt(px * px + py * py);
+      phip = std::atan2(s, c);
+      zb = zabs + tl * ts;
+    } else {
+      const double xc = x - s / kap, yc = y + c / kap;
+      const double rc = std::sqrt(xc * xc + yc * yc);
+      const double R = 1.0 / std::fabs(kap);
+      const double px = xc * (1.0 - R / rc), py = yc * (1.0 - R / rc);
+      d = std::fabs(rc - R);
+      phip = std::atan2(-((xc - px) * kap), (yc - py) * kap);
+      double dphi = std::asin(s) - phip;
+      dphi = dphi - 2.0 * kPi * std::floor((dphi + kPi) / (2.0 * kPi));  // into [-pi, pi)
+      zb = zabs - (tl * dphi) / kap;
+    }
+    const int sec = sector[k];
+    const double alpha = ((sec % 18) + 0.5) * (20.0 * kPi / 180.0);
+    double ph = phip + alpha;
+    ph = ph - 2.0 * kPi * std::floor(ph / (2.0 * kPi));
+    const double side = sec < 18 ? 1.0 : -1.0;
+    phi0[k] = (float)ph;
+    z0[k] = (float)zb;
+    dca[k] = (float)d;
+    t0[k] = (float)(-(side * zb) / v_drift);
+  }
+}

@@ -78,6 +78,7 @@ def lib():
         L.orc_update_f32.restype = C.c_float
         L.orc_update_f64.restype = C.c_double
         L.orc_links.restype = C.c_int64
+        L.orc_beamline.restype = None
         L.orc_select.restype = C.c_int64
         _lib = L
     return _lib
@@ -198,6 +199,19 @@ def fit(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, precision="f32"
                                      _ptr(fh), _ptr(th), _ptr(par), _ptr(cov), _ptr(xref), _ptr(zref), _ptr(chi2),
                                      _ptr(ndf))
     return dict(par=par, cov=cov, xref=xref, zref=zref, chi2=chi2, ndf=ndf)
+
+
+def beamline(p, par, xref, zref, sector, v_drift=2.58):
+    """R24: closest approach to the beam line of fp32 track states par[5,K] at xref: dict(phi0, z0, dca, t0) (fp32)."""
+    P = make_params(p, "f32")          # the tracker's fp32-rounded field constant
+    par = np.ascontiguousarray(par, np.float32)
+    K = par.shape[1]
+    xref = np.ascontiguousarray(xref, np.float32); zref = np.ascontiguousarray(zref, np.float32)
+    sector = np.ascontiguousarray(sector, np.int32)
+    out = {k: np.empty(K, np.float32) for k in ("phi0", "z0", "dca", "t0")}
+    lib().orc_beamline(C.byref(P), C.c_int64(K), _ptr(par), C.c_int64(K), _ptr(xref), _ptr(zref), _ptr(sector),
+                       C.c_double(v_drift), _ptr(out["phi0"]), _ptr(out["z0"]), _ptr(out["dca"]), _ptr(out["t0"]))
+    return out
 
 
 def propagate(p, par5, cov15, dx, precision="f64"):

@@ -27,7 +27,7 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
+           "tpc_track_time", "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
 
 
 class tpc_params_t(C.Structure):
@@ -223,6 +223,17 @@ class Tracker:
                                        C.c_int64(self.max_tracks), _dp(self.trk_nhits), _dp(self.trk_first_hit),
                                        _dp(self.trk_hits), _dp(self.par), _dp(self.cov), _dp(self.xref), _dp(self.zref),
                                        _dp(self.chi2), _dp(self.ndf), _stream()), "tpc_fit_tracks")
+
+    def track_time(self, v_drift: float = 2.58):
+        """tpc_track_time (R24) on the last fit: dict(phi0, z0, dca, t0) as numpy fp32 [K]; synchronises."""
+        t = self.torch
+        K = self.max_tracks
+        out = {k: t.empty(K, dtype=t.float32, device=self.device) for k in ("phi0", "z0", "dca", "t0")}
+        _check(self.lib.tpc_track_time(C.byref(self.P), _dp(self.counters), C.c_int64(K), _dp(self.trk_sector), _dp(self.par),
+                                       _dp(self.xref), _dp(self.zref), C.c_float(v_drift), _dp(out["phi0"]), _dp(out["z0"]),
+                                       _dp(out["dca"]), _dp(out["t0"]), _stream()), "tpc_track_time")
+        k = int(self.counters[CNT_TRACKS].item())
+        return {n: v[:k].cpu().numpy() for n, v in out.items()}
 
     def step(self, y, z, sector_row):
         """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""

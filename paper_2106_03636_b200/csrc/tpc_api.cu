@@ -25,7 +25,7 @@ Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
-                                         "k_fit", "k_export_*"};
+                                         "k_fit", "k_track_time", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -287,6 +287,19 @@ int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
   const cudaError_t e = tpc::launch_fit(pr.G, workspace ? &pr.W : nullptr, n_clusters, y, z, sector_row, counters, max_tracks,
                                         trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf,
                                         (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int64_t max_tracks, const int32_t* trk_sector,
+                   const float* par, const float* xref, const float* zref, float v_drift, float* phi0, float* z0, float* dca,
+                   float* t0, void* stream) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (max_tracks < 1 || !(v_drift > 0.0f) || !counters || !trk_sector || !par || !xref || !zref || !phi0 || !z0 || !dca || !t0)
+    return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_track_time(G, (double)v_drift, counters, max_tracks, trk_sector, par, xref, zref, phi0, z0,
+                                               dca, t0, (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

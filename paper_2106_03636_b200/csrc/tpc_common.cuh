@@ -206,6 +206,10 @@ cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, con
                        const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
                        float* zref, float* chi2, int32_t* ndf, cudaStream_t st);
 
+cudaError_t launch_track_time(const Geo& g, double v_drift, const int32_t* counters, int64_t max_tracks,
+                              const int32_t* trk_sector, const float* par, const float* xref, const float* zref, float* phi0,
+                              float* z0, float* dca, float* t0, cudaStream_t st);
+
 // ---- device helpers -------------------------------------------------------------------------
 // R7: clamp-to-range binning; NaN and negatives go to bin 0.
 __device__ __forceinline__ int clampbin(float v, int n) {

@@ -52,7 +52,6 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   const int n_starts = ws_counters[WC_N_STARTS];
   const int lane = threadIdx.x & 31;
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
-  unsigned long long work[3] = {0ull, 0ull, 0ull};
 
   // per-lane tracklet state
   int phase = PH_FETCH;
@@ -60,8 +59,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   float zref = 0.0f;
   int t = 0, s = 0, r0 = 0, r_at = 0, r = 0, hn = -1, p0 = 0, orig0 = 0;
   int misses = 0, nh = 0, lo = 0, hi = 0;
-  unsigned nprop = 0, nupd = 0, ncand = 0;
-  int32_t* my_hits = row_hit;
+  unsigned nprop = 0, nupd = 0, ncand = 0;  // work counters of this lane over all its tracklets (TPC_CNT_PROP/UPD/CAND)
   int pf_ka = -1;  // first grid position of the bin the NEXT step is expected to search (-1: no prediction)
 #pragma unroll
   for (int k = 0; k < 5; k++) st.p[k] = 0.0f;
@@ -100,10 +98,8 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
           st.p[3] = (a.w - a.y) / ch;
           st.p[4] = 0.0f;
           reset_cov(st, sc.cov0);
-          my_hits = row_hit + (int64_t)t * nrows;
           nh = 0;
           lo = hi = r_at = r0;
-          nprop = nupd = ncand = 0;
           phase = PH_INIT;
         }
       }
@@ -310,7 +306,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     // ---- bookkeeping and phase transitions ---------------------------------------------------------------
     __syncwarp();
     const bool searched = leg && ok && !edge_out;
-    if (upd || searched) my_hits[rn] = upd ? mk : -1;
+    if (upd || searched) row_hit[(int64_t)t * nrows + rn] = upd ? mk : -1;
     bool finish = false;
     if (isI) {
       phase = PH_CHAIN;
@@ -338,16 +334,13 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     if (finish) {  // R18 record; the R20 key is pushed by k_push_keys
       tl_info[t] = nh | (lo << 8) | (hi << 16);
       tl_key[t] = sel_key(nh, orig0, t);
-      work[0] += nprop;
-      work[1] += nupd;
-      work[2] += ncand;
       phase = PH_FETCH;
     }
   }
   // one 64-bit atomic per warp and counter
 #pragma unroll
   for (int k = 0; k < 3; k++) {
-    unsigned long long v = work[k];
+    unsigned long long v = k == 0 ? nprop : (k == 1 ? nupd : ncand);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(kFull, v, d);
     if (lane == 0 && v) atomicAdd((unsigned long long*)(ws_counters + WC_PROP64) + k, v);

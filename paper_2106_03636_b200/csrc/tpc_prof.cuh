@@ -28,6 +28,7 @@ enum KernelId {
   KID_COUNT_KEPT,
   KID_WRITE_TRACKS,
   KID_FIT,
+  KID_TRACK_TIME,
   KID_EXPORT,
   KID_N
 };
