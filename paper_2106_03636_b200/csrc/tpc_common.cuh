@@ -85,7 +85,13 @@ struct Layout {
 // carrying t lets the per-cluster passes find the owning tracklet without a search.
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
-constexpr int kMaxBuckets = 32768;  // grid build: first-level buckets of the counting sort
+#ifndef TPC_MAX_BUCKETS
+#define TPC_MAX_BUCKETS 32768
+#endif
+#ifndef TPC_BUCKET_SHIFT0
+#define TPC_BUCKET_SHIFT0 13
+#endif
+constexpr int kMaxBuckets = TPC_MAX_BUCKETS;  // grid build: first-level buckets of the counting sort
 constexpr int kMaskWords = 5;  // kept-row mask per tracklet (rows 0..159)
 
 // Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.

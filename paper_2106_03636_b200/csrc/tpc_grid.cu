@@ -86,8 +86,14 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
     for (int j = 0; j < kUnroll; j++) {
       int bk = -1;
       if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], &clamped) >> bucket_shift;
-      const unsigned peers = __match_any_sync(kFull, bk);  // inputs ordered by row put a whole warp in one bucket
-      if (bk >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + bk, __popc(peers));
+      // inputs ordered by row put a whole warp in one bucket: one add of 32; otherwise shared-memory atomics
+      // (same-address lanes are merged by the hardware)
+      const int bk0 = __shfl_sync(kFull, bk, 0);
+      if (__all_sync(kFull, bk == bk0)) {
+        if (bk >= 0 && (threadIdx.x & 31) == 0) atomicAdd(hist + bk, 32);
+      } else if (bk >= 0) {
+        atomicAdd(hist + bk, 1);
+      }
     }
   }
   __syncthreads();
@@ -124,13 +130,21 @@ k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, con
       const int64_t i = i0 + j * 32 + lane;
       int bk = -1;
       if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift;
-      const unsigned peers = __match_any_sync(kFull, bk);
-      const int leader = __ffs(peers) - 1;
-      int base = 0;
-      if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
-      base = __shfl_sync(kFull, base, leader);
-      if (bk >= 0)
-        tmp[base + __popc(peers & ((1u << lane) - 1u))] = make_float4(yv[j], zv[j], __int_as_float((int)i), __int_as_float(srv[j]));
+      // Warp-aggregated append.  match.any is slow when all 32 keys differ (shuffled input), and then there is
+      // nothing to aggregate: it is only used when some neighbouring lanes share a bucket (inputs ordered by row,
+      // where it turns up to 32 same-address atomics into one).
+      int slot;
+      if (__any_sync(kFull, bk == __shfl_xor_sync(kFull, bk, 1))) {
+        const unsigned peers = __match_any_sync(kFull, bk);
+        const int leader = __ffs(peers) - 1;
+        int base = 0;
+        if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
+        base = __shfl_sync(kFull, base, leader);
+        slot = base + __popc(peers & ((1u << lane) - 1u));
+      } else {
+        slot = bk >= 0 ? atomicAdd(cursor + bk, 1) : 0;
+      }
+      if (bk >= 0) tmp[slot] = make_float4(yv[j], zv[j], __int_as_float((int)i), __int_as_float(srv[j]));
     }
   }
 }
@@ -229,7 +243,7 @@ k_export_sorted(int64_t n, const Rec* __restrict__ rec, int32_t* __restrict__ so
 
 // bucket geometry: 8192 bins per bucket, doubled until at most 32768 buckets remain (nb <= 2^30)
 static inline int bucket_shift_for(int64_t nb) {
-  int sh = 13;
+  int sh = TPC_BUCKET_SHIFT0;
   while (((nb + ((int64_t)1 << sh) - 1) >> sh) > kMaxBuckets) sh++;
   return sh;
 }
