@@ -15,6 +15,7 @@
  *                                        selection with exclusive cluster assignment (R20)
  *   tpc_fit_tracks   step 3b (R21-R22)   3-point seed + outward/inward Kalman refit, fp32
  *   tpc_track_time   next     (R24)       per-track closest approach to the beam line, z0, time offset
+ *   tpc_find_collisions next  (R25)       collisions = peaks of the per-track time offsets; track -> collision
  *
  * Conventions.
  *  - Every pointer is a DEVICE pointer unless its name ends in `_host`.  Every call only enqueues
@@ -192,6 +193,26 @@ int tpc_fit_tracks(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
 int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int64_t max_tracks,
                    const int32_t* trk_sector, const float* par, const float* xref, const float* zref,
                    float v_drift, float* phi0, float* z0, float* dca, float* t0, void* stream);
+
+/* Collisions from the per-track time offsets (R25).  Integer work on
+ * a time histogram of n_bins bins of bin_width [us] starting at t_lo:
+ *   used tracks: finite t0, dca <= dca_max, t_lo <= t0 < t_lo + n_bins*bin_width, on the selected TPC side
+ *                (side_sel = +1: sectors < 18, -1: sectors >= 18, 0: both; trk_sector may be NULL for 0).  The two sides
+ *                see a collision at t -/+ z_vertex/v_drift (R5), so they are clustered separately and paired afterwards;
+ *   s[b] = tracks in bins b-2..b+2;  bin b is a collision iff s[b] >= n_min, s[b] > s[b-j] and s[b] >= s[b+j], j = 1..3;
+ *   coll_time [max_collisions]    : mean t0 of the tracks in the collision's 5 bins (exact: accumulated as
+ *                                   round(1024 (t0 - t_lo)) in int64), collisions in ascending time order
+ *   coll_ntracks, coll_bin [max_collisions] : tracks in those 5 bins; the peak bin
+ *   trk_collision [max_tracks]    : nearest collision within 5 bins of the track's bin (ties: the earlier), -1 = none
+ *   n_collisions [2] (device)     : collisions found; collisions written (clamped to max_collisions)
+ * K = counters[TPC_CNT_TRACKS] is read on the device.  workspace: tpc_collisions_workspace_bytes(n_bins,
+ * max_tracks) bytes, 256-byte aligned, caller-owned.  Enqueue only. */
+int tpc_collisions_workspace_bytes(int64_t n_bins, int64_t max_tracks, size_t* bytes_host);
+int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float* t0, const float* dca,
+                        const int32_t* trk_sector, int32_t side_sel, double t_lo, double bin_width, int64_t n_bins, double dca_max, int32_t n_min,
+                        void* workspace, size_t ws_bytes, int64_t max_collisions, float* coll_time,
+                        int32_t* coll_ntracks, int32_t* coll_bin, int32_t* trk_collision,
+                        int32_t* n_collisions, void* stream);
 
 /* Host-buffer convenience for end-to-end measurement (bench.py `e2e`): copies the five input
  * arrays host->device into caller-provided device staging buffers, runs the three steps, and

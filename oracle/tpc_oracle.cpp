@@ -758,3 +758,73 @@ ORC_API void orc_beamline(const OrcParams* P, int64_t K, const float* par, int64
     t0[k] = (float)(-(side * zb) / v_drift);
   }
 }
+
+// ---------------------------------------------------------------------------------------------
+// R25 (second half): collisions from the per-track time offsets of R24.
+// Integer work throughout (times are accumulated as round(t0 * 1024) in int64), so the result is unique:
+//   1. tracks used: finite t0, dca <= dca_max, t_lo <= t0 < t_lo + nb*w, and on the selected TPC side (side_sel = +1:
+//      sectors < 18, -1: sectors >= 18, 0: both -- the two sides see a collision at t -/+ z_vertex / v_d, so they are
+//      clustered separately and paired afterwards);  bin b = floor((t0 - t_lo) / w)
+//   2. h[b] = tracks in bin b;  s[b] = h[b-2] + ... + h[b+2]  (out-of-range bins count 0)
+//   3. bin b is a peak iff s[b] >= n_min, s[b] > s[b-j] and s[b] >= s[b+j] for j = 1..3
+//   4. collisions = peaks in ascending b;  time = t_lo + (sum of q over the peak's 5 bins / tracks there) / 1024
+//      with q = round((t0 - t_lo) * 1024);  n_tracks = tracks in those 5 bins
+//   5. a used track belongs to the peak nearest to its bin (ties: the earlier peak) if within 5 bins, else -1;
+//      unused tracks get -1
+// Returns the number of collisions; coll_* hold at most coll_cap entries.
+// ---------------------------------------------------------------------------------------------
+ORC_API int64_t orc_collisions(int64_t K, const float* t0, const float* dca, const int32_t* sector, int32_t side_sel, double t_lo, double w, int64_t nb, double dca_max,
+                               int32_t n_min, int64_t coll_cap, float* coll_time, int32_t* coll_ntracks, int32_t* coll_bin,
+                               int32_t* trk_collision) {
+  std::vector<int32_t> h((size_t)nb, 0), bin((size_t)K, -1);
+  std::vector<int64_t> q((size_t)nb, 0);
+  for (int64_t k = 0; k < K; k++) {
+    const double t = t0[k];
+    if (!(t == t) || !((double)dca[k] <= dca_max)) continue;   // NaN or displaced
+    if (side_sel != 0 && (side_sel > 0) != (sector[k] < 18)) continue;
+    const double u = (t - t_lo) / w;
+    if (!(u >= 0.0) || !(u < (double)nb)) continue;
+    const int64_t b = (int64_t)std::floor(u);
+    bin[(size_t)k] = (int32_t)b;
+    h[(size_t)b] += 1;
+    q[(size_t)b] += (int64_t)std::llround((t - t_lo) * 1024.0);
+  }
+  auto H = [&](int64_t b) -> int64_t { return (b >= 0 && b < nb) ? h[(size_t)b] : 0; };
+  auto S = [&](int64_t b) -> int64_t { return H(b - 2) + H(b - 1) + H(b) + H(b + 1) + H(b + 2); };
+  std::vector<int32_t> peaks;
+  for (int64_t b = 0; b < nb; b++) {
+    const int64_t s = S(b);
+    if (s < n_min) continue;
+    bool peak = true;
+    for (int j = 1; j <= 3; j++) peak = peak && s > S(b - j) && s >= S(b + j);
+    if (peak) peaks.push_back((int32_t)b);
+  }
+  const int64_t C = (int64_t)peaks.size();
+  for (int64_t c = 0; c < C && c < coll_cap; c++) {
+    const int64_t b = peaks[(size_t)c];
+    int64_t cnt = 0, sum = 0;
+    for (int64_t bb = b - 2; bb <= b + 2; bb++)
+      if (bb >= 0 && bb < nb) {
+        cnt += h[(size_t)bb];
+        sum += q[(size_t)bb];
+      }
+    coll_time[c] = (float)(t_lo + ((double)sum / (double)cnt) / 1024.0);
+    coll_ntracks[c] = (int32_t)cnt;
+    coll_bin[c] = (int32_t)b;
+  }
+  for (int64_t k = 0; k < K; k++) {
+    int32_t best = -1;
+    int64_t bestd = 6;
+    if (bin[(size_t)k] >= 0)
+      for (int64_t c = 0; c < C; c++) {   // plain scan: the oracle is allowed to be slow
+        int64_t d = (int64_t)peaks[(size_t)c] - bin[(size_t)k];
+        if (d < 0) d = -d;
+        if (d < bestd) {
+          bestd = d;
+          best = (int32_t)c;
+        }
+      }
+    trk_collision[k] = (best >= 0 && best < coll_cap) ? best : -1;
+  }
+  return C;
+}

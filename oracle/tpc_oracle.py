@@ -13,6 +13,7 @@ so the parity tests can compare stage by stage.
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 import time
@@ -212,6 +213,22 @@ def beamline(p, par, xref, zref, sector, v_drift=2.58):
     lib().orc_beamline(C.byref(P), C.c_int64(K), _ptr(par), C.c_int64(K), _ptr(xref), _ptr(zref), _ptr(sector),
                        C.c_double(v_drift), _ptr(out["phi0"]), _ptr(out["z0"]), _ptr(out["dca"]), _ptr(out["t0"]))
     return out
+
+
+def collisions(t0, dca, t_lo, t_hi, w=1.0, dca_max=3.0, n_min=5, sector=None, side=0):
+    """R25: dict(coll_time, coll_ntracks, coll_bin, trk_collision) from per-track t0 / dca (R24)."""
+    t0 = np.ascontiguousarray(t0, np.float32); dca = np.ascontiguousarray(dca, np.float32)
+    K = t0.size
+    sector = np.zeros(K, np.int32) if sector is None else np.ascontiguousarray(sector, np.int32)
+    nb = int(math.ceil((t_hi - t_lo) / w))
+    ct = np.empty(max(nb, 1), np.float32); cn = np.empty(max(nb, 1), np.int32); cb = np.empty(max(nb, 1), np.int32)
+    tc = np.empty(max(K, 1), np.int32)
+    L = lib()
+    L.orc_collisions.restype = C.c_int64
+    n = L.orc_collisions(C.c_int64(K), _ptr(t0), _ptr(dca), _ptr(sector), C.c_int32(side), C.c_double(t_lo), C.c_double(w), C.c_int64(nb),
+                         C.c_double(dca_max), C.c_int32(n_min), C.c_int64(ct.size), _ptr(ct), _ptr(cn), _ptr(cb), _ptr(tc))
+    n = int(n)
+    return dict(coll_time=ct[:n], coll_ntracks=cn[:n], coll_bin=cb[:n], trk_collision=tc[:K])
 
 
 def propagate(p, par5, cov15, dx, precision="f64"):

@@ -27,7 +27,7 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_time", "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
+           "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
 
 
 class tpc_params_t(C.Structure):
@@ -234,6 +234,36 @@ class Tracker:
                                        _dp(out["dca"]), _dp(out["t0"]), _stream()), "tpc_track_time")
         k = int(self.counters[CNT_TRACKS].item())
         return {n: v[:k].cpu().numpy() for n, v in out.items()}
+
+    def find_collisions(self, t_lo: float, t_hi: float, v_drift: float = 2.58, bin_width: float = 1.0, dca_max: float = 3.0,
+                        n_min: int = 5, max_collisions: int = 1 << 16, side: int = 0):
+        """tpc_track_time + tpc_find_collisions (R24, R25) on the last fit; numpy results; synchronises."""
+        import math
+        t = self.torch
+        K = self.max_tracks
+        dev = self.device
+        tt = {k: t.empty(K, dtype=t.float32, device=dev) for k in ("phi0", "z0", "dca", "t0")}
+        _check(self.lib.tpc_track_time(C.byref(self.P), _dp(self.counters), C.c_int64(K), _dp(self.trk_sector), _dp(self.par),
+                                       _dp(self.xref), _dp(self.zref), C.c_float(v_drift), _dp(tt["phi0"]), _dp(tt["z0"]),
+                                       _dp(tt["dca"]), _dp(tt["t0"]), _stream()), "tpc_track_time")
+        nb = int(math.ceil((t_hi - t_lo) / bin_width))
+        wsb = C.c_size_t(0)
+        _check(self.lib.tpc_collisions_workspace_bytes(C.c_int64(nb), C.c_int64(K), C.byref(wsb)), "tpc_collisions_workspace_bytes")
+        ws = t.empty(int(wsb.value), dtype=t.uint8, device=dev)
+        ct = t.empty(max_collisions, dtype=t.float32, device=dev)
+        cn = t.empty(max_collisions, dtype=t.int32, device=dev)
+        cb = t.empty(max_collisions, dtype=t.int32, device=dev)
+        tc = t.empty(K, dtype=t.int32, device=dev)
+        nc = t.zeros(2, dtype=t.int32, device=dev)
+        _check(self.lib.tpc_find_collisions(_dp(self.counters), C.c_int64(K), _dp(tt["t0"]), _dp(tt["dca"]), _dp(self.trk_sector),
+                                            C.c_int32(side), C.c_double(t_lo),
+                                            C.c_double(bin_width), C.c_int64(nb), C.c_double(dca_max), C.c_int32(n_min), _dp(ws),
+                                            C.c_size_t(int(wsb.value)), C.c_int64(max_collisions), _dp(ct), _dp(cn), _dp(cb),
+                                            _dp(tc), _dp(nc), _stream()), "tpc_find_collisions")
+        k = int(self.counters[CNT_TRACKS].item())
+        found, n = (int(v) for v in nc.cpu().numpy())
+        return dict(n_found=found, coll_time=ct[:n].cpu().numpy(), coll_ntracks=cn[:n].cpu().numpy(), coll_bin=cb[:n].cpu().numpy(),
+                    trk_collision=tc[:k].cpu().numpy(), t0=tt["t0"][:k].cpu().numpy(), dca=tt["dca"][:k].cpu().numpy())
 
     def step(self, y, z, sector_row):
         """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""

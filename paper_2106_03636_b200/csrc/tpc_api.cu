@@ -25,7 +25,7 @@ Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
-                                         "k_fit", "k_track_time", "k_export_*"};
+                                         "k_fit", "k_track_time", "k_t0_*", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -300,6 +300,29 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
     return TPC_EINVAL;
   const cudaError_t e = tpc::launch_track_time(G, (double)v_drift, counters, max_tracks, trk_sector, par, xref, zref, phi0, z0,
                                                dca, t0, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_collisions_workspace_bytes(int64_t n_bins, int64_t max_tracks, size_t* bytes_host) {
+  if (!bytes_host || n_bins < 1 || n_bins > 2147483000ll || max_tracks < 1 || max_tracks > 2147483000ll) return TPC_EINVAL;
+  *bytes_host = tpc::collisions_ws_bytes(n_bins, max_tracks);
+  return TPC_OK;
+}
+
+int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float* t0, const float* dca,
+                        const int32_t* trk_sector, int32_t side_sel, double t_lo,
+                        double bin_width, int64_t n_bins, double dca_max, int32_t n_min, void* workspace, size_t ws_bytes,
+                        int64_t max_collisions, float* coll_time, int32_t* coll_ntracks, int32_t* coll_bin,
+                        int32_t* trk_collision, int32_t* n_collisions, void* stream) {
+  if (n_bins < 1 || n_bins > 2147483000ll || max_tracks < 1 || max_tracks > 2147483000ll || max_collisions < 1 ||
+      !(bin_width > 0.0) || n_min < 1 || !counters || !t0 || !dca || (side_sel != 0 && !trk_sector) || side_sel < -1 || side_sel > 1 || !workspace || !coll_time || !coll_ntracks || !coll_bin ||
+      !trk_collision || !n_collisions)
+    return TPC_EINVAL;
+  if (((uintptr_t)workspace & 255) != 0) return TPC_EINVAL;
+  if (ws_bytes < tpc::collisions_ws_bytes(n_bins, max_tracks)) return TPC_ENOMEM_WS;
+  const cudaError_t e = tpc::launch_collisions(counters, max_tracks, t0, dca, trk_sector, side_sel, t_lo, bin_width, n_bins, dca_max, n_min, workspace,
+                                               max_collisions, coll_time, coll_ntracks, coll_bin, trk_collision, n_collisions,
+                                               (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

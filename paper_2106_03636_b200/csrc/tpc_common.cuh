@@ -216,6 +216,13 @@ cudaError_t launch_track_time(const Geo& g, double v_drift, const int32_t* count
                               const int32_t* trk_sector, const float* par, const float* xref, const float* zref, float* phi0,
                               float* z0, float* dca, float* t0, cudaStream_t st);
 
+size_t collisions_ws_bytes(int64_t nb, int64_t max_tracks);
+cudaError_t launch_collisions(const int32_t* counters, int64_t max_tracks, const float* t0, const float* dca,
+                              const int32_t* trk_sector, int side_sel, double t_lo,
+                              double w, int64_t nb, double dca_max, int32_t n_min, void* workspace, int64_t max_collisions,
+                              float* coll_time, int32_t* coll_ntracks, int32_t* coll_bin, int32_t* trk_collision,
+                              int32_t* n_collisions, cudaStream_t st);
+
 // ---- device helpers -------------------------------------------------------------------------
 // R7: clamp-to-range binning; NaN and negatives go to bin 0.
 __device__ __forceinline__ int clampbin(float v, int n) {

@@ -29,6 +29,7 @@ enum KernelId {
   KID_WRITE_TRACKS,
   KID_FIT,
   KID_TRACK_TIME,
+  KID_COLLISIONS,
   KID_EXPORT,
   KID_N
 };

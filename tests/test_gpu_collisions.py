@@ -1,0 +1,70 @@
+"""-m gpu: tpc_find_collisions (R25) against the oracle (integer work: bit-exact) and against the
+generator's collision list on a short 50 kHz Pb-Pb slice (configs[4] recipe, 8 orbits)."""
+import numpy as np
+import pytest
+
+from paper_2106_03636_b200.synth import V_DRIFT, make_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def slice8():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: -m gpu tests must run on the B200 box")
+    from paper_2106_03636_b200 import binding
+    ev = make_config(4, n_orbits=8)
+    trk = binding.Tracker(ev.params, ev.n)
+    res = trk.run(torch.from_numpy(ev.y).cuda(), torch.from_numpy(ev.z).cuda(), torch.from_numpy(ev.sector_row).cuda())
+    t_lo = float(np.floor(-ev.params.z_hi / V_DRIFT)) - 2.0
+    t_hi = float(np.ceil(-ev.params.z_lo / V_DRIFT)) + 2.0
+    g = {side: trk.find_collisions(t_lo, t_hi, V_DRIFT, side=side) for side in (0, 1, -1)}
+    return ev, res, g, t_lo, t_hi
+
+
+@pytest.mark.parametrize("side", [0, 1, -1])
+def test_collisions_match_oracle_exactly(slice8, orc, side):
+    ev, res, g, t_lo, t_hi = slice8
+    g = g[side]
+    o = orc.collisions(g["t0"], g["dca"], t_lo, t_hi, sector=res["trk_sector"], side=side)
+    assert g["n_found"] == o["coll_time"].size > 10
+    for k in ("coll_bin", "coll_ntracks", "trk_collision"):
+        assert np.array_equal(g[k], o[k]), k
+    assert np.array_equal(g["coll_time"], o["coll_time"])
+
+
+@pytest.mark.parametrize("side", [1, -1])
+def test_isolated_collisions_are_found_at_their_time(slice8, side):
+    """A TPC side sees a collision at t - side * z_vertex / v_d (R5, R24): with the sides clustered separately every
+    isolated collision with enough tracks is found within 1.5 us of that time, and its tracks are assigned to it."""
+    ev, res, g, t_lo, t_hi = slice8
+    g = g[side]
+    t_true, idx = np.unique(ev.trk["t_us"], return_index=True)
+    ntrk = np.array([np.count_nonzero(ev.trk["t_us"] == t) for t in t_true])
+    vz = np.array([np.median(ev.trk["vz"][ev.trk["t_us"] == t]) for t in t_true])      # 85 % primaries share the vertex
+    gap = np.minimum(np.diff(t_true, prepend=-1e9), np.diff(t_true, append=1e9))
+    good = (gap > 12.0) & (ntrk >= 100)
+    assert good.sum() >= 5
+    first, nh = res["trk_first_hit"], res["trk_nhits"]
+    tt = ev.true_track[res["trk_hits"][first + nh // 2]]
+    on_side = (res["trk_sector"] < 18) == (side > 0)
+    for t, z in zip(t_true[good], vz[good]):
+        expect = t - side * z / V_DRIFT
+        d = np.abs(g["coll_time"] - expect)
+        assert d.min() < 1.5, f"collision at {t:.1f} us (side time {expect:.1f}) not found (nearest {g['coll_time'][d.argmin()]:.1f})"
+        c = int(d.argmin())
+        mine = (tt >= 0) & (nh >= 60) & (g["dca"] < 1.0) & on_side
+        mine[mine] &= ev.trk["t_us"][tt[mine]] == t
+        if mine.sum() > 20:
+            assert np.mean(g["trk_collision"][mine] == c) > 0.9
+    assert np.all(g["trk_collision"][~on_side] == -1)
+
+
+def test_collisions_argument_errors():
+    from paper_2106_03636_b200 import binding
+    import ctypes as C
+    L = binding.load()
+    out = C.c_size_t(0)
+    assert L.tpc_collisions_workspace_bytes(C.c_int64(0), C.c_int64(10), C.byref(out)) == -1
+    assert L.tpc_collisions_workspace_bytes(C.c_int64(100), C.c_int64(10), C.byref(out)) == 0 and out.value > 0
