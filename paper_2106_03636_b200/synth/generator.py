@@ -196,12 +196,19 @@ def _trace_loopers(t, idx, row_x, tan_half, max_turns=2):
 # ----------------------------------------------------------------------------------------
 # event assembly
 # ----------------------------------------------------------------------------------------
-def choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi, lo=1.0, hi=8.0):
-    """Square grid cell with mean occupancy ~1 (R7: 'bins ~ N'), clamped to [lo, hi] cm."""
+def choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi, occupancy=0.35, cz_min=5.5, lo=1.0, hi=8.0):
+    """Grid cell (cell_y, cell_z) in cm for a mean bin occupancy of `occupancy` (R7; R8: results do not depend on it).
+
+    Measured on the Time Frame of configs[4]: about three bins per cluster is the optimum --
+    the follower and the CA finder test fewer candidates per lookup, the grid build pays for the extra bins.  The
+    drift cell is kept >= 5.5 cm, the height of the CA window (2 * ca_max_dzdx * pitch = 5.3 cm), so that every
+    window spans at most two z-bin rows; the rest of the area budget goes to y.  Quarter-cm steps: exact in fp32."""
     area = n_sectors * float(np.sum(2.0 * row_x.astype(np.float64) * tan_half)) * (z_hi - z_lo)
-    dens = max(n, 1) / area
-    c = min(max(math.sqrt(1.0 / dens), lo), hi)
-    return float(np.float32(round(c * 4.0) / 4.0))      # quarter-cm steps: exact in fp32
+    cell_area = occupancy * area / max(n, 1)
+    q = lambda v: float(np.float32(round(min(max(v, lo), hi) * 4.0) / 4.0))
+    cz = q(max(math.sqrt(cell_area), cz_min))
+    cy = q(cell_area / cz)
+    return cy, cz
 
 
 def _trace_signal(rng, t, t_us, sigma_y, sigma_z, dropout, single_sector, smear=True):
@@ -274,8 +281,8 @@ def _finish(name, rng, t, t_us, sig, noise_frac, single_sector, params_kw=None, 
     z_lo = float(np.floor(zeta.min() - 1.0)) if n else -1.0
     z_hi = float(np.ceil(zeta.max() + 1.0)) if n else Z_MAX + 1.0
     del zeta, sgn
-    cell = choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi)
-    kw = dict(n_sectors=n_sectors, z_lo=z_lo, z_hi=z_hi, cell_y=cell, cell_z=cell)
+    cell_y, cell_z = choose_cells(n, n_sectors, row_x, tan_half, z_lo, z_hi)
+    kw = dict(n_sectors=n_sectors, z_lo=z_lo, z_hi=z_hi, cell_y=cell_y, cell_z=cell_z)
     kw.update(params_kw or {})
     p = TpcParams(**kw)
     trk = {k: np.asarray(v) for k, v in t.items()}
