@@ -106,7 +106,7 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
     G->row.ny[r] = ny;
     G->row.rowbase[r] = (int32_t)base;
     base += (int64_t)ny * s.nz;
-    if (base * s.nsec > 1073741824ll) return false;       // bin ids: int32, and <= 32768 buckets of <= 32768 bins
+    if (base * s.nsec > 1073741824ll) return false;       // bin ids: int32, and <= kMaxBuckets buckets of <= 32768 bins
   }
   G->row.rowbase[s.nrows] = (int32_t)base;
   s.bins_per_sector = (int32_t)base;

@@ -86,7 +86,7 @@ struct Layout {
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
 #ifndef TPC_MAX_BUCKETS
-#define TPC_MAX_BUCKETS 32768
+#define TPC_MAX_BUCKETS 49152
 #endif
 #ifndef TPC_BUCKET_SHIFT0
 #define TPC_BUCKET_SHIFT0 13

@@ -28,6 +28,7 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kHistThreads = 1024;  // the bucket histogram takes up to 192 KB of shared memory: one or two big blocks per SM
 constexpr int kUnroll = 4;  // independent loads in flight per thread in the streaming passes
 
 struct GridSmem {
@@ -57,22 +58,22 @@ __device__ __forceinline__ int bin_of(const GridSmem& sm, const Scalars& sc, int
 // shared-memory index with one pad word per 32: conflict-free both for t*32+k and for random access
 __device__ __forceinline__ int pad32(int j) { return j + (j >> 5); }
 
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kHistThreads)
 k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nbuckets, const float* __restrict__ y,
               const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ bucket_cnt,
               int32_t* __restrict__ ws_counters) {
   extern __shared__ int32_t hist[];  // [nbuckets]
   __shared__ GridSmem sm;
   load_grid_rows(sm, g);
-  for (int j = threadIdx.x; j < nbuckets; j += kThreads) hist[j] = 0;
+  for (int j = threadIdx.x; j < nbuckets; j += kHistThreads) hist[j] = 0;
   __syncthreads();
   const Scalars& sc = g.s;
   bool clamped = false;
   // every block takes one contiguous slice of the input (the tail of the loop keeps the warp whole for match_any)
-  const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kThreads * kUnroll - 1) / (kThreads * kUnroll) * (kThreads * kUnroll);
+  const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kHistThreads * kUnroll - 1) / (kHistThreads * kUnroll) * (kHistThreads * kUnroll);
   const int64_t lo = (int64_t)blockIdx.x * per, hi = lo + per < n ? lo + per : n;
   // a warp takes kUnroll x 32 consecutive clusters per iteration: all loads are issued before the first use
-  for (int64_t i0 = lo + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < hi; i0 += (int64_t)kThreads * kUnroll) {
+  for (int64_t i0 = lo + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < hi; i0 += (int64_t)kHistThreads * kUnroll) {
     int srv[kUnroll];
     float yv[kUnroll], zv[kUnroll];
 #pragma unroll
@@ -97,7 +98,7 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
     }
   }
   __syncthreads();
-  for (int j = threadIdx.x; j < nbuckets; j += kThreads) {
+  for (int j = threadIdx.x; j < nbuckets; j += kHistThreads) {
     const int c = hist[j];
     if (c) atomicAdd(bucket_cnt + j, c);
   }
@@ -241,7 +242,7 @@ k_export_sorted(int64_t n, const Rec* __restrict__ rec, int32_t* __restrict__ so
 
 }  // namespace
 
-// bucket geometry: 8192 bins per bucket, doubled until at most 32768 buckets remain (nb <= 2^30)
+// bucket geometry: 8192 bins per bucket, doubled until at most kMaxBuckets buckets remain (nb <= 2^30)
 static inline int bucket_shift_for(int64_t nb) {
   int sh = TPC_BUCKET_SHIFT0;
   while (((nb + ((int64_t)1 << sh) - 1) >> sh) > kMaxBuckets) sh++;
@@ -267,7 +268,8 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
   if ((e = cudaMemsetAsync(w.bucket_first, 0, sizeof(int32_t) * (size_t)(kMaxBuckets + 2), st)) != cudaSuccess) return e;
   if (n > 0)
     TPC_LAUNCH(KID_BUCKET_HIST, st,
-               (k_bucket_hist<<<blocks_for(n, kThreads * 64, 148 * 4), kThreads, hist_smem, st>>>(
+               (k_bucket_hist<<<blocks_for(n, kHistThreads * 64, 148 * (hist_smem + 2048 <= 110000 ? 2 : 1)), kHistThreads,
+                               hist_smem, st>>>(
                    g, n, sh, nbuckets, y, z, sector_row, w.bucket_first, w.counters)));
   if ((e = exclusive_scan<int32_t>(w.bucket_first, w.bucket_first, nbuckets + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
   if ((e = cudaMemcpyAsync(w.bucket_cursor, w.bucket_first, sizeof(int32_t) * (size_t)(nbuckets + 1), cudaMemcpyDeviceToDevice,
