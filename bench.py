@@ -60,9 +60,9 @@ KERNEL_MODEL = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
 # launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
-NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 3.92, "k_bucket_sort": 6.86, "k_neighbours": 6.55,
-                     "k_clean": 2.25, "k_compact_starts": 2.06, "k_follow": 11.56, "k_push_keys": 6.24,
-                     "k_count_kept": 6.16, "k_write_tracks": 23.92, "k_fit": 4.89}
+NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.14, "k_neighbours": 8.98,
+                     "k_clean": 2.26, "k_compact_starts": 2.06, "k_follow": 17.26, "k_push_keys": 5.80,
+                     "k_count_kept": 6.24, "k_write_tracks": 22.87, "k_fit": 4.87}
 
 
 def parse_args():
