@@ -9,8 +9,8 @@
 // update (R13)".  The kernel is ONE loop whose body holds a single copy of the transport and of
 // the update, so the lanes of a warp execute them together whatever phase each lane is in, and a
 // lane that finishes its tracklet pulls the next one from the queue inside the same loop (no
-// waiting for the longest tracklet of a batch).  Tracklets are queued in grid order, so
-// concurrently running lanes walk neighbouring bins (L2 locality of the R16 lookups).
+// waiting for the longest tracklet of a batch).  Tracklets are queued in (sector, z slab, row) order
+// (tpc_find.cu), so concurrently running lanes walk neighbouring bins (L2 locality of the lookups).
 //
 // Output: row_hit[t][row] (grid positions, -1 = no hit), tl_info[t] = nHits | lo<<8 | hi<<16,
 // tl_key[t] = R20 selection key.  The key is pushed onto the clusters by k_push_keys
