@@ -25,13 +25,18 @@ namespace tpc {
 
 namespace {
 
-constexpr int kFollowThreads = 128;
+#ifndef TPC_FOLLOW_THREADS
+#define TPC_FOLLOW_THREADS 64
+#endif
+// 64-thread blocks, 10 per SM: 96 registers per thread without spills and 20 resident warps per SM (measured on
+// configs[4]: 128 x 4 blocks at 112 registers = 16 warps: 28.0 ms; 64 x 10 at 96 registers, batch 3: 25.3 ms)
+constexpr int kFollowThreads = TPC_FOLLOW_THREADS;
 constexpr unsigned kFull = 0xffffffffu;
 #ifndef TPC_FOLLOW_BATCH
-#define TPC_FOLLOW_BATCH 4
+#define TPC_FOLLOW_BATCH 3
 #endif
 #ifndef TPC_FOLLOW_MIN_BLOCKS
-#define TPC_FOLLOW_MIN_BLOCKS 4
+#define TPC_FOLLOW_MIN_BLOCKS 10
 #endif
 constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
 
