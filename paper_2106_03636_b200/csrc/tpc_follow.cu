@@ -38,6 +38,9 @@ constexpr unsigned kFull = 0xffffffffu;
 #ifndef TPC_FOLLOW_MIN_BLOCKS
 #define TPC_FOLLOW_MIN_BLOCKS 10
 #endif
+#ifndef TPC_FOLLOW_PREFETCH
+#define TPC_FOLLOW_PREFETCH 1
+#endif
 constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
 
 // L1 prefetch of one line: the follower knows one step ahead roughly where it will look.
@@ -284,8 +287,8 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     //   linearly extrapolated position -- its offset is loaded now (in flight during the update) and the
     //   records behind it are prefetched at the top of the next iteration.  st still holds the state at the
     //   previous row here, so the slope costs two subtractions.
-    if (chain && upd && nxt >= 0) prefetch_l1(rec + nxt);
-    if (moved && ok && !isJ) {
+    if (TPC_FOLLOW_PREFETCH && chain && upd && nxt >= 0) prefetch_l1(rec + nxt);
+    if (TPC_FOLLOW_PREFETCH && moved && ok && !isJ) {
       const int r2 = rn + ((phase == PH_DOWN) ? -1 : 1);
       if (r2 >= 0 && r2 < nrows) {
         const float y2 = yp + (yp - st.p[0]);
