@@ -12,7 +12,8 @@
 //   orc_grid        R7      per-(sector,row) (y, zeta) grid: stable sort by bin, bin_first
 //   orc_neighbours  R9      cellular-automaton best (up,down) pair per cluster
 //   orc_links       R10     reciprocal-link cleaning, start hits
-//   orc_follow      R11-R18 Kalman following of every start hit (chain, up leg, down leg)
+//   orc_follow      R11-R18 Kalman following of every start hit: phase A chain + up leg for all, phase B
+//                           jump + down leg for those whose start hit no upward leg picked up (R17)
 //   orc_select      R20     one-shot arbitration by 64-bit key, exclusive assignment
 //   orc_fit         R21-R22 3-point seed + outward/inward Kalman refit
 //   orc_propagate / orc_update   the R12 / R13 primitives, exported for the pins (I7)
@@ -362,6 +363,7 @@ struct Follower {
 
   // R16: extrapolate row by row in direction dir (+1/-1) starting after row r_at (state is at X[r_at]).
   // Returns the row the state is at when the leg ends.
+  uint8_t* picked_up = nullptr;  // R17: set for every cluster an UPWARD leg attaches (phase A)
   int extrapolate(State<T>& st, T zref, int sector, int r_at, int r_first, int dir, int32_t* row_hit, int tracklet) {
     int misses = 0;
     for (int r = r_first; r >= 0 && r < G.nrows; r += dir) {
@@ -390,6 +392,7 @@ struct Follower {
         }
         update(st, cl.y[bi], cl.z[bi] - zref, G.sy2, G.sz2);
         row_hit[r] = bi;
+        if (picked_up && dir > 0) picked_up[bi] = 1;
         misses = 0;
       } else {
         misses++;
@@ -399,8 +402,9 @@ struct Follower {
     return r_at;
   }
 
-  // Follow start hit h0; row_hit[nrows] receives original indices (-1 = none).  Returns nHits.
-  int follow(int32_t h0, const int32_t* up_c, int32_t* row_hit, int tracklet, State<T>* final_state, T* zref_out) {
+  // Phase A of following start hit h0 (R14 init, R15 chain, R16 upward leg); row_hit[nrows] receives original
+  // indices (-1 = none).  Leaves the state where the upward leg ended (at X[*r_at_out]).
+  void follow_up(int32_t h0, const int32_t* up_c, int32_t* row_hit, int tracklet, State<T>* st_out, T* zref_out, int* r_at_out) {
     for (int r = 0; r < G.nrows; r++) row_hit[r] = -1;
     const int sector = cl.sector(h0), r0 = cl.row(h0);
     const int32_t h1 = up_c[h0];
@@ -435,13 +439,21 @@ struct Follower {
     }
     // R16 upward from the last chain hit
     r_at = extrapolate(st, zref, sector, r_at, r_at + 1, +1, row_hit, tracklet);
-    // R17: one step back to the start row (no update), then R16 downward
+    *st_out = st;
+    *zref_out = zref;
+    *r_at_out = r_at;
+  }
+
+  // Phase B (only for tracklets whose start hit no upward leg picked up, R17): one step back to the start row
+  // (no update), then R16 downward.  Returns nHits of the whole tracklet.
+  int follow_down(int32_t h0, int32_t* row_hit, int tracklet, State<T>* st_io, T zref, int r_at) {
+    const int sector = cl.sector(h0), r0 = cl.row(h0);
+    State<T> st = *st_io;
     if (propagate(st, G.X[r0] - G.X[r_at], G.kB, (T)P.max_sinphi))
       extrapolate(st, zref, sector, r0, r0 - 1, -1, row_hit, tracklet);
     int nh = 0;
     for (int r = 0; r < G.nrows; r++) nh += row_hit[r] >= 0;
-    if (final_state) *final_state = st;
-    if (zref_out) *zref_out = zref;
+    *st_io = st;
     return nh;
   }
 };
@@ -539,16 +551,30 @@ int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const
                     T* state_out, TraceRec* trace, int64_t trace_cap) {
   Ctx<T> c(*P, n, y, z, sr, use_grid);
   Follower<T> f{c.P, c.G, c.cl, c.ix, trace, trace_cap, 0};
+  // R17: phase A for every start hit, then phase B for those that no upward leg picked up; the others are
+  // absorbed (the tracklet that picked their start hit up covers them): they record nothing and claim nothing.
+  std::vector<uint8_t> picked_up((size_t)n, 0);
+  std::vector<State<T>> sts((size_t)n_starts);
+  std::vector<T> zrefs((size_t)n_starts);
+  std::vector<int> r_ats((size_t)n_starts);
+  f.picked_up = picked_up.data();
+  for (int64_t t = 0; t < n_starts; t++)
+    f.follow_up(starts[t], up_c, row_hit + t * c.G.nrows, (int)t, &sts[(size_t)t], &zrefs[(size_t)t], &r_ats[(size_t)t]);
+  f.picked_up = nullptr;
   for (int64_t t = 0; t < n_starts; t++) {
-    State<T> fs;
-    T zref;
-    n_hits[t] = f.follow(starts[t], up_c, row_hit + t * c.G.nrows, (int)t, &fs, &zref);
+    if (picked_up[(size_t)starts[t]]) {
+      n_hits[t] = 0;
+      for (int r = 0; r < c.G.nrows; r++) row_hit[t * c.G.nrows + r] = -1;
+    } else {
+      n_hits[t] = f.follow_down(starts[t], row_hit + t * c.G.nrows, (int)t, &sts[(size_t)t], zrefs[(size_t)t], r_ats[(size_t)t]);
+    }
     if (state_out) {   // 5 params, 15 cov (lower), zref : 21 values per tracklet
+      const State<T>& fs = sts[(size_t)t];
       T* o = state_out + t * 21;
       for (int i = 0; i < 5; i++) o[i] = fs.p[i];
       for (int i = 0, m = 5; i < 5; i++)
         for (int j = 0; j <= i; j++) o[m++] = fs.C[i][j];
-      o[20] = zref;
+      o[20] = zrefs[(size_t)t];
     }
   }
   return f.trace_n;
