@@ -50,7 +50,8 @@ KERNEL_MODEL = {
     "k_neighbours": ("hbm", {"cluster": 16 + 8}, None),           # own record in, two links out (neighbours from L2)
     "k_clean": ("hbm", {"cluster": 8 + 8}, None),
     "k_compact_starts": ("hbm", {"cluster": 4, "tracklet": 32}, None),
-    "k_follow": ("alu", {}, "step"),
+    "k_follow": ("alu", {}, "step"),                              # both phases (two launches per step)
+    "k_survivor_*": ("hbm", {"tracklet": 32 + 1 + 4 + 12 + 4}, None),
     "k_push_keys": ("hbm", {"claim": 4 + 8 + 8, "tracklet": 12}, None),   # row_hit in, 8-byte atomicMax RMW
     "k_count_kept": ("hbm", {"claim": 4 + 8, "tracklet": 12 + 20 + 8}, None),   # row_hit, owner in; mask, value out
     "k_write_tracks": ("hbm", {"hit": 4 + 16 + 4 + 16 + 8, "tracklet": 16 + 20}, None),  # rec in; trk_hits, hit_rec, cluster_track out
@@ -311,9 +312,11 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     launches = int(sum(v[1] for v in prof.values()))
     top = max(kern, key=lambda k: kern[k]["ms_per_step"])
     top_ms = kern[top]["ms_per_step"] / max(kern[top]["launches_per_step"], 1)
+    if top == "k_follow":      # phases A and B are two launches of one kernel; the work counters cover both
+        top_ms = kern[top]["ms_per_step"]
     nb = binding.grid_bins(ev.params)
     work = binding.work_counts(res["counters"])
-    units = {"cluster": n, "bin": nb, "tracklet": int(res["counters"][binding.CNT_TRACKLETS]), "claim": work["updates"],
+    units = {"cluster": n, "bin": nb, "tracklet": int(res["counters"][binding.CNT_TRACKLETS]), "claim": work["claims"],
              "hit": n_hits}
     roofline = kernel_roofline(top, top_ms, units, work, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
     if args.config == 4 and top in NCU_TRAFFIC_GB_C4:
@@ -321,7 +324,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         roofline["traffic_source"] = "profiles/r01_ncu_summary.md (ncu dram__bytes_read.sum + dram__bytes_write.sum)"
     for k in kern:       # every kernel's own fraction of its roof, so that the table can be read without DESIGN.md
         r = kernel_roofline(k, kern[k]["ms_per_step"] / max(kern[k]["launches_per_step"], 1) *
-                            (kern[k]["launches_per_step"] if k == "k_scan_*" else 1), units, work,
+                            (kern[k]["launches_per_step"] if k in ("k_scan_*", "k_follow", "k_survivor_*") else 1), units, work,
                             int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
         kern[k]["bound"], kern[k]["frac"] = r["bound"], round(r["frac"], 4)
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -332,7 +335,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                       "l2": f"inputs ({12 * n / 1e6:.0f} MB/step) and workspace exceed the 126 MB L2; no explicit flush",
                       "parallelism": f"tf-replicas x{world}", "gen_seconds": round(t_gen, 1)},
            "time_frames_per_s": (world / (ms_step * 1e-3)) if args.config == 4 else None,
-           "tracks_found": K_tracks, "tracklets_followed": n_tracklets, "clusters_assigned": n_hits,
+           "tracks_found": K_tracks, "tracklets_followed": n_tracklets,
+           "tracklets_followed_down": int(res["counters"][binding.CNT_FOLLOWED_DOWN]), "clusters_assigned": n_hits,
            "follower_work": work,
            "clocks": clocks, "gpu_launches": launches, "kernels": kern, "roofline": roofline}
     if not args.no_e2e:

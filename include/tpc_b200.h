@@ -65,7 +65,7 @@ enum {
   TPC_CNT_STATUS = 3,     /* bit mask of TPC_ST_*                                               */
   TPC_CNT_STARTS_FOUND = 4, /* start hits found before clamping                                 */
   TPC_CNT_TRACKS_FOUND = 5, /* accepted tracks before clamping                                  */
-  TPC_CNT_RESERVED6 = 6,
+  TPC_CNT_FOLLOWED_DOWN = 6, /* tracklets that went on to the downward leg (start hit not picked up by an upward leg, R17) */
   TPC_CNT_RESERVED7 = 7,
   TPC_CNT_PROP_LO = 8,    /* follower work (time ~ tracks x attached clusters):      */
   TPC_CNT_PROP_HI = 9,    /*   64-bit count of helix transports (R12) done by the follower, lo/hi    */
@@ -73,6 +73,8 @@ enum {
   TPC_CNT_UPD_HI = 11,
   TPC_CNT_CAND_LO = 12,   /*   64-bit count of candidate clusters chi2-tested in R16 searches, lo/hi */
   TPC_CNT_CAND_HI = 13,
+  TPC_CNT_CLAIMS_LO = 14, /*   64-bit count of hits recorded by the tracklets of TPC_CNT_FOLLOWED_DOWN (R18), lo/hi */
+  TPC_CNT_CLAIMS_HI = 15,
   TPC_N_COUNTERS = 16
 };
 #define TPC_ST_TRACKLET_OVERFLOW 1 /* more start hits than max_tracklets: the excess was dropped */

@@ -21,7 +21,8 @@ TPC_MAX_ROWS = 152
 TPC_N_COUNTERS = 16
 TPC_MAX_TRACKLETS = 1 << 25
 CNT_TRACKS, CNT_TRACKLETS, CNT_HITS, CNT_STATUS, CNT_STARTS_FOUND, CNT_TRACKS_FOUND = 0, 1, 2, 3, 4, 5
-CNT_PROP_LO, CNT_UPD_LO, CNT_CAND_LO = 8, 10, 12
+CNT_FOLLOWED_DOWN = 6
+CNT_PROP_LO, CNT_UPD_LO, CNT_CAND_LO, CNT_CLAIMS_LO = 8, 10, 12, 14
 ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
@@ -129,15 +130,22 @@ def profile_collect(reset: bool = True) -> dict:
     ms = (C.c_double * k)()
     cnt = (C.c_int64 * k)()
     _check(L.tpc_profile_collect(C.c_int(k), ms, cnt, C.c_int(int(reset))), "tpc_profile_collect")
-    return {L.tpc_profile_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
+    out = {}
+    for i in range(k):      # kernel ids that share a name (the two phases of k_follow) are summed
+        name = L.tpc_profile_name(i).decode()
+        a, b = out.get(name, (0.0, 0))
+        out[name] = (a + float(ms[i]), b + int(cnt[i]))
+    return out
 
 
 def work_counts(counters) -> dict:
-    """Follower work from the counters array: transports (R12), updates (R13), candidates tested (R16)."""
+    """Follower work from the counters array: transports (R12), updates (R13), candidates tested (R16), and the hits
+    recorded by the tracklets that went through phase B (the claims the selection works on, R18/R20)."""
     c = np.asarray(counters).astype(np.int64) & 0xFFFFFFFF
     return {"propagations": int(c[CNT_PROP_LO] | (c[CNT_PROP_LO + 1] << 32)),
             "updates": int(c[CNT_UPD_LO] | (c[CNT_UPD_LO + 1] << 32)),
-            "candidates": int(c[CNT_CAND_LO] | (c[CNT_CAND_LO + 1] << 32))}
+            "candidates": int(c[CNT_CAND_LO] | (c[CNT_CAND_LO + 1] << 32)),
+            "claims": int(c[CNT_CLAIMS_LO] | (c[CNT_CLAIMS_LO + 1] << 32))}
 
 
 def grid_bins(params) -> int:

@@ -60,9 +60,12 @@ enum {
   WC_STATUS = 2,       // TPC_ST_* bits
   WC_STARTS_FOUND = 3, // before clamping
   WC_FIT_QUEUE = 4,    // work-queue head of the cached refit
+  WC_QUEUE_B = 5,      // work-queue head of the follower's phase B
+  WC_N_SURV = 6,       // tracklets that go on to phase B (start hit not picked up by an upward leg, R17)
   WC_PROP64 = 8,       // unsigned long long at [8,9]: follower transports
   WC_UPD64 = 10,       // unsigned long long at [10,11]: follower updates
   WC_CAND64 = 12,      // unsigned long long at [12,13]: candidates tested
+  WC_CLAIMS64 = 14,    // unsigned long long at [14,15]: hits recorded by the tracklets that finished phase B
   WC_N = 16
 };
 
@@ -76,7 +79,7 @@ struct Layout {
   int64_t scan_tiles;  // capacity (elements) of the scan scratch
   size_t off_counters, off_rec, off_key, off_bucket_first, off_bucket_cursor, off_bin_first, off_link_up, off_link_dn, off_up_c,
       off_owner, off_hit_rec, off_tl_init, off_tl_info, off_tl_key, off_tl_mask, off_tl_scan, off_row_hit,
-      off_chunk_base, off_chunk_scan0, off_scan_tmp, total;
+      off_tl_state, off_surv, off_surv_scan, off_picked, off_chunk_base, off_chunk_scan0, off_scan_tmp, total;
 };
 
 // R20 selection key, 64 bits: [63:56] nHits | [55:25] 0x7FFFFFFF - original index of the start hit |
@@ -92,6 +95,8 @@ constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
 #define TPC_BUCKET_SHIFT0 13
 #endif
 constexpr int kMaxBuckets = TPC_MAX_BUCKETS;  // grid build: first-level buckets of the counting sort
+constexpr int kStateVec = 6;    // float4 per tracklet of follower state carried from phase A to phase B (24 words)
+constexpr int kStartBit = 1 << 30;  // rec.w: set on start hits by k_compact_starts (read by the upward legs, R17)
 constexpr int kMaskWords = 5;  // kept-row mask per tracklet (rows 0..159)
 
 // Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.
@@ -139,6 +144,10 @@ inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows, int64_
   L.off_tl_mask = take(sizeof(uint32_t) * kMaskWords * (size_t)(L.scap_pad + 1));
   L.off_tl_scan = take(sizeof(int64_t) * (size_t)(L.scap_pad + 2));
   L.off_row_hit = take(sizeof(int32_t) * (size_t)L.scap_pad * (size_t)nrows);  // [t][row], tracklet-major
+  L.off_tl_state = take(sizeof(float4) * kStateVec * (size_t)(L.scap_pad + 1));  // follower state between phases A and B
+  L.off_surv = take(sizeof(int32_t) * (size_t)(L.scap_pad + 2));
+  L.off_surv_scan = take(sizeof(int32_t) * (size_t)(L.scap_pad + 2));
+  L.off_picked = take((size_t)(n + 256));  // one byte per cluster: attached by some upward leg (R17)
   L.off_chunk_base = take(sizeof(int32_t) * (size_t)(nchunks + 2));   // tracklets before chunk (sector, slab, row)
   L.off_chunk_scan0 = take(sizeof(int32_t) * (size_t)(nchunks + 2));  // grid-order start count at the chunk's first cluster
   L.off_scan_tmp = take(sizeof(int64_t) * (size_t)L.scan_tiles);
@@ -162,6 +171,9 @@ struct Ws {
   long long* tl_scan;
   int32_t* row_hit;
   int32_t *chunk_base, *chunk_scan0;
+  float4* tl_state;
+  int32_t *surv, *surv_scan;
+  uint8_t* picked;
   long long* scan_tmp;
 };
 
@@ -186,6 +198,10 @@ inline Ws bind_ws(const Layout& L, void* workspace) {
   w.tl_mask = (uint32_t*)(b + L.off_tl_mask);
   w.tl_scan = (long long*)(b + L.off_tl_scan);
   w.row_hit = (int32_t*)(b + L.off_row_hit);
+  w.tl_state = (float4*)(b + L.off_tl_state);
+  w.surv = (int32_t*)(b + L.off_surv);
+  w.surv_scan = (int32_t*)(b + L.off_surv_scan);
+  w.picked = (uint8_t*)(b + L.off_picked);
   w.chunk_base = (int32_t*)(b + L.off_chunk_base);
   w.chunk_scan0 = (int32_t*)(b + L.off_chunk_scan0);
   w.scan_tmp = (long long*)(b + L.off_scan_tmp);
@@ -233,7 +249,8 @@ __device__ __forceinline__ int clampbin(float v, int n) {
 
 __device__ __forceinline__ Rec ld_rec(const Rec* __restrict__ recs, int k) { return __ldg(recs + k); }
 __device__ __forceinline__ int rec_idx(const Rec& r) { return __float_as_int(r.z); }
-__device__ __forceinline__ int rec_sr(const Rec& r) { return __float_as_int(r.w); }
+__device__ __forceinline__ int rec_sr(const Rec& r) { return __float_as_int(r.w) & (kStartBit - 1); }
+__device__ __forceinline__ bool rec_is_start(const Rec& r) { return (__float_as_int(r.w) & kStartBit) != 0; }
 
 // R20 selection key (layout above)
 __device__ __forceinline__ unsigned long long sel_key(int nh, int start_orig, int t) {

@@ -280,14 +280,17 @@ k_chunk_counts(const __grid_constant__ Geo g, int64_t nchunks, const int32_t* __
 // with full memory-level parallelism instead of as a dependent chain inside the follower.
 __global__ void __launch_bounds__(kThreads)
 k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const int32_t* __restrict__ scan,
-                 const Rec* __restrict__ rec, const int32_t* __restrict__ up_c, const int32_t* __restrict__ chunk_base,
+                 Rec* rec, const int32_t* __restrict__ up_c, const int32_t* __restrict__ chunk_base,
                  const int32_t* __restrict__ chunk_scan0, TlInit* __restrict__ tl_init, int32_t* __restrict__ ws_counters) {
   const Scalars& sc = g.s;
   for (int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x; p < n; p += (int64_t)gridDim.x * kThreads) {
     const int ex = scan[p];
     if (scan[p + 1] != ex) {
-      const Rec h0 = ld_rec(rec, (int)p);
+      const Rec h0 = rec[p];
       const int sr0 = rec_sr(h0);
+      // mark the record as a start hit: the upward legs of the follower look at this bit (R17).  Only this thread
+      // writes this word; other threads read at most y and z of this record.
+      reinterpret_cast<int*>(rec + p)[3] = sr0 | kStartBit;
       const int s = sr0 / sc.nrows, r = sr0 - s * sc.nrows;
       const float zeta = (s < 18) ? h0.y : -h0.y;  // R2/R7, the same expression the grid build bins with
       const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
@@ -295,7 +298,7 @@ k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const i
       const int t = chunk_base[q] + (ex - chunk_scan0[q]);
       if (t < scap) {
         const int p1 = up_c[p];
-        const Rec h1 = ld_rec(rec, p1);
+        const Rec h1 = rec[p1];
         float4* o = reinterpret_cast<float4*>(tl_init + t);
         o[0] = make_float4(h0.x, h0.y, h1.x, h1.y);
         o[1] = make_float4(__int_as_float((int)p), __int_as_float(p1), __int_as_float(sr0), h0.z);
@@ -355,7 +358,7 @@ cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64
   // queue heads restart; status bits from the grid build are kept
   if ((e = cudaMemsetAsync(w.counters + WC_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.counters + WC_N_STARTS, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(w.counters + WC_PROP64, 0, sizeof(int32_t) * 6, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(w.counters + WC_PROP64, 0, sizeof(int32_t) * 8, st)) != cudaSuccess) return e;
   int32_t* flag = w.key;  // the bin ids of the grid build are dead by now
   if (n > 0)
     TPC_LAUNCH(KID_NEIGHBOURS, st,

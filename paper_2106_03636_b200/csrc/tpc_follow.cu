@@ -19,6 +19,7 @@
 #include "tpc_common.cuh"
 #include "tpc_kalman.cuh"
 #include "tpc_prof.cuh"
+#include "tpc_scan.cuh"
 #include "tpc_search.cuh"
 
 namespace tpc {
@@ -48,16 +49,22 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
+// PHASE_B = false: phase A (R14 init, R15 chain, R16 upward leg) for every start hit; the state at the end of the
+// upward leg goes to tl_state, and every START hit an upward leg attaches is marked in `picked` (R17).
+// PHASE_B = true: the tracklets listed in `surv` (start hit not picked up) resume from tl_state with the R17 jump
+// and the R16 downward leg, and write their R18 record and R20 key.
+template <bool PHASE_B>
 __global__ void __launch_bounds__(kFollowThreads, TPC_FOLLOW_MIN_BLOCKS)
 k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32_t* __restrict__ bin_first,
          const int32_t* __restrict__ up_c, const TlInit* __restrict__ tl_init, int32_t* __restrict__ row_hit,
-         int32_t* __restrict__ tl_info, unsigned long long* __restrict__ tl_key, int32_t* __restrict__ ws_counters) {
+         int32_t* __restrict__ tl_info, unsigned long long* __restrict__ tl_key, float4* __restrict__ tl_state,
+         const int32_t* __restrict__ surv, uint8_t* __restrict__ picked, int32_t* __restrict__ ws_counters) {
   __shared__ SmRow sm;
   load_rows(sm, g);
   __syncthreads();
   const Scalars& sc = g.s;
   const int nrows = sc.nrows;
-  const int n_starts = ws_counters[WC_N_STARTS];
+  const int n_starts = PHASE_B ? ws_counters[WC_N_SURV] : ws_counters[WC_N_STARTS];
   const int lane = threadIdx.x & 31;
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
 
@@ -67,7 +74,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   float zref = 0.0f;
   int t = 0, s = 0, r0 = 0, r_at = 0, r = 0, hn = -1, p0 = 0, orig0 = 0;
   int misses = 0, nh = 0, lo = 0, hi = 0;
-  unsigned nprop = 0, nupd = 0, ncand = 0;  // work counters of this lane over all its tracklets (TPC_CNT_PROP/UPD/CAND)
+  unsigned nprop = 0, nupd = 0, ncand = 0, nclaims = 0;  // work counters of this lane over all its tracklets
   int pf_ka = -1;  // first grid position of the bin the NEXT step is expected to search (-1: no prediction)
 #pragma unroll
   for (int k = 0; k < 5; k++) st.p[k] = 0.0f;
@@ -80,13 +87,36 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     if (need) {
       const int leader = __ffs(need) - 1;
       int base = 0;
-      if (lane == leader) base = atomicAdd(ws_counters + WC_QUEUE, __popc(need));
+      if (lane == leader) base = atomicAdd(ws_counters + (PHASE_B ? WC_QUEUE_B : WC_QUEUE), __popc(need));
       base = __shfl_sync(kFull, base, leader);
       if (phase == PH_FETCH) {
-        t = base + __popc(need & ((1u << lane) - 1u));
-        if (t >= n_starts) {
+        const int q = base + __popc(need & ((1u << lane) - 1u));
+        if (q >= n_starts) {
           phase = PH_DONE;
+        } else if (PHASE_B) {
+          t = __ldg(surv + q);
+          const float4 b = __ldg(reinterpret_cast<const float4*>(tl_init + t) + 1);
+          const float4* sp = tl_state + (int64_t)t * kStateVec;
+          const float4 v0 = sp[0], v1 = sp[1], v2 = sp[2], v3 = sp[3], v4 = sp[4], v5 = sp[5];
+          p0 = __float_as_int(b.x);
+          const int sr0 = __float_as_int(b.z);
+          orig0 = __float_as_int(b.w);
+          s = sr0 / nrows;
+          r0 = sr0 - s * nrows;
+          st.p[0] = v0.x; st.p[1] = v0.y; st.p[2] = v0.z; st.p[3] = v0.w; st.p[4] = v1.x;
+          st.C[0] = v1.y; st.C[1] = v1.z; st.C[2] = v1.w;
+          st.C[3] = v2.x; st.C[4] = v2.y; st.C[5] = v2.z; st.C[6] = v2.w;
+          st.C[7] = v3.x; st.C[8] = v3.y; st.C[9] = v3.z; st.C[10] = v3.w;
+          st.C[11] = v4.x; st.C[12] = v4.y; st.C[13] = v4.z; st.C[14] = v4.w;
+          zref = v5.x;
+          r_at = __float_as_int(v5.y);
+          const int info = __float_as_int(v5.z);
+          nh = info & 0xff;
+          lo = (info >> 8) & 0xff;
+          hi = (info >> 16) & 0xff;
+          phase = PH_JUMP;
         } else {
+          t = q;
           const float4* ip = reinterpret_cast<const float4*>(tl_init + t);
           const float4 a = __ldg(ip), b = __ldg(ip + 1);
           p0 = __float_as_int(b.x);
@@ -115,8 +145,9 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     if (__all_sync(kFull, phase == PH_DONE)) break;
 
     // ---- target row of this step; chain steps prefetch their next link --------------------------
-    const bool isI = phase == PH_INIT, chain = phase == PH_CHAIN, isJ = phase == PH_JUMP;
-    const bool leg = phase == PH_UP || phase == PH_DOWN;
+    // phase A never sees PH_JUMP / PH_DOWN, phase B never PH_INIT / PH_CHAIN / PH_UP: the template prunes them
+    const bool isI = !PHASE_B && phase == PH_INIT, chain = !PHASE_B && phase == PH_CHAIN, isJ = PHASE_B && phase == PH_JUMP;
+    const bool leg = PHASE_B ? phase == PH_DOWN : phase == PH_UP;
     int rn = r0;                      // PH_INIT, PH_JUMP
     if (chain) rn = r_at + 1;         // links join adjacent rows (R9)
     if (leg) rn = r;
@@ -180,7 +211,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     const int n0 = e0 - ka0, n1 = e1 - ka1;
     // ---- arg-min chi2 over the candidates (ties: lowest original index) ----------------------------
     __syncwarp();
-    bool have = false;
+    bool have = false, bstart = false;  // bstart: the best candidate is a start hit (R17 marking)
     float best = 0.0f, by = 0.0f, bz = 0.0f;
     int bi = 0, bk = -1;
     const int ntot = n0 + n1;
@@ -226,6 +257,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
           bk = ks;
           by = cs.x;
           bz = cs.y;
+          bstart = rec_is_start(cs);
         }
       }
       if (inmask & (inmask - 1u)) {  // more than one slot inside the window
@@ -241,6 +273,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
               bk = kk[j];
               by = c[j].x;
               bz = c[j].y;
+              bstart = rec_is_start(c[j]);
             }
           }
         }
@@ -264,6 +297,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
             bk = k;
             by = c.x;
             bz = c.y;
+            bstart = rec_is_start(c);
           }
         }
       }
@@ -289,7 +323,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     //   previous row here, so the slope costs two subtractions.
     if (TPC_FOLLOW_PREFETCH && chain && upd && nxt >= 0) prefetch_l1(rec + nxt);
     if (TPC_FOLLOW_PREFETCH && moved && ok && !isJ) {
-      const int r2 = rn + ((phase == PH_DOWN) ? -1 : 1);
+      const int r2 = rn + (PHASE_B ? -1 : 1);
       if (r2 >= 0 && r2 < nrows) {
         const float y2 = yp + (yp - st.p[0]);
         const float z2 = zref + (dzp + (dzp - st.p[1]));
@@ -315,7 +349,8 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     __syncwarp();
     const bool searched = leg && ok && !edge_out;
     if (upd || searched) row_hit[(int64_t)t * nrows + rn] = upd ? mk : -1;
-    bool finish = false;
+    if (!PHASE_B && leg && upd && bstart) picked[mk] = 1;  // R17: an upward leg attached another tracklet's start hit
+    bool finish = false;  // phase A: end of the upward leg; phase B: end of the tracklet
     if (isI) {
       phase = PH_CHAIN;
     } else if (chain) {
@@ -324,31 +359,39 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
         phase = PH_UP;
         r = r_at + 1;
         misses = 0;
-        if (r >= nrows) phase = PH_JUMP;
+        if (r >= nrows) finish = true;
       }
     } else if (leg) {
       misses = upd ? 0 : misses + 1;
-      r += (phase == PH_UP) ? 1 : -1;
-      if (!searched || misses > sc.max_gap || r < 0 || r >= nrows) {  // end of the leg
-        if (phase == PH_UP) phase = PH_JUMP;  // R17
-        else finish = true;
-      }
-    } else if (isJ) {
+      r += PHASE_B ? -1 : 1;
+      if (!searched || misses > sc.max_gap || r < 0 || r >= nrows) finish = true;  // end of the leg
+    } else if (isJ) {  // R17
       phase = PH_DOWN;
       r = r0 - 1;
       misses = 0;
       if (!ok || r < 0) finish = true;
     }
-    if (finish) {  // R18 record; the R20 key is pushed by k_push_keys
-      tl_info[t] = nh | (lo << 8) | (hi << 16);
-      tl_key[t] = sel_key(nh, orig0, t);
+    if (finish) {
+      if (PHASE_B) {  // R18 record; the R20 key is pushed by k_push_keys
+        tl_info[t] = nh | (lo << 8) | (hi << 16);
+        tl_key[t] = sel_key(nh, orig0, t);
+        nclaims += nh;
+      } else {  // park the state: phase B resumes it if no upward leg picked this tracklet's start hit up
+        float4* sp = tl_state + (int64_t)t * kStateVec;
+        sp[0] = make_float4(st.p[0], st.p[1], st.p[2], st.p[3]);
+        sp[1] = make_float4(st.p[4], st.C[0], st.C[1], st.C[2]);
+        sp[2] = make_float4(st.C[3], st.C[4], st.C[5], st.C[6]);
+        sp[3] = make_float4(st.C[7], st.C[8], st.C[9], st.C[10]);
+        sp[4] = make_float4(st.C[11], st.C[12], st.C[13], st.C[14]);
+        sp[5] = make_float4(zref, __int_as_float(r_at), __int_as_float(nh | (lo << 8) | (hi << 16)), 0.0f);
+      }
       phase = PH_FETCH;
     }
   }
   // one 64-bit atomic per warp and counter
 #pragma unroll
-  for (int k = 0; k < 3; k++) {
-    unsigned long long v = k == 0 ? nprop : (k == 1 ? nupd : ncand);
+  for (int k = 0; k < 4; k++) {
+    unsigned long long v = k == 0 ? nprop : (k == 1 ? nupd : (k == 2 ? ncand : nclaims));
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(kFull, v, d);
     if (lane == 0 && v) atomicAdd((unsigned long long*)(ws_counters + WC_PROP64) + k, v);
@@ -359,18 +402,67 @@ int g_follow_blocks = 0;
 
 }  // namespace
 
+namespace {
+
+constexpr int kThreads = 256;
+
+// R17: a tracklet goes on to phase B iff no upward leg attached its start hit; the others are absorbed and get an
+// empty R18 record (nHits = 0, empty row range), so that selection and export skip them.
+__global__ void __launch_bounds__(kThreads)
+k_survivor_flags(int64_t scap_pad, const TlInit* __restrict__ tl_init, const uint8_t* __restrict__ picked,
+                 int32_t* __restrict__ tl_info, int32_t* __restrict__ flag, const int32_t* __restrict__ ws_counters) {
+  const int n_starts = ws_counters[WC_N_STARTS];
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t <= scap_pad; t += (int64_t)gridDim.x * kThreads) {
+    int f = 0;
+    if (t < n_starts) {
+      f = picked[tl_init[t].p0] ? 0 : 1;
+      if (!f) tl_info[t] = 0 | (1 << 8) | (0 << 16);
+    }
+    flag[t] = f;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_survivor_list(int64_t scap_pad, const int32_t* __restrict__ scan, int32_t* __restrict__ surv,
+                int32_t* __restrict__ ws_counters) {
+  const int n_starts = ws_counters[WC_N_STARTS];
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < scap_pad; t += (int64_t)gridDim.x * kThreads) {
+    if (t == 0) ws_counters[WC_N_SURV] = scan[scap_pad];
+    if (t < n_starts) {
+      const int i = scan[t];
+      if (scan[t + 1] != i) surv[i] = (int)t;
+    }
+  }
+}
+
+}  // namespace
+
 cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st) {
   cudaError_t e;
+  const int64_t scap_pad = w.L.scap_pad;
   if (g_follow_blocks == 0) {
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_follow, kFollowThreads, 0)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_follow<false>, kFollowThreads, 0)) != cudaSuccess) return e;
     g_follow_blocks = sms * (per_sm > 0 ? per_sm : 1);
   }
+  if ((e = cudaMemsetAsync(w.picked, 0, (size_t)(w.L.n + 1), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(w.counters + WC_QUEUE_B, 0, sizeof(int32_t) * 2, st)) != cudaSuccess) return e;  // + WC_N_SURV
   TPC_LAUNCH(KID_FOLLOW, st,
-             (k_follow<<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
-                                                                  w.tl_info, w.tl_key, w.counters)));
+             (k_follow<false><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                                                                         w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
+                                                                         w.counters)));
+  TPC_LAUNCH(KID_SURVIVORS, st,
+             (k_survivor_flags<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(scap_pad, w.tl_init, w.picked, w.tl_info,
+                                                                                        w.surv_scan, w.counters)));
+  if ((e = exclusive_scan<int32_t>(w.surv_scan, w.surv_scan, scap_pad + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
+  TPC_LAUNCH(KID_SURVIVORS, st,
+             (k_survivor_list<<<blocks_for(scap_pad, kThreads), kThreads, 0, st>>>(scap_pad, w.surv_scan, w.surv, w.counters)));
+  TPC_LAUNCH(KID_FOLLOW_B, st,
+             (k_follow<true><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                                                                        w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
+                                                                        w.counters)));
   return cudaGetLastError();
 }
 

@@ -24,6 +24,8 @@ enum KernelId {
   KID_CLEAN,
   KID_COMPACT_STARTS,
   KID_FOLLOW,
+  KID_SURVIVORS,
+  KID_FOLLOW_B,
   KID_PUSH_KEYS,
   KID_COUNT_KEPT,
   KID_WRITE_TRACKS,

@@ -11,7 +11,8 @@
 //                   the (y, z, row) record of every hit for the refit, cluster_track, and the
 //                   per-track arrays; the counters block
 //
-// Tracklets are numbered by (sector, z slab, row) (tpc_find.cu), so the few thousand warps in
+// Only the tracklets that went through phase B of the follower (`surv`, R17) take part.  Tracklets are numbered by
+// (sector, z slab, row) (tpc_find.cu), so the few thousand warps in
 // flight work on one z slab of one sector: the owner / record gathers and the atomics stay in L2.
 // =============================================================================================
 #include "tpc_common.cuh"
@@ -27,11 +28,12 @@ constexpr int kThreads = 256;
 __global__ void __launch_bounds__(kThreads)
 k_push_keys(int nrows, const int32_t* __restrict__ row_hit, const int32_t* __restrict__ tl_info,
             const unsigned long long* __restrict__ tl_key, unsigned long long* __restrict__ owner,
-            const int32_t* __restrict__ ws_counters) {
-  const int n_starts = ws_counters[WC_N_STARTS];
+            const int32_t* __restrict__ surv, const int32_t* __restrict__ ws_counters) {
+  const int n_surv = ws_counters[WC_N_SURV];
   const int lane = threadIdx.x & 31;
   const int64_t nwarps = (int64_t)gridDim.x * (kThreads / 32);
-  for (int64_t t = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); t < n_starts; t += nwarps) {
+  for (int64_t i = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); i < n_surv; i += nwarps) {
+    const int64_t t = __ldg(surv + i);
     const int info = __ldg(tl_info + t);
     const int lo = (info >> 8) & 0xff, hi = (info >> 16) & 0xff;
     const unsigned long long key = __ldg(tl_key + t);
@@ -55,11 +57,13 @@ k_push_keys(int nrows, const int32_t* __restrict__ row_hit, const int32_t* __res
 __global__ void __launch_bounds__(kThreads)
 k_count_kept(int nrows, int min_hits, const int32_t* __restrict__ row_hit, const int32_t* __restrict__ tl_info,
              const unsigned long long* __restrict__ tl_key, const unsigned long long* __restrict__ owner,
-             uint32_t* __restrict__ tl_mask, long long* __restrict__ tl_val, const int32_t* __restrict__ ws_counters) {
-  const int n_starts = ws_counters[WC_N_STARTS];
+             uint32_t* __restrict__ tl_mask, long long* __restrict__ tl_val, const int32_t* __restrict__ surv,
+             const int32_t* __restrict__ ws_counters) {
+  const int n_surv = ws_counters[WC_N_SURV];
   const int lane = threadIdx.x & 31;
   const int64_t nwarps = (int64_t)gridDim.x * (kThreads / 32);
-  for (int64_t t = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); t < n_starts; t += nwarps) {
+  for (int64_t i = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); i < n_surv; i += nwarps) {
+    const int64_t t = __ldg(surv + i);
     const int info = __ldg(tl_info + t);
     const int lo = (info >> 8) & 0xff, hi = (info >> 16) & 0xff;
     const unsigned long long key = __ldg(tl_key + t);
@@ -94,8 +98,9 @@ k_write_tracks(int nrows, const Rec* __restrict__ rec, const TlInit* __restrict_
                const long long* __restrict__ tl_scan, int64_t scap_pad, int64_t max_tracks,
                int32_t* __restrict__ cluster_track, int32_t* __restrict__ trk_seed, int32_t* __restrict__ trk_sector,
                int32_t* __restrict__ trk_nhits, int64_t* __restrict__ trk_first_hit, int32_t* __restrict__ trk_hits,
-               float4* __restrict__ hit_rec, int32_t* __restrict__ counters, const int32_t* __restrict__ ws_counters) {
-  const int n_starts = ws_counters[WC_N_STARTS];
+               float4* __restrict__ hit_rec, int32_t* __restrict__ counters, const int32_t* __restrict__ surv,
+               const int32_t* __restrict__ ws_counters) {
+  const int n_starts = ws_counters[WC_N_STARTS], n_surv = ws_counters[WC_N_SURV];
   const int lane = threadIdx.x & 31;
   const int64_t nwarps = (int64_t)gridDim.x * (kThreads / 32);
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -107,13 +112,12 @@ k_write_tracks(int nrows, const Rec* __restrict__ rec, const TlInit* __restrict_
     counters[TPC_CNT_STARTS_FOUND] = ws_counters[WC_STARTS_FOUND];
     if (K <= max_tracks) counters[TPC_CNT_HITS] = (int)(total & 0xffffffffll);
     counters[TPC_CNT_STATUS] = ws_counters[WC_STATUS] | (K > max_tracks ? TPC_ST_TRACK_OVERFLOW : 0);
-    counters[TPC_CNT_RESERVED6] = 0;
+    counters[TPC_CNT_FOLLOWED_DOWN] = n_surv;
     counters[TPC_CNT_RESERVED7] = 0;
-    for (int k = 0; k < 6; k++) counters[TPC_CNT_PROP_LO + k] = ws_counters[WC_PROP64 + k];
-    counters[14] = 0;
-    counters[15] = 0;
+    for (int k = 0; k < 8; k++) counters[TPC_CNT_PROP_LO + k] = ws_counters[WC_PROP64 + k];
   }
-  for (int64_t t = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); t < n_starts; t += nwarps) {
+  for (int64_t i = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); i < n_surv; i += nwarps) {
+    const int64_t t = __ldg(surv + i);
     const long long ex = __ldg(tl_scan + t), nx = __ldg(tl_scan + t + 1);
     const long long k = ex >> 32;
     if ((nx >> 32) == k) continue;  // not accepted (R20)
@@ -168,16 +172,16 @@ cudaError_t launch_select(const Geo& g, const Ws& w, int32_t* cluster_track, int
   if (n > 0) {
     if ((e = cudaMemsetAsync(cluster_track, 0xFF, sizeof(int32_t) * (size_t)n, st)) != cudaSuccess) return e;
     TPC_LAUNCH(KID_PUSH_KEYS, st,
-               (k_push_keys<<<wblocks, kThreads, 0, st>>>(nrows, w.row_hit, w.tl_info, w.tl_key, w.owner, w.counters)));
+               (k_push_keys<<<wblocks, kThreads, 0, st>>>(nrows, w.row_hit, w.tl_info, w.tl_key, w.owner, w.surv, w.counters)));
     TPC_LAUNCH(KID_COUNT_KEPT, st,
                (k_count_kept<<<wblocks, kThreads, 0, st>>>(nrows, g.s.min_hits, w.row_hit, w.tl_info, w.tl_key, w.owner,
-                                                          w.tl_mask, w.tl_scan, w.counters)));
+                                                          w.tl_mask, w.tl_scan, w.surv, w.counters)));
   }
   if ((e = exclusive_scan<long long>(w.tl_scan, w.tl_scan, scap_pad + 1, w.scan_tmp, st)) != cudaSuccess) return e;
   TPC_LAUNCH(KID_WRITE_TRACKS, st,
              (k_write_tracks<<<wblocks, kThreads, 0, st>>>(nrows, w.rec, w.tl_init, w.row_hit, w.tl_mask, w.tl_scan, scap_pad,
                                                           max_tracks, cluster_track, trk_seed, trk_sector, trk_nhits,
-                                                          trk_first_hit, trk_hits, w.hit_rec, counters, w.counters)));
+                                                          trk_first_hit, trk_hits, w.hit_rec, counters, w.surv, w.counters)));
   return cudaGetLastError();
 }
 
