@@ -624,3 +624,36 @@ def test_sector_independence_whole_event_vs_single_sector(orc):
         assert st["tracks_oracle"] == st["tracks_cuda"] == st["tracks_same_hits"] > 10
         assert st["assign_identical"] == sel.size
         assert st["par_bit_identical"] and st["cov_bit_identical"]
+
+
+# --------------------------------------------------------------------------------------------
+# R17 (two-phase following): a track cut into chain fragments by missing rows is followed to the end by ONE
+# tracklet -- the one starting at the lowest fragment; the start hits of the other fragments are picked up by its
+# upward leg and their tracklets record nothing
+# --------------------------------------------------------------------------------------------
+def test_R17_fragments_of_one_track_are_absorbed_by_the_lowest(orc):
+    ev = single_helix(0.6, math.radians(9.0), 0.4)
+    rows = ev.sector_row % 152
+    drop = np.isin(rows, [40, 41, 80, 120])            # three gaps (<= max_gap rows) -> four chain fragments
+    y, z, sr = ev.y[~drop], ev.z[~drop], ev.sector_row[~drop]
+    o = orc.run(ev.params, y, z, sr, "f32", True)
+    rsel = sr % 152
+    assert o["starts"].size == 4, "one start hit per fragment"
+    start_rows = np.sort(rsel[o["starts"]])
+    # a fragment's first cluster has no down-neighbour, hence no link pair (R9): its second cluster is the start hit
+    assert list(start_rows[1:]) == [43, 82, 122] and start_rows[0] == int(rsel.min()) + 1
+    nh = o["n_hits"][np.argsort(rsel[o["starts"]])]
+    assert nh[0] == y.size and np.all(nh[1:] == 0), f"lowest fragment follows the whole track, the others are absorbed: {nh}"
+    assert o["trk_seed"].size == 1 and o["trk_nhits"][0] == y.size
+    rh = o["row_hit"][np.argsort(rsel[o["starts"]])]
+    assert np.all(rh[1:] == -1)
+
+
+def test_R17_a_gap_too_long_to_bridge_leaves_two_tracks(orc):
+    ev = single_helix(0.6, math.radians(9.0), 0.4)
+    rows = ev.sector_row % 152
+    drop = (rows >= 60) & (rows < 70)                   # 10 missing rows > max_gap: nobody picks the upper start hit up
+    y, z, sr = ev.y[~drop], ev.z[~drop], ev.sector_row[~drop]
+    o = orc.run(ev.params, y, z, sr, "f32", True)
+    assert o["starts"].size == 2 and np.all(o["n_hits"] > 0)
+    assert o["trk_seed"].size == 2 and int(o["trk_nhits"].sum()) == y.size
