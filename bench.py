@@ -61,9 +61,9 @@ KERNEL_MODEL = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
 # launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
-NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.66, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.14, "k_neighbours": 8.99,
-                     "k_clean": 2.26, "k_compact_starts": 2.06, "k_follow": 26.43, "k_push_keys": 5.79,
-                     "k_count_kept": 6.26, "k_write_tracks": 22.90, "k_fit": 4.87}
+NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.14, "k_neighbours": 8.96,
+                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 30.06, "k_push_keys": 3.22,
+                     "k_count_kept": 2.16, "k_write_tracks": 19.06, "k_fit": 4.71}      # k_follow: phases A + B
 
 
 def parse_args():
