@@ -32,6 +32,8 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -338,6 +340,7 @@ void clean_links(int64_t n, const int32_t* link_up, const int32_t* link_dn, int3
   for (int64_t h = 0; h < n; h++) {
     up_c[h] = (link_up[h] >= 0 && link_dn[link_up[h]] == (int32_t)h) ? link_up[h] : -1;
     dn_c[h] = (link_dn[h] >= 0 && link_up[link_dn[h]] == (int32_t)h) ? link_dn[h] : -1;
+    if (up_c[h] < 0 && dn_c[h] >= 0) up_c[h] = -2;   // R10: top of a chain (linked downward only); read by R17
   }
   starts.clear();
   for (int64_t h = 0; h < n; h++)
@@ -400,6 +403,30 @@ struct Follower {
       }
     }
     return r_at;
+  }
+
+  // R17 wave test: does the backward straight line through the start hit h0 and its up-neighbour meet, within
+  // max_gap + 3 rows below, the top of a lower chain (up' = -2)?  (A chain's last cluster and a fragment's first
+  // cluster carry no links by R9, so a gap of g missing rows puts the lower chain top g + 3 rows below h0.)
+  // Tolerance 4 sigma per row of distance plus one.  Such a start hit waits for the first wave: the tracklet of the lower
+  // fragment will most likely pick it up.
+  bool has_predecessor(int32_t h0, const int32_t* up_c) const {
+    const int sector = cl.sector(h0), r0 = cl.row(h0);
+    const int32_t h1 = up_c[h0];
+    const T dxu = G.X[cl.row(h1)] - G.X[r0];
+    const T my = (cl.y[h1] - cl.y[h0]) / dxu, mz = (cl.z[h1] - cl.z[h0]) / dxu;
+    bool found = false;
+    for (int k = 1; k <= P.max_gap + 3 && !found; k++) {
+      const int r = r0 - k;
+      if (r < 0) break;
+      const T dxk = G.X[r0] - G.X[r];
+      const T yp = cl.y[h0] - my * dxk, zp = cl.z[h0] - mz * dxk;
+      const T ty = ((T)4 * (T)P.sigma_y) * (T)(k + 1), tz = ((T)4 * (T)P.sigma_z) * (T)(k + 1);
+      ix.visit(sector, r, yp - ty, yp + ty, zp - tz, zp + tz, [&](int32_t c) {
+        if (std::fabs(cl.y[c] - yp) <= ty && std::fabs(cl.z[c] - zp) <= tz && up_c[c] == -2) found = true;
+      });
+    }
+    return found;
   }
 
   // Phase A of following start hit h0 (R14 init, R15 chain, R16 upward leg); row_hit[nrows] receives original
@@ -557,12 +584,29 @@ int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const
   std::vector<State<T>> sts((size_t)n_starts);
   std::vector<T> zrefs((size_t)n_starts);
   std::vector<int> r_ats((size_t)n_starts);
+  // Two waves of phase A: start hits with a plausible predecessor below them (has_predecessor) wait; after the
+  // first wave only those of them that no upward leg picked up are followed (second wave).  The rest never run.
+  std::vector<uint8_t> waits((size_t)n_starts, 0), ran((size_t)n_starts, 0);
+  for (int64_t t = 0; t < n_starts; t++) waits[(size_t)t] = f.has_predecessor(starts[t], up_c) ? 1 : 0;
   f.picked_up = picked_up.data();
-  for (int64_t t = 0; t < n_starts; t++)
-    f.follow_up(starts[t], up_c, row_hit + t * c.G.nrows, (int)t, &sts[(size_t)t], &zrefs[(size_t)t], &r_ats[(size_t)t]);
+  for (int wave = 0; wave < 2; wave++) {
+    std::vector<int64_t> todo;
+    for (int64_t t = 0; t < n_starts; t++)
+      if (wave == 0 ? !waits[(size_t)t] : (waits[(size_t)t] && !picked_up[(size_t)starts[t]])) todo.push_back(t);
+    for (int64_t t : todo) {
+      f.follow_up(starts[t], up_c, row_hit + t * c.G.nrows, (int)t, &sts[(size_t)t], &zrefs[(size_t)t], &r_ats[(size_t)t]);
+      ran[(size_t)t] = 1;
+    }
+  }
   f.picked_up = nullptr;
+  if (std::getenv("ORC_VERBOSE")) {
+    int64_t nw = 0, nr = 0;
+    for (int64_t t = 0; t < n_starts; t++) { nw += waits[(size_t)t]; nr += ran[(size_t)t]; }
+    std::fprintf(stderr, "R17 waves: %lld start hits, %lld wait, %lld ran phase A\n", (long long)n_starts, (long long)nw, (long long)nr);
+  }
   for (int64_t t = 0; t < n_starts; t++) {
-    if (picked_up[(size_t)starts[t]]) {
+    if (!ran[(size_t)t]) sts[(size_t)t] = State<T>();
+    if (!ran[(size_t)t] || picked_up[(size_t)starts[t]]) {
       n_hits[t] = 0;
       for (int r = 0; r < c.G.nrows; r++) row_hit[t * c.G.nrows + r] = -1;
     } else {

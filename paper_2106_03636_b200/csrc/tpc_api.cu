@@ -83,6 +83,8 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
   s.kB = P->kB;
   s.sy2 = P->sigma_y * P->sigma_y;
   s.sz2 = P->sigma_z * P->sigma_z;
+  s.sig_y = P->sigma_y;
+  s.sig_z = P->sigma_z;
   s.ca_cut = P->ca_cut;
   s.chi2_cut = P->chi2_cut;
   s.chi2_chain_cut = P->chi2_chain_cut;

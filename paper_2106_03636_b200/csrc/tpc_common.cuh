@@ -41,7 +41,7 @@ struct Scalars {
   int32_t nsec, nrows, nz, bins_per_sector;
   int32_t slab_w, nslab;  // tracklet ordering: z slabs of slab_w bins, nslab = ceil(nz / slab_w)
   float inv_cy, inv_cz, z_lo, z_hi;
-  float kB, sy2, sz2;
+  float kB, sy2, sz2, sig_y, sig_z;
   float ca_cut, chi2_cut, chi2_chain_cut, win_max, max_sinphi, edge_margin;
   int32_t max_gap, min_hits, n_fit_passes;
   float cov0[5];
@@ -62,6 +62,7 @@ enum {
   WC_FIT_QUEUE = 4,    // work-queue head of the cached refit
   WC_QUEUE_B = 5,      // work-queue head of the follower's phase B
   WC_N_SURV = 6,       // tracklets that go on to phase B (start hit not picked up by an upward leg, R17)
+  WC_N_WAVE = 7,       // tracklets of the current phase-A wave (R17)
   WC_PROP64 = 8,       // unsigned long long at [8,9]: follower transports
   WC_UPD64 = 10,       // unsigned long long at [10,11]: follower updates
   WC_CAND64 = 12,      // unsigned long long at [12,13]: candidates tested

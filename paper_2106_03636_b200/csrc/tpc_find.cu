@@ -242,7 +242,7 @@ k_clean(int64_t n, const int32_t* __restrict__ link_up, const int32_t* __restric
     const int u = link_up[p], d = link_dn[p];
     const int uc = (u >= 0 && __ldg(link_dn + u) == (int)p) ? u : -1;
     const int dc = (d >= 0 && __ldg(link_up + d) == (int)p) ? d : -1;
-    up_c[p] = uc;
+    up_c[p] = (uc < 0 && dc >= 0) ? -2 : uc;  // -2: top of a chain (linked downward only); read by the R17 wave test
     flag[p] = (uc >= 0 && dc < 0) ? 1 : 0;
   }
 }
@@ -316,7 +316,7 @@ k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const i
 // ---------------------------------------------------------------------------------------------
 // parity/debug export in original indices
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int to_orig(const Rec* rec, int pos) { return pos >= 0 ? rec_idx(rec[pos]) : -1; }
+__device__ __forceinline__ int to_orig(const Rec* rec, int pos) { return pos >= 0 ? rec_idx(rec[pos]) : pos; }
 
 __global__ void __launch_bounds__(kThreads)
 k_export_links(int64_t n, const Rec* __restrict__ rec, const int32_t* __restrict__ link_up,

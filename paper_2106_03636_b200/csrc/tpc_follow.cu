@@ -49,8 +49,9 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
-// PHASE_B = false: phase A (R14 init, R15 chain, R16 upward leg) for every start hit; the state at the end of the
-// upward leg goes to tl_state, and every START hit an upward leg attaches is marked in `picked` (R17).
+// PHASE_B = false: phase A (R14 init, R15 chain, R16 upward leg) for the tracklets of one wave, listed in `surv`
+// (R17: first the start hits without a plausible predecessor, then those of the rest that nobody picked up); the
+// state at the end of the upward leg goes to tl_state, and every START hit an upward leg attaches is marked in `picked` (R17).
 // PHASE_B = true: the tracklets listed in `surv` (start hit not picked up) resume from tl_state with the R17 jump
 // and the R16 downward leg, and write their R18 record and R20 key.
 template <bool PHASE_B>
@@ -64,7 +65,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   __syncthreads();
   const Scalars& sc = g.s;
   const int nrows = sc.nrows;
-  const int n_starts = PHASE_B ? ws_counters[WC_N_SURV] : ws_counters[WC_N_STARTS];
+  const int n_starts = PHASE_B ? ws_counters[WC_N_SURV] : ws_counters[WC_N_WAVE];  // entries of `surv` to work on
   const int lane = threadIdx.x & 31;
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
 
@@ -116,7 +117,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
           hi = (info >> 16) & 0xff;
           phase = PH_JUMP;
         } else {
-          t = q;
+          t = __ldg(surv + q);
           const float4* ip = reinterpret_cast<const float4*>(tl_init + t);
           const float4 a = __ldg(ip), b = __ldg(ip + 1);
           p0 = __float_as_int(b.x);
@@ -406,31 +407,83 @@ namespace {
 
 constexpr int kThreads = 256;
 
-// R17: a tracklet goes on to phase B iff no upward leg attached its start hit; the others are absorbed and get an
-// empty R18 record (nHits = 0, empty row range), so that selection and export skip them.
+// R17 wave test, one thread per tracklet: does the backward straight line through the start hit and its up-neighbour
+// meet, within max_gap + 3 rows below, the top of a lower chain (up' == -2)?  Tolerance 4 sigma per (rows + 1).
+// Such a start hit waits for the first wave.  The answer is kept in tl_info[t] until phase B overwrites it.
 __global__ void __launch_bounds__(kThreads)
-k_survivor_flags(int64_t scap_pad, const TlInit* __restrict__ tl_init, const uint8_t* __restrict__ picked,
-                 int32_t* __restrict__ tl_info, int32_t* __restrict__ flag, const int32_t* __restrict__ ws_counters) {
+k_wave_test(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32_t* __restrict__ bin_first,
+            const int32_t* __restrict__ up_c, const TlInit* __restrict__ tl_init, int32_t* __restrict__ tl_info,
+            const int32_t* __restrict__ ws_counters) {
+  __shared__ SmRow sm;
+  load_rows(sm, g);
+  __syncthreads();
+  const Scalars& sc = g.s;
+  const int nrows = sc.nrows;
+  const int n_starts = ws_counters[WC_N_STARTS];
+  const float sig_y = sc.sig_y, sig_z = sc.sig_z;
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < n_starts; t += (int64_t)gridDim.x * kThreads) {
+    const float4* ip = reinterpret_cast<const float4*>(tl_init + t);
+    const float4 a = __ldg(ip), b = __ldg(ip + 1);
+    const int sr0 = __float_as_int(b.z);
+    const int s = sr0 / nrows, r0 = sr0 - s * nrows;
+    const float dxu = sm.X[r0 + 1] - sm.X[r0];
+    const float my = (a.z - a.x) / dxu, mz = (a.w - a.y) / dxu;
+    bool found = false;
+    for (int k = 1; k <= sc.max_gap + 3 && !found; k++) {
+      const int r = r0 - k;
+      if (r < 0) break;
+      const float dxk = sm.X[r0] - sm.X[r];
+      const float yp = a.x - my * dxk, zp = a.y - mz * dxk;
+      const float ty = (4.0f * sig_y) * (float)(k + 1), tz = (4.0f * sig_z) * (float)(k + 1);
+      const BinWin W = bin_window(sm, sc, s, r, yp - ty, yp + ty, zp - tz, zp + tz);
+      for (int zi = 0; zi < W.nzb && !found; zi++) {
+        const int b0 = W.first + zi * W.ny;
+        const int ka = __ldg(bin_first + b0), ke = __ldg(bin_first + b0 + W.ybspan);
+        for (int c = ka; c < ke; c++) {
+          const Rec h = ld_rec(rec, c);
+          if (fabsf(h.x - yp) <= ty && fabsf(h.y - zp) <= tz && __ldg(up_c + c) == -2) found = true;
+        }
+      }
+    }
+    tl_info[t] = found ? 1 : 0;
+  }
+}
+
+// R17 lists.  mode 0: first wave = start hits that do not wait;  mode 1: second wave = waiting start hits that no
+// upward leg of the first wave picked up;  mode 2: phase B = tracklets whose start hit nobody picked up -- all
+// others (absorbed, or never run) get an empty R18 record (nHits = 0, empty row range) that selection and export skip.
+__global__ void __launch_bounds__(kThreads)
+k_list_flags(int mode, int64_t scap_pad, const TlInit* __restrict__ tl_init, const uint8_t* __restrict__ picked,
+             int32_t* __restrict__ tl_info, int32_t* __restrict__ flag, const int32_t* __restrict__ ws_counters) {
   const int n_starts = ws_counters[WC_N_STARTS];
   for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t <= scap_pad; t += (int64_t)gridDim.x * kThreads) {
     int f = 0;
     if (t < n_starts) {
-      f = picked[tl_init[t].p0] ? 0 : 1;
-      if (!f) tl_info[t] = 0 | (1 << 8) | (0 << 16);
+      if (mode == 0) {
+        f = tl_info[t] ? 0 : 1;
+      } else {
+        const bool pk = picked[tl_init[t].p0] != 0;
+        if (mode == 1) {
+          f = (tl_info[t] && !pk) ? 1 : 0;
+        } else {
+          f = pk ? 0 : 1;
+          if (!f) tl_info[t] = 0 | (1 << 8) | (0 << 16);
+        }
+      }
     }
     flag[t] = f;
   }
 }
 
 __global__ void __launch_bounds__(kThreads)
-k_survivor_list(int64_t scap_pad, const int32_t* __restrict__ scan, int32_t* __restrict__ surv,
-                int32_t* __restrict__ ws_counters) {
+k_list_build(int count_index, int64_t scap_pad, const int32_t* __restrict__ scan, int32_t* __restrict__ list,
+             int32_t* __restrict__ ws_counters) {
   const int n_starts = ws_counters[WC_N_STARTS];
   for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < scap_pad; t += (int64_t)gridDim.x * kThreads) {
-    if (t == 0) ws_counters[WC_N_SURV] = scan[scap_pad];
+    if (t == 0) ws_counters[count_index] = scan[scap_pad];
     if (t < n_starts) {
       const int i = scan[t];
-      if (scan[t + 1] != i) surv[i] = (int)t;
+      if (scan[t + 1] != i) list[i] = (int)t;
     }
   }
 }
@@ -448,21 +501,31 @@ cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st) {
     g_follow_blocks = sms * (per_sm > 0 ? per_sm : 1);
   }
   if ((e = cudaMemsetAsync(w.picked, 0, (size_t)(w.L.n + 1), st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(w.counters + WC_QUEUE_B, 0, sizeof(int32_t) * 2, st)) != cudaSuccess) return e;  // + WC_N_SURV
-  TPC_LAUNCH(KID_FOLLOW, st,
-             (k_follow<false><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
-                                                                         w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
-                                                                         w.counters)));
+  if ((e = cudaMemsetAsync(w.counters + WC_QUEUE_B, 0, sizeof(int32_t) * 3, st)) != cudaSuccess) return e;  // + N_SURV, N_WAVE
   TPC_LAUNCH(KID_SURVIVORS, st,
-             (k_survivor_flags<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(scap_pad, w.tl_init, w.picked, w.tl_info,
-                                                                                        w.surv_scan, w.counters)));
-  if ((e = exclusive_scan<int32_t>(w.surv_scan, w.surv_scan, scap_pad + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
-  TPC_LAUNCH(KID_SURVIVORS, st,
-             (k_survivor_list<<<blocks_for(scap_pad, kThreads), kThreads, 0, st>>>(scap_pad, w.surv_scan, w.surv, w.counters)));
-  TPC_LAUNCH(KID_FOLLOW_B, st,
-             (k_follow<true><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
-                                                                        w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
-                                                                        w.counters)));
+             (k_wave_test<<<blocks_for(w.L.scap, kThreads), kThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.tl_info,
+                                                                              w.counters)));
+  for (int mode = 0; mode < 3; mode++) {  // two waves of phase A, then phase B
+    TPC_LAUNCH(KID_SURVIVORS, st,
+               (k_list_flags<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(mode, scap_pad, w.tl_init, w.picked, w.tl_info,
+                                                                                      w.surv_scan, w.counters)));
+    if ((e = exclusive_scan<int32_t>(w.surv_scan, w.surv_scan, scap_pad + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
+    TPC_LAUNCH(KID_SURVIVORS, st,
+               (k_list_build<<<blocks_for(scap_pad, kThreads), kThreads, 0, st>>>(mode == 2 ? WC_N_SURV : WC_N_WAVE, scap_pad,
+                                                                                  w.surv_scan, w.surv, w.counters)));
+    if (mode < 2) {
+      if ((e = cudaMemsetAsync(w.counters + WC_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
+      TPC_LAUNCH(KID_FOLLOW, st,
+                 (k_follow<false><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                                                                             w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
+                                                                             w.counters)));
+    } else {
+      TPC_LAUNCH(KID_FOLLOW_B, st,
+                 (k_follow<true><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                                                                            w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
+                                                                            w.counters)));
+    }
+  }
   return cudaGetLastError();
 }
 

@@ -246,6 +246,8 @@ def test_R10_links_brute_force(orc):
     for h in range(n):
         eu = up[h] if (up[h] >= 0 and dn[up[h]] == h) else -1
         ed = dn[h] if (dn[h] >= 0 and up[dn[h]] == h) else -1
+        if eu < 0 and ed >= 0:
+            eu = -2                                    # R10: top of a chain (linked downward only)
         assert up_c[h] == eu and dn_c[h] == ed
     assert starts.tolist() == [h for h in range(n) if up_c[h] >= 0 and dn_c[h] < 0]
 
