@@ -50,8 +50,8 @@ KERNEL_MODEL = {
     "k_neighbours": ("hbm", {"cluster": 16 + 8}, None),           # own record in, two links out (neighbours from L2)
     "k_clean": ("hbm", {"cluster": 8 + 8}, None),
     "k_compact_starts": ("hbm", {"cluster": 4, "tracklet": 32}, None),
-    "k_follow": ("alu", {}, "step"),                              # both phases (two launches per step)
-    "k_survivor_*": ("hbm", {"tracklet": 32 + 1 + 4 + 12 + 4}, None),
+    "k_follow": ("alu", {}, "step"),                              # two waves of phase A + phase B (three launches per step)
+    "k_survivor_*": ("hbm", {"tracklet": 32 + 4 + 3 * (32 + 1 + 4 + 12 + 4)}, None),   # wave test + three list builds
     "k_push_keys": ("hbm", {"claim": 4 + 8 + 8, "tracklet": 12}, None),   # row_hit in, 8-byte atomicMax RMW
     "k_count_kept": ("hbm", {"claim": 4 + 8, "tracklet": 12 + 20 + 8}, None),   # row_hit, owner in; mask, value out
     "k_write_tracks": ("hbm", {"hit": 4 + 16 + 4 + 16 + 8, "tracklet": 16 + 20}, None),  # rec in; trk_hits, hit_rec, cluster_track out
@@ -61,9 +61,9 @@ KERNEL_MODEL = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
 # launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
-NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.14, "k_neighbours": 8.96,
-                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 30.06, "k_push_keys": 3.22,
-                     "k_count_kept": 2.16, "k_write_tracks": 19.06, "k_fit": 4.71}      # k_follow: phases A + B
+NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.15, "k_neighbours": 9.00,
+                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 28.35, "k_push_keys": 3.18,
+                     "k_count_kept": 2.17, "k_write_tracks": 19.19, "k_fit": 4.73}      # k_follow: all three launches
 
 
 def parse_args():
@@ -312,7 +312,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     launches = int(sum(v[1] for v in prof.values()))
     top = max(kern, key=lambda k: kern[k]["ms_per_step"])
     top_ms = kern[top]["ms_per_step"] / max(kern[top]["launches_per_step"], 1)
-    if top == "k_follow":      # phases A and B are two launches of one kernel; the work counters cover both
+    if top == "k_follow":      # the waves of phase A and phase B are launches of one kernel; the work counters cover all
         top_ms = kern[top]["ms_per_step"]
     nb = binding.grid_bins(ev.params)
     work = binding.work_counts(res["counters"])
