@@ -30,11 +30,12 @@ namespace {
 #define TPC_FOLLOW_THREADS 64
 #endif
 // 64-thread blocks, 10 per SM: 96 registers per thread without spills and 20 resident warps per SM (measured on
-// configs[4]: 128 x 4 blocks at 112 registers = 16 warps: 28.0 ms; 64 x 10 at 96 registers, batch 3: 25.3 ms)
+// configs[4], before R17: 128 x 4 blocks at 112 registers = 16 warps: 28.0 ms; 64 x 10 at 96 registers: 25.3 ms;
+// with the R17 waves a batch of 2 candidate records is the optimum: 11.0 ms against 11.3 with 3 and 12.3 with 4)
 constexpr int kFollowThreads = TPC_FOLLOW_THREADS;
 constexpr unsigned kFull = 0xffffffffu;
 #ifndef TPC_FOLLOW_BATCH
-#define TPC_FOLLOW_BATCH 3
+#define TPC_FOLLOW_BATCH 2
 #endif
 #ifndef TPC_FOLLOW_MIN_BLOCKS
 #define TPC_FOLLOW_MIN_BLOCKS 10
