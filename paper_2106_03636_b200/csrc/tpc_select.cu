@@ -162,24 +162,27 @@ cudaError_t launch_select(const Geo& g, const Ws& w, int32_t* cluster_track, int
                           int32_t* counters, cudaStream_t st) {
   const int64_t n = w.L.n, scap_pad = w.L.scap_pad;
   const int nrows = g.s.nrows;
-  // one warp per tracklet, grid-stride over a grid several waves deep: neighbouring tracklets (same z slab, often
-  // the same clusters) then run at different times, which spreads their atomics over the L2 slices.  A one-wave
-  // grid with consecutive tracklets in flight was measured 2.5x slower on k_push_keys (same-line atomic contention).
+  // One warp per surviving tracklet.  Grid sizes are measured, not derived (configs[4], 2.0e6 survivors): push and
+  // write run fastest with (nearly) one warp per tracklet and no grid-stride loop -- consecutive tracklets in flight
+  // share z slab and cache lines (push 1.72 -> 1.20 ms, write 7.4 -> 6.1 ms against a 9472-block grid); count is
+  // fastest on the 9472-block grid-stride grid.  (Before R17, with 3 tracklets per track claiming the same clusters,
+  // consecutive tracklets in flight meant same-line atomic contention and push was 2.5x slower that way.)
   const unsigned wblocks = blocks_for(w.L.scap * 32, kThreads);
+  const unsigned wblocks_wide = blocks_for(w.L.scap * 32, kThreads, 148 * 2048);
   cudaError_t e;
   if ((e = cudaMemsetAsync(w.owner, 0, sizeof(uint64_t) * (size_t)(n + 1), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.tl_scan, 0, sizeof(long long) * (size_t)(scap_pad + 2), st)) != cudaSuccess) return e;
   if (n > 0) {
     if ((e = cudaMemsetAsync(cluster_track, 0xFF, sizeof(int32_t) * (size_t)n, st)) != cudaSuccess) return e;
     TPC_LAUNCH(KID_PUSH_KEYS, st,
-               (k_push_keys<<<wblocks, kThreads, 0, st>>>(nrows, w.row_hit, w.tl_info, w.tl_key, w.owner, w.surv, w.counters)));
+               (k_push_keys<<<wblocks_wide, kThreads, 0, st>>>(nrows, w.row_hit, w.tl_info, w.tl_key, w.owner, w.surv, w.counters)));
     TPC_LAUNCH(KID_COUNT_KEPT, st,
                (k_count_kept<<<wblocks, kThreads, 0, st>>>(nrows, g.s.min_hits, w.row_hit, w.tl_info, w.tl_key, w.owner,
                                                           w.tl_mask, w.tl_scan, w.surv, w.counters)));
   }
   if ((e = exclusive_scan<long long>(w.tl_scan, w.tl_scan, scap_pad + 1, w.scan_tmp, st)) != cudaSuccess) return e;
   TPC_LAUNCH(KID_WRITE_TRACKS, st,
-             (k_write_tracks<<<wblocks, kThreads, 0, st>>>(nrows, w.rec, w.tl_init, w.row_hit, w.tl_mask, w.tl_scan, scap_pad,
+             (k_write_tracks<<<wblocks_wide, kThreads, 0, st>>>(nrows, w.rec, w.tl_init, w.row_hit, w.tl_mask, w.tl_scan, scap_pad,
                                                           max_tracks, cluster_track, trk_seed, trk_sector, trk_nhits,
                                                           trk_first_hit, trk_hits, w.hit_rec, counters, w.surv, w.counters)));
   return cudaGetLastError();
