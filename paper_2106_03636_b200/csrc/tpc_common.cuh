@@ -260,7 +260,10 @@ __device__ __forceinline__ unsigned long long sel_key(int nh, int start_orig, in
 }
 __device__ __forceinline__ int key_tracklet(unsigned long long key) { return (int)(key & (unsigned long long)(kMaxTracklets - 1)); }
 
-inline unsigned blocks_for(int64_t n, int threads, int64_t cap = 148 * 64) {
+#ifndef TPC_BLOCK_CAP
+#define TPC_BLOCK_CAP (148 * 64)
+#endif
+inline unsigned blocks_for(int64_t n, int threads, int64_t cap = TPC_BLOCK_CAP) {
   int64_t b = (n + threads - 1) / threads;
   if (b > cap) b = cap;
   if (b < 1) b = 1;
