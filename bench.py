@@ -61,9 +61,9 @@ KERNEL_MODEL = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
 # launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
-NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.15, "k_neighbours": 9.00,
-                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 28.35, "k_push_keys": 3.18,
-                     "k_count_kept": 2.17, "k_write_tracks": 19.19, "k_fit": 4.73}      # k_follow: all three launches
+NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.15, "k_neighbours": 9.01,
+                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 28.47, "k_push_keys": 2.99,
+                     "k_count_kept": 2.17, "k_write_tracks": 13.89, "k_fit": 4.69}      # k_follow: all three launches
 
 
 def parse_args():
