@@ -456,10 +456,11 @@ k_wave_test(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const in
 __global__ void __launch_bounds__(kThreads)
 k_list_flags(int mode, int64_t scap_pad, const TlInit* __restrict__ tl_init, const uint8_t* __restrict__ picked,
              int32_t* __restrict__ tl_info, int32_t* __restrict__ flag, const int32_t* __restrict__ ws_counters) {
-  const int n_starts = ws_counters[WC_N_STARTS];
-  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t <= scap_pad; t += (int64_t)gridDim.x * kThreads) {
+  const int n_starts = ws_counters[WC_N_STARTS];  // flag[] beyond it was zeroed by the caller (memset)
+  (void)scap_pad;
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < n_starts; t += (int64_t)gridDim.x * kThreads) {
     int f = 0;
-    if (t < n_starts) {
+    {
       if (mode == 0) {
         f = tl_info[t] ? 0 : 1;
       } else {
@@ -480,12 +481,10 @@ __global__ void __launch_bounds__(kThreads)
 k_list_build(int count_index, int64_t scap_pad, const int32_t* __restrict__ scan, int32_t* __restrict__ list,
              int32_t* __restrict__ ws_counters) {
   const int n_starts = ws_counters[WC_N_STARTS];
-  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < scap_pad; t += (int64_t)gridDim.x * kThreads) {
-    if (t == 0) ws_counters[count_index] = scan[scap_pad];
-    if (t < n_starts) {
-      const int i = scan[t];
-      if (scan[t + 1] != i) list[i] = (int)t;
-    }
+  if (blockIdx.x == 0 && threadIdx.x == 0) ws_counters[count_index] = scan[scap_pad];
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < n_starts; t += (int64_t)gridDim.x * kThreads) {
+    const int i = scan[t];
+    if (scan[t + 1] != i) list[i] = (int)t;
   }
 }
 
@@ -507,6 +506,7 @@ cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st) {
              (k_wave_test<<<blocks_for(w.L.scap, kThreads), kThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.tl_info,
                                                                               w.counters)));
   for (int mode = 0; mode < 3; mode++) {  // two waves of phase A, then phase B
+    if ((e = cudaMemsetAsync(w.surv_scan, 0, sizeof(int32_t) * (size_t)(scap_pad + 2), st)) != cudaSuccess) return e;
     TPC_LAUNCH(KID_SURVIVORS, st,
                (k_list_flags<<<blocks_for(scap_pad + 1, kThreads), kThreads, 0, st>>>(mode, scap_pad, w.tl_init, w.picked, w.tl_info,
                                                                                       w.surv_scan, w.counters)));
