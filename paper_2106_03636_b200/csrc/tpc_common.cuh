@@ -86,7 +86,7 @@ struct Layout {
 // R20 selection key, 64 bits: [63:56] nHits | [55:25] 0x7FFFFFFF - original index of the start hit |
 // [24:0] tracklet number t.  (nHits, start index) is unique per tracklet, so the low field never
 // decides a comparison: max(key) = most hits, ties to the lowest original start index, as R20 asks;
-// carrying t lets the per-cluster passes find the owning tracklet without a search.
+// t makes the key of a tracklet unique even among tracklets dropped for capacity and names the owner in a dump.
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
 #ifndef TPC_MAX_BUCKETS
@@ -258,7 +258,6 @@ __device__ __forceinline__ unsigned long long sel_key(int nh, int start_orig, in
   return ((unsigned long long)(unsigned)nh << 56) | ((unsigned long long)(0x7FFFFFFFu - (unsigned)start_orig) << kKeyTBits) |
          (unsigned long long)(unsigned)t;
 }
-__device__ __forceinline__ int key_tracklet(unsigned long long key) { return (int)(key & (unsigned long long)(kMaxTracklets - 1)); }
 
 #ifndef TPC_BLOCK_CAP
 #define TPC_BLOCK_CAP (148 * 64)

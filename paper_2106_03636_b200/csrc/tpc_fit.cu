@@ -94,6 +94,43 @@ k_fit_gather(const __grid_constant__ Geo g, const float* __restrict__ y, const f
   }
 }
 
+// R21 seeds for the cached refit, one thread per track (full memory parallelism for the four hit gathers and no
+// divergence, instead of a few lanes of a warp doing it inside the fit loop).  seed[k] = two float4:
+// (y1, sinphi, tanlambda, q/pT), (zRef, x1, first hit's y/z are re-read by the fit loop, -, -).
+__global__ void __launch_bounds__(256)
+k_fit_seed(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const int32_t* __restrict__ counters,
+           int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+           float4* __restrict__ seed) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  const float kB = sc.kB, ms = sc.max_sinphi;
+  for (int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x; k < K; k += (int64_t)gridDim.x * 256) {
+    const int n = trk_nhits[k];
+    const float4* hits = hit_rec + trk_first_hit[k];
+    // R21: seed from the first, middle and last hit
+    const float4 a = __ldg(hits), b = __ldg(hits + n / 2), c = __ldg(hits + (n - 1)), h1 = __ldg(hits + (n > 1 ? 1 : 0));
+    const float x1 = sX[__float_as_int(a.z)], y1 = a.x, x2 = sX[__float_as_int(b.z)], y2 = b.x,
+                x3 = sX[__float_as_int(c.z)], y3 = c.x;
+    const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+    const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+    const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+    const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+    const float kappa = (2.0f * cross) / ((d12 * d23) * d13);  // signed curvature of the circumcircle
+    const float dx = sX[__float_as_int(h1.z)] - x1, dy = h1.x - y1;
+    const float ch = sqrtf(dx * dx + dy * dy);
+    float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);  // chord direction rotated back by half the turn
+    if (sphi > ms) sphi = ms;
+    if (sphi < -ms) sphi = -ms;
+    const float zref = a.y;
+    seed[2 * k] = make_float4(y1, sphi, (h1.y - zref) / ch, -(kappa / kB));
+    seed[2 * k + 1] = make_float4(zref, x1, 0.0f, 0.0f);
+  }
+}
+
 constexpr unsigned kFull = 0xffffffffu;
 enum FitPhase { F_FETCH = 0, F_RUN, F_DONE };
 
@@ -101,7 +138,8 @@ __global__ void __launch_bounds__(kFitThreads)
 k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const int32_t* __restrict__ counters,
       int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
       float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref, float* __restrict__ zref_out,
-      float* __restrict__ chi2_out, int32_t* __restrict__ ndf, int32_t* __restrict__ ws_counters) {
+      float* __restrict__ chi2_out, int32_t* __restrict__ ndf, const float4* __restrict__ seed,
+      int32_t* __restrict__ ws_counters) {
   __shared__ float sX[kMaxRows];
   const Scalars& sc = g.s;
   for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
@@ -138,26 +176,16 @@ k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const i
         } else {
           n = trk_nhits[k];
           hits = hit_rec + trk_first_hit[k];
-          // R21: seed from the first, middle and last hit
-          const float4 a = __ldg(hits), b = __ldg(hits + n / 2), c = __ldg(hits + (n - 1)), h1 = __ldg(hits + (n > 1 ? 1 : 0));
-          const float x1 = sX[__float_as_int(a.z)], y1 = a.x, x2 = sX[__float_as_int(b.z)], y2 = b.x,
-                      x3 = sX[__float_as_int(c.z)], y3 = c.x;
-          const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
-          const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
-          const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
-          const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
-          const float kappa = (2.0f * cross) / ((d12 * d23) * d13);  // signed curvature of the circumcircle
-          const float dx = sX[__float_as_int(h1.z)] - x1, dy = h1.x - y1;
-          const float ch = sqrtf(dx * dx + dy * dy);
-          float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);  // chord direction rotated back by half the turn
-          if (sphi > ms) sphi = ms;
-          if (sphi < -ms) sphi = -ms;
-          zref = a.y;
-          st.p[0] = y1;
+          // R21 seed, prepared by k_fit_seed
+          const float4 s0 = __ldg(seed + 2 * (int64_t)k), s1 = __ldg(seed + 2 * (int64_t)k + 1);
+          const float4 a = __ldg(hits);
+          zref = s1.x;
+          const float x1 = s1.y;
+          st.p[0] = s0.x;
           st.p[1] = 0.0f;
-          st.p[2] = sphi;
-          st.p[3] = (h1.y - zref) / ch;
-          st.p[4] = -(kappa / kB);
+          st.p[2] = s0.y;
+          st.p[3] = s0.z;
+          st.p[4] = s0.w;
           reset_cov(st, sc.cov0);  // R22: covariance reset at the start of every pass
           x_at = x1;
           chi2 = 0.0f;
@@ -242,9 +270,16 @@ cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, con
     int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
     if (blocks > g_fit_blocks) blocks = g_fit_blocks;
     if ((e = cudaMemsetAsync(w->counters + WC_FIT_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
+    // seeds go where the follower parked its states (dead by now; at least 96 bytes per tracklet >= 32 per track)
+    float4* seed = w->tl_state;
+    int64_t sblocks = (max_tracks + 255) / 256;
+    if (sblocks > 148 * 64) sblocks = 148 * 64;
+    if (max_tracks > w->L.scap_pad * (int64_t)(kStateVec / 2)) return cudaErrorInvalidValue;  // cannot happen: K <= tracklets
+    TPC_LAUNCH(KID_FIT, st,
+               (k_fit_seed<<<(unsigned)sblocks, 256, 0, st>>>(g, w->hit_rec, counters, max_tracks, trk_nhits, trk_first_hit, seed)));
     TPC_LAUNCH(KID_FIT, st,
                (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, w->hit_rec, counters, max_tracks, trk_nhits, trk_first_hit,
-                                                               par, cov, xref, zref, chi2, ndf, w->counters)));
+                                                               par, cov, xref, zref, chi2, ndf, seed, w->counters)));
     return cudaGetLastError();
   }
   int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
