@@ -12,11 +12,14 @@
 //   orc_grid        R7      per-(sector,row) (y, zeta) grid: stable sort by bin, bin_first
 //   orc_neighbours  R9      cellular-automaton best (up,down) pair per cluster
 //   orc_links       R10     reciprocal-link cleaning, start hits
-//   orc_follow      R11-R18 Kalman following of every start hit: phase A chain + up leg for all, phase B
-//                           jump + down leg for those whose start hit no upward leg picked up (R17)
+//   orc_follow      R11-R18 Kalman following of the start hits in the order R17 fixes: wave test, two waves of
+//                           phase A (init, chain, up leg), phase B (jump, down leg) for the start hits that no
+//                           upward leg picked up; the others are absorbed
 //   orc_select      R20     one-shot arbitration by 64-bit key, exclusive assignment
 //   orc_fit         R21-R22 3-point seed + outward/inward Kalman refit
 //   orc_propagate / orc_update   the R12 / R13 primitives, exported for the pins (I7)
+//   orc_beamline    R24     closest approach of a fitted helix to the beam line, z there, time offset
+//   orc_collisions  R25     collisions as peaks of the per-track time offsets; track -> collision
 //
 // Every function exists for real_t = float (suffix _f32: reproduces the GPU's arithmetic, one
 // IEEE operation per written operation, no contraction: build with -ffp-contract=off) and for
