@@ -28,7 +28,9 @@
 // reordered.  The grid is only an acceleration structure (R8): every search is defined over all
 // clusters of a row, and `use_grid = 0` runs exactly that brute force.
 //
-// Pins (tests/test_oracle_pins.py, -m "not gpu"): I1-I10 of SURVEY.md §8(c).  Track count,
+// Pins (-m "not gpu"): tests/test_oracle_pins.py (I1-I10 of SURVEY.md §8(c)), tests/test_oracle_r17.py (R17: the
+// wave test line by line, the wave loop, the three R17 modes measured against one another, configs[0] against the
+// stored summary), tests/test_oracle_beamline.py (R24), tests/test_oracle_collisions.py (R25).  Track count,
 // efficiency and fake rate themselves are "parity unpinned" by the paper (it publishes no number
 // for any synthetic workload); they are fixed only by oracle == GPU.
 // =============================================================================================
@@ -575,23 +577,44 @@ void neighbours_impl(const OrcParams* P, int64_t n, const T* y, const T* z, cons
   neighbours(c.P, c.G, c.cl, c.ix, link_up, link_dn);
 }
 
+// R17 modes (R17).  The paper fixes none of this (PAPER.md l.47 only says the tracker derives from the
+// Run-2 HLT tracker), so the reading is stated three ways and the tests measure one against the other:
+//   mode 0  SURVEY.md §8(c) R17 as first written: every start hit is followed in full (R14 init, R15 chain, R16
+//           upward leg, one-step jump back, R16 downward leg); nothing is marked, nobody is absorbed
+//   mode 1  phases: phase A (R14, R15, R16 upward) for every start hit, every cluster an upward leg attaches is
+//           marked; a tracklet whose start hit is marked is absorbed (records nothing, claims nothing); the others
+//           run phase B (jump + R16 downward)
+//   mode 2  phases + waves (the method the CUDA path implements; the default): phase A runs in two waves -- first
+//           the start hits for which wave_test() is false, then those of the rest that no first-wave leg marked
+enum { R17_NAIVE = 0, R17_PHASES = 1, R17_WAVES = 2 };
+
+template <class T>
+void wave_test_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int use_grid,
+                    const int32_t* up_c, int64_t n_starts, const int32_t* starts, uint8_t* waits) {
+  Ctx<T> c(*P, n, y, z, sr, use_grid);
+  Follower<T> f{c.P, c.G, c.cl, c.ix, nullptr, 0, 0};
+  for (int64_t t = 0; t < n_starts; t++) waits[t] = f.has_predecessor(starts[t], up_c) ? 1 : 0;
+}
+
 template <class T>
 int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int use_grid,
                     const int32_t* up_c, int64_t n_starts, const int32_t* starts, int32_t* row_hit, int32_t* n_hits,
-                    T* state_out, TraceRec* trace, int64_t trace_cap) {
+                    T* state_out, TraceRec* trace, int64_t trace_cap, int r17_mode, uint8_t* ran_out) {
   Ctx<T> c(*P, n, y, z, sr, use_grid);
   Follower<T> f{c.P, c.G, c.cl, c.ix, trace, trace_cap, 0};
-  // R17: phase A for every start hit, then phase B for those that no upward leg picked up; the others are
-  // absorbed (the tracklet that picked their start hit up covers them): they record nothing and claim nothing.
   std::vector<uint8_t> picked_up((size_t)n, 0);
   std::vector<State<T>> sts((size_t)n_starts);
   std::vector<T> zrefs((size_t)n_starts);
   std::vector<int> r_ats((size_t)n_starts);
-  // Two waves of phase A: start hits with a plausible predecessor below them (has_predecessor) wait; after the
-  // first wave only those of them that no upward leg picked up are followed (second wave).  The rest never run.
   std::vector<uint8_t> waits((size_t)n_starts, 0), ran((size_t)n_starts, 0);
-  for (int64_t t = 0; t < n_starts; t++) waits[(size_t)t] = f.has_predecessor(starts[t], up_c) ? 1 : 0;
-  f.picked_up = picked_up.data();
+  // (i) wave test (mode 2 only): start hits with a plausible predecessor below them wait for the first wave
+  if (r17_mode == R17_WAVES)
+    for (int64_t t = 0; t < n_starts; t++) waits[(size_t)t] = f.has_predecessor(starts[t], up_c) ? 1 : 0;
+  // marks are only made in modes 1 and 2
+  f.picked_up = (r17_mode == R17_NAIVE) ? nullptr : picked_up.data();
+  // (ii) first wave: the start hits that do not wait (all of them in modes 0 and 1);
+  // (iii) second wave: the waiting start hits that no upward leg of the first wave marked.
+  // The list of a wave is fixed BEFORE the wave runs (whole-wave barrier): marks made during a wave do not change it.
   for (int wave = 0; wave < 2; wave++) {
     std::vector<int64_t> todo;
     for (int64_t t = 0; t < n_starts; t++)
@@ -605,8 +628,10 @@ int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const
   if (std::getenv("ORC_VERBOSE")) {
     int64_t nw = 0, nr = 0;
     for (int64_t t = 0; t < n_starts; t++) { nw += waits[(size_t)t]; nr += ran[(size_t)t]; }
-    std::fprintf(stderr, "R17 waves: %lld start hits, %lld wait, %lld ran phase A\n", (long long)n_starts, (long long)nw, (long long)nr);
+    std::fprintf(stderr, "R17 mode %d: %lld start hits, %lld wait, %lld ran phase A\n", r17_mode, (long long)n_starts, (long long)nw, (long long)nr);
   }
+  // (iv) a tracklet whose start hit is marked after both waves -- whether it ran or not -- is absorbed: it records
+  // nothing and claims nothing (R18: nHits = 0, empty table); all others run phase B.
   for (int64_t t = 0; t < n_starts; t++) {
     if (!ran[(size_t)t]) sts[(size_t)t] = State<T>();
     if (!ran[(size_t)t] || picked_up[(size_t)starts[t]]) {
@@ -615,6 +640,7 @@ int64_t follow_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const
     } else {
       n_hits[t] = f.follow_down(starts[t], row_hit + t * c.G.nrows, (int)t, &sts[(size_t)t], zrefs[(size_t)t], r_ats[(size_t)t]);
     }
+    if (ran_out) ran_out[t] = ran[(size_t)t];
     if (state_out) {   // 5 params, 15 cov (lower), zref : 21 values per tracklet
       const State<T>& fs = sts[(size_t)t];
       T* o = state_out + t * 21;
@@ -740,15 +766,30 @@ ORC_API int64_t orc_links(int64_t n, const int32_t* link_up, const int32_t* link
   std::memcpy(starts, s.data(), sizeof(int32_t) * s.size());
   return (int64_t)s.size();
 }
+// r17_mode: 0 naive, 1 phases, 2 phases + waves (see follow_impl); ran_out[n_starts] (may be NULL): 1 if the start
+// hit ran phase A
 ORC_API int64_t orc_follow_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,
                                int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts,
-                               int32_t* row_hit, int32_t* n_hits, float* state_out, TraceRec* trace, int64_t trace_cap) {
-  return follow_impl<float>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap);
+                               int32_t* row_hit, int32_t* n_hits, float* state_out, TraceRec* trace, int64_t trace_cap,
+                               int r17_mode, uint8_t* ran_out) {
+  return follow_impl<float>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap,
+                            r17_mode, ran_out);
 }
 ORC_API int64_t orc_follow_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr,
                                int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts,
-                               int32_t* row_hit, int32_t* n_hits, double* state_out, TraceRec* trace, int64_t trace_cap) {
-  return follow_impl<double>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap);
+                               int32_t* row_hit, int32_t* n_hits, double* state_out, TraceRec* trace, int64_t trace_cap,
+                               int r17_mode, uint8_t* ran_out) {
+  return follow_impl<double>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, row_hit, n_hits, state_out, trace, trace_cap,
+                             r17_mode, ran_out);
+}
+// R17 (i): waits[t] = 1 if start hit t has a plausible predecessor below it (Follower::has_predecessor)
+ORC_API void orc_wave_test_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,
+                               int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts, uint8_t* waits) {
+  wave_test_impl<float>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, waits);
+}
+ORC_API void orc_wave_test_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr,
+                               int use_grid, const int32_t* up_c, int64_t n_starts, const int32_t* starts, uint8_t* waits) {
+  wave_test_impl<double>(P, n, y, z, sr, use_grid, up_c, n_starts, starts, waits);
 }
 ORC_API int64_t orc_select(int64_t n, int n_rows, int64_t n_starts, const int32_t* starts, const int32_t* row_hit,
                            const int32_t* n_hits, int min_hits, int32_t* cluster_track, int32_t* trk_seed,

@@ -149,8 +149,27 @@ def links(link_up, link_dn):
     return up_c, dn_c, starts[:ns].copy()
 
 
-def follow(p, y, z, sector_row, up_c, starts, precision="f32", use_grid=True, want_state=False, trace_cap=0):
-    """R14-R18: returns dict(row_hit[S, n_rows], n_hits[S], state[S,21]?, trace?)."""
+R17_NAIVE, R17_PHASES, R17_WAVES = 0, 1, 2
+
+
+def wave_test(p, y, z, sector_row, up_c, starts, precision="f32", use_grid=True):
+    """R17 (i): waits[S] (bool) -- does start hit t have a plausible predecessor below it?"""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    starts = np.ascontiguousarray(starts, np.int32); up_c = np.ascontiguousarray(up_c, np.int32)
+    waits = np.zeros(starts.size, np.uint8)
+    fn = getattr(lib(), f"orc_wave_test_{sfx}")
+    fn.restype = None
+    fn(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int(int(use_grid)), _ptr(up_c),
+       C.c_int64(starts.size), _ptr(starts), _ptr(waits))
+    return waits.astype(bool)
+
+
+def follow(p, y, z, sector_row, up_c, starts, precision="f32", use_grid=True, want_state=False, trace_cap=0,
+           r17_mode=R17_WAVES):
+    """R14-R18: returns dict(row_hit[S, n_rows], n_hits[S], ran[S], state[S,21]?, trace?).
+    r17_mode: 0 = every start hit followed in full, 1 = phases, 2 = phases + waves (R17; the default)."""
     rt, sfx = _real(precision)
     P = make_params(p, precision)
     y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
@@ -159,10 +178,12 @@ def follow(p, y, z, sector_row, up_c, starts, precision="f32", use_grid=True, wa
     row_hit = np.empty((S, P.n_rows), np.int32); n_hits = np.empty(S, np.int32)
     state = np.empty((S, 21), rt) if want_state else None
     trace = np.zeros(trace_cap, TRACE_DTYPE) if trace_cap else None
+    ran = np.zeros(S, np.uint8)
     nt = getattr(lib(), f"orc_follow_{sfx}")(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr),
                                              C.c_int(int(use_grid)), _ptr(up_c), C.c_int64(S), _ptr(starts),
-                                             _ptr(row_hit), _ptr(n_hits), _ptr(state), _ptr(trace), C.c_int64(trace_cap))
-    out = dict(row_hit=row_hit, n_hits=n_hits)
+                                             _ptr(row_hit), _ptr(n_hits), _ptr(state), _ptr(trace), C.c_int64(trace_cap),
+                                             C.c_int(int(r17_mode)), _ptr(ran))
+    out = dict(row_hit=row_hit, n_hits=n_hits, ran=ran.astype(bool))
     if want_state:
         out["state"] = state
     if trace_cap:
@@ -251,7 +272,8 @@ def update(p, par5, cov15, ym, zm, precision="f64"):
     return float(chi2), a, c
 
 
-def run(p, y, z, sector_row, precision="f32", use_grid=True, want_state=False, trace_cap=0, timings=None):
+def run(p, y, z, sector_row, precision="f32", use_grid=True, want_state=False, trace_cap=0, timings=None,
+        r17_mode=R17_WAVES):
     """Whole hot path a1..a6.  Returns every stage's output (original cluster indices everywhere)."""
     t0 = time.perf_counter()
     out = {}
@@ -262,7 +284,7 @@ def run(p, y, z, sector_row, precision="f32", use_grid=True, want_state=False, t
     t2 = time.perf_counter()
     up_c, dn_c, starts = links(up, dn)
     t3 = time.perf_counter()
-    fo = follow(p, y, z, sector_row, up_c, starts, precision, use_grid, want_state, trace_cap)
+    fo = follow(p, y, z, sector_row, up_c, starts, precision, use_grid, want_state, trace_cap, r17_mode)
     t4 = time.perf_counter()
     se = select(int(np.asarray(y).size), int(p.n_rows), starts, fo["row_hit"], fo["n_hits"], p.min_hits)
     t5 = time.perf_counter()

@@ -5,6 +5,10 @@ golden value can come from it (tests/golden/README.md); every pin below is a clo
 invariant, a textbook/library special case or a brute force on a tiny input.  None of them calls the
 CUDA path.  Each is chosen so that a plausible slip in the oracle (dropped Jacobian term, wrong
 sign of the curvature, transposed covariance index, off-by-one row, wrong tie-break) fails it.
+
+R17 (phases and waves: which start hits are followed, in which order, and who is absorbed) has its own file,
+tests/test_oracle_r17.py, whose header maps every line of Follower::has_predecessor and of the wave loop to the
+pin that constrains it; the two R17 tests at the end of this file are the first, coarser pair.
 """
 import math
 
