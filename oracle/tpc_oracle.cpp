@@ -21,9 +21,12 @@
 //   orc_beamline    R24     closest approach of a fitted helix to the beam line, z there, time offset
 //   orc_collisions  R25     collisions as peaks of the per-track time offsets; track -> collision
 //
-// Every function exists for real_t = float (suffix _f32: reproduces the GPU's arithmetic, one
-// IEEE operation per written operation, no contraction: build with -ffp-contract=off) and for
-// real_t = double (suffix _f64: analytic pins I1, I7, I8).  The step order and notation follow
+// Every function exists for real_t = float (suffix _f32: reproduces the GPU's arithmetic: one IEEE
+// operation per written operation -- build with -ffp-contract=off -- where mad(a, b, c) is the IEEE
+// fusedMultiplyAdd, ONE rounding, in the sums of products of R12 / R13)
+// and for real_t = double (suffix _f64: analytic pins I1, I7, I8).  orc_set_arith(0) evaluates every mad
+// as a multiplication followed by an addition (two roundings), so that the tests can measure one
+// rounding sequence against the other under north_star's tolerances (tests/test_oracle_arith.py).  The step order and notation follow
 // R1-R23 so the file can be checked against DESIGN.md by eye; nothing is blocked, fused or
 // reordered.  The grid is only an acceleration structure (R8): every search is defined over all
 // clusters of a row, and `use_grid = 0` runs exactly that brute force.
@@ -45,6 +48,35 @@
 namespace {
 
 constexpr int kMaxRows = 152;
+
+// Arithmetic contract: g_fused = 1 (default): mad(a,b,c) = fma(a,b,c), one rounding;
+// g_fused = 0: a*b rounded, then + c rounded (the file is compiled with -ffp-contract=off, so the compiler
+// never fuses on its own).  fma(-a, b, c) = c - a*b with one rounding (the negation is exact).
+int g_fused = 1;
+template <class T>
+inline T mad(T a, T b, T c) {
+  if (g_fused) return std::fma(a, b, c);
+  const T ab = a * b;
+  return ab + c;
+}
+
+// Decision log (tests/parity.py near-tie report): one record per decision the follower takes, in the order it
+// takes them.  kind 0: R16 search (chosen = attached cluster or -1; best / second = the two lowest chi2 inside the
+// window, +inf if absent; cut = chi2_cut);  kind 1: R15 chain step (chosen = linked cluster if accepted else -1;
+// best = its chi2; cut = chi2_chain_cut);  kind 2: a transport refused by |sinphi| > max_sinphi (best = the
+// larger |sinphi|, cut = max_sinphi);  kind 3: R16 edge test (best = |y'|, cut = ymax + edge_margin; chosen = 0
+// if the leg goes on, -1 if it stops).
+struct DecRec {
+  int32_t tracklet, row, kind, chosen;
+  double best, second, cut;
+};
+DecRec* g_dec = nullptr;
+int64_t g_dec_cap = 0, g_dec_n = 0;
+inline void log_decision(int tracklet, int row, int kind, int32_t chosen, double best, double second, double cut) {
+  if (!g_dec) return;
+  if (g_dec_n < g_dec_cap) g_dec[g_dec_n] = DecRec{tracklet, row, kind, chosen, best, second, cut};
+  g_dec_n++;
+}
 
 // Host POD filled by oracle/tpc_oracle.py (its own definition; not the CUDA library's header).
 struct OrcParams {
@@ -188,7 +220,7 @@ template <class T>
 T asin_ratio(T u) {
   if (std::fabs(u) < Thr<T>::asin_u) {
     const T u2 = u * u;
-    return (T)1 + u2 * ((T)0.16666667 + u2 * ((T)0.075 + u2 * (T)0.044642857));
+    return mad(u2, mad(u2, mad(u2, (T)0.044642857, (T)0.075), (T)0.16666667), (T)1);
   }
   const double ud = (double)u;
   return (T)(std::asin(ud) / ud);
@@ -200,16 +232,16 @@ template <class T>
 bool propagate(State<T>& st, T dx, T kB, T max_sinphi, T (*F_out)[5] = nullptr) {
   const T y = st.p[0], dz = st.p[1], s1 = st.p[2], tl = st.p[3], q = st.p[4];
   const T kappa = -(kB * q);                       // R4: dphi/ds = -kB q/pT
-  const T s2 = s1 + kappa * dx;
+  const T s2 = mad(kappa, dx, s1);
   if (!(std::fabs(s1) <= max_sinphi) || !(std::fabs(s2) <= max_sinphi)) return false;
-  const T c1 = std::sqrt((T)1 - s1 * s1), c2 = std::sqrt((T)1 - s2 * s2);
+  const T c1 = std::sqrt(mad(-s1, s1, (T)1)), c2 = std::sqrt(mad(-s2, s2, (T)1));
   const T cc = c1 + c2;
   const T t = (s1 + s2) / cc;                      // tan of the mean direction
-  const T L = dx * std::sqrt((T)1 + t * t);        // signed chord
+  const T L = dx * std::sqrt(mad(t, t, (T)1));     // signed chord
   const T u = (kappa * L) * (T)0.5;
   const T arc = L * asin_ratio(u);                 // signed arc length in the bending plane
   // Jacobian (non-trivial terms), g = 1 + c1 c2 + s1 s2
-  const T g = ((T)1 + c1 * c2) + s1 * s2;
+  const T g = mad(s1, s2, mad(c1, c2, (T)1));
   const T c1c2 = c1 * c2;
   const T f02 = (dx * g) / (cc * c1c2);                       // dy'/dsinphi
   const T f04 = -((kB * (dx * dx)) * g) / (c2 * (cc * cc));   // dy'/dq
@@ -226,21 +258,21 @@ bool propagate(State<T>& st, T dx, T kB, T max_sinphi, T (*F_out)[5] = nullptr) 
   const T f14 = -((kB * tl) * E);                             // ddz'/dq
   T F[5][5] = {{1, 0, f02, 0, f04}, {0, 1, f12, f13, f14}, {0, 0, 1, 0, f24}, {0, 0, 0, 1, 0}, {0, 0, 0, 0, 1}};
   // state
-  st.p[0] = y + dx * t;
-  st.p[1] = dz + tl * arc;
+  st.p[0] = mad(dx, t, y);
+  st.p[1] = mad(tl, arc, dz);
   st.p[2] = s2;
-  // C' = F C F^T (Q = 0, R6): dense products, sums over k ascending; lower triangle kept, mirrored.
+  // C' = F C F^T (Q = 0, R6): dense products, sums over k ascending, every term one mad; lower triangle kept, mirrored.
   T M[5][5], N[5][5];
   for (int i = 0; i < 5; i++)
     for (int j = 0; j < 5; j++) {
       T acc = 0;
-      for (int k = 0; k < 5; k++) acc += F[i][k] * st.C[k][j];
+      for (int k = 0; k < 5; k++) acc = mad(F[i][k], st.C[k][j], acc);
       M[i][j] = acc;
     }
   for (int i = 0; i < 5; i++)
     for (int j = 0; j <= i; j++) {
       T acc = 0;
-      for (int k = 0; k < 5; k++) acc += M[i][k] * F[j][k];
+      for (int k = 0; k < 5; k++) acc = mad(M[i][k], F[j][k], acc);
       N[i][j] = acc;
     }
   for (int i = 0; i < 5; i++)
@@ -262,7 +294,7 @@ Innov<T> innovation(const State<T>& st, T sy2, T sz2) {
   I.S00 = st.C[0][0] + sy2;
   I.S01 = st.C[1][0];
   I.S11 = st.C[1][1] + sz2;
-  const T det = I.S00 * I.S11 - I.S01 * I.S01;
+  const T det = mad(-I.S01, I.S01, I.S00 * I.S11);
   const T idet = (T)1 / det;
   I.Si00 = I.S11 * idet;
   I.Si01 = -(I.S01 * idet);
@@ -271,7 +303,7 @@ Innov<T> innovation(const State<T>& st, T sy2, T sz2) {
 }
 template <class T>
 T chi2_of(const Innov<T>& I, T r0, T r1) {
-  return ((r0 * r0) * I.Si00 + (T)2 * ((r0 * r1) * I.Si01)) + (r1 * r1) * I.Si11;
+  return mad(r1 * r1, I.Si11, mad((T)2 * (r0 * r1), I.Si01, (r0 * r0) * I.Si00));
 }
 // R13: Kalman update with measurement (ym, zm) (zm already relative to zRef); returns chi2.
 template <class T>
@@ -281,13 +313,13 @@ T update(State<T>& st, T ym, T zm, T sy2, T sz2) {
   const T chi2 = chi2_of(I, r0, r1);
   T K[5][2];
   for (int i = 0; i < 5; i++) {
-    K[i][0] = st.C[i][0] * I.Si00 + st.C[i][1] * I.Si01;
-    K[i][1] = st.C[i][0] * I.Si01 + st.C[i][1] * I.Si11;
+    K[i][0] = mad(st.C[i][1], I.Si01, st.C[i][0] * I.Si00);
+    K[i][1] = mad(st.C[i][1], I.Si11, st.C[i][0] * I.Si01);
   }
   T N[5][5];
   for (int i = 0; i < 5; i++)
-    for (int j = 0; j <= i; j++) N[i][j] = st.C[i][j] - (K[i][0] * st.C[0][j] + K[i][1] * st.C[1][j]);
-  for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K[i][0] * r0 + K[i][1] * r1);
+    for (int j = 0; j <= i; j++) N[i][j] = mad(-K[i][1], st.C[1][j], mad(-K[i][0], st.C[0][j], st.C[i][j]));
+  for (int i = 0; i < 5; i++) st.p[i] = mad(K[i][1], r1, mad(K[i][0], r0, st.p[i]));
   for (int i = 0; i < 5; i++)
     for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = N[i][j];
   return chi2;
@@ -372,12 +404,22 @@ struct Follower {
   // R16: extrapolate row by row in direction dir (+1/-1) starting after row r_at (state is at X[r_at]).
   // Returns the row the state is at when the leg ends.
   uint8_t* picked_up = nullptr;  // R17: set for every cluster an UPWARD leg attaches (phase A)
+  void log_sinphi(const State<T>& st, T dx, int tracklet, int r) const {   // decision log only
+    if (!g_dec) return;
+    const T s2 = mad(-(G.kB * st.p[4]), dx, st.p[2]);
+    log_decision(tracklet, r, 2, -1, std::max(std::fabs((double)st.p[2]), std::fabs((double)s2)), 0.0, P.max_sinphi);
+  }
   int extrapolate(State<T>& st, T zref, int sector, int r_at, int r_first, int dir, int32_t* row_hit, int tracklet) {
     int misses = 0;
     for (int r = r_first; r >= 0 && r < G.nrows; r += dir) {
-      if (!propagate(st, G.X[r] - G.X[r_at], G.kB, (T)P.max_sinphi)) break;   // |sinphi'| > max: stop
+      if (!propagate(st, G.X[r] - G.X[r_at], G.kB, (T)P.max_sinphi)) {         // |sinphi'| > max: stop
+        log_sinphi(st, G.X[r] - G.X[r_at], tracklet, r);
+        break;
+      }
       r_at = r;
-      if (std::fabs(st.p[0]) > G.ymax[r] + (T)P.edge_margin) break;           // left the sector
+      const bool out = std::fabs(st.p[0]) > G.ymax[r] + (T)P.edge_margin;
+      log_decision(tracklet, r, 3, out ? -1 : 0, std::fabs(st.p[0]), 0.0, G.ymax[r] + (T)P.edge_margin);
+      if (out) break;                                                          // left the sector
       const Innov<T> I = innovation(st, G.sy2, G.sz2);
       const T wy = std::min(std::sqrt((T)P.chi2_cut * I.S00), (T)P.win_max);
       const T wz = std::min(std::sqrt((T)P.chi2_cut * I.S11), (T)P.win_max);
@@ -386,12 +428,20 @@ struct Follower {
       bool have = false;
       T best = 0;
       int32_t bi = -1;
+      double second = HUGE_VAL;   // decision log only: runner-up chi2
       ix.visit(sector, r, yp - wy, yp + wy, zc - wz, zc + wz, [&](int32_t c) {
         const T r0 = cl.y[c] - yp, r1 = (cl.z[c] - zref) - dzp;
         if (!(std::fabs(r0) <= wy && std::fabs(r1) <= wz)) return;
         const T chi2 = chi2_of(I, r0, r1);
-        if (!have || chi2 < best || (chi2 == best && c < bi)) { have = true; best = chi2; bi = c; }
+        if (!have || chi2 < best || (chi2 == best && c < bi)) {
+          if (have) second = std::min(second, (double)best);
+          have = true; best = chi2; bi = c;
+        } else {
+          second = std::min(second, (double)chi2);
+        }
       });
+      log_decision(tracklet, r, 0, (have && best < (T)P.chi2_cut) ? bi : -1, have ? (double)best : HUGE_VAL, second,
+                   (double)P.chi2_cut);
       if (have && best < (T)P.chi2_cut) {
         if (trace && trace_n < trace_cap) {
           TraceRec& t = trace[trace_n++];
@@ -459,9 +509,13 @@ struct Follower {
       const int32_t hn = up_c[h];
       const int rn = cl.row(hn);
       State<T> trial = st;
-      if (!propagate(trial, G.X[rn] - G.X[r_at], G.kB, (T)P.max_sinphi)) break;
+      if (!propagate(trial, G.X[rn] - G.X[r_at], G.kB, (T)P.max_sinphi)) {
+        log_sinphi(st, G.X[rn] - G.X[r_at], tracklet, rn);
+        break;
+      }
       const Innov<T> I = innovation(trial, G.sy2, G.sz2);
       const T chi2 = chi2_of(I, cl.y[hn] - trial.p[0], (cl.z[hn] - zref) - trial.p[1]);
+      log_decision(tracklet, rn, 1, chi2 > (T)P.chi2_chain_cut ? -1 : hn, (double)chi2, HUGE_VAL, (double)P.chi2_chain_cut);
       if (chi2 > (T)P.chi2_chain_cut) break;       // discard the prediction; state stays at the previous hit
       update(trial, cl.y[hn], cl.z[hn] - zref, G.sy2, G.sz2);
       st = trial;
@@ -483,6 +537,8 @@ struct Follower {
     State<T> st = *st_io;
     if (propagate(st, G.X[r0] - G.X[r_at], G.kB, (T)P.max_sinphi))
       extrapolate(st, zref, sector, r0, r0 - 1, -1, row_hit, tracklet);
+    else
+      log_sinphi(st, G.X[r0] - G.X[r_at], tracklet, r0);
     int nh = 0;
     for (int r = 0; r < G.nrows; r++) nh += row_hit[r] >= 0;
     *st_io = st;
@@ -740,6 +796,14 @@ T update_impl(const OrcParams* P, T* p5, T* c15, T ym, T zm) {
 #define ORC_API extern "C" __attribute__((visibility("default")))
 
 ORC_API int64_t orc_sizeof_params() { return (int64_t)sizeof(OrcParams); }
+ORC_API int64_t orc_sizeof_decision() { return (int64_t)sizeof(DecRec); }
+// arithmetic contract: 1 (default) = mad is a fused multiply-add, 0 = multiplication then addition
+ORC_API void orc_set_arith(int fused) { g_fused = fused ? 1 : 0; }
+ORC_API int orc_get_arith() { return g_fused; }
+// decision log of the follower (see DecRec): records go to buf[cap] until orc_decisions_end(), which returns how
+// many decisions were taken (may exceed cap: the rest were dropped)
+ORC_API void orc_decisions_begin(DecRec* buf, int64_t cap) { g_dec = buf; g_dec_cap = cap; g_dec_n = 0; }
+ORC_API int64_t orc_decisions_end() { g_dec = nullptr; return g_dec_n; }
 ORC_API int64_t orc_sizeof_trace() { return (int64_t)sizeof(TraceRec); }
 
 ORC_API int64_t orc_grid_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr,

@@ -6,7 +6,8 @@ imports nothing from there (parameters arrive as any object with the TpcParams a
 clusters as numpy arrays).
 
 `build()` compiles the oracle with g++ (-O2 -ffp-contract=off: one IEEE operation per written
-operation, which is what makes float mode comparable with the GPU).  `run()` chains the stages
+operation -- the fused multiply-adds of the arithmetic contract are explicit std::fma calls -- which is
+what makes float mode comparable with the GPU; -mfma only turns those calls into the instruction).  `run()` chains the stages
 R7 -> R9 -> R10 -> R14-R18 -> R20 -> R21-R22 and returns every intermediate
 so the parity tests can compare stage by stage.
 """
@@ -45,6 +46,10 @@ class TraceRec(C.Structure):
                 ("S00", C.c_double), ("S01", C.c_double), ("S11", C.c_double), ("chi2", C.c_double)]
 
 
+DECISION_DTYPE = np.dtype([("tracklet", "i4"), ("row", "i4"), ("kind", "i4"), ("chosen", "i4"), ("best", "f8"),
+                           ("second", "f8"), ("cut", "f8")])
+DEC_SEARCH, DEC_CHAIN, DEC_SINPHI, DEC_EDGE = 0, 1, 2, 3
+
 TRACE_DTYPE = np.dtype([("tracklet", "i4"), ("row", "i4"), ("chosen", "i4"), ("pad", "i4"), ("y_pred", "f8"),
                         ("dz_pred", "f8"), ("zref", "f8"), ("S00", "f8"), ("S01", "f8"), ("S11", "f8"), ("chi2", "f8")])
 
@@ -56,9 +61,22 @@ def build(force: bool = False) -> str:
     tmp = _LIB + f".tmp{os.getpid()}"
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
            "-fvisibility=hidden", "-o", tmp, _SRC]
+    if _cpu_has_fma():
+        cmd.insert(1, "-mfma")      # std::fma -> vfmadd instead of a libm call; same (correctly rounded) result
     subprocess.run(cmd, check=True)
     os.replace(tmp, _LIB)
     return _LIB
+
+
+def _cpu_has_fma() -> bool:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    return " fma " in line + " "
+    except OSError:
+        pass
+    return False
 
 
 def lib():
@@ -81,8 +99,51 @@ def lib():
         L.orc_links.restype = C.c_int64
         L.orc_beamline.restype = None
         L.orc_select.restype = C.c_int64
+        L.orc_sizeof_decision.restype = C.c_int64
+        assert L.orc_sizeof_decision() == DECISION_DTYPE.itemsize, "DecRec layout mismatch"
+        L.orc_set_arith.restype = None
+        L.orc_get_arith.restype = C.c_int
+        L.orc_decisions_begin.restype = None
+        L.orc_decisions_end.restype = C.c_int64
         _lib = L
     return _lib
+
+
+class arith:
+    """with arith(fused=False): ...  -- evaluate every mad(a,b,c) of R12/R13 as a*b then +c (two roundings) instead
+    of the fused multiply-add of the arithmetic contract.  Process-global, restored on exit."""
+
+    def __init__(self, fused: bool):
+        self.fused = bool(fused)
+
+    def __enter__(self):
+        self.prev = lib().orc_get_arith()
+        lib().orc_set_arith(C.c_int(int(self.fused)))
+        return self
+
+    def __exit__(self, *exc):
+        lib().orc_set_arith(C.c_int(self.prev))
+        return False
+
+
+class decisions:
+    """with decisions(cap) as d: orc.follow(...) / orc.run(...);  d.log = every decision the follower took
+    (DECISION_DTYPE records, in the order taken; d.dropped = decisions beyond cap)."""
+
+    def __init__(self, cap: int):
+        self.buf = np.zeros(int(cap), DECISION_DTYPE)
+        self.log = self.buf[:0]
+        self.dropped = 0
+
+    def __enter__(self):
+        lib().orc_decisions_begin(_ptr(self.buf), C.c_int64(self.buf.size))
+        return self
+
+    def __exit__(self, *exc):
+        n = int(lib().orc_decisions_end())
+        self.log = self.buf[:min(n, self.buf.size)]
+        self.dropped = max(0, n - self.buf.size)
+        return False
 
 
 def make_params(p, precision: str = "f32") -> OrcParams:

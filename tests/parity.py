@@ -90,14 +90,16 @@ def compare_tracks(orc_out, res, n):
         co, cg = orc_out["cov"][COV_DIAG][:, io].astype(np.float64), res["cov"][COV_DIAG][:, ig].astype(np.float64)
         rel_c = np.abs(co - cg) / np.maximum(np.abs(co), np.abs(cg))
         st["par_max_rel"] = float(rel_p.max()) if rel_p.size else 0.0
+        st["par_median_rel"] = float(np.median(rel_p)) if rel_p.size else 0.0
         st["cov_max_rel"] = float(rel_c.max()) if rel_c.size else 0.0
         st["par_bit_identical"] = bool(np.array_equal(orc_out["par"][:, io], res["par"][:, ig]))
         st["cov_bit_identical"] = bool(np.array_equal(orc_out["cov"][:, io], res["cov"][:, ig]))
         st["chi2_max_rel"] = float(np.max(np.abs(orc_out["chi2"][io] - res["chi2"][ig]) /
                                           np.maximum(np.abs(orc_out["chi2"][io]), 1.0))) if io.size else 0.0
         assert np.array_equal(orc_out["ndf"][io], res["ndf"][ig])
-        assert np.array_equal(orc_out["xref"][io], res["xref"][ig])
-        assert np.array_equal(orc_out["zref"][io], res["zref"][ig])
+        if orc_out["par"].dtype == res["par"].dtype:      # an fp64 run holds the unrounded row positions
+            assert np.array_equal(orc_out["xref"][io], res["xref"][ig])
+            assert np.array_equal(orc_out["zref"][io], res["zref"][ig])
     return st
 
 
@@ -156,3 +158,70 @@ def check_output_invariants(res, sector_row, n_rows, min_hits):
     assert np.unique(res["trk_seed"]).size == K
     ok = res["ndf"] >= 0
     assert np.array_equal(res["ndf"][ok], 2 * nh[ok] - 5)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# near-tie report (BASELINE.json north_star: "any differences must be logged as near-tie chi2 comparisons")
+# ------------------------------------------------------------------------------------------------------------
+NEAR_TIE_KINDS = {0: "R16 search", 1: "R15 chain cut", 2: "max_sinphi", 3: "sector edge"}
+
+
+def _margin(rec):
+    """Relative distance of a logged decision (oracle DecRec) from flipping: the smallest of
+    |best - second| / max (two candidates swap) and |best - cut| / cut (the cut flips)."""
+    best, second, cut = float(rec["best"]), float(rec["second"]), float(rec["cut"])
+    m = np.inf
+    if np.isfinite(best):
+        m = abs(best - cut) / abs(cut)
+        if np.isfinite(second):
+            m = min(m, abs(best - second) / max(abs(best), abs(second), 1e-300), abs(second - cut) / abs(cut))
+    return m
+
+
+def near_tie_report(ref, other, dec_log, log=None):
+    """Explains the differences between two runs of the follower on the same input (`ref`, whose decision log
+    `dec_log` is given, against `other`; dicts with starts / row_hit / n_hits as oracle.follow and
+    Tracker.find_export return them, original cluster indices).
+
+    For every tracklet (matched by start hit) whose row table differs, the decisions `ref` took are replayed in
+    order against `other`'s table: the FIRST decision whose outcome `other` does not share is that tracklet's root
+    cause, and its margin (see _margin) says how near a tie it was.  A tracklet that differs without such a decision
+    is secondary: `other` went on where `ref` had stopped, or the tracklet was absorbed / not absorbed because an
+    upward leg of a root-cause tracklet marked its start hit differently (R17).  Returns a dict: differing tracklets,
+    root causes with their margins, secondaries; every root cause is written to `log` (a list of strings)."""
+    oi = np.argsort(ref["starts"])
+    gi = np.argsort(other["starts"])
+    assert np.array_equal(ref["starts"][oi], other["starts"][gi]), "the two runs do not share their start hits"
+    g_of_o = np.empty(oi.size, np.int64)
+    g_of_o[oi] = gi                                   # tracklet number in `other` of ref's tracklet t
+    differ = np.nonzero(np.any(ref["row_hit"] != other["row_hit"][g_of_o], axis=1))[0]
+    out = dict(tracklets=int(oi.size), differing=int(differ.size), roots=[], secondary=0, absorbed_flip=0)
+    if differ.size == 0:
+        return out
+    order = np.argsort(dec_log["tracklet"], kind="stable")
+    lo = np.searchsorted(dec_log["tracklet"][order], differ, "left")
+    hi = np.searchsorted(dec_log["tracklet"][order], differ, "right")
+    for t, a, b in zip(differ, lo, hi):
+        rh_other = other["row_hit"][g_of_o[t]]
+        if (ref["n_hits"][t] == 0) != (other["n_hits"][g_of_o[t]] == 0):
+            out["absorbed_flip"] += 1                 # R17: marked by somebody else's upward leg in one run only
+            continue
+        root = None
+        for rec in dec_log[order[a:b]]:
+            kind, row, chosen = int(rec["kind"]), int(rec["row"]), int(rec["chosen"])
+            if kind in (0, 1) and rh_other[row] != chosen:
+                root = rec
+                break
+            if kind in (2, 3) and chosen < 0:         # ref stopped here; did `other` go on past this row?
+                root = rec
+                break
+        if root is None:
+            out["secondary"] += 1
+            continue
+        m = _margin(root)
+        out["roots"].append((int(t), int(root["kind"]), int(root["row"]), m))
+        if log is not None:
+            log.append(f"tracklet {int(t)} (start hit {int(ref['starts'][t])}): {NEAR_TIE_KINDS[int(root['kind'])]} on row "
+                       f"{int(root['row'])}: best {root['best']:.9g}, second {root['second']:.9g}, cut {root['cut']:.9g}, "
+                       f"relative margin {m:.3e}")
+    return out
