@@ -54,7 +54,8 @@ KERNEL_MODEL = {
     "k_survivor_*": ("hbm", {"tracklet": 32 + 4 + 3 * (32 + 1 + 4 + 12 + 4)}, None),   # wave test + three list builds
     "k_push_keys": ("hbm", {"claim": 4 + 8 + 8, "tracklet": 12}, None),   # row_hit in, 8-byte atomicMax RMW
     "k_count_kept": ("hbm", {"claim": 4 + 8, "tracklet": 12 + 20 + 8}, None),   # row_hit, owner in; mask, value out
-    "k_write_tracks": ("hbm", {"hit": 4 + 16 + 4 + 16 + 8, "tracklet": 16 + 20}, None),  # rec in; trk_hits, hit_rec, cluster_track out
+    "k_write_tracks": ("hbm", {"hit": 4 + 16 + 4 + 16 + 8, "tracklet": 16 + 20}, None),  # row_hit, rec in; trk_hits, hit_rec, (orig, track) pair out
+    "k_assign": ("hbm", {"hit": 8 + 4}, None),                    # pair in, cluster_track out
     "k_fit": ("alu", {}, "hit"),
 }
 

@@ -25,14 +25,19 @@ struct SmCa {
   float wu[kMaxRows], iy[kMaxRows], iz[kMaxRows], wyu[kMaxRows], wzu[kMaxRows], wyd[kMaxRows], wzd[kMaxRows];
 };
 
-// Running arg-min of R9: minimal D2; ties: lowest original u index, then lowest original d index.
+// Running arg-min of R9: minimal D2; ties: lowest original u index, then lowest original d index.  best starts at
+// +inf and the indices at INT_MAX, so the first pair offered is always taken (as "!have ||" would).
 struct BestPair {
-  bool have;
   float best;
   int bui, bdi, bu, bd;
+  __device__ __forceinline__ void reset() {
+    best = __int_as_float(0x7f800000);
+    bui = bdi = 0x7fffffff;
+    bu = bd = -1;
+  }
+  __device__ __forceinline__ bool have() const { return bu >= 0; }
   __device__ __forceinline__ void offer(float D2, int ui, int di, int k, int j) {
-    if (!have || D2 < best || (D2 == best && (ui < bui || (ui == bui && di < bdi)))) {
-      have = true;
+    if (D2 < best || (D2 == best && (ui < bui || (ui == bui && di < bdi)))) {
       best = D2;
       bui = ui;
       bdi = di;
@@ -136,10 +141,7 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
       const BinWin WU = bin_window(sm, sc, s, r + 1, yh - wyu, yh + wyu, zh - wzu, zh + wzu);
       const BinWin WD = bin_window(sm, sc, s, r - 1, yh - wyd, yh + wyd, zh - wzd, zh + wzd);
       BestPair B;
-      B.have = false;
-      B.best = 0.0f;
-      B.bui = B.bdi = 0;
-      B.bu = B.bd = -1;
+      B.reset();
       bool slow = WU.nzb > 2 || WD.nzb > 2;
       if (!slow) {
         const Ranges RU = load_ranges(bin_first, WU), RD = load_ranges(bin_first, WD);
@@ -215,10 +217,10 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
         }
       }
       if (slow) {
-        B.have = false;
+        B.reset();
         neighbours_nested(rec, bin_first, WU, WD, yh, zh, wu, iy, iz, wyu, wzu, wyd, wzd, B);
       }
-      if (B.have && B.best < sc.ca_cut) {
+      if (B.have() && B.best < sc.ca_cut) {
         bu = B.bu;
         bd = B.bd;
       }

@@ -40,13 +40,7 @@ constexpr unsigned kFull = 0xffffffffu;
 #ifndef TPC_FOLLOW_MIN_BLOCKS
 #define TPC_FOLLOW_MIN_BLOCKS 10
 #endif
-#ifndef TPC_FOLLOW_PREFETCH
-#define TPC_FOLLOW_PREFETCH 1
-#endif
 constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
-
-// L1 prefetch of one line: the follower knows one step ahead roughly where it will look.
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
@@ -77,7 +71,6 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   int t = 0, s = 0, r0 = 0, r_at = 0, r = 0, hn = -1, p0 = 0, orig0 = 0;
   int misses = 0, nh = 0, lo = 0, hi = 0;
   unsigned nprop = 0, nupd = 0, ncand = 0, nclaims = 0;  // work counters of this lane over all its tracklets
-  int pf_ka = -1;  // first grid position of the bin the NEXT step is expected to search (-1: no prediction)
 #pragma unroll
   for (int k = 0; k < 5; k++) st.p[k] = 0.0f;
 #pragma unroll
@@ -123,7 +116,6 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
           const float4 a = __ldg(ip), b = __ldg(ip + 1);
           p0 = __float_as_int(b.x);
           hn = __float_as_int(b.y);
-          prefetch_l1(rec + hn);
           const int sr0 = __float_as_int(b.z);
           orig0 = __float_as_int(b.w);
           s = sr0 / nrows;
@@ -155,10 +147,6 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
     if (leg) rn = r;
     int nxt = -1;
     if (chain) nxt = __ldg(up_c + hn);
-    // the bin offset requested during the previous step has arrived by now: pull the records it points to
-    // into L1 while the transport below is computed
-    if (pf_ka >= 0) prefetch_l1(rec + pf_ka);
-    pf_ka = -1;
     // ---- R12 transport (one copy for every phase; __syncwarp keeps the compiler from cloning it
     //      into the phase branches, which would serialise the lanes again) --------------------------
     __syncwarp();
@@ -317,24 +305,6 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
       my = by;
       mz = bz - zref;
       mk = bk;
-    }
-    // ---- look one step ahead (prefetch only: nothing below depends on it) ---------------------------
-    //   next chain cluster: its record;  next row of a leg (or the first row after the chain): the bin at the
-    //   linearly extrapolated position -- its offset is loaded now (in flight during the update) and the
-    //   records behind it are prefetched at the top of the next iteration.  st still holds the state at the
-    //   previous row here, so the slope costs two subtractions.
-    if (TPC_FOLLOW_PREFETCH && chain && upd && nxt >= 0) prefetch_l1(rec + nxt);
-    if (TPC_FOLLOW_PREFETCH && moved && ok && !isJ) {
-      const int r2 = rn + (PHASE_B ? -1 : 1);
-      if (r2 >= 0 && r2 < nrows) {
-        const float y2 = yp + (yp - st.p[0]);
-        const float z2 = zref + (dzp + (dzp - st.p[1]));
-        const float zeta = (s < 18) ? z2 : -z2;
-        const int ny2 = sm.ny[r2];
-        const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
-        const int yb = clampbin((y2 + sm.ymax[r2]) * sc.inv_cy, ny2);
-        pf_ka = __ldg(bin_first + (s * sc.bins_per_sector + sm.rowbase[r2] + zb * ny2 + yb));
-      }
     }
     // ---- commit the transport, R13 update (one copy for every phase) --------------------------------
     __syncwarp();

@@ -29,6 +29,7 @@ enum KernelId {
   KID_PUSH_KEYS,
   KID_COUNT_KEPT,
   KID_WRITE_TRACKS,
+  KID_ASSIGN,
   KID_FIT,
   KID_TRACK_TIME,
   KID_COLLISIONS,
