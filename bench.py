@@ -7,11 +7,19 @@ One "step" = one pass of the whole hot path (tpc_grid_build -> tpc_find_tracks -
 §8(a) rows a1..a6) over one synthetic event.  The default workload is BASELINE.json configs[4]: one 128-orbit
 50 kHz min-bias Pb-Pb Time Frame (~1.4e8 clusters, seeded synthetic).
 
- value        clusters/s with the clusters resident in HBM (CUDA events, max over ranks)
- e2e          same metric through tpc_track_host: pinned host buffers, H2D + D2H inside the timed region
- roofline     the dominant kernel (by CUDA-event time measured live on the launching stream, tpc_profile_*)
- cpu_baseline the CPU oracle, as it stands, on a bounded sample of the same event (rank 0, N = 1 only)
+ value        clusters/s with the clusters resident in HBM (CUDA events around K steps, no per-kernel events inside;
+              max over ranks)
+ e2e          same metric through tpc_track_host_async / tpc_track_host_fetch: pinned host buffers, H2D of the inputs
+              and D2H of EVERY output inside the timed region, two Time Frames in flight
+ kernels      per-kernel CUDA-event times from a second, separately profiled loop (tpc_profile_*)
+ roofline     the dominant kernel of that table; the FP32 roof is measured by the library (tpc_fp32_peak, FFMA chains),
+              the HBM roof is MEASURED_PEAKS.json; `traffic` comes from profiles/*_ncu_traffic.csv and is null when
+              csrc/ has changed since that capture
+ cpu_baseline the CPU oracle, as it stands: the whole Time Frame with its sectors dealt to all host cores, and one
+              thread on a slab of one sector beside it (rank 0, N = 1 only)
  --impl reference : times the oracle alone on the host cores (this tier's reference arm)
+ --ncu-traffic RAW.csv --out profiles/NAME.csv : turn `ncu -i REP --page raw --csv` output into the stamped
+              per-kernel DRAM traffic table `roofline.traffic` reads (no GPU needed)
 
 N > 1 (torchrun): every rank tracks its OWN Time Frame (TF-level replicas: GPUs process
 independent TFs); no data-path collective; "scaling": "weak".
@@ -19,6 +27,9 @@ independent TFs); no data-path collective; "scaling": "weak".
 from __future__ import annotations
 
 import argparse
+import csv
+import glob
+import hashlib
 import json
 import os
 import subprocess
@@ -60,11 +71,78 @@ KERNEL_MODEL = {
 }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on the configs[4] workload, from the `ncu --set full` /
-# launch-list captures summarised in profiles/r01_ncu_summary.md (GB).  Only quoted for --config 4.
-NCU_TRAFFIC_GB_C4 = {"k_bucket_hist": 1.65, "k_bucket_scatter": 4.03, "k_bucket_sort": 6.15, "k_neighbours": 9.01,
-                     "k_clean": 2.26, "k_compact_starts": 2.22, "k_follow": 28.47, "k_push_keys": 2.99,
-                     "k_count_kept": 2.17, "k_write_tracks": 13.89, "k_fit": 4.69}      # k_follow: all three launches
+# ------------------------------------------------------------------------------------------------
+# roofline.traffic: ncu DRAM bytes per kernel, from a tracked capture stamped with the csrc/ it was taken on
+# ------------------------------------------------------------------------------------------------
+CSRC = os.path.join(ROOT, "paper_2106_03636_b200", "csrc")
+
+
+def csrc_digest() -> str:
+    """sha256 over the CUDA sources (names and contents): identifies the build a capture belongs to."""
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(CSRC)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            with open(os.path.join(CSRC, f), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()
+
+
+KERNEL_GROUPS = (("k_follow", "k_follow"), ("k_fit", "k_fit"), ("k_scan", "k_scan_*"), ("k_wave_test", "k_survivor_*"),
+                 ("k_list_", "k_survivor_*"), ("k_chunk_counts", "k_compact_starts"))
+
+
+def bench_kernel_name(ncu_name: str) -> str:
+    """Name of the bench table row a kernel of the ncu launch list belongs to."""
+    base = ncu_name.split("(")[0].split("::")[-1].split("<")[0].strip()
+    for prefix, row in KERNEL_GROUPS:
+        if base.startswith(prefix):
+            return row
+    return base
+
+
+def write_ncu_traffic(raw_csv: str, out_csv: str, config: int, steps_captured: int):
+    """profiles/*_ncu_traffic.csv from `ncu -i REP --page raw --csv`: DRAM read + write bytes per bench kernel row,
+    summed over its launches and divided by the number of steps captured."""
+    with open(raw_csv) as f:
+        rows = list(csv.reader(f))
+    hdr, units = rows[0], rows[1]
+    ik, ir, iw = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    tot = {}
+    for r in rows[2:]:
+        if len(r) <= max(ik, ir, iw):
+            continue
+        name = bench_kernel_name(r[ik])
+        by = float(r[ir].replace(",", "")) * scale[units[ir]] + float(r[iw].replace(",", "")) * scale[units[iw]]
+        a = tot.setdefault(name, [0.0, 0])
+        a[0] += by
+        a[1] += 1
+    with open(out_csv, "w") as f:
+        f.write(f"# csrc_sha256: {csrc_digest()}\n# config: {config}\n# steps_captured: {steps_captured}\n")
+        f.write("kernel,dram_bytes_per_step,launches_per_step\n")
+        for k in sorted(tot):
+            f.write(f"{k},{tot[k][0] / steps_captured:.0f},{tot[k][1] / steps_captured:g}\n")
+    print(f"wrote {out_csv}: {len(tot)} kernels, csrc {csrc_digest()[:12]}")
+
+
+def load_ncu_traffic(config: int):
+    """({kernel: DRAM bytes per step}, source) of the newest tracked capture taken on exactly these csrc/ sources and
+    this config; ({}, reason) otherwise -- a capture of another build says nothing about this one."""
+    want = csrc_digest()
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_traffic.csv")), reverse=True):
+        meta, table = {}, {}
+        with open(path) as f:
+            for ln in f:
+                if ln.startswith("#"):
+                    k, _, v = ln[1:].partition(":")
+                    meta[k.strip()] = v.strip()
+                elif ln.strip() and not ln.startswith("kernel,"):
+                    k, by, _ = ln.strip().split(",")
+                    table[k] = float(by)
+        if meta.get("csrc_sha256") == want and int(meta.get("config", -1)) == config:
+            return table, os.path.relpath(path, ROOT) + " (ncu dram__bytes_read.sum + dram__bytes_write.sum)"
+    return {}, "no ncu capture of this build and config under profiles/ (csrc/ changed since the last one)"
 
 
 def parse_args():
@@ -76,6 +154,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ncu-traffic", default=None, help="raw csv of `ncu -i REP --page raw --csv` to convert (no GPU needed)")
+    ap.add_argument("--out", default=None, help="with --ncu-traffic: the profiles/*_ncu_traffic.csv to write")
+    ap.add_argument("--steps-captured", type=int, default=1, help="with --ncu-traffic: steps the capture covers")
     return ap.parse_args()
 
 
@@ -174,6 +255,45 @@ def time_oracle(ev, y, z, sr, steps: int, warmup: int):
     return float(np.mean(times)), ntr
 
 
+_POOL_EV = None
+
+
+def _oracle_sector(sector: int):
+    """Worker of time_oracle_all_cores: the whole hot path of one sector, single-threaded (the oracle as it stands)."""
+    from oracle import tpc_oracle as orc
+    ev = _POOL_EV
+    nrows = int(ev.params.n_rows)
+    sel = np.nonzero(ev.sector_row // nrows == sector)[0]
+    p1 = ev.params
+    t0 = time.perf_counter()
+    o = orc.run(p1, ev.y[sel], ev.z[sel], ev.sector_row[sel], "f32", True)
+    return sector, int(sel.size), int(o["trk_seed"].size), int((o["cluster_track"] >= 0).sum()), time.perf_counter() - t0
+
+
+def time_oracle_all_cores(ev, cores: int | None = None):
+    """BASELINE.md §2 leg (ii): the whole event with its sectors dealt to all host cores (sectors are independent
+    through the whole hot path; the oracle stays single-threaded per sector).  Returns a dict for cpu_baseline."""
+    import multiprocessing as mp
+    global _POOL_EV
+    from oracle import tpc_oracle as orc
+    orc.build()
+    nsec = int(ev.params.n_sectors)
+    cores = max(1, min(cores or (os.cpu_count() or 1), nsec))
+    nrows = int(ev.params.n_rows)
+    sizes = np.bincount(ev.sector_row // nrows, minlength=nsec)
+    order = [int(s) for s in np.argsort(-sizes)]          # largest first: the pool deals them as workers free up
+    _POOL_EV = ev
+    t0 = time.perf_counter()
+    with mp.get_context("fork").Pool(cores) as pool:      # fork: the workers see the event without a copy
+        res = pool.map(_oracle_sector, order, chunksize=1)
+    wall = time.perf_counter() - t0
+    _POOL_EV = None
+    return {"value": ev.n / wall, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"whole event: {ev.n} clusters, {nsec} sectors dealt to {cores} processes (one oracle thread each)",
+            "seconds": wall, "cpu_seconds": float(sum(r[4] for r in res)), "tracks_found": int(sum(r[2] for r in res)),
+            "clusters_assigned": int(sum(r[3] for r in res)), "host_cores_available": os.cpu_count()}
+
+
 def run_reference(args, rank: int):
     """This tier's reference arm: the CPU oracle, as it stands, on a bounded sample per step."""
     if rank != 0:
@@ -252,9 +372,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     if int(cnt[binding.CNT_STATUS]) & (binding.ST_TRACKLET_OVERFLOW | binding.ST_TRACK_OVERFLOW):
         raise RuntimeError(f"capacity overflow, status bits {int(cnt[binding.CNT_STATUS])}: the run would skip work")
 
-    # ---- timed region: K steps, inputs resident in HBM, CUDA events on the launching stream -----
+    # ---- timed region: K steps, inputs resident in HBM, CUDA events on the launching stream, no per-kernel events ----
+    binding.profile_enable(False)
     binding.profile_collect(reset=True)
-    binding.profile_enable(True)
     sampler = ClockSampler(local_rank)
     time.sleep(0.3)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -268,36 +388,60 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     w1 = time.perf_counter()
     clocks = sampler.stop(w0, w1)
     ms_total = e0.elapsed_time(e1)
-    prof = binding.profile_collect(reset=True)
-    binding.profile_enable(False)
+    launches = int(sum(v[1] for v in binding.profile_collect(reset=True).values()))   # counted always, timed only below
     res = trk.results()
     K_tracks = int(res["trk_seed"].size)
     n_tracklets = int(res["counters"][binding.CNT_TRACKLETS])
     n_hits = int(res["counters"][binding.CNT_HITS])
 
-    # ---- end to end through the host-buffer entry point -----------------------------------------
+    # ---- per-kernel table: a second loop with an event pair around every launch ---------------------
+    binding.profile_enable(True)
+    for _ in range(args.steps):
+        trk.step(y, z, sr)
+    torch.cuda.synchronize()
+    prof = binding.profile_collect(reset=True)
+    binding.profile_enable(False)
+    fp32_peak = binding.fp32_peak(dev)
+
+    # ---- end to end through the host-buffer entry points -----------------------------------------
     # Two Time Frames in flight (two Tracker contexts, own workspace / staging / pinned outputs, one stream each):
     # the H2D copy of one TF overlaps the tracking of the previous one and the D2H of the one before -- the
-    # steady state of a continuous TF stream.  Every step still copies its inputs from
-    # pinned host memory and reads counters + cluster_track + parameters back inside the timed region.
+    # steady state of a continuous TF stream.  Every step copies its inputs from pinned host
+    # memory and reads EVERY output back (counters and cluster_track with the step; the per-track arrays and the hit
+    # lists, whose sizes the host only knows from the counters, by tpc_track_host_fetch once those have arrived).
     t_e2e, h2d, d2h = 0.0, 0, 0
+    NC = 3     # Time Frames in flight: a stream's H2D + tracking + D2H chain is ~2.5x the step time
     if not args.no_e2e:
-        ctx = [trk, binding.Tracker(ev.params, n, device=dev)]
-        streams = [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
+        ctx = [trk] + [binding.Tracker(ev.params, n, device=dev) for _ in range(NC - 1)]
+        streams = [torch.cuda.Stream(device=dev) for _ in range(NC)]
+        events = [torch.cuda.Event() for _ in range(NC)]
         for c, st in zip(ctx, streams):
             c.make_host_staging()
             with torch.cuda.stream(st):
-                c.track_host(hy, hz, hs)                 # warm-up (first-touch of the staging buffers), synchronous
+                h2d, d2h = c.track_host(hy, hz, hs)      # warm-up (first touch of the staging buffers), synchronous
         barrier(); torch.cuda.synchronize()
+
+        def fetch(j):                                    # TF j: wait for its counters, then enqueue the exact-size copies
+            events[j % NC].synchronize()
+            with torch.cuda.stream(streams[j % NC]):
+                ctx[j % NC].track_host_fetch()
+
         t0 = time.perf_counter()
         for i in range(args.steps):
-            with torch.cuda.stream(streams[i % 2]):
-                h2d, d2h = ctx[i % 2].track_host(hy, hz, hs, sync=False)
+            with torch.cuda.stream(streams[i % NC]):
+                ctx[i % NC].track_host_async(hy, hz, hs)
+                events[i % NC].record()
+            if i >= NC - 1:                              # its context is the one the next iteration reuses
+                fetch(i - (NC - 1))
+        for j in range(max(args.steps - (NC - 1), 0), args.steps):
+            fetch(j)
         for st in streams:
             st.synchronize()
         t_e2e = (time.perf_counter() - t0) / args.steps
-        for c in ctx[:min(args.steps, 2)]:
-            assert int(c.counters_host[binding.CNT_TRACKS]) == K_tracks
+        for c in ctx[:min(args.steps, NC)]:
+            hr = c.host_results()
+            assert hr["trk_seed"].size == K_tracks and int(hr["trk_nhits"].sum()) == n_hits
+            assert np.array_equal(hr["par"], res["par"]) and np.array_equal(hr["trk_hits"], res["trk_hits"])
         del ctx
 
     # ---- max over ranks ----------------------------------------------------------------------------
@@ -308,26 +452,26 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     hbm_peak, sm_max_mhz, peak_src = load_peaks()
     value = tot_clusters / (ms_step * 1e-3)
     # ---- per-kernel table and roofline of the dominant kernel -----------------------------------
+    # A row sums all launches of that kernel in a step (k_follow: two waves of phase A + phase B; k_fit: seeds + fit;
+    # scans, list builds); its algorithmic bytes / flops (KERNEL_MODEL) cover the same launches.
     kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps}
             for k, v in prof.items() if v[1] > 0}
-    launches = int(sum(v[1] for v in prof.values()))
     top = max(kern, key=lambda k: kern[k]["ms_per_step"])
-    top_ms = kern[top]["ms_per_step"] / max(kern[top]["launches_per_step"], 1)
-    if top == "k_follow":      # the waves of phase A and phase B are launches of one kernel; the work counters cover all
-        top_ms = kern[top]["ms_per_step"]
     nb = binding.grid_bins(ev.params)
     work = binding.work_counts(res["counters"])
     units = {"cluster": n, "bin": nb, "tracklet": int(res["counters"][binding.CNT_TRACKLETS]), "claim": work["claims"],
              "hit": n_hits}
-    roofline = kernel_roofline(top, top_ms, units, work, int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
-    if args.config == 4 and top in NCU_TRAFFIC_GB_C4:
-        roofline["traffic"] = NCU_TRAFFIC_GB_C4[top] * 1e9
-        roofline["traffic_source"] = "profiles/r01_ncu_summary.md (ncu dram__bytes_read.sum + dram__bytes_write.sum)"
+    peaks = {"hbm": hbm_peak, "hbm_source": peak_src, "fp32": fp32_peak, "sm_max_mhz": sm_max_mhz}
+    traffic, traffic_src = load_ncu_traffic(args.config)
+    roofline = kernel_roofline(top, kern[top]["ms_per_step"], units, work, int(ev.params.n_fit_passes), peaks)
+    roofline["launches_per_step"] = kern[top]["launches_per_step"]
+    roofline["traffic"] = traffic.get(top)
+    roofline["traffic_source"] = traffic_src
     for k in kern:       # every kernel's own fraction of its roof, so that the table can be read without DESIGN.md
-        r = kernel_roofline(k, kern[k]["ms_per_step"] / max(kern[k]["launches_per_step"], 1) *
-                            (kern[k]["launches_per_step"] if k in ("k_scan_*", "k_follow", "k_survivor_*") else 1), units, work,
-                            int(ev.params.n_fit_passes), hbm_peak, sm_max_mhz, peak_src)
+        r = kernel_roofline(k, kern[k]["ms_per_step"], units, work, int(ev.params.n_fit_passes), peaks)
         kern[k]["bound"], kern[k]["frac"] = r["bound"], round(r["frac"], 4)
+        if k in traffic:
+            kern[k]["ncu_dram_gb"] = round(traffic[k] / 1e9, 3)
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic",
@@ -339,39 +483,53 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "tracks_found": K_tracks, "tracklets_followed": n_tracklets,
            "tracklets_followed_down": int(res["counters"][binding.CNT_FOLLOWED_DOWN]), "clusters_assigned": n_hits,
            "follower_work": work,
-           "clocks": clocks, "gpu_launches": launches, "kernels": kern, "roofline": roofline}
+           "clocks": clocks, "gpu_launches": launches, "kernels": kern,
+           "kernels_ms_sum": round(sum(v["ms_per_step"] for v in kern.values()), 3), "roofline": roofline}
     if not args.no_e2e:
         out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
                       "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3,
-                      "pipeline": "tpc_track_host_async, 2 Time Frames in flight on 2 streams (own workspace, staging and "
-                                  "pinned outputs each); wall clock over the K steps incl. pipeline fill"}
+                      "bound": "pcie", "h2d_gb_per_s": int(h2d) / t_e2e / 1e9, "d2h_gb_per_s": int(d2h) / t_e2e / 1e9,
+                      "returns": "every output of tpc_find_tracks + tpc_fit_tracks: counters, cluster_track, trk_seed / sector / "
+                                 "nhits / first_hit, trk_hits, par, cov, xref, zref, chi2, ndf (exactly K tracks and H hits)",
+                      "pipeline": f"tpc_track_host_async + tpc_track_host_fetch, {NC} Time Frames in flight on {NC} streams (own "
+                                  "workspace, staging and pinned outputs each); wall clock over the K steps incl. pipeline fill"}
     if world == 1 and not args.no_cpu_baseline:
         ys, zs, ss, desc = oracle_sample(ev, 1_500_000)
         dt, ntr = time_oracle(ev, ys, zs, ss, 1, 0)
-        out["cpu_baseline"] = {"value": ys.size / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-                               "seconds": dt, "host_cores_available": os.cpu_count()}
+        one = {"value": ys.size / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}
+        if int(ev.params.n_sectors) > 1:
+            out["cpu_baseline"] = time_oracle_all_cores(ev)
+            out["cpu_baseline"]["one_core"] = one
+            out["cpu_baseline"]["same_tracks_as_gpu"] = bool(out["cpu_baseline"]["tracks_found"] == K_tracks and
+                                                            out["cpu_baseline"]["clusters_assigned"] == n_hits)
+        else:
+            out["cpu_baseline"] = dict(one, host_cores_available=os.cpu_count())
     print(json.dumps(out), flush=True)
 
 
-def kernel_roofline(name, ms, units, work, n_passes, hbm_peak, sm_max_mhz, peak_src):
-    """units: {"cluster": N, "bin": B, "tracklet": S, "claim": follower updates, "hit": hits of accepted tracks}."""
+def kernel_roofline(name, ms, units, work, n_passes, peaks):
+    """Roofline entry of one row of the kernel table.  ms = summed time of the row's launches in one step;
+    units: {"cluster": N, "bin": B, "tracklet": S, "claim": follower updates, "hit": hits of accepted tracks};
+    peaks: {"hbm": GB/s (MEASURED_PEAKS.json), "fp32": TFLOP/s measured by tpc_fp32_peak, ...}."""
     bound, per_unit, unit = KERNEL_MODEL.get(name, ("hbm", {}, None))
     if bound == "hbm":
         by = sum(b * units[u] for u, b in per_unit.items())
         ach = by / (ms * 1e-3) / 1e9
-        return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                "traffic": None, "algorithmic_bytes_per_launch": by, "ms_per_launch": ms, "peak_source": peak_src}
-    # alu-bound kernels: fp32 operations actually required per unit (DESIGN.md "Kernels / follower")
+        return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"],
+                "traffic": None, "algorithmic_bytes_per_step": by, "ms_per_step": ms, "peak_source": peaks["hbm_source"]}
+    # alu-bound kernels: fp32 operations the method requires per unit (DESIGN.md "Kernels"; a fused multiply-add counts 2)
     from paper_2106_03636_b200 import flops
     if name == "k_follow":
         n_units, fl = work["propagations"], flops.follow_flop(work)
     else:
         n_units, fl = units["hit"] * n_passes, flops.fit_flop(units["hit"], n_passes)
-    peak = 148 * 128 * sm_max_mhz * 1e6 / 1e12      # fp32 lanes x clock, non-FMA (one op per lane per cycle), TFLOP/s
+    nominal = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     ach = fl / (ms * 1e-3) / 1e12
-    return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-            "traffic": None, "algorithmic_flop_per_launch": fl, "units": n_units, "unit_kind": unit, "ms_per_launch": ms,
-            "peak_source": f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz, 1 op/lane/cycle (no FMA contraction by contract)"}
+    return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peaks["fp32"], "unit": "TFLOP/s", "frac": ach / peaks["fp32"],
+            "traffic": None, "algorithmic_flop_per_step": fl, "units": n_units, "unit_kind": unit, "ms_per_step": ms,
+            "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
+            "peak_source": "measured in this run by tpc_fp32_peak (FFMA chains, 8 per thread); peak_nominal = 148 SMs x 128 "
+                           f"lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz"}
 
 
 def main():
@@ -379,6 +537,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.ncu_traffic:
+        write_ncu_traffic(args.ncu_traffic, args.out or os.path.join(ROOT, "profiles", "ncu_traffic.csv"), args.config,
+                          args.steps_captured)
+        return
     if args.impl == "reference":
         run_reference(args, rank)
         return

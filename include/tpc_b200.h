@@ -216,31 +216,52 @@ int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float
                         int32_t* coll_ntracks, int32_t* coll_bin, int32_t* trk_collision,
                         int32_t* n_collisions, void* stream);
 
-/* Host-buffer convenience for end-to-end measurement (bench.py `e2e`): copies the five input
- * arrays host->device into caller-provided device staging buffers, runs the three steps, and
- * copies counters + track parameters back.  All on `stream`; synchronises before returning. */
-int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
-                   int64_t max_tracks, const float* y_host, const float* z_host,
-                   const int32_t* sector_row_host, float* y_dev, float* z_dev, int32_t* sector_row_dev,
-                   void* workspace, size_t ws_bytes, int32_t* cluster_track_dev, int32_t* trk_seed_dev,
-                   int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
-                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev,
-                   float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
-                   int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
+/* ---- host-buffer entry points (bench.py `e2e`; a continuous stream of Time Frames through
+ * reused GPU memory) ---------------------------------------------------------------------------------------------
+ * tpc_result_t names the outputs of tpc_find_tracks + tpc_fit_tracks (layouts as documented there).  The same
+ * struct describes the DEVICE buffers of a tracking context and the pinned HOST buffers the results are copied to;
+ * in the host struct a NULL member is not copied (counters is required). */
+typedef struct {
+  int32_t* cluster_track;   /* [n_clusters] */
+  int32_t* trk_seed;        /* [max_tracks] */
+  int32_t* trk_sector;      /* [max_tracks] */
+  int32_t* trk_nhits;       /* [max_tracks] */
+  int64_t* trk_first_hit;   /* [max_tracks] */
+  int32_t* trk_hits;        /* [n_clusters] */
+  int32_t* counters;        /* [TPC_N_COUNTERS] */
+  float* par;               /* [5][max_tracks] */
+  float* cov;               /* [15][max_tracks] */
+  float* xref;              /* [max_tracks] */
+  float* zref;              /* [max_tracks] */
+  float* chi2;              /* [max_tracks] */
+  int32_t* ndf;             /* [max_tracks] */
+} tpc_result_t;
 
-/* Same work as tpc_track_host, enqueue only: returns without synchronising, so that a caller with two sets of
- * buffers on two streams can overlap the host->device copy of one Time Frame with the tracking of the previous
- * one and the device->host copy of the one before (the TF stream is continuous and GPU
- * memory is reused between steps).  The host buffers must be pinned and stay untouched until `stream` has
- * passed this call's work (cudaStreamSynchronize / an event). */
+/* tpc_track_host_async: enqueue only.  Copies y, z, sector_row host->device into the caller's staging buffers,
+ * runs tpc_grid_build, tpc_find_tracks, tpc_fit_tracks into `dev`, and copies back what has a size known to the
+ * host: counters and (if host->cluster_track) cluster_track [n_clusters].  Returns without synchronising, so that a
+ * caller with two contexts on two streams overlaps the host->device copy of one Time Frame with the tracking of
+ * the previous one and the device->host copies of the one before.  Host buffers must be pinned and stay
+ * untouched until `stream` has passed this call's work.
+ * tpc_track_host_fetch: to be called once host->counters has arrived (cudaEventSynchronize on an event recorded
+ * after tpc_track_host_async, or a stream synchronise).  Reads K = counters[TPC_CNT_TRACKS] and H =
+ * counters[TPC_CNT_HITS] from host->counters and enqueues device->host copies of exactly the first K entries of
+ * every per-track array (rows of par / cov keep their pitch of max_tracks) and the first H entries of trk_hits, for
+ * every non-NULL member of `host`.  bytes_host (may be NULL) receives the bytes it enqueued.
+ * tpc_track_host: tpc_track_host_async, synchronise, tpc_track_host_fetch, synchronise.
+ * All three: TPC_EINVAL for missing buffers; otherwise the return codes of the three steps. */
 int tpc_track_host_async(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
                          int64_t max_tracks, const float* y_host, const float* z_host,
                          const int32_t* sector_row_host, float* y_dev, float* z_dev, int32_t* sector_row_dev,
-                         void* workspace, size_t ws_bytes, int32_t* cluster_track_dev, int32_t* trk_seed_dev,
-                         int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
-                         int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev,
-                         float* xref_dev, float* zref_dev, float* chi2_dev, int32_t* ndf_dev,
-                         int32_t* counters_host, int32_t* cluster_track_host, float* par_host, void* stream);
+                         void* workspace, size_t ws_bytes, const tpc_result_t* dev, const tpc_result_t* host,
+                         void* stream);
+int tpc_track_host_fetch(int64_t max_tracks, const tpc_result_t* dev, const tpc_result_t* host,
+                         int64_t* bytes_host, void* stream);
+int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                   int64_t max_tracks, const float* y_host, const float* z_host,
+                   const int32_t* sector_row_host, float* y_dev, float* z_dev, int32_t* sector_row_dev,
+                   void* workspace, size_t ws_bytes, const tpc_result_t* dev, const tpc_result_t* host,
+                   void* stream);
 
 /* ---- measurement support (bench.py `roofline`, `gpu_launches`) --------------------------------
  * The library counts every kernel it launches, per kernel id, and can bracket each launch with a
@@ -256,6 +277,11 @@ int tpc_profile_enable(int on);
 int tpc_profile_kernels(void);
 const char* tpc_profile_name(int kernel_id);
 int tpc_profile_collect(int n_ids, double* ms_host, int64_t* launches_host, int reset);
+/* The FP32 roof the alu-bound kernels are reported against ("measure an FMA-chain peak"): runs a
+ * kernel of independent FFMA chains (8 per thread, 8 blocks of 256 threads per SM) four times on `stream`,
+ * SYNCHRONISES, and writes the best rate of the last three in TFLOP/s (2 flop per FMA) to *tflops_host.
+ * scratch_dev: >= 4 bytes of device memory (never written in practice). */
+int tpc_fp32_peak(float* scratch_dev, double* tflops_host, void* stream);
 
 #ifdef __cplusplus
 }

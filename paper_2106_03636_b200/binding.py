@@ -28,7 +28,7 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_track_host", "tpc_track_host_async", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect")
+           "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -41,6 +41,15 @@ class tpc_params_t(C.Structure):
                 ("max_sinphi", C.c_float), ("edge_margin", C.c_float),
                 ("max_gap", C.c_int32), ("min_hits", C.c_int32), ("n_fit_passes", C.c_int32),
                 ("cov0", C.c_float * 5)]
+
+
+class tpc_result_t(C.Structure):
+    """Mirror of tpc_result_t: the outputs of find + fit, as device buffers or as pinned host buffers."""
+    _fields_ = [(nm, C.c_void_p) for nm in ("cluster_track", "trk_seed", "trk_sector", "trk_nhits", "trk_first_hit", "trk_hits",
+                                            "counters", "par", "cov", "xref", "zref", "chi2", "ndf")]
+
+
+RESULT_FIELDS = tuple(f[0] for f in tpc_result_t._fields_)
 
 
 class TpcError(RuntimeError):
@@ -136,6 +145,16 @@ def profile_collect(reset: bool = True) -> dict:
         a, b = out.get(name, (0.0, 0))
         out[name] = (a + float(ms[i]), b + int(cnt[i]))
     return out
+
+
+def fp32_peak(device="cuda:0") -> float:
+    """tpc_fp32_peak: measured FFMA-chain rate of the device in TFLOP/s (synchronises)."""
+    import torch
+    scratch = torch.zeros(64, dtype=torch.float32, device=device)
+    out = C.c_double(0.0)
+    with torch.cuda.device(scratch.device):
+        _check(load().tpc_fp32_peak(_dp(scratch), C.byref(out), _stream()), "tpc_fp32_peak")
+    return float(out.value)
 
 
 def work_counts(counters) -> dict:
@@ -326,31 +345,55 @@ class Tracker:
 
     # ---- host-buffer path (bench.py e2e) ------------------------------------------------------
     def make_host_staging(self):
-        """Device staging buffers + pinned host outputs for `track_host`."""
+        """Device staging buffers for the inputs + pinned host buffers for every output (`track_host`)."""
         t = self.torch
         n1 = max(self.n, 1)
         self._y_dev = t.empty(n1, dtype=t.float32, device=self.device)
         self._z_dev = t.empty(n1, dtype=t.float32, device=self.device)
         self._sr_dev = t.empty(n1, dtype=t.int32, device=self.device)
-        self.counters_host = t.zeros(TPC_N_COUNTERS, dtype=t.int32).pin_memory()
-        self.cluster_track_host = t.empty(n1, dtype=t.int32).pin_memory()
-        self.par_host = t.empty((5, self.max_tracks), dtype=t.float32).pin_memory()
+        self.host = {nm: t.empty_like(getattr(self, nm), device="cpu").pin_memory() for nm in RESULT_FIELDS}
+        self.host["counters"].zero_()
+        self.counters_host = self.host["counters"]
+        self._res_dev = tpc_result_t(*[C.c_void_p(getattr(self, nm).data_ptr()) for nm in RESULT_FIELDS])
+        self._res_host = tpc_result_t(*[C.c_void_p(self.host[nm].data_ptr()) for nm in RESULT_FIELDS])
 
-    def track_host(self, y_host, z_host, sr_host, sync: bool = True):
-        """tpc_track_host: H2D of the inputs, a1..a6, D2H of counters + cluster_track + track parameters.
-        sync=False calls tpc_track_host_async (enqueue only on the current stream)."""
+    def _host_args(self, y_host, z_host, sr_host):
         for a in (y_host, z_host, sr_host):
             assert not a.is_cuda and a.is_contiguous() and a.numel() == self.n
         hp = lambda a: C.c_void_p(a.data_ptr())
         self._inputs = (self._y_dev, self._z_dev, self._sr_dev)
-        fn = self.lib.tpc_track_host if sync else self.lib.tpc_track_host_async
-        _check(fn(
-            C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), C.c_int64(self.max_tracks),
-            hp(y_host), hp(z_host), hp(sr_host), _dp(self._y_dev), _dp(self._z_dev), _dp(self._sr_dev),
-            _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(self.cluster_track), _dp(self.trk_seed),
-            _dp(self.trk_sector), _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits), _dp(self.counters),
-            _dp(self.par), _dp(self.cov), _dp(self.xref), _dp(self.zref), _dp(self.chi2), _dp(self.ndf),
-            hp(self.counters_host), hp(self.cluster_track_host), hp(self.par_host), _stream()), "tpc_track_host")
-        h2d = 12 * self.n
-        d2h = 4 * TPC_N_COUNTERS + 4 * self.n + 4 * 5 * self.max_tracks
-        return h2d, d2h
+        return (C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets), C.c_int64(self.max_tracks),
+                hp(y_host), hp(z_host), hp(sr_host), _dp(self._y_dev), _dp(self._z_dev), _dp(self._sr_dev),
+                _dp(self.workspace), C.c_size_t(self.ws_bytes), C.byref(self._res_dev), C.byref(self._res_host), _stream())
+
+    def track_host(self, y_host, z_host, sr_host):
+        """tpc_track_host: H2D of the inputs, a1..a6, D2H of every output; synchronous.  Returns (h2d, d2h) bytes."""
+        _check(self.lib.tpc_track_host(*self._host_args(y_host, z_host, sr_host)), "tpc_track_host")
+        return 12 * self.n, self.d2h_bytes()
+
+    def track_host_async(self, y_host, z_host, sr_host):
+        """tpc_track_host_async on the current stream: H2D, a1..a6, D2H of counters + cluster_track; enqueue only."""
+        _check(self.lib.tpc_track_host_async(*self._host_args(y_host, z_host, sr_host)), "tpc_track_host_async")
+
+    def track_host_fetch(self) -> int:
+        """tpc_track_host_fetch on the current stream (the counters must have arrived): D2H of exactly K tracks and H
+        hits of every other output.  Returns the bytes enqueued."""
+        nb = C.c_int64(0)
+        _check(self.lib.tpc_track_host_fetch(C.c_int64(self.max_tracks), C.byref(self._res_dev), C.byref(self._res_host),
+                                             C.byref(nb), _stream()), "tpc_track_host_fetch")
+        return int(nb.value)
+
+    def d2h_bytes(self) -> int:
+        """Bytes one host-buffer step copies device->host, from the counters of the last completed step."""
+        K, H = int(self.counters_host[CNT_TRACKS]), int(self.counters_host[CNT_HITS])
+        return 4 * TPC_N_COUNTERS + 4 * self.n + K * (4 * 3 + 8 + 4 * (5 + 15) + 4 * 4) + 4 * H
+
+    def host_results(self):
+        """numpy views of the pinned host buffers after a completed host-buffer step (same keys as results())."""
+        cnt = self.host["counters"].numpy()
+        K, H = int(cnt[CNT_TRACKS]), int(cnt[CNT_HITS])
+        h = {k: v.numpy() for k, v in self.host.items()}
+        return dict(counters=cnt, status=int(cnt[CNT_STATUS]), cluster_track=h["cluster_track"][:self.n],
+                    trk_seed=h["trk_seed"][:K], trk_sector=h["trk_sector"][:K], trk_nhits=h["trk_nhits"][:K],
+                    trk_first_hit=h["trk_first_hit"][:K], trk_hits=h["trk_hits"][:H], par=h["par"][:, :K], cov=h["cov"][:, :K],
+                    xref=h["xref"][:K], zref=h["zref"][:K], chi2=h["chi2"][:K], ndf=h["ndf"][:K])

@@ -328,18 +328,68 @@ int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
+namespace {
+// FFMA chains: 8 independent accumulators per thread, every step a dependent fused multiply-add on each of them.
+__global__ void __launch_bounds__(256) k_fma_chain(float* out, float b, float c, int iters) {
+  float a[8];
+#pragma unroll
+  for (int k = 0; k < 8; k++) a[k] = (float)(threadIdx.x + k);
+  for (int i = 0; i < iters; i++) {
+#pragma unroll
+    for (int k = 0; k < 8; k++) a[k] = __fmaf_rn(a[k], b, c);
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 8; k++) s += a[k];
+  if (s == 123.456f) out[0] = s;  // never true: keeps the chains alive
+}
+}  // namespace
+
+int tpc_fp32_peak(float* scratch_dev, double* tflops_host, void* stream) {
+  if (!scratch_dev || !tflops_host) return TPC_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e);
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return cuda_fail(e);
+  const int blocks = sms * 8, iters = 32768;
+  cudaEvent_t a, b;
+  if ((e = cudaEventCreate(&a)) != cudaSuccess) return cuda_fail(e);
+  if ((e = cudaEventCreate(&b)) != cudaSuccess) return cuda_fail(e);
+  double best = 0.0;
+  for (int rep = 0; rep < 4; rep++) {  // the first launch warms up; best of the rest
+    cudaEventRecord(a, st);
+    k_fma_chain<<<blocks, 256, 0, st>>>(scratch_dev, 0.999f, 0.001f, iters);
+    cudaEventRecord(b, st);
+    if ((e = cudaEventSynchronize(b)) != cudaSuccess) break;
+    float ms = 0.0f;
+    cudaEventElapsedTime(&ms, a, b);
+    const double tf = 2.0 * 8.0 * (double)iters * 256.0 * (double)blocks / ((double)ms * 1e-3) / 1e12;
+    if (rep > 0 && tf > best) best = tf;
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  if (e != cudaSuccess) return cuda_fail(e);
+  *tflops_host = best;
+  return TPC_OK;
+}
+
+namespace {
+bool result_complete(const tpc_result_t* r) {
+  return r && r->cluster_track && r->trk_seed && r->trk_sector && r->trk_nhits && r->trk_first_hit && r->trk_hits &&
+         r->counters && r->par && r->cov && r->xref && r->zref && r->chi2 && r->ndf;
+}
+}  // namespace
+
 int tpc_track_host_async(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
-                   const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
-                   int32_t* sector_row_dev, void* workspace, size_t ws_bytes, int32_t* cluster_track_dev,
-                   int32_t* trk_seed_dev, int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
-                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev, float* xref_dev,
-                   float* zref_dev, float* chi2_dev, int32_t* ndf_dev, int32_t* counters_host,
-                   int32_t* cluster_track_host, float* par_host, void* stream) {
+                         const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
+                         int32_t* sector_row_dev, void* workspace, size_t ws_bytes, const tpc_result_t* dev,
+                         const tpc_result_t* host, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
   const size_t n = (size_t)(n_clusters > 0 ? n_clusters : 0);
   if (n > 0 && (!y_host || !z_host || !sector_row_host || !y_dev || !z_dev || !sector_row_dev)) return TPC_EINVAL;
-  if (!counters_host) return TPC_EINVAL;
+  if (!result_complete(dev) || !host || !host->counters) return TPC_EINVAL;
   if (n > 0) {
     if ((e = cudaMemcpyAsync(y_dev, y_host, n * sizeof(float), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
     if ((e = cudaMemcpyAsync(z_dev, z_host, n * sizeof(float), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
@@ -349,38 +399,69 @@ int tpc_track_host_async(const tpc_params_t* params_host, int64_t n_clusters, in
   int rc = tpc_grid_build(params_host, n_clusters, max_tracklets, nullptr, y_dev, z_dev, nullptr, sector_row_dev, workspace,
                           ws_bytes, stream);
   if (rc != TPC_OK) return rc;
-  rc = tpc_find_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, cluster_track_dev, max_tracks,
-                       trk_seed_dev, trk_sector_dev, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, counters_dev, stream);
+  rc = tpc_find_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, dev->cluster_track, max_tracks,
+                       dev->trk_seed, dev->trk_sector, dev->trk_nhits, dev->trk_first_hit, dev->trk_hits, dev->counters, stream);
   if (rc != TPC_OK) return rc;
-  rc = tpc_fit_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, y_dev, z_dev, sector_row_dev, counters_dev,
-                      max_tracks, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, par_dev, cov_dev, xref_dev, zref_dev, chi2_dev,
-                      ndf_dev, stream);
+  rc = tpc_fit_tracks(params_host, n_clusters, max_tracklets, workspace, ws_bytes, y_dev, z_dev, sector_row_dev, dev->counters,
+                      max_tracks, dev->trk_nhits, dev->trk_first_hit, dev->trk_hits, dev->par, dev->cov, dev->xref, dev->zref,
+                      dev->chi2, dev->ndf, stream);
   if (rc != TPC_OK) return rc;
-  if ((e = cudaMemcpyAsync(counters_host, counters_dev, sizeof(int32_t) * TPC_N_COUNTERS, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+  if ((e = cudaMemcpyAsync(host->counters, dev->counters, sizeof(int32_t) * TPC_N_COUNTERS, cudaMemcpyDeviceToHost, st)) !=
+      cudaSuccess)
     return cuda_fail(e);
-  if (cluster_track_host && n > 0)
-    if ((e = cudaMemcpyAsync(cluster_track_host, cluster_track_dev, n * sizeof(int32_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-      return cuda_fail(e);
-  if (par_host)
-    if ((e = cudaMemcpyAsync(par_host, par_dev, sizeof(float) * 5 * (size_t)max_tracks, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+  if (host->cluster_track && n > 0)
+    if ((e = cudaMemcpyAsync(host->cluster_track, dev->cluster_track, n * sizeof(int32_t), cudaMemcpyDeviceToHost, st)) !=
+        cudaSuccess)
       return cuda_fail(e);
   return TPC_OK;
 }
 
+int tpc_track_host_fetch(int64_t max_tracks, const tpc_result_t* dev, const tpc_result_t* host, int64_t* bytes_host,
+                         void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!result_complete(dev) || !host || !host->counters || max_tracks < 1) return TPC_EINVAL;
+  int64_t K = host->counters[TPC_CNT_TRACKS], H = host->counters[TPC_CNT_HITS];
+  if (K < 0 || K > max_tracks || H < 0) return TPC_EINVAL;
+  int64_t bytes = 0;
+  cudaError_t e = cudaSuccess;
+  auto copy = [&](void* dst, const void* src, size_t elem, int64_t count) {
+    if (!dst || count <= 0 || e != cudaSuccess) return;
+    e = cudaMemcpyAsync(dst, src, elem * (size_t)count, cudaMemcpyDeviceToHost, st);
+    bytes += (int64_t)(elem * (size_t)count);
+  };
+  auto copy_rows = [&](float* dst, const float* src, int rows) {   // SoA [rows][max_tracks]: K columns of every row
+    if (!dst || K <= 0 || e != cudaSuccess) return;
+    e = cudaMemcpy2DAsync(dst, sizeof(float) * (size_t)max_tracks, src, sizeof(float) * (size_t)max_tracks,
+                          sizeof(float) * (size_t)K, (size_t)rows, cudaMemcpyDeviceToHost, st);
+    bytes += (int64_t)sizeof(float) * K * rows;
+  };
+  copy(host->trk_seed, dev->trk_seed, sizeof(int32_t), K);
+  copy(host->trk_sector, dev->trk_sector, sizeof(int32_t), K);
+  copy(host->trk_nhits, dev->trk_nhits, sizeof(int32_t), K);
+  copy(host->trk_first_hit, dev->trk_first_hit, sizeof(int64_t), K);
+  copy(host->trk_hits, dev->trk_hits, sizeof(int32_t), H);
+  copy_rows(host->par, dev->par, 5);
+  copy_rows(host->cov, dev->cov, 15);
+  copy(host->xref, dev->xref, sizeof(float), K);
+  copy(host->zref, dev->zref, sizeof(float), K);
+  copy(host->chi2, dev->chi2, sizeof(float), K);
+  copy(host->ndf, dev->ndf, sizeof(int32_t), K);
+  if (bytes_host) *bytes_host = bytes;
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
 int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, int64_t max_tracks,
                    const float* y_host, const float* z_host, const int32_t* sector_row_host, float* y_dev, float* z_dev,
-                   int32_t* sector_row_dev, void* workspace, size_t ws_bytes, int32_t* cluster_track_dev,
-                   int32_t* trk_seed_dev, int32_t* trk_sector_dev, int32_t* trk_nhits_dev, int64_t* trk_first_hit_dev,
-                   int32_t* trk_hits_dev, int32_t* counters_dev, float* par_dev, float* cov_dev, float* xref_dev,
-                   float* zref_dev, float* chi2_dev, int32_t* ndf_dev, int32_t* counters_host,
-                   int32_t* cluster_track_host, float* par_host, void* stream) {
-  const int rc = tpc_track_host_async(params_host, n_clusters, max_tracklets, max_tracks, y_host, z_host, sector_row_host, y_dev,
-                                      z_dev, sector_row_dev, workspace, ws_bytes, cluster_track_dev, trk_seed_dev,
-                                      trk_sector_dev, trk_nhits_dev, trk_first_hit_dev, trk_hits_dev, counters_dev, par_dev,
-                                      cov_dev, xref_dev, zref_dev, chi2_dev, ndf_dev, counters_host, cluster_track_host,
-                                      par_host, stream);
+                   int32_t* sector_row_dev, void* workspace, size_t ws_bytes, const tpc_result_t* dev, const tpc_result_t* host,
+                   void* stream) {
+  int rc = tpc_track_host_async(params_host, n_clusters, max_tracklets, max_tracks, y_host, z_host, sector_row_host, y_dev,
+                                z_dev, sector_row_dev, workspace, ws_bytes, dev, host, stream);
   if (rc != TPC_OK) return rc;
-  const cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+  cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(e);
+  rc = tpc_track_host_fetch(max_tracks, dev, host, nullptr, stream);
+  if (rc != TPC_OK) return rc;
+  e = cudaStreamSynchronize((cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

@@ -1,7 +1,8 @@
 """fp32 operation counts of the per-track arithmetic (bench.py `roofline` for the ALU-bound kernels).
 
-Counted from csrc/tpc_kalman.cuh with one operation per written add / mul / div / sqrt (the library is
-compiled without FMA contraction, so an FMA-capable lane retires one of these per cycle at best):
+Counted from the formulas of R12 / R13 with one operation per add / mul / div / sqrt; a fused
+multiply-add of the arithmetic contract is two of them (a multiplication and an addition), so the count does not
+depend on which terms are fused and the roof it is compared with is the FFMA rate (2 flop per lane per cycle):
 
   propagate (R12)    state + Jacobian 53, F C (rows 0-2) 60, (F C) F^T 50              = 163
   innovation (R13)   S, det, inverse                                                    =   9
