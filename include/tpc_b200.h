@@ -80,6 +80,8 @@ enum {
 #define TPC_ST_TRACKLET_OVERFLOW 1 /* more start hits than max_tracklets: the excess was dropped */
 #define TPC_ST_TRACK_OVERFLOW 2    /* more accepted tracks than max_tracks: the excess was dropped */
 #define TPC_ST_Z_CLAMPED 4         /* a cluster lay outside [z_lo,z_hi] and was put in an edge bin */
+#define TPC_ST_BAD_ROW 8           /* a sector_row outside [0, n_sectors*n_rows): that cluster is in no grid bin, no
+                                      search sees it, it stays unassigned (cluster_track = -1)            */
 
 /* Host POD, passed by pointer and copied during the call.  Every field is an input of the method
  * (SURVEY.md §8(b),(c)): geometry R1-R2, field constant R4, measurement errors R6, grid cell R7,
@@ -96,7 +98,7 @@ typedef struct {
   float ca_max_dydx, ca_max_dzdx, ca_cut;                 /* R9  (2.0, 2.5, 20)                   */
   float chi2_cut, chi2_chain_cut, win_max;                /* R15-R16 (16, 30, 5 cm)               */
   float max_sinphi, edge_margin;                          /* R12, R16 (0.95, 1 cm)                */
-  int32_t max_gap, min_hits, n_fit_passes;                /* R16, R20, R22 (4, 10, 2)             */
+  int32_t max_gap, min_hits, n_fit_passes;                /* R16, R20, R22 (4, 10, 2); min_hits >= 3 (R21) */
   float cov0[5];                 /* initial covariance diagonal (1,1,1,10,100) (R14, R22)         */
 } tpc_params_t;
 
@@ -167,7 +169,8 @@ int tpc_find_export(const tpc_params_t* params_host, int64_t n_clusters, int64_t
  *                       trk_nhits / trk_first_hit / trk_hits (same n_clusters, max_tracklets).
  *                       tpc_find_tracks stored the (y, z, row) of every hit in hit-list order
  *                       there; the fit streams those records instead of gathering, and y, z,
- *                       sector_row, trk_hits are not read (may be NULL).
+ *                       sector_row, trk_hits are not read (may be NULL).  K is clamped to the
+ *                       tracklet capacity of that workspace (find cannot have produced more).
  *   workspace == NULL : self-contained gather through y, z, sector_row (the caller's arrays,
  *                       original order) and trk_hits, so any hit lists can be refitted, e.g.
  *                       truth hits; max_tracklets and ws_bytes are ignored.

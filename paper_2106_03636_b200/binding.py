@@ -23,7 +23,7 @@ TPC_MAX_TRACKLETS = 1 << 25
 CNT_TRACKS, CNT_TRACKLETS, CNT_HITS, CNT_STATUS, CNT_STARTS_FOUND, CNT_TRACKS_FOUND = 0, 1, 2, 3, 4, 5
 CNT_FOLLOWED_DOWN = 6
 CNT_PROP_LO, CNT_UPD_LO, CNT_CAND_LO, CNT_CLAIMS_LO = 8, 10, 12, 14
-ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED = 1, 2, 4
+ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED, ST_BAD_ROW = 1, 2, 4, 8
 
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",

@@ -65,7 +65,7 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
   if (P->n_sectors < 1 || P->n_sectors > 36 || P->n_rows < 3 || P->n_rows > TPC_MAX_ROWS) return false;
   if (!(P->cell_y > 0.0f) || !(P->cell_z > 0.0f) || !(P->z_hi > P->z_lo)) return false;
   if (!(P->sigma_y > 0.0f) || !(P->sigma_z > 0.0f) || !(P->tan_half > 0.0f)) return false;
-  if (P->n_fit_passes < 1 || P->min_hits < 1 || P->max_gap < 0) return false;
+  if (P->n_fit_passes < 1 || P->min_hits < 3 || P->max_gap < 0) return false;  // R21 seeds need three distinct hits
   for (int r = 1; r < P->n_rows; r++)
     if (!(P->row_x[r] > P->row_x[r - 1])) return false;
   memset(G, 0, sizeof(*G));

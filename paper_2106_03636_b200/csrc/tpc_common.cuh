@@ -98,6 +98,8 @@ constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
 constexpr int kMaxBuckets = TPC_MAX_BUCKETS;  // grid build: first-level buckets of the counting sort
 constexpr int kStateVec = 6;    // float4 per tracklet of follower state carried from phase A to phase B (24 words)
 constexpr int kStartBit = 1 << 30;  // rec.w: set on start hits by k_compact_starts (read by the upward legs, R17)
+constexpr int kBadRow = kStartBit - 1;  // rec.w of a cluster whose sector_row names no (sector, row): parked behind the grid
+constexpr int kMaxDevices = 64;     // per-device caches of function attributes / occupancy (one entry per CUDA device)
 constexpr int kMaskWords = 5;  // kept-row mask per tracklet (rows 0..159)
 
 // Start record of a tracklet (R14 inputs), written by k_compact_starts: one 32-byte load in the follower.

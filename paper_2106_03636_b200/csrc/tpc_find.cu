@@ -134,7 +134,7 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
     const int sr = rec_sr(h);
     const int s = sr / nrows, r = sr - s * nrows;
     int bu = -1, bd = -1;
-    if (r >= 1 && r <= nrows - 2) {
+    if (s < sc.nsec && r >= 1 && r <= nrows - 2) {  // (a cluster parked behind the grid has an impossible sector)
       const float yh = h.x, zh = h.y;
       const float wu = ca.wu[r], iy = ca.iy[r], iz = ca.iz[r];
       const float wyu = ca.wyu[r], wzu = ca.wzu[r], wyd = ca.wyd[r], wzd = ca.wzd[r];
@@ -290,15 +290,15 @@ k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const i
     if (scan[p + 1] != ex) {
       const Rec h0 = rec[p];
       const int sr0 = rec_sr(h0);
-      // mark the record as a start hit: the upward legs of the follower look at this bit (R17).  Only this thread
-      // writes this word; other threads read at most y and z of this record.
-      reinterpret_cast<int*>(rec + p)[3] = sr0 | kStartBit;
       const int s = sr0 / sc.nrows, r = sr0 - s * sc.nrows;
       const float zeta = (s < 18) ? h0.y : -h0.y;  // R2/R7, the same expression the grid build bins with
       const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
       const int64_t q = ((int64_t)s * sc.nslab + zb / sc.slab_w) * sc.nrows + r;
       const int t = chunk_base[q] + (ex - chunk_scan0[q]);
       if (t < scap) {
+        // mark the record as a start hit: the upward legs of the follower look at this bit (R17).  Only this thread
+        // writes this word; other threads read at most y and z of this record.  (k_clear_start_bits undoes it.)
+        reinterpret_cast<int*>(rec + p)[3] = sr0 | kStartBit;
         const int p1 = up_c[p];
         const Rec h1 = rec[p1];
         float4* o = reinterpret_cast<float4*>(tl_init + t);
@@ -313,6 +313,15 @@ k_compact_starts(const __grid_constant__ Geo g, int64_t n, int64_t scap, const i
       if (total > scap) atomicOr(ws_counters + WC_STATUS, TPC_ST_TRACKLET_OVERFLOW);
     }
   }
+}
+
+// The start bits of the PREVIOUS tpc_find_tracks on this grid (another set of cuts gives other start hits): the old
+// start list is still in tl_init.  After tpc_grid_build the list is empty and this is a no-op.
+__global__ void __launch_bounds__(kThreads)
+k_clear_start_bits(Rec* rec, const TlInit* __restrict__ tl_init, const int32_t* __restrict__ ws_counters) {
+  const int n_starts = ws_counters[WC_N_STARTS];
+  for (int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x; t < n_starts; t += (int64_t)gridDim.x * kThreads)
+    reinterpret_cast<int*>(rec + tl_init[t].p0)[3] &= ~kStartBit;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -357,6 +366,9 @@ cudaError_t launch_find(const Geo& g, const Ws& w, int32_t* cluster_track, int64
                         int32_t* counters, cudaStream_t st) {
   const int64_t n = w.L.n, scap = w.L.scap;
   cudaError_t e;
+  if (n > 0 && scap > 0)
+    TPC_LAUNCH(KID_COMPACT_STARTS, st,
+               (k_clear_start_bits<<<blocks_for(scap, kThreads, 148 * 8), kThreads, 0, st>>>(w.rec, w.tl_init, w.counters)));
   // queue heads restart; status bits from the grid build are kept
   if ((e = cudaMemsetAsync(w.counters + WC_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.counters + WC_N_STARTS, 0, sizeof(int32_t), st)) != cudaSuccess) return e;

@@ -41,7 +41,7 @@ k_fit_gather(const __grid_constant__ Geo g, const float* __restrict__ y, const f
     const int32_t* hits = trk_hits + trk_first_hit[k];
     auto rowx = [&](int h) { return sX[__ldg(sector_row + h) % nrows]; };
     // R21: seed from the first, middle and last hit
-    const int a = hits[0], b = hits[n / 2], c = hits[n - 1], h1 = hits[1];
+    const int a = hits[0], b = hits[n / 2], c = hits[n - 1], h1 = hits[n > 1 ? 1 : 0];
     const float x1 = rowx(a), y1 = __ldg(y + a), x2 = rowx(b), y2 = __ldg(y + b), x3 = rowx(c), y3 = __ldg(y + c);
     const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
     const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
@@ -99,7 +99,7 @@ k_fit_gather(const __grid_constant__ Geo g, const float* __restrict__ y, const f
 // (y1, sinphi, tanlambda, q/pT), (zRef, x1, first hit's y/z are re-read by the fit loop, -, -).
 __global__ void __launch_bounds__(256)
 k_fit_seed(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const int32_t* __restrict__ counters,
-           int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+           int64_t max_tracks, int64_t k_cap, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
            float4* __restrict__ seed) {
   __shared__ float sX[kMaxRows];
   const Scalars& sc = g.s;
@@ -107,6 +107,7 @@ k_fit_seed(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, co
   __syncthreads();
   int64_t K = counters[TPC_CNT_TRACKS];
   if (K > max_tracks) K = max_tracks;
+  if (K > k_cap) K = k_cap;
   const float kB = sc.kB, ms = sc.max_sinphi;
   for (int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x; k < K; k += (int64_t)gridDim.x * 256) {
     const int n = trk_nhits[k];
@@ -136,7 +137,7 @@ enum FitPhase { F_FETCH = 0, F_RUN, F_DONE };
 
 __global__ void __launch_bounds__(kFitThreads)
 k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const int32_t* __restrict__ counters,
-      int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+      int64_t max_tracks, int64_t k_cap, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
       float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref, float* __restrict__ zref_out,
       float* __restrict__ chi2_out, int32_t* __restrict__ ndf, const float4* __restrict__ seed,
       int32_t* __restrict__ ws_counters) {
@@ -146,6 +147,7 @@ k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const i
   __syncthreads();
   int64_t K64 = counters[TPC_CNT_TRACKS];
   if (K64 > max_tracks) K64 = max_tracks;
+  if (K64 > k_cap) K64 = k_cap;
   const int K = (int)K64;
   const int lane = threadIdx.x & 31;
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
@@ -248,7 +250,7 @@ k_fit(const __grid_constant__ Geo g, const float4* __restrict__ hit_rec, const i
   }
 }
 
-int g_fit_blocks = 0;
+int g_fit_blocks[kMaxDevices] = {0};  // resident blocks of k_fit per device
 
 }  // namespace
 
@@ -259,26 +261,32 @@ cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, con
   (void)n;
   if (max_tracks <= 0) return cudaSuccess;
   cudaError_t e;
+  int64_t max_tracks_fit = max_tracks;  // tracks the cached path can hold seeds for (see below)
   if (w) {
-    if (g_fit_blocks == 0) {
-      int dev = 0, sms = 0, per_sm = 0;
-      if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    int& fit_blocks = g_fit_blocks[dev < kMaxDevices ? dev : kMaxDevices - 1];
+    if (fit_blocks == 0 || dev >= kMaxDevices) {
+      int sms = 0, per_sm = 0;
       if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
       if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit, kFitThreads, 0)) != cudaSuccess) return e;
-      g_fit_blocks = sms * (per_sm > 0 ? per_sm : 1);
+      fit_blocks = sms * (per_sm > 0 ? per_sm : 1);
     }
-    int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
-    if (blocks > g_fit_blocks) blocks = g_fit_blocks;
+    // the hit lists come from the tpc_find_tracks call on this workspace, so K <= its tracklets <= scap_pad; the seed
+    // scratch (the follower's parked states, dead by now) holds kStateVec / 2 seeds per tracklet
+    const int64_t seed_cap = w->L.scap_pad * (int64_t)(kStateVec / 2);
+    if (max_tracks > seed_cap) max_tracks_fit = seed_cap;
+    int64_t blocks = (max_tracks_fit + kFitThreads - 1) / kFitThreads;
+    if (blocks > fit_blocks) blocks = fit_blocks;
     if ((e = cudaMemsetAsync(w->counters + WC_FIT_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
     // seeds go where the follower parked its states (dead by now; at least 96 bytes per tracklet >= 32 per track)
     float4* seed = w->tl_state;
-    int64_t sblocks = (max_tracks + 255) / 256;
+    int64_t sblocks = (max_tracks_fit + 255) / 256;
     if (sblocks > 148 * 64) sblocks = 148 * 64;
-    if (max_tracks > w->L.scap_pad * (int64_t)(kStateVec / 2)) return cudaErrorInvalidValue;  // cannot happen: K <= tracklets
     TPC_LAUNCH(KID_FIT, st,
-               (k_fit_seed<<<(unsigned)sblocks, 256, 0, st>>>(g, w->hit_rec, counters, max_tracks, trk_nhits, trk_first_hit, seed)));
+               (k_fit_seed<<<(unsigned)sblocks, 256, 0, st>>>(g, w->hit_rec, counters, max_tracks, max_tracks_fit, trk_nhits, trk_first_hit, seed)));
     TPC_LAUNCH(KID_FIT, st,
-               (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, w->hit_rec, counters, max_tracks, trk_nhits, trk_first_hit,
+               (k_fit<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, w->hit_rec, counters, max_tracks, max_tracks_fit, trk_nhits, trk_first_hit,
                                                                par, cov, xref, zref, chi2, ndf, seed, w->counters)));
     return cudaGetLastError();
   }

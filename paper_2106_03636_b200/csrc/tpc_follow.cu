@@ -370,7 +370,7 @@ k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32
   }
 }
 
-int g_follow_blocks = 0;
+int g_follow_blocks[kMaxDevices] = {0};  // resident blocks of k_follow per device
 
 }  // namespace
 
@@ -463,12 +463,14 @@ k_list_build(int count_index, int64_t scap_pad, const int32_t* __restrict__ scan
 cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st) {
   cudaError_t e;
   const int64_t scap_pad = w.L.scap_pad;
-  if (g_follow_blocks == 0) {
-    int dev = 0, sms = 0, per_sm = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  int dev = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  int& follow_blocks = g_follow_blocks[dev < kMaxDevices ? dev : kMaxDevices - 1];
+  if (follow_blocks == 0 || dev >= kMaxDevices) {
+    int sms = 0, per_sm = 0;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_follow<false>, kFollowThreads, 0)) != cudaSuccess) return e;
-    g_follow_blocks = sms * (per_sm > 0 ? per_sm : 1);
+    follow_blocks = sms * (per_sm > 0 ? per_sm : 1);
   }
   if ((e = cudaMemsetAsync(w.picked, 0, (size_t)(w.L.n + 1), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(w.counters + WC_QUEUE_B, 0, sizeof(int32_t) * 3, st)) != cudaSuccess) return e;  // + N_SURV, N_WAVE
@@ -487,12 +489,12 @@ cudaError_t launch_follow(const Geo& g, const Ws& w, cudaStream_t st) {
     if (mode < 2) {
       if ((e = cudaMemsetAsync(w.counters + WC_QUEUE, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
       TPC_LAUNCH(KID_FOLLOW, st,
-                 (k_follow<false><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                 (k_follow<false><<<follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
                                                                              w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
                                                                              w.counters)));
     } else {
       TPC_LAUNCH(KID_FOLLOW_B, st,
-                 (k_follow<true><<<g_follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
+                 (k_follow<true><<<follow_blocks, kFollowThreads, 0, st>>>(g, w.rec, w.bin_first, w.up_c, w.tl_init, w.row_hit,
                                                                             w.tl_info, w.tl_key, w.tl_state, w.surv, w.picked,
                                                                             w.counters)));
     }

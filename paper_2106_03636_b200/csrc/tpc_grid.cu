@@ -68,13 +68,14 @@ __global__ void __launch_bounds__(kHistThreads)
 k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nbuckets, const float* __restrict__ y,
               const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ bucket_cnt,
               int32_t* __restrict__ ws_counters) {
-  extern __shared__ int32_t hist[];  // [nbuckets]
+  extern __shared__ int32_t hist[];  // [nbuckets + 1]
   __shared__ GridSmem sm;
   load_grid_rows(sm, g);
-  for (int j = threadIdx.x; j < nbuckets; j += kHistThreads) hist[j] = 0;
+  for (int j = threadIdx.x; j <= nbuckets; j += kHistThreads) hist[j] = 0;
   __syncthreads();
   const Scalars& sc = g.s;
-  bool clamped = false;
+  const int sr_end = sc.nsec * sc.nrows;
+  bool clamped = false, bad = false;
   // every block takes one contiguous slice of the input (the tail of the loop keeps the warp whole for match_any)
   const int64_t per = ((n + gridDim.x - 1) / gridDim.x + kHistThreads * kUnroll - 1) / (kHistThreads * kUnroll) * (kHistThreads * kUnroll);
   const int64_t lo = (int64_t)blockIdx.x * per, hi = lo + per < n ? lo + per : n;
@@ -85,14 +86,19 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
 #pragma unroll
     for (int j = 0; j < kUnroll; j++) {
       const int64_t i = i0 + j * 32 + (threadIdx.x & 31);
-      srv[j] = i < hi ? __ldcs(sector_row + i) : -1;
+      srv[j] = i < hi ? __ldcs(sector_row + i) : 0;
       yv[j] = i < hi ? __ldcs(y + i) : 0.0f;
       zv[j] = i < hi ? __ldcs(z + i) : 0.0f;
     }
 #pragma unroll
     for (int j = 0; j < kUnroll; j++) {
+      // a sector_row outside [0, n_sectors * n_rows) names no grid bin: the cluster goes to the extra bucket
+      // `nbuckets` behind the grid (no search ever reaches it) and a status bit is raised
       int bk = -1;
-      if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], &clamped) >> bucket_shift;
+      if (i0 + j * 32 + (threadIdx.x & 31) < hi) {
+        if ((unsigned)srv[j] < (unsigned)sr_end) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], &clamped) >> bucket_shift;
+        else { bk = nbuckets; bad = true; }
+      }
       // inputs ordered by row put a whole warp in one bucket: one add of 32; otherwise shared-memory atomics
       // (same-address lanes are merged by the hardware)
       const int bk0 = __shfl_sync(kFull, bk, 0);
@@ -104,21 +110,23 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
     }
   }
   __syncthreads();
-  for (int j = threadIdx.x; j < nbuckets; j += kHistThreads) {
+  for (int j = threadIdx.x; j <= nbuckets; j += kHistThreads) {
     const int c = hist[j];
     if (c) atomicAdd(bucket_cnt + j, c);
   }
   if (__any_sync(kFull, clamped) && (threadIdx.x & 31) == 0) atomicOr(ws_counters + WC_STATUS, TPC_ST_Z_CLAMPED);
+  if (__any_sync(kFull, bad) && (threadIdx.x & 31) == 0) atomicOr(ws_counters + WC_STATUS, TPC_ST_BAD_ROW);
 }
 
 __global__ void __launch_bounds__(kThreads)
-k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, const float* __restrict__ y,
+k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nbuckets, const float* __restrict__ y,
                  const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ cursor,
                  Rec* __restrict__ tmp) {
   __shared__ GridSmem sm;
   load_grid_rows(sm, g);
   __syncthreads();
   const Scalars& sc = g.s;
+  const int sr_end = sc.nsec * sc.nrows;
   const int lane = threadIdx.x & 31;
   const int64_t span = (int64_t)kThreads * kUnroll;
   for (int64_t i0 = (int64_t)blockIdx.x * span + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < n;
@@ -128,7 +136,7 @@ k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, con
 #pragma unroll
     for (int j = 0; j < kUnroll; j++) {
       const int64_t i = i0 + j * 32 + lane;
-      srv[j] = i < n ? __ldcs(sector_row + i) : -1;
+      srv[j] = i < n ? __ldcs(sector_row + i) : 0;
       yv[j] = i < n ? __ldcs(y + i) : 0.0f;
       zv[j] = i < n ? __ldcs(z + i) : 0.0f;
     }
@@ -136,7 +144,14 @@ k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, con
     for (int j = 0; j < kUnroll; j++) {
       const int64_t i = i0 + j * 32 + lane;
       int bk = -1;
-      if (srv[j] >= 0) bk = bin_of(sm, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift;
+      if (i < n) {
+        if ((unsigned)srv[j] < (unsigned)sr_end) {
+          bk = bin_of(sm, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift;
+        } else {  // no such (sector, row): parked behind the grid with an impossible sector_row (see k_bucket_hist)
+          bk = nbuckets;
+          srv[j] = kBadRow;
+        }
+      }
       // Warp-aggregated append.  match.any is slow when all 32 keys differ (shuffled input), and then there is
       // nothing to aggregate: it is only used when some neighbouring lanes share a bucket (inputs ordered by row,
       // where it turns up to 32 same-address atomics into one).
@@ -204,7 +219,7 @@ k_bucket_sort(const __grid_constant__ Geo g, int64_t n, int64_t nb, int bucket_s
     }
     __syncthreads();
     for (int j = tid; j < nbins; j += kSortThreads) bin_first[bin0 + j] = start + cnt[pad32(j)];  // coalesced
-    if (b == nbuckets - 1 && tid == 0) bin_first[nb] = (int)n;
+    if (b == nbuckets - 1 && tid == 0) bin_first[nb] = bucket_first[nbuckets];  // clusters of the grid (n minus the bad rows)
     __syncthreads();
     for (int i0 = start + tid; i0 < end; i0 += kSortThreads * kUnroll) {
       Rec r[kUnroll];
@@ -238,6 +253,9 @@ k_bucket_sort(const __grid_constant__ Geo g, int64_t n, int64_t nb, int bucket_s
       }
     }
   }
+  // clusters without a valid (sector, row) keep their place behind the grid (order unspecified; no bin covers them)
+  if (blockIdx.x == 0)
+    for (int i = bucket_first[nbuckets] + tid; i < bucket_first[nbuckets + 1]; i += kSortThreads) rec[i] = tmp[i];
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -261,11 +279,14 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
   cudaError_t e;
   const int sh = bucket_shift_for(nb);
   const int nbuckets = (int)((nb + ((int64_t)1 << sh) - 1) >> sh);
-  const size_t hist_smem = sizeof(int32_t) * (size_t)nbuckets;
+  const size_t hist_smem = sizeof(int32_t) * (size_t)(nbuckets + 1);
   const size_t sort_smem = sizeof(int32_t) * (size_t)(((size_t)1 << sh) + ((size_t)1 << (sh - 5)) + 32);
-  static bool attr_done = false;
-  if (!attr_done) {
-    if ((e = cudaFuncSetAttribute(k_bucket_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBuckets * 4)) != cudaSuccess) return e;
+  static bool attr_done_dev[kMaxDevices] = {false};  // function attributes are per device
+  int dev = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  bool& attr_done = attr_done_dev[dev < kMaxDevices ? dev : kMaxDevices - 1];
+  if (!attr_done || dev >= kMaxDevices) {
+    if ((e = cudaFuncSetAttribute(k_bucket_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (kMaxBuckets + 1) * 4)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_bucket_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (32768 + 1024 + 32) * 4)) != cudaSuccess)
       return e;
     attr_done = true;
@@ -277,13 +298,14 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
                (k_bucket_hist<<<blocks_for(n, kHistThreads * 64, 148 * (hist_smem + 2048 <= 110000 ? 2 : 1)), kHistThreads,
                                hist_smem, st>>>(
                    g, n, sh, nbuckets, y, z, sector_row, w.bucket_first, w.counters)));
-  if ((e = exclusive_scan<int32_t>(w.bucket_first, w.bucket_first, nbuckets + 1, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
-  if ((e = cudaMemcpyAsync(w.bucket_cursor, w.bucket_first, sizeof(int32_t) * (size_t)(nbuckets + 1), cudaMemcpyDeviceToDevice,
+  // nbuckets grid buckets + the bucket of clusters without a valid (sector, row) + the total
+  if ((e = exclusive_scan<int32_t>(w.bucket_first, w.bucket_first, nbuckets + 2, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
+  if ((e = cudaMemcpyAsync(w.bucket_cursor, w.bucket_first, sizeof(int32_t) * (size_t)(nbuckets + 2), cudaMemcpyDeviceToDevice,
                            st)) != cudaSuccess)
     return e;
   if (n > 0)
     TPC_LAUNCH(KID_BUCKET_SCATTER, st,
-               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll, TPC_SCATTER_CAP), kThreads, 0, st>>>(g, n, sh, y, z, sector_row, w.bucket_cursor,
+               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll, TPC_SCATTER_CAP), kThreads, 0, st>>>(g, n, sh, nbuckets, y, z, sector_row, w.bucket_cursor,
                                                                               (Rec*)w.hit_rec)));
   TPC_LAUNCH(KID_BUCKET_SORT, st,
              (k_bucket_sort<<<blocks_for(nbuckets, 1, TPC_SORT_CAP), kSortThreads, sort_smem, st>>>(

@@ -187,6 +187,63 @@ def test_clusters_outside_z_range_are_clamped_not_lost(torch_cuda, orc):
     assert st["assign_identical"] == ev.n
 
 
+def test_corrupt_sector_row_is_flagged_and_ignored(torch_cuda, orc):
+    """A sector_row outside [0, n_sectors * n_rows) (negative or too large) names no grid bin: the status bit is set,
+    nothing is written out of bounds, those clusters stay unassigned, and everything else is tracked exactly as if
+    they were not there (oracle on the valid clusters alone)."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(1, n_tracks=300)
+    p = ev.params
+    rng = np.random.Generator(np.random.PCG64(3))
+    sr = ev.sector_row.copy()
+    bad = rng.choice(ev.n, 37, replace=False)
+    sr[bad[:12]] = -1 - rng.integers(0, 1000, 12)
+    sr[bad[12:24]] = int(p.n_sectors) * int(p.n_rows) + rng.integers(0, 5000, 12)
+    sr[bad[24:]] = 2**31 - 1 - rng.integers(0, 100, 13)
+    trk = binding.Tracker(p, ev.n)
+    t = torch_cuda
+    res = trk.run(t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(sr).cuda())
+    assert res["status"] & binding.ST_BAD_ROW
+    assert np.all(res["cluster_track"][bad] == -1)
+    good = np.setdiff1d(np.arange(ev.n), bad)                  # ascending: index tie-breaks are preserved
+    o = orc.run(p, ev.y[good], ev.z[good], ev.sector_row[good], "f32", True)
+    new_of_old = np.full(ev.n, -1, np.int64)
+    new_of_old[good] = np.arange(good.size)
+    sub = dict(res)
+    sub["cluster_track"] = res["cluster_track"][good]
+    sub["trk_seed"] = new_of_old[res["trk_seed"]].astype(np.int32)
+    sub["trk_hits"] = new_of_old[res["trk_hits"]].astype(np.int32)
+    assert sub["trk_hits"].min() >= 0 and sub["trk_seed"].min() >= 0
+    st = parity.compare_tracks(o, sub, good.size)
+    parity.assert_contract(st, exact_count=True)
+    assert st["assign_identical"] == good.size and st["par_bit_identical"]
+    sorted_idx, bin_first = trk.grid_export()
+    assert bin_first[-1] == good.size and set(sorted_idx[good.size:].tolist()) == set(bad.tolist())
+
+
+def test_find_twice_on_one_grid_with_other_cuts(torch_cuda, orc):
+    """The grid stays valid until the next tpc_grid_build: a second tpc_find_tracks on it with other cuts (other links,
+    other start hits) must give what a fresh build with those cuts gives -- no start bit of the first call survives."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(1, n_tracks=300)
+    p2 = ev.params.with_(ca_cut=2.0, chi2_cut=9.0, max_gap=2)
+    t = torch_cuda
+    y, z, sr = t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(ev.sector_row).cuda()
+    trk = binding.Tracker(ev.params, ev.n)
+    first = trk.run(y, z, sr)
+    trk.params, trk.P = p2, binding.make_params(p2)           # same grid (cells unchanged), other cuts
+    trk.find_tracks()
+    trk.fit_tracks()
+    again = trk.results()
+    fresh = binding.Tracker(p2, ev.n).run(y, z, sr)
+    assert not np.array_equal(first["cluster_track"], fresh["cluster_track"])      # the cuts do matter
+    for k in fresh:
+        assert np.array_equal(again[k], fresh[k]), k
+    o = orc.run(p2, ev.y, ev.z, ev.sector_row, "f32", True)
+    st = parity.compare_tracks(o, again, ev.n)
+    assert st["assign_identical"] == ev.n and st["tracks_oracle"] == st["tracks_cuda"]
+
+
 def test_capacity_overflow_is_flagged_and_bounded(torch_cuda):
     from paper_2106_03636_b200 import binding
     ev = config0()
