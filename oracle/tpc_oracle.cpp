@@ -788,6 +788,296 @@ T update_impl(const OrcParams* P, T* p5, T* c15, T ym, T zm) {
   return chi2;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// R26 ("full tracking in the TPC", l.60): merging of the sector-local
+// tracks of R20-R22 across the 20-degree sector edges, across the central electrode (A side <-> C side) and across
+// holes longer than max_gap, then a refit of the merged hit list.  The paper fixes none of it: this is a reading.
+//
+//   outer state of track A  = its fitted state (R22, at the innermost hit) transported by R12 to the row of its
+//                             outermost hit, covariance included (Q = 0: the fit is one helix)
+//   relation of (A, B)      : same sector | azimuthal neighbours on one side (B's frame is rotated by D = +-20 deg) |
+//                             mirror sectors across the central electrode (same azimuth, other side)
+//   B can follow A iff        1 <= first row of B - last row of A <= max_rows, the ends are close in z
+//                             (same side: |z_B - z_A| <= dz_max; across the electrode the two sides measure
+//                             z_true -+ v_d t, so |z_B + z_A| <= dz_max), and chi2 < chi2_cut, where
+//   chi2                    : A's outer state rotated into B's frame (x' = x cosD + y sinD, y' = -x sinD + y cosD,
+//                             sinphi' = sinphi cosD - cosphi sinD, cosphi' > 0; covariance C'_ij = J_i C_ij J_j with
+//                             J = (cosphi/cosphi', 1, cosphi'/cosphi, 1, 1)), transported by R12 to the x of B's
+//                             innermost hit, d = that state - B's fitted state (z through zRef_A - zRef_B),
+//                             S = C_A' + C_B, chi2 = d^T S^-1 d by Cholesky, over (y, z, sinphi, tanlambda, q/pT);
+//                             across the electrode z is not compared (the time offset is free: 4 parameters) but
+//                             |z_A' + z_B| <= ce_tol + 2 |tanlambda_B| dx / cosphi_B must hold (z_true = 0 somewhere
+//                             on the dx = x_B - x_A between the two ends)
+//   arbitration             : succ[A] = arg-min chi2 over B, pred[B] = arg-min chi2 over A (ties: lowest seed);
+//                             A -> B is a link iff succ[A] = B and pred[B] = A (reciprocal, as R10)
+//   global tracks           = the chains of links (first rows strictly increase along a chain, so there is no cycle)
+// ---------------------------------------------------------------------------------------------
+struct OrcMergeParams {
+  double chi2_cut, dz_max, ce_tol;
+  int32_t max_rows, reserved;
+};
+
+enum { REL_NONE = 0, REL_SAME = 1, REL_NEXT = 2, REL_PREV = 3, REL_CE = 4 };  // B's sector relative to A's
+
+inline int sector_relation(int sa, int sb) {
+  if (sa == sb) return REL_SAME;
+  const int aa = sa % 18, ab = sb % 18;
+  if ((sa < 18) != (sb < 18)) return aa == ab ? REL_CE : REL_NONE;
+  if (ab == (aa + 1) % 18) return REL_NEXT;   // B's frame = A's rotated by +20 degrees
+  if (aa == (ab + 1) % 18) return REL_PREV;   // ... by -20 degrees
+  return REL_NONE;
+}
+
+// Rotation of a state at x into the frame turned by D (cd = cos D, sd = sin D).  Returns false if the track does not
+// point into the +x half of the new frame (cosphi' <= 0) or |sinphi'| > max_sinphi.
+template <class T>
+bool rotate_state(State<T>& st, T& x, T cd, T sd, T max_sinphi) {
+  const T y = st.p[0], s = st.p[2];
+  const T c = std::sqrt((T)1 - s * s);
+  const T xn = x * cd + y * sd;
+  const T yn = y * cd - x * sd;
+  const T sn = s * cd - c * sd;
+  const T cn = c * cd + s * sd;
+  if (!(cn > (T)0) || !(std::fabs(sn) <= max_sinphi)) return false;
+  T J[5] = {c / cn, (T)1, cn / c, (T)1, (T)1};
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) st.C[i][j] = st.C[j][i] = (J[i] * st.C[i][j]) * J[j];
+  st.p[0] = yn;
+  st.p[2] = sn;
+  x = xn;
+  return true;
+}
+
+// chi2 = d^T S^-1 d over the parameters idx[0..n), S symmetric positive definite, by Cholesky; -1 if S is not.
+template <class T>
+T chi2_cholesky(const T S[5][5], const T d[5], const int* idx, int n) {
+  T L[5][5], yv[5];
+  for (int i = 0; i < n; i++)
+    for (int j = 0; j <= i; j++) {
+      T sum = S[idx[i]][idx[j]];
+      for (int k = 0; k < j; k++) sum = sum - L[i][k] * L[j][k];
+      if (i == j) {
+        if (!(sum > (T)0)) return (T)-1;
+        L[i][i] = std::sqrt(sum);
+      } else {
+        L[i][j] = sum / L[j][j];
+      }
+    }
+  T chi2 = 0;
+  for (int i = 0; i < n; i++) {
+    T sum = d[idx[i]];
+    for (int k = 0; k < i; k++) sum = sum - L[i][k] * yv[k];
+    yv[i] = sum / L[i][i];
+    chi2 = chi2 + yv[i] * yv[i];
+  }
+  return chi2;
+}
+
+template <class T>
+struct TrackView {   // the fitted sector-local tracks, SoA with leading dimension ld
+  int64_t K, ld;
+  const T *par, *cov, *zref;
+  const int32_t *sector, *row_first, *row_last, *seed;
+  State<T> state(int64_t k) const {
+    State<T> st;
+    for (int i = 0; i < 5; i++) st.p[i] = par[i * ld + k];
+    for (int i = 0, m = 0; i < 5; i++)
+      for (int j = 0; j <= i; j++, m++) st.C[i][j] = st.C[j][i] = cov[m * ld + k];
+    return st;
+  }
+};
+
+constexpr double kCos20 = 0.93969262078590838405, kSin20 = 0.34202014332566873304;
+
+// chi2 of "B follows A" (see the header of this section), -1 if the pair is impossible.  `out` is A's outer state at
+// the x of A's outermost hit.
+template <class T>
+T match_chi2(const OrcParams& P, const OrcMergeParams& M, const Geo<T>& G, const TrackView<T>& tv, int64_t a, int64_t b,
+             const State<T>& out, int rel) {
+  const int dr = tv.row_first[b] - tv.row_last[a];
+  if (dr < 1 || dr > M.max_rows) return (T)-1;
+  const T zA = tv.zref[a] + out.p[1], zB = tv.zref[b] + tv.par[1 * tv.ld + b];
+  if (rel == REL_CE ? !(std::fabs(zB + zA) <= (T)M.dz_max) : !(std::fabs(zB - zA) <= (T)M.dz_max)) return (T)-1;
+  State<T> r = out;
+  T x = G.X[tv.row_last[a]];
+  if (rel == REL_NEXT || rel == REL_PREV) {
+    const T sd = rel == REL_NEXT ? (T)kSin20 : -(T)kSin20;
+    if (!rotate_state(r, x, (T)kCos20, sd, (T)P.max_sinphi)) return (T)-1;
+  }
+  const T xb = G.X[tv.row_first[b]];
+  if (!propagate(r, xb - x, G.kB, (T)P.max_sinphi)) return (T)-1;
+  const State<T> sb = tv.state(b);
+  T d[5], S[5][5];
+  d[0] = r.p[0] - sb.p[0];
+  d[1] = (tv.zref[a] - tv.zref[b]) + (r.p[1] - sb.p[1]);
+  for (int i = 2; i < 5; i++) d[i] = r.p[i] - sb.p[i];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) S[i][j] = r.C[i][j] + sb.C[i][j];
+  if (rel == REL_CE) {
+    const T zsum = (tv.zref[a] + r.p[1]) + (tv.zref[b] + sb.p[1]);
+    const T cb = std::sqrt((T)1 - sb.p[2] * sb.p[2]);
+    const T lim = (T)M.ce_tol + (((T)2 * std::fabs(sb.p[3])) * (xb - G.X[tv.row_last[a]])) / cb;
+    if (!(std::fabs(zsum) <= lim)) return (T)-1;
+    const int idx[4] = {0, 2, 3, 4};
+    return chi2_cholesky(S, d, idx, 4);
+  }
+  const int idx[5] = {0, 1, 2, 3, 4};
+  return chi2_cholesky(S, d, idx, 5);
+}
+
+template <class T>
+void merge_match_impl(const OrcParams* P, const OrcMergeParams* M, int64_t K, const T* par, const T* cov, const T* zref,
+                      const int32_t* sector, const int32_t* row_first, const int32_t* row_last, const int32_t* seed,
+                      int32_t* succ, int32_t* pred, T* succ_chi2, T* pair_chi2 /* [K*K] or NULL: every pair, for the pins */) {
+  Geo<T> G(*P);
+  TrackView<T> tv{K, K, par, cov, zref, sector, row_first, row_last, seed};
+  std::vector<T> best_s((size_t)K), best_p((size_t)K);
+  for (int64_t k = 0; k < K; k++) succ[k] = pred[k] = -1;
+  if (pair_chi2)
+    for (int64_t i = 0; i < K * K; i++) pair_chi2[i] = (T)-1;
+  std::vector<std::vector<int32_t>> by_sector((size_t)G.nsec);
+  for (int64_t k = 0; k < K; k++) by_sector[(size_t)sector[k]].push_back((int32_t)k);
+  for (int64_t a = 0; a < K; a++) {
+    State<T> out = tv.state(a);
+    if (row_last[a] != row_first[a] &&
+        !propagate(out, G.X[row_last[a]] - G.X[row_first[a]], G.kB, (T)P->max_sinphi))
+      continue;   // no outer state: A has no successor
+    for (int sb = 0; sb < G.nsec; sb++) {
+      const int rel = sector_relation(sector[a], sb);
+      if (rel == REL_NONE) continue;
+      for (int32_t b : by_sector[(size_t)sb]) {
+        if (b == a) continue;
+        const T chi2 = match_chi2(*P, *M, G, tv, a, b, out, rel);
+        if (pair_chi2) pair_chi2[a * K + b] = chi2;
+        if (!(chi2 >= (T)0) || !(chi2 < (T)M->chi2_cut)) continue;
+        if (succ[a] < 0 || chi2 < best_s[(size_t)a] || (chi2 == best_s[(size_t)a] && seed[b] < seed[succ[a]])) {
+          succ[a] = b;
+          best_s[(size_t)a] = chi2;
+        }
+        if (pred[b] < 0 || chi2 < best_p[(size_t)b] || (chi2 == best_p[(size_t)b] && seed[a] < seed[pred[b]])) {
+          pred[b] = (int32_t)a;
+          best_p[(size_t)b] = chi2;
+        }
+      }
+    }
+  }
+  // reciprocal links only
+  for (int64_t a = 0; a < K; a++) {
+    succ_chi2[a] = succ[a] >= 0 ? best_s[(size_t)a] : (T)-1;
+    if (succ[a] >= 0 && pred[succ[a]] != (int32_t)a) succ[a] = -1;
+  }
+  for (int64_t b = 0; b < K; b++)
+    if (pred[b] >= 0 && succ[pred[b]] != (int32_t)b) pred[b] = -1;
+}
+
+// Refit of the global tracks (chains of links).  A chain's hits are taken segment by segment, rows ascending; the
+// filter is R22's (pass 1 inner -> outer, pass 2 outer -> inner, covariance reset to cov0 at the start of a pass, all
+// hits used) started from the head segment's own fitted state, with two additions at a change of segment:
+//   other sector : the state is rotated into the new frame (rotate_state, D = +-20 degrees) -- outward at once (as in
+//                  the matching), inward only after a transport, in the old frame, to the plane of the next hit
+//   other side   : the time offset is free, so zRef is re-based on the first hit of the new side
+//                  (zRef <- z_hit - dz predicted there: that hit's z residual is zero, and ndf loses 1)
+// A track without links keeps its sector-local fit.  Output per global track (in ascending order of the head's
+// sector-local index): head, segments, hits, state at the innermost hit in the head's frame.
+template <class T>
+int64_t merge_fit_impl(const OrcParams* P, int64_t n, const T* y, const T* z, const int32_t* sr, int64_t K, const T* par,
+                       const T* cov, const T* xref, const T* zref, const T* chi2, const int32_t* ndf, const int32_t* sector,
+                       const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, const int32_t* succ,
+                       const int32_t* pred, int32_t* trk_global, int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, T* gpar,
+                       T* gcov, T* gxref, T* gzref, T* gchi2, int32_t* gndf) {
+  Geo<T> G(*P);
+  Clusters<T> cl{n, y, z, sr, P->n_rows};
+  int64_t Mg = 0;
+  for (int64_t h = 0; h < K; h++)
+    if (pred[h] < 0) Mg++;
+  int64_t g = 0;
+  for (int64_t h = 0; h < K; h++) {
+    if (pred[h] >= 0) continue;
+    std::vector<int32_t> seg;
+    for (int32_t k = (int32_t)h; k >= 0; k = succ[k]) seg.push_back(k);
+    int nh = 0;
+    for (int32_t k : seg) {
+      trk_global[k] = (int32_t)g;
+      nh += trk_nhits[k];
+    }
+    g_head[g] = (int32_t)h;
+    g_nseg[g] = (int32_t)seg.size();
+    g_nhits[g] = nh;
+    if (seg.size() == 1) {
+      for (int i = 0; i < 5; i++) gpar[i * Mg + g] = par[i * K + h];
+      for (int i = 0; i < 15; i++) gcov[i * Mg + g] = cov[i * K + h];
+      gxref[g] = xref[h]; gzref[g] = zref[h]; gchi2[g] = chi2[h]; gndf[g] = ndf[h];
+      g++;
+      continue;
+    }
+    // hits of the chain in order, with the sector of each
+    std::vector<int32_t> hits, hsec;
+    for (int32_t k : seg)
+      for (int i = 0; i < trk_nhits[k]; i++) {
+        hits.push_back(trk_hits[trk_first_hit[k] + i]);
+        hsec.push_back(sector[k]);
+      }
+    State<T> st;
+    for (int i = 0; i < 5; i++) st.p[i] = par[i * K + h];
+    T zr = zref[h];
+    T x_at = G.X[cl.row(hits[0])];
+    int cur_sec = sector[h];
+    T c2 = 0;
+    int lost = 0;
+    bool ok = true;
+    const int N = (int)hits.size();
+    for (int pass = 0; pass < P->n_fit_passes && ok; pass++) {
+      reset_cov(st, *P);
+      c2 = 0;
+      lost = 0;
+      const int dir = (pass % 2 == 0) ? +1 : -1;
+      int k = dir > 0 ? 0 : N - 1;
+      for (int cnt = 0; cnt < N && ok; cnt++, k += dir) {
+        const int32_t hit = hits[k];
+        const int hs = hsec[k];
+        bool rebase = false;
+        if (hs != cur_sec) {
+          const int rel = sector_relation(cur_sec, hs);
+          if (rel == REL_NEXT || rel == REL_PREV) {
+            const T cd = (T)kCos20, sd = rel == REL_NEXT ? (T)kSin20 : -(T)kSin20;
+            if (dir < 0) {
+              // inward, |sinphi| grows in the frame being entered (a track leaves a sector through the edge it bends
+              // towards): stay in the current frame up to the plane of the next hit, x = X_h cosD - y_h sinD there
+              const T xc = G.X[cl.row(hit)] * cd - cl.y[hit] * sd;
+              if (!propagate(st, xc - x_at, G.kB, (T)P->max_sinphi)) { ok = false; break; }
+              x_at = xc;
+            }
+            if (!rotate_state(st, x_at, cd, sd, (T)P->max_sinphi)) { ok = false; break; }
+          } else if (rel == REL_CE) {
+            rebase = true;
+          }
+          cur_sec = hs;
+        }
+        const T xh = G.X[cl.row(hit)];
+        if (cnt > 0) {   // the first hit of a pass is the one the state sits at
+          if (!propagate(st, xh - x_at, G.kB, (T)P->max_sinphi)) { ok = false; break; }
+          x_at = xh;
+        }
+        if (rebase) {
+          zr = cl.z[hit] - st.p[1];
+          lost++;
+        }
+        c2 += update(st, cl.y[hit], cl.z[hit] - zr, G.sy2, G.sz2);
+      }
+    }
+    for (int i = 0; i < 5; i++) gpar[i * Mg + g] = st.p[i];
+    for (int i = 0, m = 0; i < 5; i++)
+      for (int j = 0; j <= i; j++) gcov[(m++) * Mg + g] = st.C[i][j];
+    gxref[g] = x_at;
+    gzref[g] = zr;
+    gchi2[g] = ok ? c2 : (T)-1;
+    gndf[g] = ok ? 2 * N - 5 - lost : -1;
+    g++;
+  }
+  return Mg;
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -1005,4 +1295,38 @@ ORC_API int64_t orc_collisions(int64_t K, const float* t0, const float* dca, con
     trk_collision[k] = (best >= 0 && best < coll_cap) ? best : -1;
   }
   return C;
+}
+
+// ---------------------------------------------------------------------------------------------
+// R26 C surface (see the section above): track matching across sector edges / the central electrode / long holes,
+// and the refit of the merged hit lists.  pair_chi2 (may be NULL): [K*K], chi2 of "b follows a" at [a*K + b], -1 = impossible.
+// ---------------------------------------------------------------------------------------------
+ORC_API int64_t orc_sizeof_merge_params() { return (int64_t)sizeof(OrcMergeParams); }
+ORC_API void orc_merge_match_f32(const OrcParams* P, const OrcMergeParams* M, int64_t K, const float* par, const float* cov,
+                                 const float* zref, const int32_t* sector, const int32_t* row_first, const int32_t* row_last,
+                                 const int32_t* seed, int32_t* succ, int32_t* pred, float* succ_chi2, float* pair_chi2) {
+  merge_match_impl<float>(P, M, K, par, cov, zref, sector, row_first, row_last, seed, succ, pred, succ_chi2, pair_chi2);
+}
+ORC_API void orc_merge_match_f64(const OrcParams* P, const OrcMergeParams* M, int64_t K, const double* par, const double* cov,
+                                 const double* zref, const int32_t* sector, const int32_t* row_first, const int32_t* row_last,
+                                 const int32_t* seed, int32_t* succ, int32_t* pred, double* succ_chi2, double* pair_chi2) {
+  merge_match_impl<double>(P, M, K, par, cov, zref, sector, row_first, row_last, seed, succ, pred, succ_chi2, pair_chi2);
+}
+ORC_API int64_t orc_merge_fit_f32(const OrcParams* P, int64_t n, const float* y, const float* z, const int32_t* sr, int64_t K,
+                                  const float* par, const float* cov, const float* xref, const float* zref, const float* chi2,
+                                  const int32_t* ndf, const int32_t* sector, const int32_t* trk_nhits,
+                                  const int64_t* trk_first_hit, const int32_t* trk_hits, const int32_t* succ, const int32_t* pred,
+                                  int32_t* trk_global, int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar,
+                                  float* gcov, float* gxref, float* gzref, float* gchi2, int32_t* gndf) {
+  return merge_fit_impl<float>(P, n, y, z, sr, K, par, cov, xref, zref, chi2, ndf, sector, trk_nhits, trk_first_hit, trk_hits,
+                               succ, pred, trk_global, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref, gchi2, gndf);
+}
+ORC_API int64_t orc_merge_fit_f64(const OrcParams* P, int64_t n, const double* y, const double* z, const int32_t* sr, int64_t K,
+                                  const double* par, const double* cov, const double* xref, const double* zref,
+                                  const double* chi2, const int32_t* ndf, const int32_t* sector, const int32_t* trk_nhits,
+                                  const int64_t* trk_first_hit, const int32_t* trk_hits, const int32_t* succ, const int32_t* pred,
+                                  int32_t* trk_global, int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, double* gpar,
+                                  double* gcov, double* gxref, double* gzref, double* gchi2, int32_t* gndf) {
+  return merge_fit_impl<double>(P, n, y, z, sr, K, par, cov, xref, zref, chi2, ndf, sector, trk_nhits, trk_first_hit, trk_hits,
+                                succ, pred, trk_global, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref, gchi2, gndf);
 }

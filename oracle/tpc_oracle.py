@@ -313,6 +313,96 @@ def collisions(t0, dca, t_lo, t_hi, w=1.0, dca_max=3.0, n_min=5, sector=None, si
     return dict(coll_time=ct[:n], coll_ntracks=cn[:n], coll_bin=cb[:n], trk_collision=tc[:K])
 
 
+class OrcMergeParams(C.Structure):
+    _fields_ = [("chi2_cut", C.c_double), ("dz_max", C.c_double), ("ce_tol", C.c_double), ("max_rows", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+#: R26 defaults: chi2 cut over 5 (4 across the electrode) parameters, largest row distance between the
+#: two ends, z window between the ends [cm], tolerance of the electrode-crossing condition [cm]
+MERGE_DEFAULTS = dict(chi2_cut=50.0, dz_max=64.0, ce_tol=1.0, max_rows=12)
+
+
+def make_merge_params(mp=None, precision="f32") -> OrcMergeParams:
+    d = dict(MERGE_DEFAULTS)
+    if mp:
+        d.update(mp if isinstance(mp, dict) else {k: getattr(mp, k) for k in MERGE_DEFAULTS})
+    rnd = (lambda v: float(np.float32(v))) if precision == "f32" else float
+    M = OrcMergeParams()
+    M.chi2_cut, M.dz_max, M.ce_tol, M.max_rows = rnd(d["chi2_cut"]), rnd(d["dz_max"]), rnd(d["ce_tol"]), int(d["max_rows"])
+    assert lib().orc_sizeof_merge_params() == C.sizeof(OrcMergeParams)
+    return M
+
+
+def track_rows(n_rows, sector_row, trk_nhits, trk_first_hit, trk_hits):
+    """(sector, first row, last row) of every track from its hit list (rows ascend along a list)."""
+    sr = np.asarray(sector_row)
+    fh = np.asarray(trk_first_hit, np.int64); nh = np.asarray(trk_nhits, np.int64)
+    if fh.size == 0:
+        z = np.zeros(0, np.int32)
+        return z, z, z
+    first = sr[np.asarray(trk_hits)[fh]]
+    last = sr[np.asarray(trk_hits)[fh + nh - 1]]
+    return (first // n_rows).astype(np.int32), (first % n_rows).astype(np.int32), (last % n_rows).astype(np.int32)
+
+
+def merge_match(p, par, cov, zref, sector, row_first, row_last, seed, mp=None, precision="f32", want_pairs=False):
+    """R26 matching: dict(succ[K], pred[K] (track index or -1, reciprocal links only), succ_chi2[K] (chi2 of the best
+    candidate successor, -1 = none), pair_chi2[K,K]? (chi2 of "b follows a", -1 = impossible))."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision); M = make_merge_params(mp, precision)
+    par = np.ascontiguousarray(par, rt); cov = np.ascontiguousarray(cov, rt); zref = np.ascontiguousarray(zref, rt)
+    K = par.shape[1]
+    i32 = lambda a: np.ascontiguousarray(a, np.int32)
+    sector, row_first, row_last, seed = i32(sector), i32(row_first), i32(row_last), i32(seed)
+    succ = np.empty(K, np.int32); pred = np.empty(K, np.int32); sc = np.empty(K, rt)
+    pairs = np.empty((K, K), rt) if want_pairs else None
+    fn = getattr(lib(), f"orc_merge_match_{sfx}")
+    fn.restype = None
+    fn(C.byref(P), C.byref(M), C.c_int64(K), _ptr(par), _ptr(cov), _ptr(zref), _ptr(sector), _ptr(row_first), _ptr(row_last),
+       _ptr(seed), _ptr(succ), _ptr(pred), _ptr(sc), _ptr(pairs))
+    out = dict(succ=succ, pred=pred, succ_chi2=sc)
+    if want_pairs:
+        out["pair_chi2"] = pairs
+    return out
+
+
+def merge_fit(p, y, z, sector_row, fit, sector, trk_nhits, trk_first_hit, trk_hits, succ, pred, precision="f32"):
+    """R26 refit of the chains: dict(trk_global[K], g_head[M], g_nseg, g_nhits, gpar[5,M], gcov[15,M], gxref, gzref,
+    gchi2, gndf).  `fit` = the dict orc.fit returned for the sector-local tracks."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    c = lambda a: np.ascontiguousarray(a, rt)
+    i32 = lambda a: np.ascontiguousarray(a, np.int32)
+    K = int(np.asarray(succ).size)
+    pred = i32(pred); succ = i32(succ)
+    Mg = int(np.count_nonzero(pred < 0))
+    tg = np.empty(K, np.int32); gh = np.empty(Mg, np.int32); gs = np.empty(Mg, np.int32); gn = np.empty(Mg, np.int32)
+    gpar = np.empty((5, Mg), rt); gcov = np.empty((15, Mg), rt)
+    gx = np.empty(Mg, rt); gz = np.empty(Mg, rt); gc = np.empty(Mg, rt); gndf = np.empty(Mg, np.int32)
+    fn = getattr(lib(), f"orc_merge_fit_{sfx}")
+    fn.restype = C.c_int64
+    par, cov, xref, zref, chi2 = c(fit["par"]), c(fit["cov"]), c(fit["xref"]), c(fit["zref"]), c(fit["chi2"])
+    ndf = i32(fit["ndf"]); sector = i32(sector); nh = i32(trk_nhits); th = i32(trk_hits)
+    fh = np.ascontiguousarray(trk_first_hit, np.int64)
+    m = fn(C.byref(P), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int64(K), _ptr(par), _ptr(cov), _ptr(xref), _ptr(zref),
+           _ptr(chi2), _ptr(ndf), _ptr(sector), _ptr(nh), _ptr(fh), _ptr(th), _ptr(succ), _ptr(pred), _ptr(tg), _ptr(gh), _ptr(gs),
+           _ptr(gn), _ptr(gpar), _ptr(gcov), _ptr(gx), _ptr(gz), _ptr(gc), _ptr(gndf))
+    assert int(m) == Mg
+    return dict(trk_global=tg, g_head=gh, g_nseg=gs, g_nhits=gn, gpar=gpar, gcov=gcov, gxref=gx, gzref=gz, gchi2=gc, gndf=gndf)
+
+
+def merge(p, y, z, sector_row, o, mp=None, precision="f32", want_pairs=False):
+    """R26 on the output `o` of run(): matching + refit of the chains.  Returns the two dicts merged, plus the
+    per-track (sector, row_first, row_last) it derived from the hit lists."""
+    sector, rf, rl = track_rows(int(p.n_rows), sector_row, o["trk_nhits"], o["trk_first_hit"], o["trk_hits"])
+    m = merge_match(p, o["par"], o["cov"], o["zref"], sector, rf, rl, o["trk_seed"], mp, precision, want_pairs)
+    f = merge_fit(p, y, z, sector_row, o, sector, o["trk_nhits"], o["trk_first_hit"], o["trk_hits"], m["succ"], m["pred"],
+                  precision)
+    return dict(trk_sector=sector, row_first=rf, row_last=rl, **m, **f)
+
+
 def propagate(p, par5, cov15, dx, precision="f64"):
     """R12 primitive: returns (ok, par5', cov15', F[5,5])."""
     rt, sfx = _real(precision)
