@@ -403,6 +403,23 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     binding.profile_enable(False)
     fp32_peak = binding.fp32_peak(dev)
 
+    # ---- after the hot path (not part of `value`): tpc_merge_tracks (R26) on the tracks of the last step ----------
+    merge = None
+    if int(ev.params.n_sectors) > 1:
+        trk.merge_enqueue()
+        torch.cuda.synchronize()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        for _ in range(3):
+            trk.merge_enqueue()
+        m1.record()
+        torch.cuda.synchronize()
+        ng = trk._merge["out"]["n_global"].cpu().numpy()
+        merge = {"ms": m0.elapsed_time(m1) / 3, "global_tracks": int(ng[0]), "links": int(ng[1]),
+                 "what": "tpc_merge_tracks: sector-local tracks linked across sector edges / the central electrode / long "
+                         "holes, merged hit lists refitted (DESIGN.md R26); not included in `value`"}
+        binding.profile_collect(reset=True)
+
     # ---- end to end through the host-buffer entry points -----------------------------------------
     # Two Time Frames in flight (two Tracker contexts, own workspace / staging / pinned outputs, one stream each):
     # the H2D copy of one TF overlaps the tracking of the previous one and the D2H of the one before -- the
@@ -484,7 +501,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "tracklets_followed_down": int(res["counters"][binding.CNT_FOLLOWED_DOWN]), "clusters_assigned": n_hits,
            "follower_work": work,
            "clocks": clocks, "gpu_launches": launches, "kernels": kern,
-           "kernels_ms_sum": round(sum(v["ms_per_step"] for v in kern.values()), 3), "roofline": roofline}
+           "kernels_ms_sum": round(sum(v["ms_per_step"] for v in kern.values()), 3), "roofline": roofline,
+           "after_hot_path": {"merge": merge}}
     if not args.no_e2e:
         out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
                       "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3,

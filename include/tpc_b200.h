@@ -266,6 +266,64 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
                    void* workspace, size_t ws_bytes, const tpc_result_t* dev, const tpc_result_t* host,
                    void* stream);
 
+/* ---- merging of the sector-local tracks ("full tracking in the TPC", l.60;
+ * DESIGN.md R26) ------------------------------------------------------------------------------------------------
+ * tpc_find_tracks leaves a particle that crosses a 20-degree sector edge, the central electrode or a hole longer than
+ * max_gap as several tracks.  tpc_merge_tracks links them and refits the merged hit lists:
+ *   B can follow A iff B's sector is A's, an azimuthal neighbour on the same side or the mirror sector across the
+ *   electrode; 1 <= first row of B - last row of A <= max_rows; |z_B - z_A| <= dz_max between the two ends
+ *   (|z_B + z_A| across the electrode: the sides measure z_true -+ v_d t); and chi2 < chi2_cut, chi2 = d^T S^-1 d over
+ *   (y, z, sinphi, tanlambda, q/pT) between A's state -- transported by R12 to its outermost hit, rotated into B's
+ *   frame, transported to B's innermost hit -- and B's state, S the sum of the two covariances.  Across the electrode
+ *   z is left out (free time offset) and |z_A' + z_B| <= ce_tol + 2 |tanlambda_B| dx / cosphi_B is required instead.
+ *   Links are the reciprocal arg-mins (ties: lowest trk_seed); global tracks are the chains of links.
+ * Inputs: `dev` = the outputs of tpc_find_tracks + tpc_fit_tracks (cluster_track, trk_hits, counters of the struct are
+ * not read; counters is passed separately), find_workspace = the workspace of that tpc_find_tracks call (its cached
+ * hit records are read).  merge_workspace: tpc_merge_workspace_bytes(params, max_tracks) bytes, 256-byte aligned.
+ * Outputs (device, caller-owned, `out`):
+ *   trk_succ, trk_pred [max_tracks] : linked successor / predecessor of a track, -1 = none
+ *   trk_succ_chi2 [max_tracks]      : chi2 of the best candidate successor (before reciprocity), -1 = none
+ *   trk_global [max_tracks]         : global track of a sector-local track
+ *   n_global [2]                    : global tracks M; links
+ *   g_head, g_nseg, g_nhits [max_tracks] : first (innermost) piece, pieces and hits of global track g < M, in
+ *                                     ascending order of g_head
+ *   gpar [5][max_tracks], gcov [15][max_tracks], gxref, gzref, gchi2, gndf [max_tracks] : refit of the merged hit
+ *                                     list at its innermost hit, in the head piece's frame (R22's passes; at a change
+ *                                     of piece the state is rotated into the new frame, at a change of side zRef is
+ *                                     re-based on the first hit of the new side and ndf loses 1); a chain of one piece
+ *                                     keeps its tpc_fit_tracks result; chi2 = ndf = -1 if a transport ran into max_sinphi
+ * K = counters[TPC_CNT_TRACKS] is read on the device.  Enqueue only.  TPC_EINVAL for missing buffers or parameters
+ * out of range (chi2_cut, dz_max > 0, ce_tol >= 0, 1 <= max_rows <= 151), TPC_ENOMEM_WS for a short workspace. */
+typedef struct {
+  float chi2_cut;    /* 50  */
+  float dz_max;      /* 64 cm */
+  float ce_tol;      /* 1 cm */
+  int32_t max_rows;  /* 12 */
+} tpc_merge_params_t;
+
+typedef struct {
+  int32_t* trk_succ;
+  int32_t* trk_pred;
+  float* trk_succ_chi2;
+  int32_t* trk_global;
+  int32_t* n_global;
+  int32_t* g_head;
+  int32_t* g_nseg;
+  int32_t* g_nhits;
+  float* gpar;
+  float* gcov;
+  float* gxref;
+  float* gzref;
+  float* gchi2;
+  int32_t* gndf;
+} tpc_merged_t;
+
+int tpc_merge_workspace_bytes(const tpc_params_t* params_host, int64_t max_tracks, size_t* bytes_host);
+int tpc_merge_tracks(const tpc_params_t* params_host, const tpc_merge_params_t* merge_host, int64_t n_clusters,
+                     int64_t max_tracklets, const void* find_workspace, size_t find_ws_bytes,
+                     const int32_t* counters, int64_t max_tracks, const tpc_result_t* dev, void* merge_workspace,
+                     size_t merge_ws_bytes, const tpc_merged_t* out, void* stream);
+
 /* ---- measurement support (bench.py `roofline`, `gpu_launches`) --------------------------------
  * The library counts every kernel it launches, per kernel id, and can bracket each launch with a
  * cudaEvent pair recorded on the launching stream.  Host-side state, one driving thread per GPU

@@ -28,7 +28,8 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED, ST_BAD_ROW = 1, 2, 4, 8
 #: every symbol include/tpc_b200.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
-           "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
+           "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_merge_workspace_bytes",
+           "tpc_merge_tracks", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -50,6 +51,19 @@ class tpc_result_t(C.Structure):
 
 
 RESULT_FIELDS = tuple(f[0] for f in tpc_result_t._fields_)
+
+
+class tpc_merge_params_t(C.Structure):
+    _fields_ = [("chi2_cut", C.c_float), ("dz_max", C.c_float), ("ce_tol", C.c_float), ("max_rows", C.c_int32)]
+
+
+class tpc_merged_t(C.Structure):
+    """Mirror of tpc_merged_t: device outputs of tpc_merge_tracks (R26)."""
+    _fields_ = [(nm, C.c_void_p) for nm in ("trk_succ", "trk_pred", "trk_succ_chi2", "trk_global", "n_global", "g_head", "g_nseg",
+                                            "g_nhits", "gpar", "gcov", "gxref", "gzref", "gchi2", "gndf")]
+
+
+MERGE_DEFAULTS = dict(chi2_cut=50.0, dz_max=64.0, ce_tol=1.0, max_rows=12)
 
 
 class TpcError(RuntimeError):
@@ -291,6 +305,50 @@ class Tracker:
         found, n = (int(v) for v in nc.cpu().numpy())
         return dict(n_found=found, coll_time=ct[:n].cpu().numpy(), coll_ntracks=cn[:n].cpu().numpy(), coll_bin=cb[:n].cpu().numpy(),
                     trk_collision=tc[:k].cpu().numpy(), t0=tt["t0"][:k].cpu().numpy(), dca=tt["dca"][:k].cpu().numpy())
+
+    def merge_alloc(self):
+        """Workspace and device outputs of tpc_merge_tracks (allocated once per Tracker)."""
+        if getattr(self, "_merge", None) is not None:
+            return self._merge
+        t = self.torch
+        K, dev = self.max_tracks, self.device
+        wsb = C.c_size_t(0)
+        _check(self.lib.tpc_merge_workspace_bytes(C.byref(self.P), C.c_int64(K), C.byref(wsb)), "tpc_merge_workspace_bytes")
+        i32, f32 = t.int32, t.float32
+        o = dict(trk_succ=t.empty(K, dtype=i32, device=dev), trk_pred=t.empty(K, dtype=i32, device=dev),
+                 trk_succ_chi2=t.empty(K, dtype=f32, device=dev), trk_global=t.empty(K, dtype=i32, device=dev),
+                 n_global=t.zeros(2, dtype=i32, device=dev), g_head=t.empty(K, dtype=i32, device=dev),
+                 g_nseg=t.empty(K, dtype=i32, device=dev), g_nhits=t.empty(K, dtype=i32, device=dev),
+                 gpar=t.empty((5, K), dtype=f32, device=dev), gcov=t.empty((15, K), dtype=f32, device=dev),
+                 gxref=t.empty(K, dtype=f32, device=dev), gzref=t.empty(K, dtype=f32, device=dev),
+                 gchi2=t.empty(K, dtype=f32, device=dev), gndf=t.empty(K, dtype=i32, device=dev))
+        self._merge = dict(ws=t.empty(int(wsb.value), dtype=t.uint8, device=dev), ws_bytes=int(wsb.value), out=o,
+                           out_c=tpc_merged_t(*[C.c_void_p(o[nm].data_ptr()) for nm, _ in tpc_merged_t._fields_]),
+                           dev_c=tpc_result_t(*[C.c_void_p(getattr(self, nm).data_ptr()) for nm in RESULT_FIELDS]))
+        return self._merge
+
+    def merge_enqueue(self, **mp):
+        """tpc_merge_tracks (R26) on the last find + fit; asynchronous."""
+        m = self.merge_alloc()
+        d = dict(MERGE_DEFAULTS, **mp)
+        M = tpc_merge_params_t(float(d["chi2_cut"]), float(d["dz_max"]), float(d["ce_tol"]), int(d["max_rows"]))
+        _check(self.lib.tpc_merge_tracks(C.byref(self.P), C.byref(M), C.c_int64(self.n), C.c_int64(self.max_tracklets),
+                                         _dp(self.workspace), C.c_size_t(self.ws_bytes), _dp(self.counters),
+                                         C.c_int64(self.max_tracks), C.byref(m["dev_c"]), _dp(m["ws"]), C.c_size_t(m["ws_bytes"]),
+                                         C.byref(m["out_c"]), _stream()), "tpc_merge_tracks")
+
+    def merge_tracks(self, **mp):
+        """merge_enqueue + numpy results (links, global tracks, merged fits); synchronises."""
+        self.merge_enqueue(**mp)
+        o = self._merge["out"]
+        k = int(self.counters[CNT_TRACKS].item())
+        m, links = (int(v) for v in o["n_global"].cpu().numpy())
+        per_trk = ("trk_succ", "trk_pred", "trk_succ_chi2", "trk_global")
+        res = {nm: o[nm][:k].cpu().numpy() for nm in per_trk}
+        res.update({nm: (o[nm][:, :m] if o[nm].dim() == 2 else o[nm][:m]).cpu().numpy()
+                    for nm in o if nm not in per_trk and nm != "n_global"})
+        res.update(n_global=m, n_links=links)
+        return res
 
     def step(self, y, z, sector_row):
         """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""

@@ -25,7 +25,7 @@ Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_survivor_*", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
-                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_export_*"};
+                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -302,6 +302,41 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
     return TPC_EINVAL;
   const cudaError_t e = tpc::launch_track_time(G, (double)v_drift, counters, max_tracks, trk_sector, par, xref, zref, phi0, z0,
                                                dca, t0, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_merge_workspace_bytes(const tpc_params_t* params_host, int64_t max_tracks, size_t* bytes_host) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!bytes_host || max_tracks < 1 || max_tracks > 2147483000ll || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  *bytes_host = tpc::merge_ws_bytes(G, max_tracks);
+  return TPC_OK;
+}
+
+int tpc_merge_tracks(const tpc_params_t* params_host, const tpc_merge_params_t* merge_host, int64_t n_clusters,
+                     int64_t max_tracklets, const void* find_workspace, size_t find_ws_bytes, const int32_t* counters,
+                     int64_t max_tracks, const tpc_result_t* dev, void* merge_workspace, size_t merge_ws_bytes,
+                     const tpc_merged_t* out, void* stream) {
+  Prep pr;
+  const int rc = prepare(params_host, n_clusters, max_tracklets, find_workspace, find_ws_bytes, &pr);
+  if (rc != TPC_OK) return rc;
+  if (!merge_host || !(merge_host->chi2_cut > 0.0f) || !(merge_host->dz_max > 0.0f) || !(merge_host->ce_tol >= 0.0f) ||
+      merge_host->max_rows < 1 || merge_host->max_rows > 151)
+    return TPC_EINVAL;
+  if (max_tracks < 1 || max_tracks > 2147483000ll || !counters || !dev || !dev->trk_seed || !dev->trk_sector || !dev->trk_nhits ||
+      !dev->trk_first_hit || !dev->par || !dev->cov || !dev->xref || !dev->zref || !dev->chi2 || !dev->ndf)
+    return TPC_EINVAL;
+  if (!out || !out->trk_succ || !out->trk_pred || !out->trk_succ_chi2 || !out->trk_global || !out->n_global || !out->g_head ||
+      !out->g_nseg || !out->g_nhits || !out->gpar || !out->gcov || !out->gxref || !out->gzref || !out->gchi2 || !out->gndf)
+    return TPC_EINVAL;
+  if (!merge_workspace || ((uintptr_t)merge_workspace & 255) != 0) return TPC_EINVAL;
+  if (merge_ws_bytes < tpc::merge_ws_bytes(pr.G, max_tracks)) return TPC_ENOMEM_WS;
+  const cudaError_t e = tpc::launch_merge(pr.G, pr.W, merge_host->chi2_cut, merge_host->dz_max, merge_host->ce_tol,
+                                          merge_host->max_rows, counters, max_tracks, dev->trk_seed, dev->trk_sector,
+                                          dev->trk_nhits, dev->trk_first_hit, dev->par, dev->cov, dev->xref, dev->zref, dev->chi2,
+                                          dev->ndf, merge_workspace, out->trk_succ, out->trk_pred, out->trk_succ_chi2,
+                                          out->trk_global, out->n_global, out->g_head, out->g_nseg, out->g_nhits, out->gpar,
+                                          out->gcov, out->gxref, out->gzref, out->gchi2, out->gndf, (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

@@ -235,6 +235,16 @@ cudaError_t launch_track_time(const Geo& g, double v_drift, const int32_t* count
                               const int32_t* trk_sector, const float* par, const float* xref, const float* zref, float* phi0,
                               float* z0, float* dca, float* t0, cudaStream_t st);
 
+// tpc_merge.cu (R26)
+size_t merge_ws_bytes(const Geo& g, int64_t max_tracks);
+cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_max, float ce_tol, int max_rows,
+                         const int32_t* counters, int64_t max_tracks, const int32_t* trk_seed, const int32_t* trk_sector,
+                         const int32_t* trk_nhits, const int64_t* trk_first_hit, const float* par, const float* cov,
+                         const float* xref, const float* zref, const float* chi2, const int32_t* ndf, void* merge_ws,
+                         int32_t* trk_succ, int32_t* trk_pred, float* trk_succ_chi2, int32_t* trk_global, int32_t* n_global,
+                         int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
+                         float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st);
+
 size_t collisions_ws_bytes(int64_t nb, int64_t max_tracks);
 cudaError_t launch_collisions(const int32_t* counters, int64_t max_tracks, const float* t0, const float* dca,
                               const int32_t* trk_sector, int side_sel, double t_lo,

@@ -1,0 +1,528 @@
+// =============================================================================================
+// tpc_merge.cu -- the step right after the hot path ("full tracking in
+// the TPC", l.60; R26): merging of the sector-local tracks across the 20-degree sector edges,
+// across the central electrode and across holes longer than max_gap, and the refit of the merged hit lists.
+//
+//   k_merge_ends     per track: rows of its first / last hit (from the hit records tpc_find_tracks cached), z of
+//                    its inner end, bucket (sector, z slab) of that end; bucket histogram
+//   k_merge_scatter  end records into bucket order (the order inside a bucket is irrelevant: every arg-min below
+//                    breaks ties by seed)
+//   k_merge_match    one thread per track A: outer state by R12, then every track B whose inner end lies in the
+//                    buckets the R26 windows can reach: row window, z window, rotation into B's frame, transport to
+//                    B's first hit, Cholesky chi2.  A keeps its best successor; every passing pair offers
+//                    (chi2, seed of A) to B by a 64-bit atomicMin -- B's best predecessor
+//   k_merge_link     A -> B is a link iff B's best predecessor is A (reciprocal arg-mins)
+//   k_merge_chains   heads (no predecessor) are numbered by a scan; each walks its chain: trk_global, pieces, hits;
+//                    a track without links keeps its sector-local fit
+//   k_merge_refit    one thread per merged chain: R22's two passes over the concatenated hit records, with the
+//                    frame rotation at a change of sector and the zRef re-basing at a change of side
+//
+// The arithmetic restates R26 operator by operator in fp32 (the library is compiled with -fmad=false; R26 has no
+// mad), so the integer decisions (links) and the merged parameters equal the CPU oracle's bit for bit.
+// =============================================================================================
+#include "tpc_common.cuh"
+#include "tpc_kalman.cuh"
+#include "tpc_prof.cuh"
+#include "tpc_scan.cuh"
+
+namespace tpc {
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr float kSlabCm = 128.0f;  // z slab of the end buckets (>= dz_max is not required: the lookup covers a range)
+constexpr float kCos20 = 0.93969262078590838405f, kSin20 = 0.34202014332566873304f;
+enum { REL_NONE = 0, REL_SAME = 1, REL_NEXT = 2, REL_PREV = 3, REL_CE = 4 };
+
+struct MergeP {
+  float chi2_cut, dz_max, ce_tol;
+  int max_rows;
+  int nslab;  // z slabs per sector
+};
+
+// inner end of a track, in bucket order: all the R26 windows need before the states are touched
+struct EndRec {
+  float z_in;   // zRef + dz at the innermost hit
+  int rows;     // first row | last row << 8 | sector << 16
+  int seed;     // original index of the start hit: tie-break
+  int track;    // index of the track
+};
+
+struct MergeWs {
+  EndRec* ends;       // [K] bucket order
+  int32_t* bucket;    // [K] bucket of track k
+  int32_t* bfirst;    // [nbuckets + 2]
+  int32_t* bcursor;   // [nbuckets + 2]
+  int32_t* rows;      // [K] first | last << 8 | sector << 16, track order
+  float* z_in;        // [K]
+  int32_t* cand;      // [K] best candidate successor (before reciprocity)
+  unsigned long long* pred_key;  // [K] (chi2 bits << 32 | seed of the best predecessor)
+  int32_t* flag;      // [K + 1] head flags and their scan
+  int32_t* scan_tmp;
+};
+
+__device__ __forceinline__ int sector_relation(int sa, int sb) {
+  if (sa == sb) return REL_SAME;
+  const int aa = sa % 18, ab = sb % 18;
+  if ((sa < 18) != (sb < 18)) return aa == ab ? REL_CE : REL_NONE;
+  if (ab == (aa + 1) % 18) return REL_NEXT;
+  if (aa == (ab + 1) % 18) return REL_PREV;
+  return REL_NONE;
+}
+
+__device__ __forceinline__ int slab_of(float zeta, float z_lo, int nslab) {
+  const float v = (zeta - z_lo) * (1.0f / kSlabCm);
+  if (!(v > 0.0f)) return 0;
+  if (v >= (float)nslab) return nslab - 1;
+  return (int)v;
+}
+
+__device__ __forceinline__ void load_state(KState& st, const float* __restrict__ par, const float* __restrict__ cov, int64_t ld,
+                                           int64_t k) {
+#pragma unroll
+  for (int i = 0; i < 5; i++) st.p[i] = __ldg(par + i * ld + k);
+#pragma unroll
+  for (int i = 0; i < 15; i++) st.C[i] = __ldg(cov + i * ld + k);
+}
+
+// R26 rotation of a state at x into the frame turned by D (cd = cos D, sd = sin D)
+__device__ __forceinline__ bool rotate_state(KState& st, float& x, float cd, float sd, float max_sinphi) {
+  const float y = st.p[0], s = st.p[2];
+  const float c = sqrtf(1.0f - s * s);
+  const float xn = x * cd + y * sd;
+  const float yn = y * cd - x * sd;
+  const float sn = s * cd - c * sd;
+  const float cn = c * cd + s * sd;
+  if (!(cn > 0.0f) || !(fabsf(sn) <= max_sinphi)) return false;
+  const float j0 = c / cn, j2 = cn / c;
+  // C'_ij = (J_i C_ij) J_j with J = (j0, 1, j2, 1, 1); a factor 1 changes nothing
+  st.C[TPC_CI(0, 0)] = (j0 * st.C[TPC_CI(0, 0)]) * j0;
+  st.C[TPC_CI(1, 0)] = st.C[TPC_CI(1, 0)] * j0;
+  st.C[TPC_CI(2, 0)] = (j2 * st.C[TPC_CI(2, 0)]) * j0;
+  st.C[TPC_CI(2, 1)] = j2 * st.C[TPC_CI(2, 1)];
+  st.C[TPC_CI(2, 2)] = (j2 * st.C[TPC_CI(2, 2)]) * j2;
+  st.C[TPC_CI(3, 0)] = st.C[TPC_CI(3, 0)] * j0;
+  st.C[TPC_CI(3, 2)] = st.C[TPC_CI(3, 2)] * j2;
+  st.C[TPC_CI(4, 0)] = st.C[TPC_CI(4, 0)] * j0;
+  st.C[TPC_CI(4, 2)] = st.C[TPC_CI(4, 2)] * j2;
+  st.p[0] = yn;
+  st.p[2] = sn;
+  x = xn;
+  return true;
+}
+
+// chi2 = d^T S^-1 d over N of the 5 parameters (index map idx), S = lower triangle of a + lower triangle of b
+template <int N>
+__device__ __forceinline__ float chi2_cholesky(const float (&Sa)[15], const float (&Sb)[15], const float (&d)[5], const int (&idx)[N]) {
+  float L[N][N], yv[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+#pragma unroll
+    for (int j = 0; j <= i; j++) {
+      float sum = Sa[TPC_CI(idx[i], idx[j])] + Sb[TPC_CI(idx[i], idx[j])];
+#pragma unroll
+      for (int k = 0; k < j; k++) sum = sum - L[i][k] * L[j][k];
+      if (i == j) {
+        if (!(sum > 0.0f)) return -1.0f;
+        L[i][i] = sqrtf(sum);
+      } else {
+        L[i][j] = sum / L[j][j];
+      }
+    }
+  }
+  float chi2 = 0.0f;
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    float sum = d[idx[i]];
+#pragma unroll
+    for (int k = 0; k < i; k++) sum = sum - L[i][k] * yv[k];
+    yv[i] = sum / L[i][i];
+    chi2 = chi2 + yv[i] * yv[i];
+  }
+  return chi2;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_ends(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict__ counters, int64_t max_tracks,
+             const int32_t* __restrict__ trk_seed, const int32_t* __restrict__ trk_sector, const int32_t* __restrict__ trk_nhits,
+             const int64_t* __restrict__ trk_first_hit, const float4* __restrict__ hit_rec, const float* __restrict__ par,
+             const float* __restrict__ zref, MergeWs w) {
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kThreads) {
+    const int64_t f = trk_first_hit[k];
+    const int n = trk_nhits[k], s = trk_sector[k];
+    const int rf = __float_as_int(__ldg(hit_rec + f).z), rl = __float_as_int(__ldg(hit_rec + f + n - 1).z);
+    const float z = zref[k] + par[1 * max_tracks + k];
+    const float zeta = s < 18 ? z : -z;
+    const int b = s * mp.nslab + slab_of(zeta, g.s.z_lo, mp.nslab);
+    w.rows[k] = rf | (rl << 8) | (s << 16);
+    w.z_in[k] = z;
+    w.bucket[k] = b;
+    w.cand[k] = -1;
+    w.pred_key[k] = ~0ull;
+    atomicAdd(w.bfirst + b, 1);
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_scatter(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_seed, MergeWs w) {
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kThreads) {
+    const int slot = atomicAdd(w.bcursor + w.bucket[k], 1);
+    EndRec e;
+    e.z_in = w.z_in[k];
+    e.rows = w.rows[k];
+    e.seed = trk_seed[k];
+    e.track = (int)k;
+    reinterpret_cast<float4*>(w.ends)[slot] = make_float4(e.z_in, __int_as_float(e.rows), __int_as_float(e.seed), __int_as_float(e.track));
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict__ counters, int64_t max_tracks,
+              const int32_t* __restrict__ trk_seed, const float* __restrict__ par, const float* __restrict__ cov,
+              const float* __restrict__ zref, MergeWs w, float* __restrict__ succ_chi2) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  const float kB = sc.kB, ms = sc.max_sinphi;
+  for (int64_t a = (int64_t)blockIdx.x * kThreads + threadIdx.x; a < K; a += (int64_t)gridDim.x * kThreads) {
+    const int rows_a = w.rows[a];
+    const int rf_a = rows_a & 0xff, rl_a = (rows_a >> 8) & 0xff, s_a = rows_a >> 16;
+    const int seed_a = trk_seed[a];
+    const float zref_a = zref[a];
+    KState out;
+    load_state(out, par, cov, max_tracks, a);
+    int best_b = -1, best_seed = 0;
+    float best = 0.0f;
+    bool have_out = true;
+    if (rl_a != rf_a) have_out = propagate(out, sX[rl_a] - sX[rf_a], kB, ms);
+    if (have_out) {
+      const float zA = zref_a + out.p[1];
+      const float x_a = sX[rl_a];
+      for (int sb = 0; sb < sc.nsec; sb++) {
+        const int rel = sector_relation(s_a, sb);
+        if (rel == REL_NONE) continue;
+        // z of B's inner end: within dz_max of zA (same side) or of -zA (across the electrode); as zeta of B's side
+        const float zc = rel == REL_CE ? -zA : zA;
+        const float side_b = sb < 18 ? 1.0f : -1.0f;
+        const float za = (zc - mp.dz_max) * side_b, zb = (zc + mp.dz_max) * side_b;
+        int s0 = slab_of(fminf(za, zb), sc.z_lo, mp.nslab) - 1, s1 = slab_of(fmaxf(za, zb), sc.z_lo, mp.nslab) + 1;
+        if (s0 < 0) s0 = 0;
+        if (s1 > mp.nslab - 1) s1 = mp.nslab - 1;
+        const int e0 = w.bfirst[sb * mp.nslab + s0], e1 = w.bfirst[sb * mp.nslab + s1 + 1];
+        for (int e = e0; e < e1; e++) {
+          const float4 er = __ldg(reinterpret_cast<const float4*>(w.ends) + e);
+          const int rows_b = __float_as_int(er.y), b = __float_as_int(er.w);
+          const int rf_b = rows_b & 0xff;
+          const int dr = rf_b - rl_a;
+          if (dr < 1 || dr > mp.max_rows || b == (int)a) continue;
+          const float zB = er.x;
+          if (rel == REL_CE ? !(fabsf(zB + zA) <= mp.dz_max) : !(fabsf(zB - zA) <= mp.dz_max)) continue;
+          KState r = out;
+          float x = x_a;
+          if (rel == REL_NEXT || rel == REL_PREV) {
+            const float sd = rel == REL_NEXT ? kSin20 : -kSin20;
+            if (!rotate_state(r, x, kCos20, sd, ms)) continue;
+          }
+          const float xb = sX[rf_b];
+          if (!propagate(r, xb - x, kB, ms)) continue;
+          KState sbst;
+          load_state(sbst, par, cov, max_tracks, b);
+          const float zref_b = zref[b];
+          float d[5];
+          d[0] = r.p[0] - sbst.p[0];
+          d[1] = (zref_a - zref_b) + (r.p[1] - sbst.p[1]);
+          d[2] = r.p[2] - sbst.p[2];
+          d[3] = r.p[3] - sbst.p[3];
+          d[4] = r.p[4] - sbst.p[4];
+          float chi2;
+          if (rel == REL_CE) {
+            const float zsum = (zref_a + r.p[1]) + (zref_b + sbst.p[1]);
+            const float cb = sqrtf(1.0f - sbst.p[2] * sbst.p[2]);
+            const float lim = mp.ce_tol + ((2.0f * fabsf(sbst.p[3])) * (xb - x_a)) / cb;
+            if (!(fabsf(zsum) <= lim)) continue;
+            const int idx[4] = {0, 2, 3, 4};
+            chi2 = chi2_cholesky<4>(r.C, sbst.C, d, idx);
+          } else {
+            const int idx[5] = {0, 1, 2, 3, 4};
+            chi2 = chi2_cholesky<5>(r.C, sbst.C, d, idx);
+          }
+          if (!(chi2 >= 0.0f) || !(chi2 < mp.chi2_cut)) continue;
+          const int seed_b = __float_as_int(er.z);
+          if (best_b < 0 || chi2 < best || (chi2 == best && seed_b < best_seed)) {
+            best_b = b;
+            best = chi2;
+            best_seed = seed_b;
+          }
+          atomicMin(w.pred_key + b, ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned long long)(unsigned)seed_a);
+        }
+      }
+    }
+    w.cand[a] = best_b;
+    succ_chi2[a] = best_b >= 0 ? best : -1.0f;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_link(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_seed, MergeWs w,
+             const float* __restrict__ succ_chi2, int32_t* __restrict__ succ, int32_t* __restrict__ pred) {
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  for (int64_t a = (int64_t)blockIdx.x * kThreads + threadIdx.x; a < K; a += (int64_t)gridDim.x * kThreads) {
+    const int b = w.cand[a];
+    int s = -1;
+    if (b >= 0) {
+      const unsigned long long key = ((unsigned long long)__float_as_uint(succ_chi2[a]) << 32) | (unsigned long long)(unsigned)trk_seed[a];
+      if (w.pred_key[b] == key) {
+        s = b;
+        pred[b] = (int)a;  // at most one track passes this test for b
+      }
+    }
+    succ[a] = s;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_heads(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ pred, int32_t* __restrict__ flag) {
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k <= max_tracks; k += (int64_t)gridDim.x * kThreads)
+    flag[k] = (k < K && pred[k] < 0) ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_chains(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_nhits,
+               const float* __restrict__ par, const float* __restrict__ cov, const float* __restrict__ xref,
+               const float* __restrict__ zref, const float* __restrict__ chi2, const int32_t* __restrict__ ndf,
+               const int32_t* __restrict__ succ, const int32_t* __restrict__ pred, const int32_t* __restrict__ scan,
+               int32_t* __restrict__ trk_global, int32_t* __restrict__ n_global, int32_t* __restrict__ g_head,
+               int32_t* __restrict__ g_nseg, int32_t* __restrict__ g_nhits, float* __restrict__ gpar, float* __restrict__ gcov,
+               float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2, int32_t* __restrict__ gndf) {
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    n_global[0] = scan[max_tracks];
+    n_global[1] = (int)K - scan[max_tracks];  // links
+  }
+  for (int64_t h = (int64_t)blockIdx.x * kThreads + threadIdx.x; h < K; h += (int64_t)gridDim.x * kThreads) {
+    if (pred[h] >= 0) continue;
+    const int gi = scan[h];
+    int nseg = 0, nh = 0;
+    for (int k = (int)h; k >= 0; k = succ[k]) {
+      trk_global[k] = gi;
+      nseg++;
+      nh += trk_nhits[k];
+    }
+    g_head[gi] = (int)h;
+    g_nseg[gi] = nseg;
+    g_nhits[gi] = nh;
+    if (nseg == 1) {  // no links: the sector-local fit stands
+#pragma unroll
+      for (int i = 0; i < 5; i++) gpar[i * max_tracks + gi] = par[i * max_tracks + h];
+#pragma unroll
+      for (int i = 0; i < 15; i++) gcov[i * max_tracks + gi] = cov[i * max_tracks + h];
+      gxref[gi] = xref[h];
+      gzref[gi] = zref[h];
+      gchi2[gi] = chi2[h];
+      gndf[gi] = ndf[h];
+    }
+  }
+}
+
+// R26 refit of one chain per thread.  The hits of a chain are walked piece by piece in the direction of the pass;
+// `piece` / `i` address the current hit, prev[] is rebuilt from succ[] on the way out (chains are a few pieces long).
+constexpr int kMaxPieces = 16;
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_global, int64_t max_tracks,
+              const int32_t* __restrict__ trk_sector, const int32_t* __restrict__ trk_nhits,
+              const int64_t* __restrict__ trk_first_hit, const float4* __restrict__ hit_rec, const float* __restrict__ par,
+              const float* __restrict__ zref, const int32_t* __restrict__ succ, const int32_t* __restrict__ g_head,
+              const int32_t* __restrict__ g_nseg, const int32_t* __restrict__ g_nhits, float* __restrict__ gpar,
+              float* __restrict__ gcov, float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2,
+              int32_t* __restrict__ gndf) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  const int M = n_global[0];
+  const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
+  for (int64_t gi = (int64_t)blockIdx.x * kThreads + threadIdx.x; gi < M; gi += (int64_t)gridDim.x * kThreads) {
+    const int nseg = g_nseg[gi];
+    if (nseg < 2) continue;
+    const int h = g_head[gi];
+    int seg[kMaxPieces];
+    int np = 0;
+    for (int k = h; k >= 0 && np < kMaxPieces; k = succ[k]) seg[np++] = k;
+    bool ok = nseg <= kMaxPieces;  // longer chains do not occur (a chain crosses a sector edge per piece); flagged if they do
+    KState st;
+#pragma unroll
+    for (int i = 0; i < 5; i++) st.p[i] = par[i * max_tracks + h];
+#pragma unroll
+    for (int i = 0; i < 15; i++) st.C[i] = 0.0f;
+    float zr = zref[h];
+    int cur_sec = trk_sector[h];
+    float x_at = sX[__float_as_int(__ldg(hit_rec + trk_first_hit[h]).z)];
+    float c2 = 0.0f;
+    int lost = 0;
+    const int N = g_nhits[gi];
+    for (int pass = 0; pass < sc.n_fit_passes && ok; pass++) {
+      reset_cov(st, sc.cov0);
+      c2 = 0.0f;
+      lost = 0;
+      const int dir = (pass & 1) ? -1 : 1;
+      int piece = dir > 0 ? 0 : np - 1;
+      int i = dir > 0 ? 0 : trk_nhits[seg[piece]] - 1;
+      for (int cnt = 0; cnt < N && ok; cnt++) {
+        const int k = seg[piece];
+        const float4 hit = __ldg(hit_rec + trk_first_hit[k] + i);
+        const int hs = trk_sector[k];
+        const float xh = sX[__float_as_int(hit.z)];
+        bool rebase = false;
+        if (hs != cur_sec) {
+          const int rel = sector_relation(cur_sec, hs);
+          if (rel == REL_NEXT || rel == REL_PREV) {
+            const float cd = kCos20, sd = rel == REL_NEXT ? kSin20 : -kSin20;
+            if (dir < 0) {  // inward: stay in the old frame up to the plane of the next hit (R26)
+              const float xc = xh * cd - hit.x * sd;
+              if (!propagate(st, xc - x_at, kB, ms)) { ok = false; break; }
+              x_at = xc;
+            }
+            if (!rotate_state(st, x_at, cd, sd, ms)) { ok = false; break; }
+          } else if (rel == REL_CE) {
+            rebase = true;
+          }
+          cur_sec = hs;
+        }
+        if (cnt > 0) {
+          if (!propagate(st, xh - x_at, kB, ms)) { ok = false; break; }
+          x_at = xh;
+        }
+        if (rebase) {
+          zr = hit.y - st.p[1];
+          lost++;
+        }
+        const Innov I = innovation(st, sy2, sz2);
+        c2 = c2 + update(st, I, hit.x, hit.y - zr);
+        // next hit in the direction of the pass
+        i += dir;
+        if (i < 0 || i >= trk_nhits[k]) {
+          piece += dir;
+          if (piece >= 0 && piece < np) i = dir > 0 ? 0 : trk_nhits[seg[piece]] - 1;
+        }
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 5; i++) gpar[i * max_tracks + gi] = st.p[i];
+#pragma unroll
+    for (int i = 0; i < 15; i++) gcov[i * max_tracks + gi] = st.C[i];
+    gxref[gi] = x_at;
+    gzref[gi] = zr;
+    gchi2[gi] = ok ? c2 : -1.0f;
+    gndf[gi] = ok ? 2 * N - 5 - lost : -1;
+  }
+}
+
+inline int merge_nslab(const Geo& g) {
+  int n = (int)ceilf((g.s.z_hi - g.s.z_lo) / kSlabCm) + 1;
+  if (n < 1) n = 1;
+  if (n > 4096) n = 4096;
+  return n;
+}
+
+struct MergeLayout {
+  size_t off_ends, off_bucket, off_bfirst, off_bcursor, off_rows, off_z, off_cand, off_key, off_flag, off_tmp, total;
+  int64_t nbuckets;
+};
+
+inline MergeLayout merge_layout(int nsec, int nslab, int64_t max_tracks) {
+  MergeLayout L{};
+  L.nbuckets = (int64_t)nsec * nslab;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = align256(o + bytes);
+    return at;
+  };
+  const size_t K = (size_t)max_tracks + 1;
+  L.off_ends = take(sizeof(EndRec) * K);
+  L.off_bucket = take(sizeof(int32_t) * K);
+  L.off_bfirst = take(sizeof(int32_t) * (size_t)(L.nbuckets + 2));
+  L.off_bcursor = take(sizeof(int32_t) * (size_t)(L.nbuckets + 2));
+  L.off_rows = take(sizeof(int32_t) * K);
+  L.off_z = take(sizeof(float) * K);
+  L.off_cand = take(sizeof(int32_t) * K);
+  L.off_key = take(sizeof(unsigned long long) * K);
+  L.off_flag = take(sizeof(int32_t) * (K + 1));
+  const int64_t longest = (int64_t)K + 1 > L.nbuckets + 2 ? (int64_t)K + 1 : L.nbuckets + 2;
+  L.off_tmp = take(sizeof(int64_t) * (size_t)((longest + kScanTile - 1) / kScanTile + 2));
+  L.total = o;
+  return L;
+}
+
+}  // namespace
+
+size_t merge_ws_bytes(const Geo& g, int64_t max_tracks) { return merge_layout(g.s.nsec, merge_nslab(g), max_tracks).total; }
+
+cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_max, float ce_tol, int max_rows,
+                         const int32_t* counters, int64_t max_tracks, const int32_t* trk_seed, const int32_t* trk_sector,
+                         const int32_t* trk_nhits, const int64_t* trk_first_hit, const float* par, const float* cov,
+                         const float* xref, const float* zref, const float* chi2, const int32_t* ndf, void* merge_ws,
+                         int32_t* trk_succ, int32_t* trk_pred, float* trk_succ_chi2, int32_t* trk_global, int32_t* n_global,
+                         int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
+                         float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st) {
+  MergeP mp;
+  mp.chi2_cut = chi2_cut;
+  mp.dz_max = dz_max;
+  mp.ce_tol = ce_tol;
+  mp.max_rows = max_rows;
+  mp.nslab = merge_nslab(g);
+  const MergeLayout L = merge_layout(g.s.nsec, mp.nslab, max_tracks);
+  char* b = (char*)merge_ws;
+  MergeWs w;
+  w.ends = (EndRec*)(b + L.off_ends);
+  w.bucket = (int32_t*)(b + L.off_bucket);
+  w.bfirst = (int32_t*)(b + L.off_bfirst);
+  w.bcursor = (int32_t*)(b + L.off_bcursor);
+  w.rows = (int32_t*)(b + L.off_rows);
+  w.z_in = (float*)(b + L.off_z);
+  w.cand = (int32_t*)(b + L.off_cand);
+  w.pred_key = (unsigned long long*)(b + L.off_key);
+  w.flag = (int32_t*)(b + L.off_flag);
+  w.scan_tmp = (int32_t*)(b + L.off_tmp);
+  cudaError_t e;
+  const unsigned blocks = blocks_for(max_tracks, kThreads, 148 * 16);
+  if ((e = cudaMemsetAsync(w.bfirst, 0, sizeof(int32_t) * (size_t)(L.nbuckets + 2), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(trk_pred, 0xFF, sizeof(int32_t) * (size_t)max_tracks, st)) != cudaSuccess) return e;
+  TPC_LAUNCH(KID_MERGE, st,
+             (k_merge_ends<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, trk_sector, trk_nhits, trk_first_hit,
+                                                       fw.hit_rec, par, zref, w)));
+  if ((e = exclusive_scan<int32_t>(w.bfirst, w.bfirst, L.nbuckets + 1, w.scan_tmp, st)) != cudaSuccess) return e;
+  if ((e = cudaMemcpyAsync(w.bcursor, w.bfirst, sizeof(int32_t) * (size_t)(L.nbuckets + 1), cudaMemcpyDeviceToDevice, st)) !=
+      cudaSuccess)
+    return e;
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_scatter<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, w)));
+  TPC_LAUNCH(KID_MERGE, st,
+             (k_merge_match<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, par, cov, zref, w, trk_succ_chi2)));
+  TPC_LAUNCH(KID_MERGE, st,
+             (k_merge_link<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, w, trk_succ_chi2, trk_succ, trk_pred)));
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_heads<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_pred, w.flag)));
+  if ((e = exclusive_scan<int32_t>(w.flag, w.flag, max_tracks + 1, w.scan_tmp, st)) != cudaSuccess) return e;
+  TPC_LAUNCH(KID_MERGE, st,
+             (k_merge_chains<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_nhits, par, cov, xref, zref, chi2, ndf, trk_succ,
+                                                         trk_pred, w.flag, trk_global, n_global, g_head, g_nseg, g_nhits, gpar,
+                                                         gcov, gxref, gzref, gchi2, gndf)));
+  TPC_LAUNCH(KID_MERGE, st,
+             (k_merge_refit<<<blocks, kThreads, 0, st>>>(g, n_global, max_tracks, trk_sector, trk_nhits, trk_first_hit, fw.hit_rec,
+                                                        par, zref, trk_succ, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref,
+                                                        gchi2, gndf)));
+  return cudaGetLastError();
+}
+
+}  // namespace tpc

@@ -33,6 +33,7 @@ enum KernelId {
   KID_FIT,
   KID_TRACK_TIME,
   KID_COLLISIONS,
+  KID_MERGE,
   KID_EXPORT,
   KID_N
 };

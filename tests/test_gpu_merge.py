@@ -1,0 +1,87 @@
+"""R26 on the GPU: tpc_merge_tracks against the CPU oracle on the same events (-m gpu).
+
+The sector-local tracks of the two sides are bit-identical (tests/test_gpu_parity.py), so the links -- integer
+decisions taken from the same fp32 arithmetic -- and the merged fits must be too.  Tracks are matched by seed (the
+order of the track list differs between the two), global tracks by the seed of their head piece."""
+import numpy as np
+import pytest
+
+from paper_2106_03636_b200.synth import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def compare_merge(orc, ev, res, gm):
+    o = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)
+    m = orc.merge(ev.params, ev.y, ev.z, ev.sector_row, o, None, "f32")
+    assert res["trk_seed"].size == o["trk_seed"].size
+    g_of_seed = {int(s): i for i, s in enumerate(res["trk_seed"])}
+    to_g = np.array([g_of_seed[int(s)] for s in o["trk_seed"]])            # oracle track -> cuda track
+
+    def seed_or_none(idx, seeds):
+        return np.where(idx >= 0, seeds[np.maximum(idx, 0)], -1)
+
+    # links, as (seed, seed of successor / predecessor)
+    for key in ("succ", "pred"):
+        a = seed_or_none(m[key], o["trk_seed"])
+        b = seed_or_none(gm["trk_" + key][to_g], res["trk_seed"])
+        assert np.array_equal(a, b), f"{key}: {np.count_nonzero(a != b)} of {a.size} links differ"
+    assert np.array_equal(m["succ_chi2"], gm["trk_succ_chi2"][to_g]), "chi2 of the best successor differs"
+    n_links = int((m["succ"] >= 0).sum())
+    assert gm["n_links"] == n_links and gm["n_global"] == m["g_head"].size == o["trk_seed"].size - n_links
+    # global tracks, matched by the seed of the head
+    og = {int(o["trk_seed"][h]): i for i, h in enumerate(m["g_head"])}
+    order = np.array([og[int(res["trk_seed"][h])] for h in gm["g_head"]])  # cuda global -> oracle global
+    for key in ("g_nseg", "g_nhits", "gndf"):
+        assert np.array_equal(m[key][order], gm[key]), key
+    for key in ("gxref", "gzref", "gchi2"):
+        assert np.array_equal(m[key][order], gm[key]), key
+    assert np.array_equal(m["gpar"][:, order], gm["gpar"]) and np.array_equal(m["gcov"][:, order], gm["gcov"])
+    # trk_global is consistent with the heads
+    assert np.array_equal(order[gm["trk_global"][to_g]], m["trk_global"])
+    return n_links, int((m["g_nseg"] > 1).sum())
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (2, {}), (3, dict(n_coll=2, n_tracks=2500))])
+def test_merge_matches_oracle(torch_cuda, orc, cfg, kw):
+    from paper_2106_03636_b200 import binding
+    ev = make_config(cfg, **kw)
+    t = torch_cuda
+    trk = binding.Tracker(ev.params, ev.n)
+    res = trk.run(t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(ev.sector_row).cuda())
+    gm = trk.merge_tracks()
+    links, merged = compare_merge(orc, ev, res, gm)
+    print(f"\nmerge c{cfg}: {res['trk_seed'].size} sector-local tracks, {links} links, {merged} merged global tracks of "
+          f"{gm['n_global']}")
+    assert links > 50
+
+
+def test_merge_single_sector_has_nothing_to_link_but_gaps(torch_cuda, orc):
+    """configs[0]: one sector -- only same-sector links (holes longer than max_gap) are possible."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(0)
+    t = torch_cuda
+    trk = binding.Tracker(ev.params, ev.n)
+    res = trk.run(t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(ev.sector_row).cuda())
+    gm = trk.merge_tracks()
+    compare_merge(orc, ev, res, gm)
+
+
+def test_merge_argument_errors(torch_cuda):
+    from paper_2106_03636_b200 import binding
+    ev = make_config(0)
+    t = torch_cuda
+    trk = binding.Tracker(ev.params, ev.n)
+    trk.run(t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(ev.sector_row).cuda())
+    with pytest.raises(binding.TpcError):
+        trk.merge_tracks(chi2_cut=0.0)
+    with pytest.raises(binding.TpcError):
+        trk.merge_tracks(max_rows=0)
