@@ -800,7 +800,10 @@ T update_impl(const OrcParams* P, T* p5, T* c15, T ym, T zm) {
 //                             mirror sectors across the central electrode (same azimuth, other side)
 //   B can follow A iff        1 <= first row of B - last row of A <= max_rows, the ends are close in z
 //                             (same side: |z_B - z_A| <= dz_max; across the electrode the two sides measure
-//                             z_true -+ v_d t, so |z_B + z_A| <= dz_max), and chi2 < chi2_cut, where
+//                             z_true -+ v_d t, so |z_B + z_A| <= dz_max), tanlambda and q/pT are not hopelessly
+//                             apart (d_i^2 <= 4 chi2_cut (C_A,ii + C_B,ii), i = tanlambda, q/pT: a gate that only
+//                             removes pairs the chi2 cut would remove, since chi2 >= d_i^2 / S_ii), and
+//                             chi2 < chi2_cut, where
 //   chi2                    : A's outer state rotated into B's frame (x' = x cosD + y sinD, y' = -x sinD + y cosD,
 //                             sinphi' = sinphi cosD - cosphi sinD, cosphi' > 0; covariance C'_ij = J_i C_ij J_j with
 //                             J = (cosphi/cosphi', 1, cosphi'/cosphi, 1, 1)), transported by R12 to the x of B's
@@ -899,6 +902,13 @@ T match_chi2(const OrcParams& P, const OrcMergeParams& M, const Geo<T>& G, const
   if (dr < 1 || dr > M.max_rows) return (T)-1;
   const T zA = tv.zref[a] + out.p[1], zB = tv.zref[b] + tv.par[1 * tv.ld + b];
   if (rel == REL_CE ? !(std::fabs(zB + zA) <= (T)M.dz_max) : !(std::fabs(zB - zA) <= (T)M.dz_max)) return (T)-1;
+  // gate: tanlambda and q/pT are untouched by rotation and transport, and so are their variances; chi2 >= d_i^2 / S_ii
+  // for every single parameter (S positive definite), so a pair four times beyond the cut in one of them cannot pass
+  for (int i = 3; i < 5; i++) {
+    const T di = out.p[i] - tv.par[i * tv.ld + b];
+    const T sii = out.C[i][i] + tv.cov[(i * (i + 1) / 2 + i) * tv.ld + b];
+    if (!(di * di <= ((T)4 * (T)M.chi2_cut) * sii)) return (T)-1;
+  }
   State<T> r = out;
   T x = G.X[tv.row_last[a]];
   if (rel == REL_NEXT || rel == REL_PREV) {

@@ -6,7 +6,8 @@ geometry and statistics, never from a run of the CUDA path:
   * a noiseless helix that crosses a 20-degree edge is found as one track per sector, the pieces are linked, the
     global track holds every cluster, and its refit returns the generating q/pT, tan(lambda), direction and vertex z
   * the same across the central electrode, with a non-zero collision time (the two sides measure z_true -+ v_d t)
-  * two different tracks that end / start at the same edge are not linked
+  * two different tracks that end / start at the same edge are not linked (by the chi2 if they share curvature and
+    dip, by the (tanlambda, q/pT) gate -- a necessary condition of the chi2 cut -- otherwise)
   * relabelling the sectors (rotation by 20 degrees, A <-> C mirror) relabels the links and nothing else
   * with the configs' smearing the chi2 of true links is chi2-distributed with 5 (4 across the electrode) degrees of
     freedom -- this pins the rotation Jacobian, the transported covariance and the Cholesky chi2 in one number
@@ -112,10 +113,12 @@ def test_noiseless_helix_across_the_central_electrode(orc):
 
 
 def test_different_tracks_at_the_same_edge_are_not_linked(orc):
-    """Two particles leave the same sector through the same edge a few rows and ~10 cm in z apart (q/pT 2.0 and 2.1,
-    tan(lambda) 0.4 and 0.5).  The piece of one in the first sector and the piece of the other in the second pass every
-    window of R26 (sector relation, rows, z) -- they are compared, and fail the chi2; each particle's own pieces link."""
-    t = dict(qpt=[2.0, 2.1], phi=[math.radians(12.0)] * 2, tanl=[0.4, 0.5], vx=[0.0, 0.0], vy=[0.0, 0.0], vz=[3.0, 3.0])
+    """Two particles of the SAME curvature and dip leave a sector through the same edge, 0.6 degrees and 7 cm in z
+    apart: the piece of one in the first sector and the piece of the other in the second pass every window and the
+    (tanlambda, q/pT) gate of R26 -- they are compared, and it is the chi2 (position and direction) that keeps them
+    apart; each particle's own pieces link.  A pair that differs in curvature instead never reaches the chi2 (gate)."""
+    t = dict(qpt=[2.0, 2.0], phi=[math.radians(12.0), math.radians(12.6)], tanl=[0.4, 0.4], vx=[0.0, 0.0], vy=[0.0, 0.0],
+             vz=[3.0, 10.0])
     ev = tracks_event(t)
     o, m = run_merge(orc, ev)
     lab = np.array([np.bincount(ev.true_track[o["trk_hits"][f:f + n]]).argmax()
@@ -126,6 +129,15 @@ def test_different_tracks_at_the_same_edge_are_not_linked(orc):
     cross = np.concatenate([m["pair_chi2"][np.ix_(lab == 0, lab == 1)].ravel(), m["pair_chi2"][np.ix_(lab == 1, lab == 0)].ravel()])
     assert (cross > 50.0).any(), "the cross pairs were looked at: a finite chi2, far above the cut"
     assert not ((cross >= 0) & (cross < 50.0)).any()
+    # other curvature (q/pT 2.0 and 2.1): removed by the gate, chi2 never formed, own pieces still linked
+    t["qpt"] = [2.0, 2.1]; t["phi"] = [math.radians(12.0)] * 2; t["tanl"] = [0.4, 0.5]; t["vz"] = [3.0, 3.0]
+    ev = tracks_event(t)
+    o, m = run_merge(orc, ev)
+    lab = np.array([np.bincount(ev.true_track[o["trk_hits"][f:f + n]]).argmax()
+                    for f, n in zip(o["trk_first_hit"], o["trk_nhits"])])
+    a = np.nonzero(m["succ"] >= 0)[0]
+    assert a.size == 2 and np.all(lab[a] == lab[m["succ"][a]])
+    assert np.all(m["pair_chi2"][np.ix_(lab == 0, lab == 1)] == -1) and np.all(m["pair_chi2"][np.ix_(lab == 1, lab == 0)] == -1)
 
 
 def test_links_follow_a_relabelling_of_the_sectors(orc):
