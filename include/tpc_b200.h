@@ -272,7 +272,8 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
  * max_gap as several tracks.  tpc_merge_tracks links them and refits the merged hit lists:
  *   B can follow A iff B's sector is A's, an azimuthal neighbour on the same side or the mirror sector across the
  *   electrode; 1 <= first row of B - last row of A <= max_rows; |z_B - z_A| <= dz_max between the two ends
- *   (|z_B + z_A| across the electrode: the sides measure z_true -+ v_d t); and chi2 < chi2_cut, chi2 = d^T S^-1 d over
+ *   (|z_B + z_A| across the electrode: the sides measure z_true -+ v_d t); tanlambda and q/pT differ by no more than
+ *   d^2 <= 4 chi2_cut (C_A + C_B) each (a necessary condition of the cut); and chi2 < chi2_cut, chi2 = d^T S^-1 d over
  *   (y, z, sinphi, tanlambda, q/pT) between A's state -- transported by R12 to its outermost hit, rotated into B's
  *   frame, transported to B's innermost hit -- and B's state, S the sum of the two covariances.  Across the electrode
  *   z is left out (free time offset) and |z_A' + z_B| <= ce_tol + 2 |tanlambda_B| dx / cosphi_B is required instead.
@@ -293,7 +294,8 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
  *                                     re-based on the first hit of the new side and ndf loses 1); a chain of one piece
  *                                     keeps its tpc_fit_tracks result; chi2 = ndf = -1 if a transport ran into max_sinphi
  * K = counters[TPC_CNT_TRACKS] is read on the device.  Enqueue only.  TPC_EINVAL for missing buffers or parameters
- * out of range (chi2_cut, dz_max > 0, ce_tol >= 0, 1 <= max_rows <= 151), TPC_ENOMEM_WS for a short workspace. */
+ * out of range (chi2_cut, dz_max > 0, ce_tol >= 0, 1 <= max_rows <= 151, max_tracks <= 2^28), TPC_ENOMEM_WS for a short
+ * workspace. */
 typedef struct {
   float chi2_cut;    /* 50  */
   float dz_max;      /* 64 cm */

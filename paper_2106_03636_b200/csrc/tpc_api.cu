@@ -308,7 +308,7 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
 int tpc_merge_workspace_bytes(const tpc_params_t* params_host, int64_t max_tracks, size_t* bytes_host) {
   tpc::Geo G;
   int64_t nb = 0;
-  if (!bytes_host || max_tracks < 1 || max_tracks > 2147483000ll || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (!bytes_host || max_tracks < 1 || max_tracks > (1ll << 28) || !make_geo(params_host, &G, &nb)) return TPC_EINVAL;
   *bytes_host = tpc::merge_ws_bytes(G, max_tracks);
   return TPC_OK;
 }
@@ -323,7 +323,7 @@ int tpc_merge_tracks(const tpc_params_t* params_host, const tpc_merge_params_t* 
   if (!merge_host || !(merge_host->chi2_cut > 0.0f) || !(merge_host->dz_max > 0.0f) || !(merge_host->ce_tol >= 0.0f) ||
       merge_host->max_rows < 1 || merge_host->max_rows > 151)
     return TPC_EINVAL;
-  if (max_tracks < 1 || max_tracks > 2147483000ll || !counters || !dev || !dev->trk_seed || !dev->trk_sector || !dev->trk_nhits ||
+  if (max_tracks < 1 || max_tracks > (1ll << 28) || !counters || !dev || !dev->trk_seed || !dev->trk_sector || !dev->trk_nhits ||
       !dev->trk_first_hit || !dev->par || !dev->cov || !dev->xref || !dev->zref || !dev->chi2 || !dev->ndf)
     return TPC_EINVAL;
   if (!out || !out->trk_succ || !out->trk_pred || !out->trk_succ_chi2 || !out->trk_global || !out->n_global || !out->g_head ||

@@ -4,7 +4,7 @@
 // across the central electrode and across holes longer than max_gap, and the refit of the merged hit lists.
 //
 //   k_merge_ends     per track: rows of its first / last hit (from the hit records tpc_find_tracks cached), z of
-//                    its inner end, bucket (sector, z slab) of that end; bucket histogram
+//                    its inner end, bucket (sector, z slab, group of 8 first rows) of that end; bucket histogram
 //   k_merge_scatter  end records into bucket order (the order inside a bucket is irrelevant: every arg-min below
 //                    breaks ties by seed)
 //   k_merge_match    one thread per track A: outer state by R12, then every track B whose inner end lies in the
@@ -31,6 +31,8 @@ namespace {
 
 constexpr int kThreads = 128;
 constexpr float kSlabCm = 128.0f;  // z slab of the end buckets (>= dz_max is not required: the lookup covers a range)
+constexpr int kRowGroups = 19;     // first rows in groups of 8: a bucket is (sector, z slab, row group)
+constexpr float kSlabEps = 0.01f;  // cm; widens a z lookup beyond any rounding of its fp32 window test
 constexpr float kCos20 = 0.93969262078590838405f, kSin20 = 0.34202014332566873304f;
 enum { REL_NONE = 0, REL_SAME = 1, REL_NEXT = 2, REL_PREV = 3, REL_CE = 4 };
 
@@ -46,6 +48,7 @@ struct EndRec {
   int rows;     // first row | last row << 8 | sector << 16
   int seed;     // original index of the start hit: tie-break
   int track;    // index of the track
+  float tanl, qpt, c33, c44;  // the gate of R26: tanlambda, q/pT and their variances
 };
 
 struct MergeWs {
@@ -58,6 +61,7 @@ struct MergeWs {
   int32_t* cand;      // [K] best candidate successor (before reciprocity)
   unsigned long long* pred_key;  // [K] (chi2 bits << 32 | seed of the best predecessor)
   int32_t* flag;      // [K + 1] head flags and their scan
+  int32_t* mlist;     // [K] global tracks of more than one piece (any order); mlist[K] = their number
   int32_t* scan_tmp;
 };
 
@@ -155,7 +159,7 @@ k_merge_ends(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict
     const int rf = __float_as_int(__ldg(hit_rec + f).z), rl = __float_as_int(__ldg(hit_rec + f + n - 1).z);
     const float z = zref[k] + par[1 * max_tracks + k];
     const float zeta = s < 18 ? z : -z;
-    const int b = s * mp.nslab + slab_of(zeta, g.s.z_lo, mp.nslab);
+    const int b = (s * mp.nslab + slab_of(zeta, g.s.z_lo, mp.nslab)) * kRowGroups + (rf >> 3);
     w.rows[k] = rf | (rl << 8) | (s << 16);
     w.z_in[k] = z;
     w.bucket[k] = b;
@@ -166,7 +170,8 @@ k_merge_ends(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict
 }
 
 __global__ void __launch_bounds__(kThreads)
-k_merge_scatter(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_seed, MergeWs w) {
+k_merge_scatter(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_seed,
+                const float* __restrict__ par, const float* __restrict__ cov, MergeWs w) {
   int64_t K = counters[TPC_CNT_TRACKS];
   if (K > max_tracks) K = max_tracks;
   for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kThreads) {
@@ -176,9 +181,51 @@ k_merge_scatter(const int32_t* __restrict__ counters, int64_t max_tracks, const 
     e.rows = w.rows[k];
     e.seed = trk_seed[k];
     e.track = (int)k;
-    reinterpret_cast<float4*>(w.ends)[slot] = make_float4(e.z_in, __int_as_float(e.rows), __int_as_float(e.seed), __int_as_float(e.track));
+    float4* dst = reinterpret_cast<float4*>(w.ends + slot);
+    dst[0] = make_float4(e.z_in, __int_as_float(e.rows), __int_as_float(e.seed), __int_as_float(e.track));
+    dst[1] = make_float4(par[3 * max_tracks + k], par[4 * max_tracks + k], cov[TPC_CI(3, 3) * max_tracks + k],
+                         cov[TPC_CI(4, 4) * max_tracks + k]);
   }
 }
+
+// chi2 of "B follows A" for a pair that passed the windows and the gate (R26); -1 = impossible
+__device__ __forceinline__ float pair_chi2(const KState& out, float x_a, float zref_a, int rel, int b, int rf_b, const float* sX,
+                                           const float* __restrict__ par, const float* __restrict__ cov,
+                                           const float* __restrict__ zref, int64_t max_tracks, float kB, float ms, float ce_tol) {
+  KState r = out;
+  float x = x_a;
+  if (rel == REL_NEXT || rel == REL_PREV) {
+    const float sd = rel == REL_NEXT ? kSin20 : -kSin20;
+    if (!rotate_state(r, x, kCos20, sd, ms)) return -1.0f;
+  }
+  const float xb = sX[rf_b];
+  if (!propagate(r, xb - x, kB, ms)) return -1.0f;
+  KState sbst;
+  load_state(sbst, par, cov, max_tracks, b);
+  const float zref_b = zref[b];
+  float d[5];
+  d[0] = r.p[0] - sbst.p[0];
+  d[1] = (zref_a - zref_b) + (r.p[1] - sbst.p[1]);
+  d[2] = r.p[2] - sbst.p[2];
+  d[3] = r.p[3] - sbst.p[3];
+  d[4] = r.p[4] - sbst.p[4];
+  if (rel == REL_CE) {
+    const float zsum = (zref_a + r.p[1]) + (zref_b + sbst.p[1]);
+    const float cb = sqrtf(1.0f - sbst.p[2] * sbst.p[2]);
+    const float lim = ce_tol + ((2.0f * fabsf(sbst.p[3])) * (xb - x_a)) / cb;
+    if (!(fabsf(zsum) <= lim)) return -1.0f;
+    const int idx[4] = {0, 2, 3, 4};
+    return chi2_cholesky<4>(r.C, sbst.C, d, idx);
+  }
+  const int idx[5] = {0, 1, 2, 3, 4};
+  return chi2_cholesky<5>(r.C, sbst.C, d, idx);
+}
+
+// One thread per track A.  The candidate loop applies only what needs no arithmetic on the states -- row window,
+// z window, (tanlambda, q/pT) gate -- to the 32-byte end records and keeps the survivors (nearly always the true
+// continuation and nobody else); the chi2 of the survivors is then formed in a second loop in which the lanes of a
+// warp work on their k-th survivor together.
+constexpr int kMaxSurv = 4;
 
 __global__ void __launch_bounds__(kThreads)
 k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict__ counters, int64_t max_tracks,
@@ -191,10 +238,11 @@ k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restric
   int64_t K = counters[TPC_CNT_TRACKS];
   if (K > max_tracks) K = max_tracks;
   const float kB = sc.kB, ms = sc.max_sinphi;
+  const float gate = 4.0f * mp.chi2_cut;
   for (int64_t a = (int64_t)blockIdx.x * kThreads + threadIdx.x; a < K; a += (int64_t)gridDim.x * kThreads) {
     const int rows_a = w.rows[a];
     const int rf_a = rows_a & 0xff, rl_a = (rows_a >> 8) & 0xff, s_a = rows_a >> 16;
-    const int seed_a = trk_seed[a];
+    const unsigned long long seed_a = (unsigned long long)(unsigned)trk_seed[a];
     const float zref_a = zref[a];
     KState out;
     load_state(out, par, cov, max_tracks, a);
@@ -202,66 +250,64 @@ k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restric
     float best = 0.0f;
     bool have_out = true;
     if (rl_a != rf_a) have_out = propagate(out, sX[rl_a] - sX[rf_a], kB, ms);
+    const float x_a = sX[rl_a];
+    const float zA = zref_a + out.p[1];
+    int surv[kMaxSurv];     // track of the survivor | relation << 28 (tracks < 2^28 by the tracklet limit of 2^25)
+    int surv_rf[kMaxSurv];
+    int nsurv = 0;
+    auto evaluate = [&](int b, int rel, int rf_b, int seed_b) {
+      const float chi2 = pair_chi2(out, x_a, zref_a, rel, b, rf_b, sX, par, cov, zref, max_tracks, kB, ms, mp.ce_tol);
+      if (!(chi2 >= 0.0f) || !(chi2 < mp.chi2_cut)) return;
+      if (best_b < 0 || chi2 < best || (chi2 == best && seed_b < best_seed)) {
+        best_b = b;
+        best = chi2;
+        best_seed = seed_b;
+      }
+      atomicMin(w.pred_key + b, ((unsigned long long)__float_as_uint(chi2) << 32) | seed_a);
+    };
     if (have_out) {
-      const float zA = zref_a + out.p[1];
-      const float x_a = sX[rl_a];
-      for (int sb = 0; sb < sc.nsec; sb++) {
+      const int g0 = (rl_a + 1) >> 3;
+      int g1 = (rl_a + mp.max_rows) >> 3;
+      if (g1 > kRowGroups - 1) g1 = kRowGroups - 1;
+      for (int sb = 0; sb < sc.nsec && g0 <= g1; sb++) {
         const int rel = sector_relation(s_a, sb);
         if (rel == REL_NONE) continue;
         // z of B's inner end: within dz_max of zA (same side) or of -zA (across the electrode); as zeta of B's side
         const float zc = rel == REL_CE ? -zA : zA;
         const float side_b = sb < 18 ? 1.0f : -1.0f;
-        const float za = (zc - mp.dz_max) * side_b, zb = (zc + mp.dz_max) * side_b;
-        int s0 = slab_of(fminf(za, zb), sc.z_lo, mp.nslab) - 1, s1 = slab_of(fmaxf(za, zb), sc.z_lo, mp.nslab) + 1;
-        if (s0 < 0) s0 = 0;
-        if (s1 > mp.nslab - 1) s1 = mp.nslab - 1;
-        const int e0 = w.bfirst[sb * mp.nslab + s0], e1 = w.bfirst[sb * mp.nslab + s1 + 1];
-        for (int e = e0; e < e1; e++) {
-          const float4 er = __ldg(reinterpret_cast<const float4*>(w.ends) + e);
-          const int rows_b = __float_as_int(er.y), b = __float_as_int(er.w);
-          const int rf_b = rows_b & 0xff;
-          const int dr = rf_b - rl_a;
-          if (dr < 1 || dr > mp.max_rows || b == (int)a) continue;
-          const float zB = er.x;
-          if (rel == REL_CE ? !(fabsf(zB + zA) <= mp.dz_max) : !(fabsf(zB - zA) <= mp.dz_max)) continue;
-          KState r = out;
-          float x = x_a;
-          if (rel == REL_NEXT || rel == REL_PREV) {
-            const float sd = rel == REL_NEXT ? kSin20 : -kSin20;
-            if (!rotate_state(r, x, kCos20, sd, ms)) continue;
+        const float za = (zc - (mp.dz_max + kSlabEps)) * side_b, zb = (zc + (mp.dz_max + kSlabEps)) * side_b;
+        const int s0 = slab_of(fminf(za, zb), sc.z_lo, mp.nslab), s1 = slab_of(fmaxf(za, zb), sc.z_lo, mp.nslab);
+        for (int sl = s0; sl <= s1; sl++) {
+          // first rows rl_a + 1 .. rl_a + max_rows: a contiguous run of row groups inside every (sector, slab)
+          const int bb = (sb * mp.nslab + sl) * kRowGroups;
+          const int e0 = w.bfirst[bb + g0], e1 = w.bfirst[bb + g1 + 1];
+          for (int e = e0; e < e1; e++) {
+            const float4 er = __ldg(reinterpret_cast<const float4*>(w.ends + e));
+            const int rows_b = __float_as_int(er.y), b = __float_as_int(er.w);
+            const int rf_b = rows_b & 0xff;
+            const int dr = rf_b - rl_a;
+            if (dr < 1 || dr > mp.max_rows || b == (int)a) continue;
+            const float zB = er.x;
+            if (rel == REL_CE ? !(fabsf(zB + zA) <= mp.dz_max) : !(fabsf(zB - zA) <= mp.dz_max)) continue;
+            const float4 gt = __ldg(reinterpret_cast<const float4*>(w.ends + e) + 1);
+            const float d3 = out.p[3] - gt.x, d4 = out.p[4] - gt.y;
+            const float s33 = out.C[TPC_CI(3, 3)] + gt.z, s44 = out.C[TPC_CI(4, 4)] + gt.w;
+            if (!(d3 * d3 <= gate * s33) || !(d4 * d4 <= gate * s44)) continue;
+            if (nsurv < kMaxSurv) {
+              surv[nsurv] = b | (rel << 28);
+              surv_rf[nsurv] = rf_b;
+              nsurv++;
+            } else {
+              evaluate(b, rel, rf_b, __float_as_int(er.z));
+            }
           }
-          const float xb = sX[rf_b];
-          if (!propagate(r, xb - x, kB, ms)) continue;
-          KState sbst;
-          load_state(sbst, par, cov, max_tracks, b);
-          const float zref_b = zref[b];
-          float d[5];
-          d[0] = r.p[0] - sbst.p[0];
-          d[1] = (zref_a - zref_b) + (r.p[1] - sbst.p[1]);
-          d[2] = r.p[2] - sbst.p[2];
-          d[3] = r.p[3] - sbst.p[3];
-          d[4] = r.p[4] - sbst.p[4];
-          float chi2;
-          if (rel == REL_CE) {
-            const float zsum = (zref_a + r.p[1]) + (zref_b + sbst.p[1]);
-            const float cb = sqrtf(1.0f - sbst.p[2] * sbst.p[2]);
-            const float lim = mp.ce_tol + ((2.0f * fabsf(sbst.p[3])) * (xb - x_a)) / cb;
-            if (!(fabsf(zsum) <= lim)) continue;
-            const int idx[4] = {0, 2, 3, 4};
-            chi2 = chi2_cholesky<4>(r.C, sbst.C, d, idx);
-          } else {
-            const int idx[5] = {0, 1, 2, 3, 4};
-            chi2 = chi2_cholesky<5>(r.C, sbst.C, d, idx);
-          }
-          if (!(chi2 >= 0.0f) || !(chi2 < mp.chi2_cut)) continue;
-          const int seed_b = __float_as_int(er.z);
-          if (best_b < 0 || chi2 < best || (chi2 == best && seed_b < best_seed)) {
-            best_b = b;
-            best = chi2;
-            best_seed = seed_b;
-          }
-          atomicMin(w.pred_key + b, ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned long long)(unsigned)seed_a);
         }
+      }
+    }
+    for (int k = 0; k < kMaxSurv; k++) {
+      if (k < nsurv) {
+        const int b = surv[k] & 0x0fffffff, rel = surv[k] >> 28;
+        evaluate(b, rel, surv_rf[k] & 0xff, trk_seed[b]);
       }
     }
     w.cand[a] = best_b;
@@ -303,7 +349,8 @@ k_merge_chains(const int32_t* __restrict__ counters, int64_t max_tracks, const i
                const int32_t* __restrict__ succ, const int32_t* __restrict__ pred, const int32_t* __restrict__ scan,
                int32_t* __restrict__ trk_global, int32_t* __restrict__ n_global, int32_t* __restrict__ g_head,
                int32_t* __restrict__ g_nseg, int32_t* __restrict__ g_nhits, float* __restrict__ gpar, float* __restrict__ gcov,
-               float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2, int32_t* __restrict__ gndf) {
+               float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2, int32_t* __restrict__ gndf,
+               int32_t* __restrict__ mlist) {
   int64_t K = counters[TPC_CNT_TRACKS];
   if (K > max_tracks) K = max_tracks;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -331,6 +378,8 @@ k_merge_chains(const int32_t* __restrict__ counters, int64_t max_tracks, const i
       gzref[gi] = zref[h];
       gchi2[gi] = chi2[h];
       gndf[gi] = ndf[h];
+    } else {
+      mlist[atomicAdd(mlist + max_tracks, 1)] = gi;
     }
   }
 }
@@ -346,16 +395,17 @@ k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_globa
               const float* __restrict__ zref, const int32_t* __restrict__ succ, const int32_t* __restrict__ g_head,
               const int32_t* __restrict__ g_nseg, const int32_t* __restrict__ g_nhits, float* __restrict__ gpar,
               float* __restrict__ gcov, float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2,
-              int32_t* __restrict__ gndf) {
+              int32_t* __restrict__ gndf, const int32_t* __restrict__ mlist) {
   __shared__ float sX[kMaxRows];
   const Scalars& sc = g.s;
   for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
   __syncthreads();
-  const int M = n_global[0];
+  (void)n_global;
+  const int M = mlist[max_tracks];
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
-  for (int64_t gi = (int64_t)blockIdx.x * kThreads + threadIdx.x; gi < M; gi += (int64_t)gridDim.x * kThreads) {
+  for (int64_t li = (int64_t)blockIdx.x * kThreads + threadIdx.x; li < M; li += (int64_t)gridDim.x * kThreads) {
+    const int gi = mlist[li];
     const int nseg = g_nseg[gi];
-    if (nseg < 2) continue;
     const int h = g_head[gi];
     int seg[kMaxPieces];
     int np = 0;
@@ -437,13 +487,13 @@ inline int merge_nslab(const Geo& g) {
 }
 
 struct MergeLayout {
-  size_t off_ends, off_bucket, off_bfirst, off_bcursor, off_rows, off_z, off_cand, off_key, off_flag, off_tmp, total;
+  size_t off_ends, off_bucket, off_bfirst, off_bcursor, off_rows, off_z, off_cand, off_key, off_flag, off_mlist, off_tmp, total;
   int64_t nbuckets;
 };
 
 inline MergeLayout merge_layout(int nsec, int nslab, int64_t max_tracks) {
   MergeLayout L{};
-  L.nbuckets = (int64_t)nsec * nslab;
+  L.nbuckets = (int64_t)nsec * nslab * kRowGroups;
   size_t o = 0;
   auto take = [&](size_t bytes) {
     size_t at = o;
@@ -460,6 +510,7 @@ inline MergeLayout merge_layout(int nsec, int nslab, int64_t max_tracks) {
   L.off_cand = take(sizeof(int32_t) * K);
   L.off_key = take(sizeof(unsigned long long) * K);
   L.off_flag = take(sizeof(int32_t) * (K + 1));
+  L.off_mlist = take(sizeof(int32_t) * (K + 1));
   const int64_t longest = (int64_t)K + 1 > L.nbuckets + 2 ? (int64_t)K + 1 : L.nbuckets + 2;
   L.off_tmp = take(sizeof(int64_t) * (size_t)((longest + kScanTile - 1) / kScanTile + 2));
   L.total = o;
@@ -495,11 +546,13 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
   w.cand = (int32_t*)(b + L.off_cand);
   w.pred_key = (unsigned long long*)(b + L.off_key);
   w.flag = (int32_t*)(b + L.off_flag);
+  w.mlist = (int32_t*)(b + L.off_mlist);
   w.scan_tmp = (int32_t*)(b + L.off_tmp);
   cudaError_t e;
   const unsigned blocks = blocks_for(max_tracks, kThreads, 148 * 16);
   if ((e = cudaMemsetAsync(w.bfirst, 0, sizeof(int32_t) * (size_t)(L.nbuckets + 2), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(trk_pred, 0xFF, sizeof(int32_t) * (size_t)max_tracks, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(w.mlist + max_tracks, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_ends<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, trk_sector, trk_nhits, trk_first_hit,
                                                        fw.hit_rec, par, zref, w)));
@@ -507,7 +560,7 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
   if ((e = cudaMemcpyAsync(w.bcursor, w.bfirst, sizeof(int32_t) * (size_t)(L.nbuckets + 1), cudaMemcpyDeviceToDevice, st)) !=
       cudaSuccess)
     return e;
-  TPC_LAUNCH(KID_MERGE, st, (k_merge_scatter<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, w)));
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_scatter<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, par, cov, w)));
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_match<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, par, cov, zref, w, trk_succ_chi2)));
   TPC_LAUNCH(KID_MERGE, st,
@@ -517,11 +570,11 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_chains<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_nhits, par, cov, xref, zref, chi2, ndf, trk_succ,
                                                          trk_pred, w.flag, trk_global, n_global, g_head, g_nseg, g_nhits, gpar,
-                                                         gcov, gxref, gzref, gchi2, gndf)));
+                                                         gcov, gxref, gzref, gchi2, gndf, w.mlist)));
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_refit<<<blocks, kThreads, 0, st>>>(g, n_global, max_tracks, trk_sector, trk_nhits, trk_first_hit, fw.hit_rec,
                                                         par, zref, trk_succ, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref,
-                                                        gchi2, gndf)));
+                                                        gchi2, gndf, w.mlist)));
   return cudaGetLastError();
 }
 
