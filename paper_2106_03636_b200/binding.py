@@ -78,8 +78,8 @@ def load(rebuild: bool = False):
     global _lib
     if _lib is not None and not rebuild:
         return _lib
-    path = os.environ.get("TPC_B200_LIB") or _build.LIB      # override: an alternative build of the same sources
-    if path == _build.LIB and (rebuild or not _build.up_to_date()):
+    path = _build.LIB
+    if rebuild or not _build.up_to_date():
         try:
             path = _build.build_library(force=rebuild)
         except Exception as e:  # no nvcc on this machine: use the shipped binary if there is one

@@ -2,7 +2,8 @@
 
 `python -m paper_2106_03636_b200.build` or `build_library()`; nvcc cross-compiles without a GPU.
 Flags that are part of the arithmetic contract: `-fmad=false` (one IEEE rounding per written
-fp32 operation on the device) and `-ffp-contract=off` for the host-side geometry tables.
+fp32 operation on the device; the fused multiply-adds of the contract are explicit __fmaf_rn) and
+`-ffp-contract=off` for the host-side geometry tables.
 """
 from __future__ import annotations
 
@@ -43,7 +44,6 @@ def build_library(force: bool = False, verbose: bool = False, out: str | None = 
            "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared", "-o", tmp]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += os.environ.get("TPC_B200_NVCC_FLAGS", "").split()     # tuning macros (-DTPC_FOLLOW_BATCH=...), optional
     cmd += [os.path.join(CSRC, s) for s in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:

@@ -89,13 +89,8 @@ struct Layout {
 // t makes the key of a tracklet unique even among tracklets dropped for capacity and names the owner in a dump.
 constexpr int kKeyTBits = 25;
 constexpr int64_t kMaxTracklets = (int64_t)1 << kKeyTBits;  // 33,554,432
-#ifndef TPC_MAX_BUCKETS
-#define TPC_MAX_BUCKETS 49152
-#endif
-#ifndef TPC_BUCKET_SHIFT0
-#define TPC_BUCKET_SHIFT0 13
-#endif
-constexpr int kMaxBuckets = TPC_MAX_BUCKETS;  // grid build: first-level buckets of the counting sort
+constexpr int kMaxBuckets = 49152;   // grid build: first-level buckets of the counting sort (their histogram fits shared memory)
+constexpr int kBucketShift0 = 13;    // ... of at least 2^13 bins each  // grid build: first-level buckets of the counting sort
 constexpr int kStateVec = 6;    // float4 per tracklet of follower state carried from phase A to phase B (24 words)
 constexpr int kStartBit = 1 << 30;  // rec.w: set on start hits by k_compact_starts (read by the upward legs, R17)
 constexpr int kBadRow = kStartBit - 1;  // rec.w of a cluster whose sector_row names no (sector, row): parked behind the grid
@@ -271,10 +266,8 @@ __device__ __forceinline__ unsigned long long sel_key(int nh, int start_orig, in
          (unsigned long long)(unsigned)t;
 }
 
-#ifndef TPC_BLOCK_CAP
-#define TPC_BLOCK_CAP (148 * 64)
-#endif
-inline unsigned blocks_for(int64_t n, int threads, int64_t cap = TPC_BLOCK_CAP) {
+constexpr int64_t kBlockCap = 148 * 64;  // grid-stride kernels: blocks per launch (per-block table set-up is amortised; measured optimum)
+inline unsigned blocks_for(int64_t n, int threads, int64_t cap = kBlockCap) {
   int64_t b = (n + threads - 1) / threads;
   if (b > cap) b = cap;
   if (b < 1) b = 1;

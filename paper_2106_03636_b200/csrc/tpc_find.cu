@@ -86,10 +86,7 @@ __device__ __noinline__ void neighbours_nested(const Rec* __restrict__ rec, cons
 // the tie-break is explicit.  Windows over more than two z-bin rows, or more than kMaxCand staged
 // candidates, take the plain nested loops.
 // ---------------------------------------------------------------------------------------------
-#ifndef TPC_CA_BATCH
-#define TPC_CA_BATCH 4
-#endif
-constexpr int kCaBatch = TPC_CA_BATCH;
+constexpr int kCaBatch = 4;  // candidate records in flight per thread and side (measured optimum)
 
 struct Ranges {
   int ka0, n0, ka1, n1;

@@ -26,21 +26,13 @@ namespace tpc {
 
 namespace {
 
-#ifndef TPC_FOLLOW_THREADS
-#define TPC_FOLLOW_THREADS 64
-#endif
 // 64-thread blocks, 10 per SM: 96 registers per thread without spills and 20 resident warps per SM (measured on
 // configs[4], before R17: 128 x 4 blocks at 112 registers = 16 warps: 28.0 ms; 64 x 10 at 96 registers: 25.3 ms;
 // with the R17 waves a batch of 2 candidate records is the optimum: 11.0 ms against 11.3 with 3 and 12.3 with 4)
-constexpr int kFollowThreads = TPC_FOLLOW_THREADS;
+constexpr int kFollowThreads = 64;
+constexpr int kFollowMinBlocks = 10;
 constexpr unsigned kFull = 0xffffffffu;
-#ifndef TPC_FOLLOW_BATCH
-#define TPC_FOLLOW_BATCH 2
-#endif
-#ifndef TPC_FOLLOW_MIN_BLOCKS
-#define TPC_FOLLOW_MIN_BLOCKS 10
-#endif
-constexpr int kBatch = TPC_FOLLOW_BATCH;  // candidate records in flight per lane in the R15/R16 search
+constexpr int kBatch = 2;  // candidate records in flight per lane in the R15/R16 search
 
 enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE };
 
@@ -50,7 +42,7 @@ enum Phase { PH_FETCH = 0, PH_INIT, PH_CHAIN, PH_UP, PH_JUMP, PH_DOWN, PH_DONE }
 // PHASE_B = true: the tracklets listed in `surv` (start hit not picked up) resume from tl_state with the R17 jump
 // and the R16 downward leg, and write their R18 record and R20 key.
 template <bool PHASE_B>
-__global__ void __launch_bounds__(kFollowThreads, TPC_FOLLOW_MIN_BLOCKS)
+__global__ void __launch_bounds__(kFollowThreads, kFollowMinBlocks)
 k_follow(const __grid_constant__ Geo g, const Rec* __restrict__ rec, const int32_t* __restrict__ bin_first,
          const int32_t* __restrict__ up_c, const TlInit* __restrict__ tl_init, int32_t* __restrict__ row_hit,
          int32_t* __restrict__ tl_info, unsigned long long* __restrict__ tl_key, float4* __restrict__ tl_state,

@@ -28,12 +28,8 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr unsigned kFull = 0xffffffffu;
-#ifndef TPC_SCATTER_CAP
-#define TPC_SCATTER_CAP (148 * 1024) /* no grid-stride loop: measured 3.33 -> 3.12 ms on configs[4] */
-#endif
-#ifndef TPC_SORT_CAP
-#define TPC_SORT_CAP kMaxBuckets /* one block per bucket: measured 2.62 -> 2.37 ms */
-#endif
+constexpr int64_t kScatterCap = 148 * 1024;  // no grid-stride loop: measured 3.33 -> 3.12 ms on configs[4]
+constexpr int64_t kSortCap = kMaxBuckets;    // one block per bucket: measured 2.62 -> 2.37 ms
 constexpr int kHistThreads = 1024;  // the bucket histogram takes up to 192 KB of shared memory: one or two big blocks per SM
 constexpr int kUnroll = 4;  // independent loads in flight per thread in the streaming passes
 
@@ -268,7 +264,7 @@ k_export_sorted(int64_t n, const Rec* __restrict__ rec, int32_t* __restrict__ so
 
 // bucket geometry: 8192 bins per bucket, doubled until at most kMaxBuckets buckets remain (nb <= 2^30)
 static inline int bucket_shift_for(int64_t nb) {
-  int sh = TPC_BUCKET_SHIFT0;
+  int sh = kBucketShift0;
   while (((nb + ((int64_t)1 << sh) - 1) >> sh) > kMaxBuckets) sh++;
   return sh;
 }
@@ -305,10 +301,10 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
     return e;
   if (n > 0)
     TPC_LAUNCH(KID_BUCKET_SCATTER, st,
-               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll, TPC_SCATTER_CAP), kThreads, 0, st>>>(g, n, sh, nbuckets, y, z, sector_row, w.bucket_cursor,
+               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll, kScatterCap), kThreads, 0, st>>>(g, n, sh, nbuckets, y, z, sector_row, w.bucket_cursor,
                                                                               (Rec*)w.hit_rec)));
   TPC_LAUNCH(KID_BUCKET_SORT, st,
-             (k_bucket_sort<<<blocks_for(nbuckets, 1, TPC_SORT_CAP), kSortThreads, sort_smem, st>>>(
+             (k_bucket_sort<<<blocks_for(nbuckets, 1, kSortCap), kSortThreads, sort_smem, st>>>(
                  g, n, nb, sh, nbuckets, w.bucket_first, (const Rec*)w.hit_rec, w.rec, w.bin_first)));
   return cudaGetLastError();
 }
