@@ -1340,3 +1340,75 @@ ORC_API int64_t orc_merge_fit_f64(const OrcParams* P, int64_t n, const double* y
   return merge_fit_impl<double>(P, n, y, z, sr, K, par, cov, xref, zref, chi2, ndf, sector, trk_nhits, trk_first_hit, trk_hits,
                                 succ, pred, trk_global, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref, gchi2, gndf);
 }
+
+// ---------------------------------------------------------------------------------------------
+// R27 (the TPC clusterizer is the step that feeds the tracker).
+// Input: zero-suppressed digits (sector_row, pad, time bin, ADC), any order; two digits of the same cell add up.
+// The paper gives no algorithm; this is the textbook reading:
+//   peak    : a digit of ADC a >= peak_min that beats its 8 neighbours in (pad, time) -- strictly the four "earlier"
+//             ones (time - 1 at any pad, and pad - 1 at the same time), at least equal to the four "later" ones, so a
+//             plateau yields exactly one peak; a missing neighbour counts as 0
+//   cluster : centre of gravity of the 3 x 3 cells around a peak (p0, t0), integer sums S = sum a, Sp = sum a dp,
+//             St = sum a dt; in fp32, one operation per operator:
+//               y    = ((p0 + 0.5) + Sp / S) * pad_width - ymax_row            (pad p covers [p, p + 1) pad widths)
+//               zeta = ((t0 + 0.5) + St / S) * time_width + z_lo,  z = side * zeta   (R2)
+//               q    = S
+// Output: clusters in ascending (sector_row, time, pad) order of their peaks, with the peak cell of each.
+// Returns the number of clusters found (at most `cap` are written).
+// ---------------------------------------------------------------------------------------------
+ORC_API int64_t orc_clusterize(const OrcParams* P, int64_t n, const int32_t* sr, const int32_t* pad, const int32_t* tim,
+                               const int32_t* adc, double pad_width, double time_width, int32_t peak_min, int64_t cap,
+                               float* y, float* z, float* q, int32_t* out_sr, int32_t* out_pad, int32_t* out_time) {
+  Geo<float> G(*P);
+  std::vector<std::pair<uint64_t, int64_t>> cells((size_t)n);
+  auto key = [](int64_t s, int64_t t, int64_t p) { return ((uint64_t)s << 40) | ((uint64_t)t << 16) | (uint64_t)p; };
+  for (int64_t i = 0; i < n; i++) cells[(size_t)i] = {key(sr[i], tim[i], pad[i]), (int64_t)adc[i]};
+  std::sort(cells.begin(), cells.end());
+  size_t m = 0;   // cells of the same key add up
+  for (size_t i = 0; i < cells.size(); i++) {
+    if (m > 0 && cells[m - 1].first == cells[i].first) cells[m - 1].second += cells[i].second;
+    else cells[m++] = cells[i];
+  }
+  cells.resize(m);
+  auto value = [&](int64_t s, int64_t t, int64_t p) -> int64_t {
+    if (t < 0 || p < 0 || p > 65535) return 0;
+    const uint64_t k = key(s, t, p);
+    auto it = std::lower_bound(cells.begin(), cells.end(), std::make_pair(k, (int64_t)INT64_MIN));
+    return (it != cells.end() && it->first == k) ? it->second : 0;
+  };
+  const float pw = (float)pad_width, tw = (float)time_width;
+  int64_t found = 0;
+  for (const auto& c : cells) {
+    const int64_t s = (int64_t)(c.first >> 40), t0 = (int64_t)((c.first >> 16) & 0xFFFFFF), p0 = (int64_t)(c.first & 0xFFFF);
+    const int64_t a = c.second;
+    if (a < peak_min) continue;
+    bool peak = true;
+    int64_t S = 0, Sp = 0, St = 0;
+    for (int dt = -1; dt <= 1; dt++)
+      for (int dp = -1; dp <= 1; dp++) {
+        const int64_t b = (dt == 0 && dp == 0) ? a : value(s, t0 + dt, p0 + dp);
+        if (dt != 0 || dp != 0) {
+          const bool earlier = dt < 0 || (dt == 0 && dp < 0);
+          if (earlier ? !(a > b) : !(a >= b)) peak = false;
+        }
+        S += b;
+        Sp += b * dp;
+        St += b * dt;
+      }
+    if (!peak) continue;
+    if (found < cap) {
+      const int sector = (int)(s / G.nrows), r = (int)(s % G.nrows);
+      const float fp = (float)Sp / (float)S, ft = (float)St / (float)S;
+      const float yc = (((float)p0 + 0.5f) + fp) * pw - G.ymax[r];
+      const float zeta = (((float)t0 + 0.5f) + ft) * tw + G.z_lo;
+      y[found] = yc;
+      z[found] = G.side(sector) * zeta;
+      q[found] = (float)S;
+      out_sr[found] = (int32_t)s;
+      out_pad[found] = (int32_t)p0;
+      out_time[found] = (int32_t)t0;
+    }
+    found++;
+  }
+  return found;
+}

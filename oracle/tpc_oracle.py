@@ -403,6 +403,25 @@ def merge(p, y, z, sector_row, o, mp=None, precision="f32", want_pairs=False):
     return dict(trk_sector=sector, row_first=rf, row_last=rl, **m, **f)
 
 
+def clusterize(p, sector_row, pad, time, adc, pad_width, time_width, peak_min=6, cap=None):
+    """R27: clusters from digits: dict(y, z, q (fp32), sector_row, pad, time (peak cell)), ascending (sector_row, time, pad)."""
+    P = make_params(p, "f32")
+    i32 = lambda a: np.ascontiguousarray(a, np.int32)
+    sr, pad, time, adc = i32(sector_row), i32(pad), i32(time), i32(adc)
+    n = sr.size
+    cap = int(cap if cap is not None else max(n, 1))
+    out = dict(y=np.empty(cap, np.float32), z=np.empty(cap, np.float32), q=np.empty(cap, np.float32),
+               sector_row=np.empty(cap, np.int32), pad=np.empty(cap, np.int32), time=np.empty(cap, np.int32))
+    L = lib()
+    L.orc_clusterize.restype = C.c_int64
+    k = int(L.orc_clusterize(C.byref(P), C.c_int64(n), _ptr(sr), _ptr(pad), _ptr(time), _ptr(adc), C.c_double(pad_width),
+                             C.c_double(time_width), C.c_int32(int(peak_min)), C.c_int64(cap), _ptr(out["y"]), _ptr(out["z"]),
+                             _ptr(out["q"]), _ptr(out["sector_row"]), _ptr(out["pad"]), _ptr(out["time"])))
+    out = {a: b[:min(k, cap)].copy() for a, b in out.items()}
+    out["n_found"] = k
+    return out
+
+
 def propagate(p, par5, cov15, dx, precision="f64"):
     """R12 primitive: returns (ok, par5', cov15', F[5,5])."""
     rt, sfx = _real(precision)
