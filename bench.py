@@ -420,6 +420,29 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                          "holes, merged hit lists refitted (DESIGN.md R26); not included in `value`"}
         binding.profile_collect(reset=True)
 
+    # ---- in front of the hot path (not part of `value`): tpc_clusterize (R27) on the digits of a slab of the event ---
+    cluster = None
+    if world == 1 and not args.no_cpu_baseline:
+        from types import SimpleNamespace
+        from paper_2106_03636_b200.synth import digitize
+        ys, zs, ss, desc = oracle_sample(ev, 1_000_000)
+        qs = np.full(ys.size, 50.0, np.float32)
+        d = digitize(SimpleNamespace(params=ev.params, y=ys, z=zs, q=qs, sector_row=ss))
+        dd = [torch.from_numpy(a).to(dev) for a in (d.sector_row, d.pad, d.time, d.adc)]
+        binding.clusterize(ev.params, *dd, d.pad_width, d.time_width)                   # warm-up
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(3):
+            r = binding.clusterize(ev.params, *dd, d.pad_width, d.time_width, want_numpy=False)
+        c1.record()
+        torch.cuda.synchronize()
+        ms = c0.elapsed_time(c1) / 3
+        cluster = {"ms": ms, "digits": d.n, "clusters": int(r["n_clusters"][0].item()), "digits_per_s": d.n / (ms * 1e-3),
+                   "sample": desc, "what": "tpc_clusterize on synthetic digits of that slab (DESIGN.md R27; hash-table build + "
+                                           "peak finding + centre of gravity; includes the table memsets); not included in `value`"}
+        del dd, r
+        binding.profile_collect(reset=True)
+
     # ---- end to end through the host-buffer entry points -----------------------------------------
     # Two Time Frames in flight (two Tracker contexts, own workspace / staging / pinned outputs, one stream each):
     # the H2D copy of one TF overlaps the tracking of the previous one and the D2H of the one before -- the
@@ -502,7 +525,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "follower_work": work,
            "clocks": clocks, "gpu_launches": launches, "kernels": kern,
            "kernels_ms_sum": round(sum(v["ms_per_step"] for v in kern.values()), 3), "roofline": roofline,
-           "after_hot_path": {"merge": merge}}
+           "after_hot_path": {"merge": merge}, "before_hot_path": {"clusterizer": cluster}}
     if not args.no_e2e:
         out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
                       "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3,

@@ -29,7 +29,7 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED, ST_BAD_ROW = 1, 2, 4, 8
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
            "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_merge_workspace_bytes",
-           "tpc_merge_tracks", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
+           "tpc_merge_tracks", "tpc_clusterize_workspace_bytes", "tpc_clusterize", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -169,6 +169,36 @@ def fp32_peak(device="cuda:0") -> float:
     with torch.cuda.device(scratch.device):
         _check(load().tpc_fp32_peak(_dp(scratch), C.byref(out), _stream()), "tpc_fp32_peak")
     return float(out.value)
+
+
+def clusterize(params, sector_row, pad, time, adc, pad_width, time_width, peak_min=6, max_clusters=None, want_numpy=True):
+    """tpc_clusterize (R27) on CUDA int32 tensors of digits.  Returns dict(y, z, q, sector_row, pad, time, n_found) --
+    numpy arrays of the clusters written (order unspecified) -- or, with want_numpy=False, the device tensors and the
+    device counter (asynchronous)."""
+    import torch
+    L = load()
+    n = int(sector_row.numel())
+    dev = sector_row.device
+    cap = int(max_clusters if max_clusters is not None else max(n, 1))
+    wsb = C.c_size_t(0)
+    _check(L.tpc_clusterize_workspace_bytes(C.c_int64(n), C.byref(wsb)), "tpc_clusterize_workspace_bytes")
+    ws = torch.empty(int(wsb.value), dtype=torch.uint8, device=dev)
+    f32, i32 = torch.float32, torch.int32
+    out = dict(y=torch.empty(cap, dtype=f32, device=dev), z=torch.empty(cap, dtype=f32, device=dev),
+               q=torch.empty(cap, dtype=f32, device=dev), sector_row=torch.empty(cap, dtype=i32, device=dev),
+               pad=torch.empty(cap, dtype=i32, device=dev), time=torch.empty(cap, dtype=i32, device=dev))
+    cnt = torch.zeros(2, dtype=i32, device=dev)
+    with torch.cuda.device(dev):
+        _check(L.tpc_clusterize(C.byref(make_params(params)), C.c_int64(n), _dp(sector_row), _dp(pad), _dp(time), _dp(adc),
+                                C.c_float(pad_width), C.c_float(time_width), C.c_int32(int(peak_min)), _dp(ws),
+                                C.c_size_t(int(wsb.value)), C.c_int64(cap), _dp(out["y"]), _dp(out["z"]), _dp(out["q"]),
+                                _dp(out["sector_row"]), _dp(out["pad"]), _dp(out["time"]), _dp(cnt), _stream()), "tpc_clusterize")
+    if not want_numpy:
+        return dict(out, n_clusters=cnt, workspace=ws)
+    found, written = (int(v) for v in cnt.cpu().numpy())
+    res = {k: v[:written].cpu().numpy() for k, v in out.items()}
+    res["n_found"] = found
+    return res
 
 
 def work_counts(counters) -> dict:

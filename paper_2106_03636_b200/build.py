@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpc_b200.so")
-SOURCES = ["tpc_api.cu", "tpc_grid.cu", "tpc_find.cu", "tpc_follow.cu", "tpc_select.cu", "tpc_fit.cu", "tpc_vertex.cu", "tpc_collisions.cu", "tpc_merge.cu"]
+SOURCES = ["tpc_api.cu", "tpc_grid.cu", "tpc_find.cu", "tpc_follow.cu", "tpc_select.cu", "tpc_fit.cu", "tpc_vertex.cu", "tpc_collisions.cu", "tpc_merge.cu", "tpc_cluster.cu"]
 HEADERS = ["tpc_common.cuh", "tpc_kalman.cuh", "tpc_scan.cuh", "tpc_search.cuh", "tpc_prof.cuh", os.path.join("..", "..", "include", "tpc_b200.h")]
 
 

@@ -25,7 +25,7 @@ Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_survivor_*", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
-                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_export_*"};
+                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_digit_*", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -302,6 +302,31 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
     return TPC_EINVAL;
   const cudaError_t e = tpc::launch_track_time(G, (double)v_drift, counters, max_tracks, trk_sector, par, xref, zref, phi0, z0,
                                                dca, t0, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_clusterize_workspace_bytes(int64_t n_digits, size_t* bytes_host) {
+  if (!bytes_host || n_digits < 0 || n_digits > (1ll << 31)) return TPC_EINVAL;
+  *bytes_host = tpc::cluster_ws_bytes(n_digits);
+  return TPC_OK;
+}
+
+int tpc_clusterize(const tpc_params_t* params_host, int64_t n_digits, const int32_t* sector_row, const int32_t* pad,
+                   const int32_t* time_bin, const int32_t* adc, float pad_width, float time_width, int32_t peak_min,
+                   void* workspace, size_t ws_bytes, int64_t max_clusters, float* y, float* z, float* q,
+                   int32_t* out_sector_row, int32_t* out_pad, int32_t* out_time, int32_t* n_clusters, void* stream) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (n_digits < 0 || n_digits > (1ll << 31) || max_clusters < 1 || max_clusters > 2147483000ll || !(pad_width > 0.0f) ||
+      !(time_width > 0.0f) || peak_min < 1 || !y || !z || !q || !out_sector_row || !out_pad || !out_time || !n_clusters)
+    return TPC_EINVAL;
+  if (n_digits > 0 && (!sector_row || !pad || !time_bin || !adc)) return TPC_EINVAL;
+  if (!workspace || ((uintptr_t)workspace & 255) != 0) return TPC_EINVAL;
+  if (ws_bytes < tpc::cluster_ws_bytes(n_digits)) return TPC_ENOMEM_WS;
+  const cudaError_t e = tpc::launch_clusterize(G, n_digits, sector_row, pad, time_bin, adc, pad_width, time_width, peak_min,
+                                               workspace, max_clusters, y, z, q, out_sector_row, out_pad, out_time, n_clusters,
+                                               (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

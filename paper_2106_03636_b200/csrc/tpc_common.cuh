@@ -240,6 +240,13 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
                          int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
                          float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st);
 
+// tpc_cluster.cu (R27)
+size_t cluster_ws_bytes(int64_t n_digits);
+cudaError_t launch_clusterize(const Geo& g, int64_t n, const int32_t* sr, const int32_t* pad, const int32_t* tim,
+                              const int32_t* adc, float pad_width, float time_width, int peak_min, void* workspace,
+                              int64_t max_clusters, float* y, float* z, float* q, int32_t* out_sr, int32_t* out_pad,
+                              int32_t* out_time, int32_t* n_clusters, cudaStream_t st);
+
 size_t collisions_ws_bytes(int64_t nb, int64_t max_tracks);
 cudaError_t launch_collisions(const int32_t* counters, int64_t max_tracks, const float* t0, const float* dca,
                               const int32_t* trk_sector, int side_sel, double t_lo,

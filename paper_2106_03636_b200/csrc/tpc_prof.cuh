@@ -34,6 +34,7 @@ enum KernelId {
   KID_TRACK_TIME,
   KID_COLLISIONS,
   KID_MERGE,
+  KID_CLUSTERIZE,
   KID_EXPORT,
   KID_N
 };
