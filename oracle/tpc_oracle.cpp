@@ -1412,3 +1412,154 @@ ORC_API int64_t orc_clusterize(const OrcParams* P, int64_t n, const int32_t* sr,
   }
   return found;
 }
+
+
+// ---------------------------------------------------------------------------------------------
+// R28 (synchronous tracking exists for the "removal of hits of tracks
+// not used for physics", l.47).  The paper gives no formula; the reading is the textbook one:
+//   R28a process noise.  After every transport of the refit over a path of L = |arc| sqrt(1 + tanl^2) cm through
+//        material of radiation length X0 (x0inv = 1/X0 per cm), multiple scattering with the Highland width without
+//        its logarithm, beta = 1:  theta0^2 = (0.0136 GeV)^2 (q/pT)^2 / (1 + tanl^2) * L * x0inv   (p = pT sqrt(1+tanl^2))
+//        is added to the covariance of the directions:  C22 += theta0^2 (1 - s^2)(1 + tl^2),  C33 += theta0^2 (1 + tl^2)^2,
+//        C43 += theta0^2 tl q (1 + tl^2),  C44 += theta0^2 tl^2 q^2   (s = sinphi, tl = tanl, q = q/pT).
+//        x0inv = 0 (the synthetic events have no material) reproduces R22 bit for bit.
+//   R28b outlier rejection.  In the LAST pass a hit whose chi2 against the predicted state exceeds outlier_cut is not
+//        used: no update, hit_flag = 1, ndf loses 2.  outlier_cut <= 0 switches it off.
+//   R28c cluster tags (what a compression step would drop): per cluster, bit 0 = attached to a track; bit 1 = that
+//        track is not used for physics: its refit failed (ndf < 0) or |q/pT| > qpt_max (low-pT loopers);
+//        bit 2 = the hit was rejected by R28b.  An unattached cluster has tag 0.
+// ---------------------------------------------------------------------------------------------
+struct OrcFitOptions {
+  double x0inv, outlier_cut;
+};
+
+template <class T>
+void add_scattering(State<T>& st, T arc, T x0inv) {
+  if (!(x0inv > (T)0)) return;
+  const T s = st.p[2], tl = st.p[3], q = st.p[4];
+  const T one_tl2 = (T)1 + tl * tl;
+  const T L = std::fabs(arc) * std::sqrt(one_tl2);
+  const T th2 = ((((T)0.0136 * (T)0.0136) * (q * q)) / one_tl2) * (L * x0inv);
+  st.C[2][2] = st.C[2][2] + (th2 * ((T)1 - s * s)) * one_tl2;
+  st.C[3][3] = st.C[3][3] + (th2 * one_tl2) * one_tl2;
+  const T c43 = ((th2 * tl) * q) * one_tl2;
+  st.C[4][3] = st.C[4][3] + c43;
+  st.C[3][4] = st.C[4][3];
+  st.C[4][4] = st.C[4][4] + ((th2 * tl) * tl) * (q * q);
+}
+
+// fit_one (R21-R22) with the R28 options; hit_flag[n] receives 1 for hits rejected in the last pass
+template <class T>
+bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G, const Clusters<T>& cl, const int32_t* hits,
+                     int n, T* par, T* cov, T* xref, T* zref_out, T* chi2_out, int32_t* ndf, uint8_t* hit_flag) {
+  const int32_t a = hits[0], b = hits[n / 2], c = hits[n - 1];
+  const T x1 = G.X[cl.row(a)], y1 = cl.y[a], x2 = G.X[cl.row(b)], y2 = cl.y[b], x3 = G.X[cl.row(c)], y3 = cl.y[c];
+  const T cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+  const T d12 = std::sqrt((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+  const T d23 = std::sqrt((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+  const T d13 = std::sqrt((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+  const T kappa = ((T)2 * cross) / ((d12 * d23) * d13);
+  const int32_t h1 = hits[1];
+  const T dx = G.X[cl.row(h1)] - x1, dy = cl.y[h1] - y1;
+  const T ch = std::sqrt(dx * dx + dy * dy);
+  T sphi = dy / ch - ((kappa * ch) * (T)0.5) * (dx / ch);
+  const T ms = (T)P.max_sinphi;
+  if (sphi > ms) sphi = ms;
+  if (sphi < -ms) sphi = -ms;
+  const T zref = cl.z[a];
+  State<T> st;
+  st.p[0] = y1; st.p[1] = 0; st.p[2] = sphi; st.p[3] = (cl.z[h1] - zref) / ch; st.p[4] = -(kappa / G.kB);
+  T chi2 = 0;
+  int at = 0, nrej = 0;
+  bool ok = true;
+  for (int i = 0; i < n; i++) hit_flag[i] = 0;
+  for (int pass = 0; pass < P.n_fit_passes && ok; pass++) {
+    reset_cov(st, P);
+    chi2 = 0;
+    const bool last = pass == P.n_fit_passes - 1;
+    const int dir = (pass % 2 == 0) ? +1 : -1;
+    const int first = (dir > 0) ? 0 : n - 1;
+    for (int k = first; k >= 0 && k < n; k += dir) {
+      const int32_t h = hits[k];
+      if (k != at) {
+        const T dxk = G.X[cl.row(h)] - G.X[cl.row(hits[at])];
+        // arc length of this step (the same expression R12 forms), for the scattering width
+        const T s1 = st.p[2], kap = -(G.kB * st.p[4]);
+        if (!propagate(st, dxk, G.kB, (T)P.max_sinphi)) { ok = false; break; }
+        const T s2 = st.p[2];
+        const T c1 = std::sqrt(mad(-s1, s1, (T)1)), c2 = std::sqrt(mad(-s2, s2, (T)1));
+        const T t = (s1 + s2) / (c1 + c2);
+        const T Lc = dxk * std::sqrt(mad(t, t, (T)1));
+        const T arc = Lc * asin_ratio((kap * Lc) * (T)0.5);
+        add_scattering(st, arc, (T)O.x0inv);
+        at = k;
+      }
+      if (last && O.outlier_cut > 0) {
+        const Innov<T> I = innovation(st, G.sy2, G.sz2);
+        const T c2h = chi2_of(I, cl.y[h] - st.p[0], (cl.z[h] - zref) - st.p[1]);
+        if (c2h > (T)O.outlier_cut) {
+          hit_flag[k] = 1;
+          nrej++;
+          continue;
+        }
+      }
+      chi2 += update(st, cl.y[h], cl.z[h] - zref, G.sy2, G.sz2);
+    }
+  }
+  for (int i = 0; i < 5; i++) par[i] = st.p[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) cov[m++] = st.C[i][j];
+  *xref = G.X[cl.row(hits[at])];
+  *zref_out = zref;
+  *chi2_out = ok ? chi2 : (T)-1;
+  *ndf = ok ? 2 * (n - nrej) - 5 : -1;
+  return ok;
+}
+
+template <class T>
+void fit_physics_impl(const OrcParams* P, const OrcFitOptions* O, int64_t n, const T* y, const T* z, const int32_t* sr, int64_t K,
+                      const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, T* par, T* cov, T* xref,
+                      T* zref, T* chi2, int32_t* ndf, uint8_t* hit_flag) {
+  OrcParams Pp = *P;
+  Geo<T> G(Pp);
+  Clusters<T> cl{n, y, z, sr, Pp.n_rows};
+  for (int64_t k = 0; k < K; k++) {
+    T p5[5], c15[15];
+    fit_one_physics(Pp, *O, G, cl, trk_hits + trk_first_hit[k], trk_nhits[k], p5, c15, xref + k, zref + k, chi2 + k, ndf + k,
+                    hit_flag + trk_first_hit[k]);
+    for (int i = 0; i < 5; i++) par[i * K + k] = p5[i];
+    for (int i = 0; i < 15; i++) cov[i * K + k] = c15[i];
+  }
+}
+
+ORC_API void orc_fit_physics_f32(const OrcParams* P, const OrcFitOptions* O, int64_t n, const float* y, const float* z,
+                                 const int32_t* sr, int64_t K, const int32_t* trk_nhits, const int64_t* trk_first_hit,
+                                 const int32_t* trk_hits, float* par, float* cov, float* xref, float* zref, float* chi2,
+                                 int32_t* ndf, uint8_t* hit_flag) {
+  fit_physics_impl<float>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag);
+}
+ORC_API void orc_fit_physics_f64(const OrcParams* P, const OrcFitOptions* O, int64_t n, const double* y, const double* z,
+                                 const int32_t* sr, int64_t K, const int32_t* trk_nhits, const int64_t* trk_first_hit,
+                                 const int32_t* trk_hits, double* par, double* cov, double* xref, double* zref, double* chi2,
+                                 int32_t* ndf, uint8_t* hit_flag) {
+  fit_physics_impl<double>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag);
+}
+// R28c: tag[n] from cluster_track[n], the per-track q/pT (par row 4, leading dimension ldp) and ndf, and hit_flag in
+// hit-list order (may be NULL)
+ORC_API void orc_tag_clusters(int64_t n, const int32_t* cluster_track, int64_t K, const float* qpt, const int32_t* ndf,
+                              const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
+                              const uint8_t* hit_flag, double qpt_max, uint8_t* tag) {
+  for (int64_t c = 0; c < n; c++) {
+    const int32_t k = cluster_track[c];
+    uint8_t t = 0;
+    if (k >= 0) {
+      t = 1;
+      if (ndf[k] < 0 || std::fabs((double)qpt[k]) > qpt_max) t |= 2;
+    }
+    tag[c] = t;
+  }
+  if (hit_flag)
+    for (int64_t k = 0; k < K; k++)
+      for (int i = 0; i < trk_nhits[k]; i++)
+        if (hit_flag[trk_first_hit[k] + i]) tag[trk_hits[trk_first_hit[k] + i]] |= 4;
+}

@@ -403,6 +403,46 @@ def merge(p, y, z, sector_row, o, mp=None, precision="f32", want_pairs=False):
     return dict(trk_sector=sector, row_first=rf, row_last=rl, **m, **f)
 
 
+class OrcFitOptions(C.Structure):
+    _fields_ = [("x0inv", C.c_double), ("outlier_cut", C.c_double)]
+
+
+def fit_physics(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, x0inv=0.0, outlier_cut=0.0, precision="f32"):
+    """R21-R22 with the R28 options (process noise per unit path, outlier rejection in the last pass):
+    dict(par, cov, xref, zref, chi2, ndf, hit_flag[n_hits])."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    rnd = (lambda v: float(np.float32(v))) if precision == "f32" else float
+    O = OrcFitOptions(rnd(x0inv), rnd(outlier_cut))
+    y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
+    nh = np.ascontiguousarray(trk_nhits, np.int32); fh = np.ascontiguousarray(trk_first_hit, np.int64)
+    th = np.ascontiguousarray(trk_hits, np.int32)
+    K = nh.size
+    par = np.empty((5, K), rt); cov = np.empty((15, K), rt)
+    xref = np.empty(K, rt); zref = np.empty(K, rt); chi2 = np.empty(K, rt); ndf = np.empty(K, np.int32)
+    flag = np.zeros(max(th.size, 1), np.uint8)
+    fn = getattr(lib(), f"orc_fit_physics_{sfx}")
+    fn.restype = None
+    fn(C.byref(P), C.byref(O), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int64(K), _ptr(nh), _ptr(fh), _ptr(th), _ptr(par),
+       _ptr(cov), _ptr(xref), _ptr(zref), _ptr(chi2), _ptr(ndf), _ptr(flag))
+    return dict(par=par, cov=cov, xref=xref, zref=zref, chi2=chi2, ndf=ndf, hit_flag=flag[:th.size])
+
+
+def tag_clusters(cluster_track, qpt, ndf, trk_nhits, trk_first_hit, trk_hits, hit_flag=None, qpt_max=10.0):
+    """R28c: uint8 tag per cluster (bit 0 attached, bit 1 track not used for physics, bit 2 rejected hit)."""
+    ct = np.ascontiguousarray(cluster_track, np.int32)
+    qpt = np.ascontiguousarray(qpt, np.float32); ndf = np.ascontiguousarray(ndf, np.int32)
+    nh = np.ascontiguousarray(trk_nhits, np.int32); fh = np.ascontiguousarray(trk_first_hit, np.int64)
+    th = np.ascontiguousarray(trk_hits, np.int32)
+    hf = None if hit_flag is None else np.ascontiguousarray(hit_flag, np.uint8)
+    tag = np.empty(ct.size, np.uint8)
+    fn = lib().orc_tag_clusters
+    fn.restype = None
+    fn(C.c_int64(ct.size), _ptr(ct), C.c_int64(nh.size), _ptr(qpt), _ptr(ndf), _ptr(nh), _ptr(fh), _ptr(th), _ptr(hf),
+       C.c_double(qpt_max), _ptr(tag))
+    return tag
+
+
 def clusterize(p, sector_row, pad, time, adc, pad_width, time_width, peak_min=6, cap=None):
     """R27: clusters from digits: dict(y, z, q (fp32), sector_row, pad, time (peak cell)), ascending (sector_row, time, pad)."""
     P = make_params(p, "f32")
