@@ -266,6 +266,27 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
                    void* workspace, size_t ws_bytes, const tpc_result_t* dev, const tpc_result_t* host,
                    void* stream);
 
+/* ---- physics options of the refit and cluster tags ("removal of hits of tracks
+ * not used for physics"; R28) -------------------------------------------------------------------------
+ * tpc_fit_tracks_physics: tpc_fit_tracks' self-contained path (hits gathered through y, z, sector_row, trk_hits;
+ * no workspace) with two options: x0inv > 0 adds multiple-scattering process noise after every transport over a path
+ * of L cm, theta0^2 = (0.0136 GeV)^2 (q/pT)^2 / (1 + tanl^2) L x0inv (x0inv = 1 / radiation length, per cm), to the
+ * covariance of sinphi, tanlambda and q/pT (R28a); outlier_cut > 0 leaves out, in the last pass, every hit whose chi2
+ * against the predicted state exceeds it: hit_flag = 1, ndf loses 2 (R28b).  hit_flag [n_clusters], in hit-list
+ * order (same indexing as trk_hits), is always written (0 = used).  x0inv = 0 and outlier_cut <= 0 give
+ * tpc_fit_tracks' results bit for bit.  TPC_EINVAL for x0inv < 0, NaN options or missing buffers.
+ * tpc_tag_clusters: tag [n_clusters] (uint8): bit 0 = attached to a track; bit 1 = that track is not used for
+ * physics: ndf < 0 or |q/pT| = |par[4][track]| > qpt_max (low-pT loopers); bit 2 = rejected by R28b (hit_flag may be
+ * NULL: bit 2 is then never set); 0 = unattached.  H = counters[TPC_CNT_HITS] is read on the device.  Enqueue only. */
+int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
+                           const int32_t* sector_row, const int32_t* counters, int64_t max_tracks,
+                           const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
+                           float x0inv, float outlier_cut, float* par, float* cov, float* xref, float* zref,
+                           float* chi2, int32_t* ndf, uint8_t* hit_flag, void* stream);
+int tpc_tag_clusters(int64_t n_clusters, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
+                     const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag,
+                     double qpt_max, uint8_t* tag, void* stream);
+
 /* ---- clusterizer (the step that feeds the tracker; R27) --------
  * Clusters from zero-suppressed digits (sector_row, pad, time_bin, adc), any order; two digits of one cell add up;
  * a digit with sector_row outside [0, n_sectors*n_rows), pad outside [0, 65535] or time_bin outside [0, 2^24) is

@@ -29,7 +29,8 @@ ST_TRACKLET_OVERFLOW, ST_TRACK_OVERFLOW, ST_Z_CLAMPED, ST_BAD_ROW = 1, 2, 4, 8
 SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins", "tpc_workspace_bytes",
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
            "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_merge_workspace_bytes",
-           "tpc_merge_tracks", "tpc_clusterize_workspace_bytes", "tpc_clusterize", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
+           "tpc_merge_tracks", "tpc_clusterize_workspace_bytes", "tpc_clusterize", "tpc_fit_tracks_physics",
+           "tpc_tag_clusters", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -335,6 +336,38 @@ class Tracker:
         found, n = (int(v) for v in nc.cpu().numpy())
         return dict(n_found=found, coll_time=ct[:n].cpu().numpy(), coll_ntracks=cn[:n].cpu().numpy(), coll_bin=cb[:n].cpu().numpy(),
                     trk_collision=tc[:k].cpu().numpy(), t0=tt["t0"][:k].cpu().numpy(), dca=tt["dca"][:k].cpu().numpy())
+
+    def fit_tracks_physics(self, x0inv: float = 0.0, outlier_cut: float = 0.0):
+        """tpc_fit_tracks_physics (R28a/b) on the hit lists of the last find: numpy dict(par, cov, xref, zref, chi2, ndf,
+        hit_flag); the Tracker's own fit outputs are left untouched.  Synchronises."""
+        t = self.torch
+        K, dev = self.max_tracks, self.device
+        y, z, sr = self._inputs
+        o = dict(par=t.empty((5, K), dtype=t.float32, device=dev), cov=t.empty((15, K), dtype=t.float32, device=dev),
+                 xref=t.empty(K, dtype=t.float32, device=dev), zref=t.empty(K, dtype=t.float32, device=dev),
+                 chi2=t.empty(K, dtype=t.float32, device=dev), ndf=t.empty(K, dtype=t.int32, device=dev),
+                 hit_flag=t.zeros(max(self.n, 1), dtype=t.uint8, device=dev))
+        _check(self.lib.tpc_fit_tracks_physics(C.byref(self.P), C.c_int64(self.n), _dp(y), _dp(z), _dp(sr), _dp(self.counters),
+                                               C.c_int64(K), _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits),
+                                               C.c_float(x0inv), C.c_float(outlier_cut), _dp(o["par"]), _dp(o["cov"]),
+                                               _dp(o["xref"]), _dp(o["zref"]), _dp(o["chi2"]), _dp(o["ndf"]), _dp(o["hit_flag"]),
+                                               _stream()), "tpc_fit_tracks_physics")
+        self._physics = o
+        cnt = self.counters.cpu().numpy()
+        k, h = int(cnt[CNT_TRACKS]), int(cnt[CNT_HITS])
+        return dict(par=o["par"][:, :k].cpu().numpy(), cov=o["cov"][:, :k].cpu().numpy(), xref=o["xref"][:k].cpu().numpy(),
+                    zref=o["zref"][:k].cpu().numpy(), chi2=o["chi2"][:k].cpu().numpy(), ndf=o["ndf"][:k].cpu().numpy(),
+                    hit_flag=o["hit_flag"][:h].cpu().numpy())
+
+    def tag_clusters(self, qpt_max: float = 10.0, use_physics_fit: bool = False):
+        """tpc_tag_clusters (R28c): uint8 tag per cluster, from the Tracker's fit or from the last fit_tracks_physics."""
+        t = self.torch
+        tag = t.empty(max(self.n, 1), dtype=t.uint8, device=self.device)
+        src = self._physics if use_physics_fit else dict(par=self.par, ndf=self.ndf, hit_flag=None)
+        _check(self.lib.tpc_tag_clusters(C.c_int64(self.n), _dp(self.cluster_track), _dp(self.counters), C.c_int64(self.max_tracks),
+                                         _dp(src["par"]), _dp(src["ndf"]), _dp(self.trk_hits), _dp(src["hit_flag"]),
+                                         C.c_double(qpt_max), _dp(tag), _stream()), "tpc_tag_clusters")
+        return tag[:self.n].cpu().numpy()
 
     def merge_alloc(self):
         """Workspace and device outputs of tpc_merge_tracks (allocated once per Tracker)."""

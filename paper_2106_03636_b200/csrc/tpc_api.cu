@@ -25,7 +25,7 @@ Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
 const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_survivor_*", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
-                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_digit_*", "k_export_*"};
+                                         "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_digit_*", "k_fit_physics+k_tag_*", "k_export_*"};
 }  // namespace
 
 void prof_begin(int id, cudaStream_t st) {
@@ -302,6 +302,33 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
     return TPC_EINVAL;
   const cudaError_t e = tpc::launch_track_time(G, (double)v_drift, counters, max_tracks, trk_sector, par, xref, zref, phi0, z0,
                                                dca, t0, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
+                           const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                           const int64_t* trk_first_hit, const int32_t* trk_hits, float x0inv, float outlier_cut, float* par,
+                           float* cov, float* xref, float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, void* stream) {
+  tpc::Geo G;
+  int64_t nb = 0;
+  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
+  if (n_clusters < 0 || max_tracks < 1 || !(x0inv >= 0.0f) || outlier_cut != outlier_cut || !counters || !trk_nhits ||
+      !trk_first_hit || !par || !cov || !xref || !zref || !chi2 || !ndf)
+    return TPC_EINVAL;
+  if (n_clusters > 0 && (!y || !z || !sector_row || !trk_hits || !hit_flag)) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_fit_physics(G, x0inv, outlier_cut, y, z, sector_row, counters, max_tracks, trk_nhits,
+                                                trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag,
+                                                (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
+int tpc_tag_clusters(int64_t n_clusters, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
+                     const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag, double qpt_max,
+                     uint8_t* tag, void* stream) {
+  if (n_clusters < 0 || max_tracks < 1 || !(qpt_max > 0.0) || !counters || !par || !ndf) return TPC_EINVAL;
+  if (n_clusters > 0 && (!cluster_track || !tag || (hit_flag && !trk_hits))) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_tag_clusters(n_clusters, cluster_track, counters, max_tracks, par, ndf, trk_hits, hit_flag,
+                                                 qpt_max, tag, (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

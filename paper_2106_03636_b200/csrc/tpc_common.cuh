@@ -240,6 +240,15 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
                          int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
                          float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st);
 
+// tpc_fit.cu (R28)
+cudaError_t launch_fit_physics(const Geo& g, float x0inv, float outlier_cut, const float* y, const float* z,
+                               const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                               const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
+                               float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st);
+cudaError_t launch_tag_clusters(int64_t n, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
+                                const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag,
+                                double qpt_max, uint8_t* tag, cudaStream_t st);
+
 // tpc_cluster.cu (R27)
 size_t cluster_ws_bytes(int64_t n_digits);
 cudaError_t launch_clusterize(const Geo& g, int64_t n, const int32_t* sr, const int32_t* pad, const int32_t* tim,

@@ -94,6 +94,131 @@ k_fit_gather(const __grid_constant__ Geo g, const float* __restrict__ y, const f
   }
 }
 
+// R28: k_fit_gather with process noise after every transport (R28a) and outlier
+// rejection in the last pass (R28b).  x0inv = 0 and outlier_cut <= 0 give k_fit_gather's results bit for bit.
+__device__ __forceinline__ void add_scattering(KState& st, float arc, float x0inv) {
+  if (!(x0inv > 0.0f)) return;
+  const float s = st.p[2], tl = st.p[3], q = st.p[4];
+  const float one_tl2 = 1.0f + tl * tl;
+  const float L = fabsf(arc) * sqrtf(one_tl2);
+  const float th2 = (((0.0136f * 0.0136f) * (q * q)) / one_tl2) * (L * x0inv);
+  st.C[TPC_CI(2, 2)] = st.C[TPC_CI(2, 2)] + (th2 * (1.0f - s * s)) * one_tl2;
+  st.C[TPC_CI(3, 3)] = st.C[TPC_CI(3, 3)] + (th2 * one_tl2) * one_tl2;
+  st.C[TPC_CI(4, 3)] = st.C[TPC_CI(4, 3)] + ((th2 * tl) * q) * one_tl2;
+  st.C[TPC_CI(4, 4)] = st.C[TPC_CI(4, 4)] + ((th2 * tl) * tl) * (q * q);
+}
+
+__global__ void __launch_bounds__(kFitThreads)
+k_fit_physics(const __grid_constant__ Geo g, float x0inv, float outlier_cut, const float* __restrict__ y,
+              const float* __restrict__ z, const int32_t* __restrict__ sector_row, const int32_t* __restrict__ counters,
+              int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
+              const int32_t* __restrict__ trk_hits, float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref,
+              float* __restrict__ zref_out, float* __restrict__ chi2_out, int32_t* __restrict__ ndf, uint8_t* __restrict__ hit_flag) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  const int nrows = sc.nrows;
+  for (int r = threadIdx.x; r < nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t K = counters[TPC_CNT_TRACKS];
+  if (K > max_tracks) K = max_tracks;
+  const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
+  for (int64_t k = (int64_t)blockIdx.x * kFitThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kFitThreads) {
+    const int n = trk_nhits[k];
+    const int64_t first = trk_first_hit[k];
+    const int32_t* hits = trk_hits + first;
+    auto rowx = [&](int h) { return sX[__ldg(sector_row + h) % nrows]; };
+    const int a = hits[0], b = hits[n / 2], c = hits[n - 1], h1 = hits[n > 1 ? 1 : 0];
+    const float x1 = rowx(a), y1 = __ldg(y + a), x2 = rowx(b), y2 = __ldg(y + b), x3 = rowx(c), y3 = __ldg(y + c);
+    const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+    const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
+    const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
+    const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
+    const float kappa = (2.0f * cross) / ((d12 * d23) * d13);
+    const float dx = rowx(h1) - x1, dy = __ldg(y + h1) - y1;
+    const float ch = sqrtf(dx * dx + dy * dy);
+    float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);
+    if (sphi > ms) sphi = ms;
+    if (sphi < -ms) sphi = -ms;
+    const float zref = __ldg(z + a);
+    KState st;
+    st.p[0] = y1;
+    st.p[1] = 0.0f;
+    st.p[2] = sphi;
+    st.p[3] = (__ldg(z + h1) - zref) / ch;
+    st.p[4] = -(kappa / kB);
+    float chi2 = 0.0f;
+    float x_at = x1;
+    int nrej = 0;
+    bool ok = true;
+    for (int i = 0; i < n; i++) hit_flag[first + i] = 0;
+    for (int pass = 0; pass < sc.n_fit_passes && ok; pass++) {
+      reset_cov(st, sc.cov0);
+      chi2 = 0.0f;
+      const bool last = pass == sc.n_fit_passes - 1;
+      const int dir = (pass & 1) ? -1 : 1;
+      int i = dir > 0 ? 0 : n - 1;
+      for (int cnt = 0; cnt < n; cnt++, i += dir) {
+        const int h = hits[i];
+        const float xh = rowx(h);
+        if (cnt > 0) {  // the first hit of a pass is the one the state already sits at (no transport)
+          const float dxk = xh - x_at;
+          const float s1 = st.p[2], kap = -(kB * st.p[4]);
+          if (!propagate(st, dxk, kB, ms)) {
+            ok = false;
+            break;
+          }
+          const float s2 = st.p[2];
+          const float c1 = sqrtf(mad(-s1, s1, 1.0f)), c2 = sqrtf(mad(-s2, s2, 1.0f));
+          const float t = (s1 + s2) / (c1 + c2);
+          const float Lc = dxk * sqrtf(mad(t, t, 1.0f));
+          add_scattering(st, Lc * asin_ratio((kap * Lc) * 0.5f), x0inv);
+          x_at = xh;
+        }
+        const Innov I = innovation(st, sy2, sz2);
+        const float yh = __ldg(y + h), zh = __ldg(z + h) - zref;
+        if (last && outlier_cut > 0.0f && chi2_of(I, yh - st.p[0], zh - st.p[1]) > outlier_cut) {
+          hit_flag[first + i] = 1;
+          nrej++;
+          continue;
+        }
+        chi2 = chi2 + update(st, I, yh, zh);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 5; i++) par[(int64_t)i * max_tracks + k] = st.p[i];
+#pragma unroll
+    for (int i = 0; i < 15; i++) cov[(int64_t)i * max_tracks + k] = st.C[i];
+    xref[k] = x_at;
+    zref_out[k] = zref;
+    chi2_out[k] = ok ? chi2 : -1.0f;
+    ndf[k] = ok ? 2 * (n - nrej) - 5 : -1;
+  }
+}
+
+// R28c cluster tags: bit 0 attached, bit 1 track not used for physics (refit failed or |q/pT| > qpt_max), bit 2 hit
+// rejected by R28b
+__global__ void __launch_bounds__(256)
+k_tag_tracks(int64_t n, const int32_t* __restrict__ cluster_track, int64_t max_tracks, const float* __restrict__ par,
+             const int32_t* __restrict__ ndf, double qpt_max, uint8_t* __restrict__ tag) {
+  for (int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x; c < n; c += (int64_t)gridDim.x * 256) {
+    const int k = cluster_track[c];
+    uint8_t t = 0;
+    if (k >= 0) {
+      t = 1;
+      if (__ldg(ndf + k) < 0 || (double)fabsf(__ldg(par + 4 * max_tracks + k)) > qpt_max) t |= 2;
+    }
+    tag[c] = t;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_tag_hits(const int32_t* __restrict__ counters, const int32_t* __restrict__ trk_hits, const uint8_t* __restrict__ hit_flag,
+           uint8_t* __restrict__ tag) {
+  const int64_t H = counters[TPC_CNT_HITS];
+  for (int64_t j = (int64_t)blockIdx.x * 256 + threadIdx.x; j < H; j += (int64_t)gridDim.x * 256)
+    if (hit_flag[j]) tag[trk_hits[j]] |= 4;  // a cluster is in one hit list at most: no other thread touches this byte
+}
+
 // R21 seeds for the cached refit, one thread per track (full memory parallelism for the four hit gathers and no
 // divergence, instead of a few lanes of a warp doing it inside the fit loop).  seed[k] = two float4:
 // (y1, sinphi, tanlambda, q/pT), (zRef, x1, first hit's y/z are re-read by the fit loop, -, -).
@@ -295,6 +420,31 @@ cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, con
   TPC_LAUNCH(KID_FIT, st,
              (k_fit_gather<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, y, z, sector_row, counters, max_tracks, trk_nhits,
                                                                     trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf)));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fit_physics(const Geo& g, float x0inv, float outlier_cut, const float* y, const float* z,
+                               const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                               const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
+                               float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st) {
+  if (max_tracks <= 0) return cudaSuccess;
+  int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  TPC_LAUNCH(KID_FIT_PHYSICS, st,
+             (k_fit_physics<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, x0inv, outlier_cut, y, z, sector_row, counters, max_tracks,
+                                                                     trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2,
+                                                                     ndf, hit_flag)));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tag_clusters(int64_t n, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
+                                const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag,
+                                double qpt_max, uint8_t* tag, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  TPC_LAUNCH(KID_FIT_PHYSICS, st,
+             (k_tag_tracks<<<blocks_for(n, 256), 256, 0, st>>>(n, cluster_track, max_tracks, par, ndf, qpt_max, tag)));
+  if (hit_flag)
+    TPC_LAUNCH(KID_FIT_PHYSICS, st, (k_tag_hits<<<blocks_for(n, 256), 256, 0, st>>>(counters, trk_hits, hit_flag, tag)));
   return cudaGetLastError();
 }
 

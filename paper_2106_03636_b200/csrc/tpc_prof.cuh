@@ -35,6 +35,7 @@ enum KernelId {
   KID_COLLISIONS,
   KID_MERGE,
   KID_CLUSTERIZE,
+  KID_FIT_PHYSICS,
   KID_EXPORT,
   KID_N
 };
