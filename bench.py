@@ -88,13 +88,17 @@ def csrc_digest() -> str:
     return h.hexdigest()
 
 
-KERNEL_GROUPS = (("k_follow", "k_follow"), ("k_fit", "k_fit"), ("k_scan", "k_scan_*"), ("k_wave_test", "k_survivor_*"),
-                 ("k_list_", "k_survivor_*"), ("k_chunk_counts", "k_compact_starts"))
+KERNEL_GROUPS = (("k_follow", "k_follow"), ("k_fit_seed", "k_fit"), ("k_fit_gather", "k_fit"), ("k_scan", "k_scan_*"), ("k_wave_test", "k_survivor_*"),
+                 ("k_list_", "k_survivor_*"), ("k_chunk_counts", "k_compact_starts"), ("k_clear_start_bits", "k_compact_starts"),
+                 ("k_fit_physics", "k_fit_physics+k_tag_*"), ("k_tag_", "k_fit_physics+k_tag_*"), ("k_merge_", "k_merge_*"),
+                 ("k_digit_", "k_digit_*"), ("k_cluster_count", "k_digit_*"))
 
 
 def bench_kernel_name(ncu_name: str) -> str:
     """Name of the bench table row a kernel of the ncu launch list belongs to."""
-    base = ncu_name.split("(")[0].split("::")[-1].split("<")[0].strip()
+    base = ncu_name.split("(")[0].split("::")[-1].split("<")[0].strip().split(" ")[-1]     # drops "void", namespaces, template arguments
+    if base == "k_fit":
+        return "k_fit"
     for prefix, row in KERNEL_GROUPS:
         if base.startswith(prefix):
             return row
