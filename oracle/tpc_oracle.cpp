@@ -1563,3 +1563,45 @@ ORC_API void orc_tag_clusters(int64_t n, const int32_t* cluster_track, int64_t K
       for (int i = 0; i < trk_nhits[k]; i++)
         if (hit_flag[trk_first_hit[k] + i]) tag[trk_hits[trk_first_hit[k] + i]] |= 4;
 }
+
+// ---------------------------------------------------------------------------------------------
+// R29 (last part): pairing of the collisions found on the two TPC sides (R25 with
+// side_sel = +1 and -1).  By R5 a collision at time t with vertex z_v is seen at t - z_v/v_d by side A and at
+// t + z_v/v_d by side C, with about the same number of tracks on either side.
+//   admissible : |t_C - t_A| <= dt_max (= 2 z_max / v_d)
+//   cost       : ((t_C - t_A) / sigma_t)^2 + (n_A - n_C)^2 / (n_A + n_C + 1)     (double, in this order)
+//   pairs      : best_C[i] = arg-min cost over admissible j, best_A[j] = arg-min over admissible i (ties: the lower
+//                index); (i, j) is a pair iff best_C[i] = j and best_A[j] = i -- reciprocal, as R10 and R26
+//   result     : t = (t_A + t_C) / 2,  z_v = v_d (t_C - t_A) / 2,  per pair, in ascending i
+// pair_of_a[nA], pair_of_c[nC] receive the partner's index or -1.  Returns the number of pairs.
+// ---------------------------------------------------------------------------------------------
+ORC_API int64_t orc_pair_sides(int64_t nA, const float* tA, const int32_t* cntA, int64_t nC, const float* tC, const int32_t* cntC,
+                               double dt_max, double sigma_t, double v_drift, int32_t* pair_of_a, int32_t* pair_of_c,
+                               float* t_out, float* zv_out) {
+  std::vector<int32_t> bestC((size_t)nA, -1), bestA((size_t)nC, -1);
+  std::vector<double> costA((size_t)nA, 0.0), costC((size_t)nC, 0.0);
+  for (int64_t i = 0; i < nA; i++)
+    for (int64_t j = 0; j < nC; j++) {
+      const double dt = (double)tC[j] - (double)tA[i];
+      if (!(std::fabs(dt) <= dt_max)) continue;
+      const double u = dt / sigma_t, dn = (double)cntA[i] - (double)cntC[j];
+      const double cost = u * u + (dn * dn) / ((double)cntA[i] + (double)cntC[j] + 1.0);
+      if (bestC[(size_t)i] < 0 || cost < costA[(size_t)i]) { bestC[(size_t)i] = (int32_t)j; costA[(size_t)i] = cost; }
+      if (bestA[(size_t)j] < 0 || cost < costC[(size_t)j]) { bestA[(size_t)j] = (int32_t)i; costC[(size_t)j] = cost; }
+    }
+  for (int64_t j = 0; j < nC; j++) pair_of_c[j] = -1;
+  int64_t np = 0;
+  for (int64_t i = 0; i < nA; i++) {
+    const int32_t j = bestC[(size_t)i];
+    if (j >= 0 && bestA[(size_t)j] == (int32_t)i) {
+      pair_of_a[i] = j;
+      pair_of_c[j] = (int32_t)i;
+      t_out[np] = (float)(((double)tA[i] + (double)tC[j]) * 0.5);
+      zv_out[np] = (float)((v_drift * ((double)tC[j] - (double)tA[i])) * 0.5);
+      np++;
+    } else {
+      pair_of_a[i] = -1;
+    }
+  }
+  return np;
+}

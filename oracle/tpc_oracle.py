@@ -462,6 +462,19 @@ def clusterize(p, sector_row, pad, time, adc, pad_width, time_width, peak_min=6,
     return out
 
 
+def pair_sides(tA, nA, tC, nC, dt_max=15.5, sigma_t=3.88, v_drift=2.58):
+    """R29: dict(pair_of_a[nA], pair_of_c[nC], t[np], z_vertex[np]) from the per-side collision times / track counts."""
+    tA = np.ascontiguousarray(tA, np.float32); tC = np.ascontiguousarray(tC, np.float32)
+    nA = np.ascontiguousarray(nA, np.int32); nC = np.ascontiguousarray(nC, np.int32)
+    pa = np.empty(max(tA.size, 1), np.int32); pc = np.empty(max(tC.size, 1), np.int32)
+    t = np.empty(max(min(tA.size, tC.size), 1), np.float32); zv = np.empty_like(t)
+    fn = lib().orc_pair_sides
+    fn.restype = C.c_int64
+    k = int(fn(C.c_int64(tA.size), _ptr(tA), _ptr(nA), C.c_int64(tC.size), _ptr(tC), _ptr(nC), C.c_double(dt_max),
+               C.c_double(sigma_t), C.c_double(v_drift), _ptr(pa), _ptr(pc), _ptr(t), _ptr(zv)))
+    return dict(pair_of_a=pa[:tA.size], pair_of_c=pc[:tC.size], t=t[:k], z_vertex=zv[:k])
+
+
 def propagate(p, par5, cov15, dx, precision="f64"):
     """R12 primitive: returns (ok, par5', cov15', F[5,5])."""
     rt, sfx = _real(precision)

@@ -86,3 +86,58 @@ def test_R25_side_selection_separates_the_two_halves_of_a_collision(orc):
     assert np.all(a["trk_collision"][:60] == 0) and np.all(a["trk_collision"][60:] == -1)
     assert 0.5 * (a["coll_time"][0] + c["coll_time"][0]) == pytest.approx(t_c, abs=0.15)
     assert 0.5 * (c["coll_time"][0] - a["coll_time"][0]) * vd == pytest.approx(zv, abs=0.4)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# R29: pairing of the two sides' collisions into (t, z_vertex)
+# ------------------------------------------------------------------------------------------------------------
+def _two_sides(rng, n_coll, rate_us, sigma_z=5.0, vd=2.58):
+    t = np.cumsum(rng.exponential(rate_us, n_coll)) + 50.0
+    zv = rng.normal(0.0, sigma_z, n_coll)
+    mult = rng.integers(20, 400, n_coll)
+    nA = rng.binomial(mult, 0.5); nC = mult - nA
+    return t, zv, (t - zv / vd).astype(np.float32), nA.astype(np.int32), (t + zv / vd).astype(np.float32), nC.astype(np.int32)
+
+
+def test_R29_pairs_give_back_time_and_vertex(orc):
+    """Collisions 20 us apart on average (50 kHz), vertex spread 5 cm: the two halves are 2 z_v / v_d <= ~12 us apart;
+    the reciprocal arg-min of (dt / sigma_t)^2 + (n_A - n_C)^2 / (n_A + n_C + 1) pairs 85 % of them correctly at this
+    pile-up (every collision at a tenth of the rate), and a correct pair returns t and z_v exactly (up to fp32)."""
+    rng = np.random.default_rng(40)
+    t, zv, tA, nA, tC, nC = _two_sides(rng, 400, 20.0)
+    permC = rng.permutation(400)                      # the C list in another order: the pairing is by value
+    r = orc.pair_sides(tA, nA, tC[permC], nC[permC])
+    inv = np.empty(400, np.int64); inv[permC] = np.arange(400)
+    good = r["pair_of_a"] == inv
+    assert good.mean() > 0.80
+    t2, zv2, tA2, nA2, tC2, nC2 = _two_sides(rng, 200, 200.0)
+    r2 = orc.pair_sides(tA2, nA2, tC2, nC2)
+    ok2 = r2["pair_of_a"] == np.arange(200)
+    assert ok2.mean() > 0.97                     # a few gaps of the Poisson process are still shorter than the window
+    paired = np.nonzero(r2["pair_of_a"] >= 0)[0]
+    np.testing.assert_allclose(r2["z_vertex"][ok2[paired]], zv2[paired][ok2[paired]], atol=2e-2)
+    idx = np.nonzero(r["pair_of_a"] >= 0)[0]
+    assert np.array_equal(r["pair_of_c"][r["pair_of_a"][idx]], idx), "the two partner tables must agree"
+    ok = good[idx]
+    np.testing.assert_allclose(r["t"][ok], t[idx][ok], atol=2e-3)
+    np.testing.assert_allclose(r["z_vertex"][ok], zv[idx][ok], atol=5e-3)
+
+
+def test_R29_is_the_reciprocal_argmin_of_the_stated_cost(orc):
+    rng = np.random.default_rng(41)
+    t, zv, tA, nA, tC, nC = _two_sides(rng, 120, 6.0)     # heavy pile-up: many admissible partners
+    dt_max, sig = 15.5, 3.88
+    r = orc.pair_sides(tA, nA, tC, nC, dt_max, sig)
+    dt = tC.astype(np.float64)[None, :] - tA.astype(np.float64)[:, None]
+    dn = nA.astype(np.float64)[:, None] - nC.astype(np.float64)[None, :]
+    cost = (dt / sig) ** 2 + dn * dn / (nA[:, None] + nC[None, :] + 1.0)
+    cost = np.where(np.abs(dt) <= dt_max, cost, np.inf)
+    bc = np.where(np.isfinite(cost).any(1), cost.argmin(1), -1)
+    ba = np.where(np.isfinite(cost).any(0), cost.argmin(0), -1)
+    want = np.array([j if j >= 0 and ba[j] == i else -1 for i, j in enumerate(bc)])
+    assert np.array_equal(r["pair_of_a"], want) and (want >= 0).sum() > 60
+    # nothing outside the window is ever paired; a lone half stays unpaired
+    lone = orc.pair_sides([100.0], [50], [130.0], [50])
+    assert lone["pair_of_a"][0] == -1 and lone["t"].size == 0
+    one = orc.pair_sides([100.0], [50], [107.0], [48])
+    assert one["pair_of_a"][0] == 0 and one["t"][0] == pytest.approx(103.5) and one["z_vertex"][0] == pytest.approx(2.58 * 3.5)
