@@ -219,6 +219,22 @@ int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float
                         int32_t* coll_ntracks, int32_t* coll_bin, int32_t* trk_collision,
                         int32_t* n_collisions, void* stream);
 
+/* Pairing of the two sides' collisions into (t, z_vertex) (last part; R29).  Inputs: the
+ * outputs of two tpc_find_collisions calls, side_sel = +1 (`_a`) and -1 (`_c`): n_collisions [2], coll_time,
+ * coll_ntracks (device; the number written, n_collisions[1], is read on the device).  A collision at time t with
+ * vertex z_v is seen at t - z_v/v_drift by side A and at t + z_v/v_drift by side C.  (i, j) is admissible iff
+ * |t_c[j] - t_a[i]| <= dt_max; cost = ((t_c - t_a) / sigma_t)^2 + (n_a - n_c)^2 / (n_a + n_c + 1) in double; pairs are
+ * the reciprocal arg-mins (ties: the lower index).  Outputs (device): pair_of_a, pair_of_c [max_collisions] (partner
+ * or -1), t, z_vertex [max_collisions] per pair in ascending side-A index (t = (t_a + t_c)/2, z_vertex =
+ * v_drift (t_c - t_a)/2), n_pairs [1].  workspace: tpc_pair_sides_workspace_bytes(max_collisions), 256-byte aligned.
+ * Enqueue only. */
+int tpc_pair_sides_workspace_bytes(int64_t max_collisions, size_t* bytes_host);
+int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, const int32_t* coll_ntracks_a,
+                   const int32_t* n_collisions_c, const float* coll_time_c, const int32_t* coll_ntracks_c,
+                   int64_t max_collisions, double dt_max, double sigma_t, double v_drift, void* workspace,
+                   size_t ws_bytes, int32_t* pair_of_a, int32_t* pair_of_c, float* t, float* z_vertex,
+                   int32_t* n_pairs, void* stream);
+
 /* ---- host-buffer entry points (bench.py `e2e`; a continuous stream of Time Frames through
  * reused GPU memory) ---------------------------------------------------------------------------------------------
  * tpc_result_t names the outputs of tpc_find_tracks + tpc_fit_tracks (layouts as documented there).  The same

@@ -30,7 +30,7 @@ SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins"
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
            "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_merge_workspace_bytes",
            "tpc_merge_tracks", "tpc_clusterize_workspace_bytes", "tpc_clusterize", "tpc_fit_tracks_physics",
-           "tpc_tag_clusters", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
+           "tpc_tag_clusters", "tpc_pair_sides_workspace_bytes", "tpc_pair_sides", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -334,6 +334,8 @@ class Tracker:
                                             _dp(tc), _dp(nc), _stream()), "tpc_find_collisions")
         k = int(self.counters[CNT_TRACKS].item())
         found, n = (int(v) for v in nc.cpu().numpy())
+        self._coll = getattr(self, "_coll", {})
+        self._coll[side] = dict(n=nc, time=ct, ntracks=cn, cap=max_collisions)      # device views for pair_sides
         return dict(n_found=found, coll_time=ct[:n].cpu().numpy(), coll_ntracks=cn[:n].cpu().numpy(), coll_bin=cb[:n].cpu().numpy(),
                     trk_collision=tc[:k].cpu().numpy(), t0=tt["t0"][:k].cpu().numpy(), dca=tt["dca"][:k].cpu().numpy())
 
@@ -412,6 +414,27 @@ class Tracker:
                     for nm in o if nm not in per_trk and nm != "n_global"})
         res.update(n_global=m, n_links=links)
         return res
+
+    def pair_sides(self, dt_max: float = 15.5, sigma_t: float = 3.88, v_drift: float = 2.58):
+        """tpc_pair_sides (R29) on the last find_collisions(side=+1) and find_collisions(side=-1): numpy dict(pair_of_a,
+        pair_of_c, t, z_vertex); synchronises."""
+        t = self.torch
+        a, c = self._coll[1], self._coll[-1]
+        cap = min(a["cap"], c["cap"])
+        wsb = C.c_size_t(0)
+        _check(self.lib.tpc_pair_sides_workspace_bytes(C.c_int64(cap), C.byref(wsb)), "tpc_pair_sides_workspace_bytes")
+        ws = t.empty(int(wsb.value), dtype=t.uint8, device=self.device)
+        pa = t.empty(cap, dtype=t.int32, device=self.device); pc = t.empty(cap, dtype=t.int32, device=self.device)
+        tt = t.empty(cap, dtype=t.float32, device=self.device); zv = t.empty(cap, dtype=t.float32, device=self.device)
+        npairs = t.zeros(1, dtype=t.int32, device=self.device)
+        _check(self.lib.tpc_pair_sides(_dp(a["n"]), _dp(a["time"]), _dp(a["ntracks"]), _dp(c["n"]), _dp(c["time"]), _dp(c["ntracks"]),
+                                       C.c_int64(cap), C.c_double(dt_max), C.c_double(sigma_t), C.c_double(v_drift), _dp(ws),
+                                       C.c_size_t(int(wsb.value)), _dp(pa), _dp(pc), _dp(tt), _dp(zv), _dp(npairs), _stream()),
+               "tpc_pair_sides")
+        k = int(npairs.item())
+        na, nc_ = int(a["n"][1].item()), int(c["n"][1].item())
+        return dict(pair_of_a=pa[:na].cpu().numpy(), pair_of_c=pc[:nc_].cpu().numpy(), t=tt[:k].cpu().numpy(),
+                    z_vertex=zv[:k].cpu().numpy())
 
     def step(self, y, z, sector_row):
         """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""

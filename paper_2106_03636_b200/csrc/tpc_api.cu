@@ -305,6 +305,28 @@ int tpc_track_time(const tpc_params_t* params_host, const int32_t* counters, int
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
+int tpc_pair_sides_workspace_bytes(int64_t max_collisions, size_t* bytes_host) {
+  if (!bytes_host || max_collisions < 1 || max_collisions > 2147483000ll) return TPC_EINVAL;
+  *bytes_host = tpc::pair_sides_ws_bytes(max_collisions);
+  return TPC_OK;
+}
+
+int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, const int32_t* coll_ntracks_a,
+                   const int32_t* n_collisions_c, const float* coll_time_c, const int32_t* coll_ntracks_c, int64_t max_collisions,
+                   double dt_max, double sigma_t, double v_drift, void* workspace, size_t ws_bytes, int32_t* pair_of_a,
+                   int32_t* pair_of_c, float* t, float* z_vertex, int32_t* n_pairs, void* stream) {
+  if (max_collisions < 1 || max_collisions > 2147483000ll || !(dt_max > 0.0) || !(sigma_t > 0.0) || !(v_drift > 0.0) ||
+      !n_collisions_a || !coll_time_a || !coll_ntracks_a || !n_collisions_c || !coll_time_c || !coll_ntracks_c || !pair_of_a ||
+      !pair_of_c || !t || !z_vertex || !n_pairs)
+    return TPC_EINVAL;
+  if (!workspace || ((uintptr_t)workspace & 255) != 0) return TPC_EINVAL;
+  if (ws_bytes < tpc::pair_sides_ws_bytes(max_collisions)) return TPC_ENOMEM_WS;
+  const cudaError_t e = tpc::launch_pair_sides(n_collisions_a, coll_time_a, coll_ntracks_a, n_collisions_c, coll_time_c,
+                                               coll_ntracks_c, max_collisions, dt_max, sigma_t, v_drift, workspace, pair_of_a,
+                                               pair_of_c, t, z_vertex, n_pairs, (cudaStream_t)stream);
+  return e == cudaSuccess ? TPC_OK : cuda_fail(e);
+}
+
 int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
                            const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
                            const int64_t* trk_first_hit, const int32_t* trk_hits, float x0inv, float outlier_cut, float* par,

@@ -111,7 +111,73 @@ k_t0_assign(const int32_t* __restrict__ counters, int64_t max_tracks, int64_t nb
   }
 }
 
+// R29: pairing of the two sides' collisions.  which = 0: thread i of side A looks for its best partner on side C;
+// which = 1: thread j of side C for its best partner on side A.  The cost is formed in double in R29's operation
+// order; ties go to the lower index (strict < while the partner index ascends).
+__global__ void __launch_bounds__(kThreads)
+k_pair_best(int which, const int32_t* __restrict__ n_a, const float* __restrict__ t_a, const int32_t* __restrict__ c_a,
+            const int32_t* __restrict__ n_c, const float* __restrict__ t_c, const int32_t* __restrict__ c_c, double dt_max,
+            double sigma_t, int32_t* __restrict__ best) {
+  const int nA = n_a[1], nC = n_c[1];
+  const int n_own = which == 0 ? nA : nC, n_oth = which == 0 ? nC : nA;
+  for (int i = blockIdx.x * kThreads + threadIdx.x; i < n_own; i += gridDim.x * kThreads) {
+    int b = -1;
+    double bc = 0.0;
+    for (int j = 0; j < n_oth; j++) {
+      const int ia = which == 0 ? i : j, ic = which == 0 ? j : i;
+      const double dt = (double)t_c[ic] - (double)t_a[ia];
+      if (!(fabs(dt) <= dt_max)) continue;
+      const double u = dt / sigma_t, dn = (double)c_a[ia] - (double)c_c[ic];
+      const double cost = u * u + (dn * dn) / ((double)c_a[ia] + (double)c_c[ic] + 1.0);
+      if (b < 0 || cost < bc) {
+        b = j;
+        bc = cost;
+      }
+    }
+    best[i] = b;
+  }
+}
+
+// reciprocal pairs in ascending order of the side-A index (a Time Frame holds a few hundred collisions: one thread)
+__global__ void k_pair_emit(const int32_t* __restrict__ n_a, const float* __restrict__ t_a, const int32_t* __restrict__ n_c,
+                            const float* __restrict__ t_c, const int32_t* __restrict__ best_c, const int32_t* __restrict__ best_a,
+                            double v_drift, int32_t* __restrict__ pair_of_a, int32_t* __restrict__ pair_of_c, float* __restrict__ t_out,
+                            float* __restrict__ zv_out, int32_t* __restrict__ n_pairs) {
+  const int nA = n_a[1], nC = n_c[1];
+  for (int j = 0; j < nC; j++) pair_of_c[j] = -1;
+  int np = 0;
+  for (int i = 0; i < nA; i++) {
+    const int j = best_c[i];
+    if (j >= 0 && best_a[j] == i) {
+      pair_of_a[i] = j;
+      pair_of_c[j] = i;
+      t_out[np] = (float)(((double)t_a[i] + (double)t_c[j]) * 0.5);
+      zv_out[np] = (float)((v_drift * ((double)t_c[j] - (double)t_a[i])) * 0.5);
+      np++;
+    } else {
+      pair_of_a[i] = -1;
+    }
+  }
+  n_pairs[0] = np;
+}
+
 }  // namespace
+
+size_t pair_sides_ws_bytes(int64_t max_collisions) { return 2 * align256(sizeof(int32_t) * (size_t)(max_collisions + 1)); }
+
+cudaError_t launch_pair_sides(const int32_t* n_a, const float* t_a, const int32_t* c_a, const int32_t* n_c, const float* t_c,
+                              const int32_t* c_c, int64_t max_collisions, double dt_max, double sigma_t, double v_drift,
+                              void* workspace, int32_t* pair_of_a, int32_t* pair_of_c, float* t_out, float* zv_out,
+                              int32_t* n_pairs, cudaStream_t st) {
+  int32_t* best_c = (int32_t*)workspace;
+  int32_t* best_a = (int32_t*)((char*)workspace + align256(sizeof(int32_t) * (size_t)(max_collisions + 1)));
+  const unsigned blocks = blocks_for(max_collisions, kThreads, 148 * 4);
+  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(0, n_a, t_a, c_a, n_c, t_c, c_c, dt_max, sigma_t, best_c)));
+  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(1, n_a, t_a, c_a, n_c, t_c, c_c, dt_max, sigma_t, best_a)));
+  TPC_LAUNCH(KID_COLLISIONS, st,
+             (k_pair_emit<<<1, 1, 0, st>>>(n_a, t_a, n_c, t_c, best_c, best_a, v_drift, pair_of_a, pair_of_c, t_out, zv_out, n_pairs)));
+  return cudaGetLastError();
+}
 
 size_t collisions_ws_bytes(int64_t nb, int64_t max_tracks) {
   size_t o = 0;

@@ -240,6 +240,12 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
                          int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
                          float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st);
 
+size_t pair_sides_ws_bytes(int64_t max_collisions);
+cudaError_t launch_pair_sides(const int32_t* n_a, const float* t_a, const int32_t* c_a, const int32_t* n_c, const float* t_c,
+                              const int32_t* c_c, int64_t max_collisions, double dt_max, double sigma_t, double v_drift,
+                              void* workspace, int32_t* pair_of_a, int32_t* pair_of_c, float* t_out, float* zv_out,
+                              int32_t* n_pairs, cudaStream_t st);
+
 // tpc_fit.cu (R28)
 cudaError_t launch_fit_physics(const Geo& g, float x0inv, float outlier_cut, const float* y, const float* z,
                                const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,

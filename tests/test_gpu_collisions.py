@@ -68,3 +68,31 @@ def test_collisions_argument_errors():
     out = C.c_size_t(0)
     assert L.tpc_collisions_workspace_bytes(C.c_int64(0), C.c_int64(10), C.byref(out)) == -1
     assert L.tpc_collisions_workspace_bytes(C.c_int64(100), C.c_int64(10), C.byref(out)) == 0 and out.value > 0
+
+
+def test_pair_sides_matches_oracle_and_truth(slice8, orc):
+    """R29: tpc_pair_sides on the two per-side collision lists equals the oracle's pairing, and the paired (t, z_vertex)
+    are the generator's for the collisions whose halves were both found (isolated ones)."""
+    import torch
+    from paper_2106_03636_b200 import binding
+    ev, res, g, t_lo, t_hi = slice8
+    trk = binding.Tracker(ev.params, ev.n)
+    trk.run(torch.from_numpy(ev.y).cuda(), torch.from_numpy(ev.z).cuda(), torch.from_numpy(ev.sector_row).cuda())
+    a = trk.find_collisions(t_lo, t_hi, V_DRIFT, side=1)
+    c = trk.find_collisions(t_lo, t_hi, V_DRIFT, side=-1)
+    p = trk.pair_sides()
+    o = orc.pair_sides(a["coll_time"], a["coll_ntracks"], c["coll_time"], c["coll_ntracks"])
+    for k in ("pair_of_a", "pair_of_c", "t", "z_vertex"):
+        assert np.array_equal(p[k], o[k]), k
+    assert p["t"].size >= 5
+    # against the generator: every isolated, well-populated collision comes back as a pair at its time and vertex
+    t_true = np.unique(ev.trk["t_us"])
+    ntrk = np.array([np.count_nonzero(ev.trk["t_us"] == t) for t in t_true])
+    vz = np.array([np.median(ev.trk["vz"][ev.trk["t_us"] == t]) for t in t_true])
+    gap = np.minimum(np.diff(t_true, prepend=-1e9), np.diff(t_true, append=1e9))
+    good = (gap > 25.0) & (ntrk >= 200)
+    assert good.sum() >= 3
+    for t, z in zip(t_true[good], vz[good]):
+        d = np.abs(p["t"] - t)
+        assert d.min() < 1.0, f"collision at {t:.1f} us has no pair (nearest {p['t'][d.argmin()]:.1f})"
+        assert abs(p["z_vertex"][d.argmin()] - z) < 2.0
