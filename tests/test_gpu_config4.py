@@ -34,6 +34,8 @@ def c4_run():
     res = trk.run(y, z, sr)
     assert res["status"] == 0, f"device status bits {res['status']}"
     work = binding.work_counts(res["counters"])
+    res["merge"] = trk.merge_tracks()                 # R26 on the whole Time Frame (invariants below)
+    res["tags"] = trk.tag_clusters(qpt_max=10.0)      # R28c
     del trk, y, z, sr
     torch.cuda.empty_cache()
     return ev, res, work
@@ -67,6 +69,34 @@ def test_c4_size_and_whole_output_invariants(c4_run):
     parity.check_output_invariants(res, ev.sector_row, int(ev.params.n_rows), int(ev.params.min_hits))
     # the follower's work is what scales: every recorded update is preceded by a transport
     assert work["propagations"] >= work["updates"] - int(res["counters"][1]) > 0
+
+
+def test_c4_merge_and_tags_invariants(c4_run):
+    """tpc_merge_tracks / tpc_tag_clusters at the full size (the oracle cannot merge 1.8e6 tracks in test time; it is
+    compared link for link on configs 0-3 in tests/test_gpu_merge.py): properties that hold at any size."""
+    ev, res, _ = c4_run
+    m, K = res["merge"], res["trk_seed"].size
+    succ, pred = m["trk_succ"], m["trk_pred"]
+    a = np.nonzero(succ >= 0)[0]
+    assert np.array_equal(pred[succ[a]], a), "succ and pred must be inverse to one another"
+    assert np.unique(succ[a]).size == a.size, "a track follows at most one track"
+    assert (pred >= 0).sum() == a.size == m["n_links"] and m["n_global"] == K - a.size
+    sec = res["trk_sector"]
+    rel_ok = (sec[a] == sec[succ[a]]) | (np.abs(sec[a] % 18 - sec[succ[a]] % 18) % 16 <= 1)
+    assert rel_ok.all(), "links only join a sector with itself, a neighbour or its mirror"
+    assert int(m["g_nhits"].sum()) == int(res["trk_nhits"].sum()) and int(m["g_nseg"].sum()) == K
+    assert np.array_equal(np.bincount(m["trk_global"], minlength=m["n_global"]), m["g_nseg"])
+    assert np.all(np.diff(m["g_head"]) > 0) and np.all(pred[m["g_head"]] < 0)
+    single = m["g_nseg"] == 1
+    assert np.array_equal(m["gpar"][:, single], res["par"][:, m["g_head"][single]])
+    merged_ok = (~single) & (m["gndf"] > 0)
+    assert merged_ok.sum() > 0.9 * (~single).sum()
+    assert 0.8 < np.median(m["gchi2"][merged_ok] / m["gndf"][merged_ok]) < 1.3
+    assert a.size > 0.3 * K, "about half of the sector-local tracks of a Time Frame are pieces of longer ones"
+    tags = res["tags"]
+    assert np.array_equal(tags > 0, res["cluster_track"] >= 0) and np.all(tags <= 3)
+    low = np.abs(res["par"][4]) > 10.0
+    assert np.array_equal((tags & 2) > 0, (res["cluster_track"] >= 0) & (low | (res["ndf"] < 0))[np.maximum(res["cluster_track"], 0)])
 
 
 @pytest.mark.parametrize("sector", SAMPLED_SECTORS)
