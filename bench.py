@@ -570,9 +570,15 @@ def kernel_roofline(name, ms, units, work, n_passes, peaks):
         n_units, fl = units["hit"] * n_passes, flops.fit_flop(units["hit"], n_passes)
     nominal = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     ach = fl / (ms * 1e-3) / 1e12
+    # SURVEY.md 8(d) asks for both views of the per-track kernels: the follower gathers ~100 bytes of 32-byte sectors
+    # per transport when nothing hits L2 (two bin-offset sectors, one or two cluster records, its row_hit entry); the
+    # refit streams 16 bytes per hit and pass
+    gather = (work["propagations"] * 100) if name == "k_follow" else (units["hit"] * n_passes * 16)
+    hbm_view = {"bound": "hbm", "algorithmic_bytes_per_step": gather, "achieved": gather / (ms * 1e-3) / 1e9,
+                "peak": peaks["hbm"], "unit": "GB/s", "frac": gather / (ms * 1e-3) / 1e9 / peaks["hbm"]}
     return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peaks["fp32"], "unit": "TFLOP/s", "frac": ach / peaks["fp32"],
             "traffic": None, "algorithmic_flop_per_step": fl, "units": n_units, "unit_kind": unit, "ms_per_step": ms,
-            "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
+            "peak_nominal": nominal, "frac_of_nominal": ach / nominal, "hbm_view": hbm_view,
             "peak_source": "measured in this run by tpc_fp32_peak (FFMA chains, 8 per thread); peak_nominal = 148 SMs x 128 "
                            f"lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz"}
 
