@@ -382,7 +382,7 @@ class Tracker:
         i32, f32 = t.int32, t.float32
         o = dict(trk_succ=t.empty(K, dtype=i32, device=dev), trk_pred=t.empty(K, dtype=i32, device=dev),
                  trk_succ_chi2=t.empty(K, dtype=f32, device=dev), trk_global=t.empty(K, dtype=i32, device=dev),
-                 n_global=t.zeros(2, dtype=i32, device=dev), g_head=t.empty(K, dtype=i32, device=dev),
+                 n_global=t.zeros(4, dtype=i32, device=dev), g_head=t.empty(K, dtype=i32, device=dev),
                  g_nseg=t.empty(K, dtype=i32, device=dev), g_nhits=t.empty(K, dtype=i32, device=dev),
                  gpar=t.empty((5, K), dtype=f32, device=dev), gcov=t.empty((15, K), dtype=f32, device=dev),
                  gxref=t.empty(K, dtype=f32, device=dev), gzref=t.empty(K, dtype=f32, device=dev),
@@ -407,12 +407,12 @@ class Tracker:
         self.merge_enqueue(**mp)
         o = self._merge["out"]
         k = int(self.counters[CNT_TRACKS].item())
-        m, links = (int(v) for v in o["n_global"].cpu().numpy())
+        m, links, pairs, dropped = (int(v) for v in o["n_global"].cpu().numpy())
         per_trk = ("trk_succ", "trk_pred", "trk_succ_chi2", "trk_global")
         res = {nm: o[nm][:k].cpu().numpy() for nm in per_trk}
         res.update({nm: (o[nm][:, :m] if o[nm].dim() == 2 else o[nm][:m]).cpu().numpy()
                     for nm in o if nm not in per_trk and nm != "n_global"})
-        res.update(n_global=m, n_links=links)
+        res.update(n_global=m, n_links=links, n_pairs=pairs, n_pairs_dropped=dropped)
         return res
 
     def pair_sides(self, dt_max: float = 15.5, sigma_t: float = 3.88, v_drift: float = 2.58):

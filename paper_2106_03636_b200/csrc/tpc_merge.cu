@@ -7,11 +7,15 @@
 //                    its inner end, bucket (sector, z slab, group of 8 first rows) of that end; bucket histogram
 //   k_merge_scatter  end records into bucket order (the order inside a bucket is irrelevant: every arg-min below
 //                    breaks ties by seed)
-//   k_merge_match    one thread per track A: outer state by R12, then every track B whose inner end lies in the
-//                    buckets the R26 windows can reach: row window, z window, rotation into B's frame, transport to
-//                    B's first hit, Cholesky chi2.  A keeps its best successor; every passing pair offers
-//                    (chi2, seed of A) to B by a 64-bit atomicMin -- B's best predecessor
-//   k_merge_link     A -> B is a link iff B's best predecessor is A (reciprocal arg-mins)
+//   k_merge_scan     one thread per track A: every track B whose inner end lies in the buckets the R26 windows can
+//                    reach is put to the tests that need no arithmetic on the states -- row window, z window,
+//                    (tanlambda, q/pT) gate -- on its 32-byte end record; the survivors (nearly always the true
+//                    continuation and nobody else) are appended to a pair list
+//   k_merge_eval     one thread per pair: A's outer state by R12, rotation into B's frame, transport to B's first
+//                    hit, Cholesky chi2; a pair under the cut offers (chi2, seed of B) to A and (chi2, seed of A) to
+//                    B by 64-bit atomicMin: the best successor / predecessor (ties: lowest seed)
+//   k_merge_link     one thread per pair: it is A's best successor iff A's key is its own; A -> B is a link iff B's
+//                    key is the pair's too (reciprocal arg-mins)
 //   k_merge_chains   heads (no predecessor) are numbered by a scan; each walks its chain: trk_global, pieces, hits;
 //                    a track without links keeps its sector-local fit
 //   k_merge_refit    one thread per merged chain: R22's two passes over the concatenated hit records, with the
@@ -24,6 +28,8 @@
 #include "tpc_kalman.cuh"
 #include "tpc_prof.cuh"
 #include "tpc_scan.cuh"
+
+#include <cstring>
 
 namespace tpc {
 
@@ -58,8 +64,13 @@ struct MergeWs {
   int32_t* bcursor;   // [nbuckets + 2]
   int32_t* rows;      // [K] first | last << 8 | sector << 16, track order
   float* z_in;        // [K]
-  int32_t* cand;      // [K] best candidate successor (before reciprocity)
+  unsigned long long* succ_key;  // [K] (chi2 bits << 32 | seed of the best successor)
   unsigned long long* pred_key;  // [K] (chi2 bits << 32 | seed of the best predecessor)
+  int32_t* pair_a;    // [pair_cap] pairs that passed the windows and the gate: track A,
+  int32_t* pair_b;    //            track B | relation << 28,
+  float* pair_chi2;   //            chi2 (-1: impossible or above the cut)
+  int32_t* n_pairs;   // [1]
+  int64_t pair_cap;
   int32_t* flag;      // [K + 1] head flags and their scan
   int32_t* mlist;     // [K] global tracks of more than one piece (any order); mlist[K] = their number
   int32_t* scan_tmp;
@@ -163,7 +174,7 @@ k_merge_ends(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict
     w.rows[k] = rf | (rl << 8) | (s << 16);
     w.z_in[k] = z;
     w.bucket[k] = b;
-    w.cand[k] = -1;
+    w.succ_key[k] = ~0ull;
     w.pred_key[k] = ~0ull;
     atomicAdd(w.bfirst + b, 1);
   }
@@ -221,16 +232,29 @@ __device__ __forceinline__ float pair_chi2(const KState& out, float x_a, float z
   return chi2_cholesky<5>(r.C, sbst.C, d, idx);
 }
 
-// One thread per track A.  The candidate loop applies only what needs no arithmetic on the states -- row window,
-// z window, (tanlambda, q/pT) gate -- to the 32-byte end records and keeps the survivors (nearly always the true
-// continuation and nobody else); the chi2 of the survivors is then formed in a second loop in which the lanes of a
-// warp work on their k-th survivor together.
-constexpr int kMaxSurv = 4;
+__device__ __forceinline__ unsigned long long chi2_key(float chi2, int seed) {
+  return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned long long)(unsigned)seed;  // chi2 >= 0: ordered as uint
+}
+
+// chi2 of one pair and its offers to both ends (R26 arbitration)
+__device__ __forceinline__ float eval_pair(const MergeP& mp, const float* sX, int a, int b, int rel, int rows_a, int rf_b,
+                                           const int32_t* __restrict__ trk_seed, const float* __restrict__ par,
+                                           const float* __restrict__ cov, const float* __restrict__ zref, int64_t max_tracks,
+                                           float kB, float ms, const MergeWs& w) {
+  const int rf_a = rows_a & 0xff, rl_a = (rows_a >> 8) & 0xff;
+  KState out;
+  load_state(out, par, cov, max_tracks, a);
+  if (rl_a != rf_a && !propagate(out, sX[rl_a] - sX[rf_a], kB, ms)) return -1.0f;
+  const float chi2 = pair_chi2(out, sX[rl_a], zref[a], rel, b, rf_b, sX, par, cov, zref, max_tracks, kB, ms, mp.ce_tol);
+  if (!(chi2 >= 0.0f) || !(chi2 < mp.chi2_cut)) return -1.0f;
+  atomicMin(w.succ_key + a, chi2_key(chi2, trk_seed[b]));
+  atomicMin(w.pred_key + b, chi2_key(chi2, trk_seed[a]));
+  return chi2;
+}
 
 __global__ void __launch_bounds__(kThreads)
-k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict__ counters, int64_t max_tracks,
-              const int32_t* __restrict__ trk_seed, const float* __restrict__ par, const float* __restrict__ cov,
-              const float* __restrict__ zref, MergeWs w, float* __restrict__ succ_chi2) {
+k_merge_scan(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restrict__ counters, int64_t max_tracks,
+             const int32_t* __restrict__ trk_seed, const float* __restrict__ par, const float* __restrict__ cov, const float* __restrict__ zref, MergeWs w) {
   __shared__ float sX[kMaxRows];
   const Scalars& sc = g.s;
   for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
@@ -242,95 +266,88 @@ k_merge_match(const __grid_constant__ Geo g, MergeP mp, const int32_t* __restric
   for (int64_t a = (int64_t)blockIdx.x * kThreads + threadIdx.x; a < K; a += (int64_t)gridDim.x * kThreads) {
     const int rows_a = w.rows[a];
     const int rf_a = rows_a & 0xff, rl_a = (rows_a >> 8) & 0xff, s_a = rows_a >> 16;
-    const unsigned long long seed_a = (unsigned long long)(unsigned)trk_seed[a];
-    const float zref_a = zref[a];
-    KState out;
-    load_state(out, par, cov, max_tracks, a);
-    int best_b = -1, best_seed = 0;
-    float best = 0.0f;
-    bool have_out = true;
-    if (rl_a != rf_a) have_out = propagate(out, sX[rl_a] - sX[rf_a], kB, ms);
-    const float x_a = sX[rl_a];
-    const float zA = zref_a + out.p[1];
-    int surv[kMaxSurv];     // track of the survivor | relation << 28 (tracks < 2^28 by the tracklet limit of 2^25)
-    int surv_rf[kMaxSurv];
-    int nsurv = 0;
-    auto evaluate = [&](int b, int rel, int rf_b, int seed_b) {
-      const float chi2 = pair_chi2(out, x_a, zref_a, rel, b, rf_b, sX, par, cov, zref, max_tracks, kB, ms, mp.ce_tol);
-      if (!(chi2 >= 0.0f) || !(chi2 < mp.chi2_cut)) return;
-      if (best_b < 0 || chi2 < best || (chi2 == best && seed_b < best_seed)) {
-        best_b = b;
-        best = chi2;
-        best_seed = seed_b;
-      }
-      atomicMin(w.pred_key + b, ((unsigned long long)__float_as_uint(chi2) << 32) | seed_a);
-    };
-    if (have_out) {
-      const int g0 = (rl_a + 1) >> 3;
-      int g1 = (rl_a + mp.max_rows) >> 3;
-      if (g1 > kRowGroups - 1) g1 = kRowGroups - 1;
-      for (int sb = 0; sb < sc.nsec && g0 <= g1; sb++) {
-        const int rel = sector_relation(s_a, sb);
-        if (rel == REL_NONE) continue;
-        // z of B's inner end: within dz_max of zA (same side) or of -zA (across the electrode); as zeta of B's side
-        const float zc = rel == REL_CE ? -zA : zA;
-        const float side_b = sb < 18 ? 1.0f : -1.0f;
-        const float za = (zc - (mp.dz_max + kSlabEps)) * side_b, zb = (zc + (mp.dz_max + kSlabEps)) * side_b;
-        const int s0 = slab_of(fminf(za, zb), sc.z_lo, mp.nslab), s1 = slab_of(fmaxf(za, zb), sc.z_lo, mp.nslab);
-        for (int sl = s0; sl <= s1; sl++) {
-          // first rows rl_a + 1 .. rl_a + max_rows: a contiguous run of row groups inside every (sector, slab)
-          const int bb = (sb * mp.nslab + sl) * kRowGroups;
-          const int e0 = w.bfirst[bb + g0], e1 = w.bfirst[bb + g1 + 1];
-          for (int e = e0; e < e1; e++) {
-            const float4 er = __ldg(reinterpret_cast<const float4*>(w.ends + e));
-            const int rows_b = __float_as_int(er.y), b = __float_as_int(er.w);
-            const int rf_b = rows_b & 0xff;
-            const int dr = rf_b - rl_a;
-            if (dr < 1 || dr > mp.max_rows || b == (int)a) continue;
-            const float zB = er.x;
-            if (rel == REL_CE ? !(fabsf(zB + zA) <= mp.dz_max) : !(fabsf(zB - zA) <= mp.dz_max)) continue;
-            const float4 gt = __ldg(reinterpret_cast<const float4*>(w.ends + e) + 1);
-            const float d3 = out.p[3] - gt.x, d4 = out.p[4] - gt.y;
-            const float s33 = out.C[TPC_CI(3, 3)] + gt.z, s44 = out.C[TPC_CI(4, 4)] + gt.w;
-            if (!(d3 * d3 <= gate * s33) || !(d4 * d4 <= gate * s44)) continue;
-            if (nsurv < kMaxSurv) {
-              surv[nsurv] = b | (rel << 28);
-              surv_rf[nsurv] = rf_b;
-              nsurv++;
-            } else {
-              evaluate(b, rel, rf_b, __float_as_int(er.z));
-            }
-          }
+    // what the tests need of A's outer state: dz (transported), tanlambda and q/pT with their variances (unchanged by R12)
+    float dz_out = par[1 * max_tracks + a];
+    const float tl_a = par[3 * max_tracks + a], q_a = par[4 * max_tracks + a];
+    const float c33_a = cov[TPC_CI(3, 3) * max_tracks + a], c44_a = cov[TPC_CI(4, 4) * max_tracks + a];
+    if (rl_a != rf_a) {
+      KState st;
+      load_state(st, par, cov, max_tracks, a);
+      Transport T;
+      if (!transport_state(st, sX[rl_a] - sX[rf_a], kB, ms, T)) continue;  // no outer state: A has no successor
+      dz_out = T.dz;
+    }
+    const float zA = zref[a] + dz_out;
+    const int g0 = (rl_a + 1) >> 3;
+    int g1 = (rl_a + mp.max_rows) >> 3;
+    if (g1 > kRowGroups - 1) g1 = kRowGroups - 1;
+    if (g0 > g1) continue;
+    for (int sb = 0; sb < sc.nsec; sb++) {
+      const int rel = sector_relation(s_a, sb);
+      if (rel == REL_NONE) continue;
+      // z of B's inner end: within dz_max of zA (same side) or of -zA (across the electrode); as zeta of B's side
+      const float zc = rel == REL_CE ? -zA : zA;
+      const float side_b = sb < 18 ? 1.0f : -1.0f;
+      const float za = (zc - (mp.dz_max + kSlabEps)) * side_b, zb = (zc + (mp.dz_max + kSlabEps)) * side_b;
+      const int s0 = slab_of(fminf(za, zb), sc.z_lo, mp.nslab), s1 = slab_of(fmaxf(za, zb), sc.z_lo, mp.nslab);
+      for (int sl = s0; sl <= s1; sl++) {
+        // first rows rl_a + 1 .. rl_a + max_rows: a contiguous run of row groups inside every (sector, slab)
+        const int bb = (sb * mp.nslab + sl) * kRowGroups;
+        const int e0 = w.bfirst[bb + g0], e1 = w.bfirst[bb + g1 + 1];
+        for (int e = e0; e < e1; e++) {
+          const float4 er = __ldg(reinterpret_cast<const float4*>(w.ends + e));
+          const int rows_b = __float_as_int(er.y), b = __float_as_int(er.w);
+          const int rf_b = rows_b & 0xff;
+          const int dr = rf_b - rl_a;
+          if (dr < 1 || dr > mp.max_rows || b == (int)a) continue;
+          const float zB = er.x;
+          if (rel == REL_CE ? !(fabsf(zB + zA) <= mp.dz_max) : !(fabsf(zB - zA) <= mp.dz_max)) continue;
+          const float4 gt = __ldg(reinterpret_cast<const float4*>(w.ends + e) + 1);
+          const float d3 = tl_a - gt.x, d4 = q_a - gt.y;
+          if (!(d3 * d3 <= gate * (c33_a + gt.z)) || !(d4 * d4 <= gate * (c44_a + gt.w))) continue;
+          const int slot = atomicAdd(w.n_pairs, 1);
+          if (slot < w.pair_cap) {
+            w.pair_a[slot] = (int)a;
+            w.pair_b[slot] = b | (rel << 28);
+          }  // else: list full (4 survivors per track on average: never seen); counted in n_global[3]
         }
       }
     }
-    for (int k = 0; k < kMaxSurv; k++) {
-      if (k < nsurv) {
-        const int b = surv[k] & 0x0fffffff, rel = surv[k] >> 28;
-        evaluate(b, rel, surv_rf[k] & 0xff, trk_seed[b]);
-      }
-    }
-    w.cand[a] = best_b;
-    succ_chi2[a] = best_b >= 0 ? best : -1.0f;
   }
 }
 
 __global__ void __launch_bounds__(kThreads)
-k_merge_link(const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_seed, MergeWs w,
-             const float* __restrict__ succ_chi2, int32_t* __restrict__ succ, int32_t* __restrict__ pred) {
-  int64_t K = counters[TPC_CNT_TRACKS];
-  if (K > max_tracks) K = max_tracks;
-  for (int64_t a = (int64_t)blockIdx.x * kThreads + threadIdx.x; a < K; a += (int64_t)gridDim.x * kThreads) {
-    const int b = w.cand[a];
-    int s = -1;
-    if (b >= 0) {
-      const unsigned long long key = ((unsigned long long)__float_as_uint(succ_chi2[a]) << 32) | (unsigned long long)(unsigned)trk_seed[a];
-      if (w.pred_key[b] == key) {
-        s = b;
-        pred[b] = (int)a;  // at most one track passes this test for b
-      }
+k_merge_eval(const __grid_constant__ Geo g, MergeP mp, int64_t max_tracks, const int32_t* __restrict__ trk_seed,
+             const float* __restrict__ par, const float* __restrict__ cov, const float* __restrict__ zref, MergeWs w) {
+  __shared__ float sX[kMaxRows];
+  const Scalars& sc = g.s;
+  for (int r = threadIdx.x; r < sc.nrows; r += blockDim.x) sX[r] = g.row.X[r];
+  __syncthreads();
+  int64_t np = w.n_pairs[0];
+  if (np > w.pair_cap) np = w.pair_cap;
+  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < np; i += (int64_t)gridDim.x * kThreads) {
+    const int a = w.pair_a[i], pb = w.pair_b[i];
+    const int b = pb & 0x0fffffff, rel = pb >> 28;
+    w.pair_chi2[i] = eval_pair(mp, sX, a, b, rel, w.rows[a], w.rows[b] & 0xff, trk_seed, par, cov, zref, max_tracks, sc.kB,
+                               sc.max_sinphi, w);
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_merge_link(const int32_t* __restrict__ trk_seed, MergeWs w, float* __restrict__ succ_chi2, int32_t* __restrict__ succ,
+             int32_t* __restrict__ pred) {
+  int64_t np = w.n_pairs[0];
+  if (np > w.pair_cap) np = w.pair_cap;
+  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < np; i += (int64_t)gridDim.x * kThreads) {
+    const float chi2 = w.pair_chi2[i];
+    if (!(chi2 >= 0.0f)) continue;
+    const int a = w.pair_a[i], b = w.pair_b[i] & 0x0fffffff;
+    if (w.succ_key[a] != chi2_key(chi2, trk_seed[b])) continue;
+    succ_chi2[a] = chi2;  // B is A's best candidate successor ...
+    if (w.pred_key[b] == chi2_key(chi2, trk_seed[a])) {  // ... and A is B's best candidate predecessor: a link
+      succ[a] = b;
+      pred[b] = a;
     }
-    succ[a] = s;
   }
 }
 
@@ -350,12 +367,14 @@ k_merge_chains(const int32_t* __restrict__ counters, int64_t max_tracks, const i
                int32_t* __restrict__ trk_global, int32_t* __restrict__ n_global, int32_t* __restrict__ g_head,
                int32_t* __restrict__ g_nseg, int32_t* __restrict__ g_nhits, float* __restrict__ gpar, float* __restrict__ gcov,
                float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2, int32_t* __restrict__ gndf,
-               int32_t* __restrict__ mlist) {
+               int32_t* __restrict__ mlist, const int32_t* __restrict__ n_pairs, int64_t pair_cap) {
   int64_t K = counters[TPC_CNT_TRACKS];
   if (K > max_tracks) K = max_tracks;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     n_global[0] = scan[max_tracks];
     n_global[1] = (int)K - scan[max_tracks];  // links
+    n_global[2] = n_pairs[0];                 // pairs that passed the windows and the gate
+    n_global[3] = n_pairs[0] > pair_cap ? (int)(n_pairs[0] - pair_cap) : 0;  // ... of which not tested (list full)
   }
   for (int64_t h = (int64_t)blockIdx.x * kThreads + threadIdx.x; h < K; h += (int64_t)gridDim.x * kThreads) {
     if (pred[h] >= 0) continue;
@@ -479,6 +498,14 @@ k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_globa
   }
 }
 
+__global__ void __launch_bounds__(256) k_fill_u32(unsigned* p, unsigned v, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) p[i] = v;
+}
+inline cudaError_t cudaMemsetD32Async_compat(void* p, unsigned v, size_t n, cudaStream_t st) {
+  k_fill_u32<<<blocks_for((int64_t)n, 256, 148 * 8), 256, 0, st>>>((unsigned*)p, v, n);
+  return cudaGetLastError();
+}
+
 inline int merge_nslab(const Geo& g) {
   int n = (int)ceilf((g.s.z_hi - g.s.z_lo) / kSlabCm) + 1;
   if (n < 1) n = 1;
@@ -487,7 +514,8 @@ inline int merge_nslab(const Geo& g) {
 }
 
 struct MergeLayout {
-  size_t off_ends, off_bucket, off_bfirst, off_bcursor, off_rows, off_z, off_cand, off_key, off_flag, off_mlist, off_tmp, total;
+  size_t off_ends, off_bucket, off_bfirst, off_bcursor, off_rows, off_z, off_skey, off_key, off_flag, off_mlist, off_pa, off_pb, off_pc, off_np, off_tmp, total;
+  int64_t pair_cap;
   int64_t nbuckets;
 };
 
@@ -507,10 +535,15 @@ inline MergeLayout merge_layout(int nsec, int nslab, int64_t max_tracks) {
   L.off_bcursor = take(sizeof(int32_t) * (size_t)(L.nbuckets + 2));
   L.off_rows = take(sizeof(int32_t) * K);
   L.off_z = take(sizeof(float) * K);
-  L.off_cand = take(sizeof(int32_t) * K);
+  L.off_skey = take(sizeof(unsigned long long) * K);
   L.off_key = take(sizeof(unsigned long long) * K);
   L.off_flag = take(sizeof(int32_t) * (K + 1));
   L.off_mlist = take(sizeof(int32_t) * (K + 1));
+  L.pair_cap = 4 * max_tracks;  // pairs that pass the windows and the gate: one or two per track that has any
+  L.off_pa = take(sizeof(int32_t) * (size_t)L.pair_cap);
+  L.off_pb = take(sizeof(int32_t) * (size_t)L.pair_cap);
+  L.off_pc = take(sizeof(float) * (size_t)L.pair_cap);
+  L.off_np = take(sizeof(int32_t) * 4);
   const int64_t longest = (int64_t)K + 1 > L.nbuckets + 2 ? (int64_t)K + 1 : L.nbuckets + 2;
   L.off_tmp = take(sizeof(int64_t) * (size_t)((longest + kScanTile - 1) / kScanTile + 2));
   L.total = o;
@@ -543,7 +576,12 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
   w.bcursor = (int32_t*)(b + L.off_bcursor);
   w.rows = (int32_t*)(b + L.off_rows);
   w.z_in = (float*)(b + L.off_z);
-  w.cand = (int32_t*)(b + L.off_cand);
+  w.succ_key = (unsigned long long*)(b + L.off_skey);
+  w.pair_a = (int32_t*)(b + L.off_pa);
+  w.pair_b = (int32_t*)(b + L.off_pb);
+  w.pair_chi2 = (float*)(b + L.off_pc);
+  w.n_pairs = (int32_t*)(b + L.off_np);
+  w.pair_cap = L.pair_cap;
   w.pred_key = (unsigned long long*)(b + L.off_key);
   w.flag = (int32_t*)(b + L.off_flag);
   w.mlist = (int32_t*)(b + L.off_mlist);
@@ -561,16 +599,24 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
       cudaSuccess)
     return e;
   TPC_LAUNCH(KID_MERGE, st, (k_merge_scatter<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, par, cov, w)));
-  TPC_LAUNCH(KID_MERGE, st,
-             (k_merge_match<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, par, cov, zref, w, trk_succ_chi2)));
-  TPC_LAUNCH(KID_MERGE, st,
-             (k_merge_link<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_seed, w, trk_succ_chi2, trk_succ, trk_pred)));
+  if ((e = cudaMemsetAsync(w.n_pairs, 0, sizeof(int32_t), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(trk_succ, 0xFF, sizeof(int32_t) * (size_t)max_tracks, st)) != cudaSuccess) return e;
+  {
+    const float minus1 = -1.0f;
+    unsigned bits;
+    memcpy(&bits, &minus1, sizeof(bits));
+    if ((e = cudaMemsetD32Async_compat(trk_succ_chi2, bits, (size_t)max_tracks, st)) != cudaSuccess) return e;
+  }
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_scan<<<blocks, kThreads, 0, st>>>(g, mp, counters, max_tracks, trk_seed, par, cov, zref, w)));
+  const unsigned pblocks = blocks_for(L.pair_cap, kThreads, 148 * 16);
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_eval<<<pblocks, kThreads, 0, st>>>(g, mp, max_tracks, trk_seed, par, cov, zref, w)));
+  TPC_LAUNCH(KID_MERGE, st, (k_merge_link<<<pblocks, kThreads, 0, st>>>(trk_seed, w, trk_succ_chi2, trk_succ, trk_pred)));
   TPC_LAUNCH(KID_MERGE, st, (k_merge_heads<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_pred, w.flag)));
   if ((e = exclusive_scan<int32_t>(w.flag, w.flag, max_tracks + 1, w.scan_tmp, st)) != cudaSuccess) return e;
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_chains<<<blocks, kThreads, 0, st>>>(counters, max_tracks, trk_nhits, par, cov, xref, zref, chi2, ndf, trk_succ,
                                                          trk_pred, w.flag, trk_global, n_global, g_head, g_nseg, g_nhits, gpar,
-                                                         gcov, gxref, gzref, gchi2, gndf, w.mlist)));
+                                                         gcov, gxref, gzref, gchi2, gndf, w.mlist, w.n_pairs, w.pair_cap)));
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_refit<<<blocks, kThreads, 0, st>>>(g, n_global, max_tracks, trk_sector, trk_nhits, trk_first_hit, fw.hit_rec,
                                                         par, zref, trk_succ, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref,
