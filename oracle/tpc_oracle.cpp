@@ -20,6 +20,13 @@
 //   orc_propagate / orc_update   the R12 / R13 primitives, exported for the pins (I7)
 //   orc_beamline    R24     closest approach of a fitted helix to the beam line, z there, time offset
 //   orc_collisions  R25     collisions as peaks of the per-track time offsets; track -> collision
+//   orc_merge_match / orc_merge_fit  R26  links between sector-local tracks (sector edges, central electrode, long
+//                           holes) by a 5-parameter chi2, reciprocal arg-mins; refit of the merged hit lists
+//   orc_clusterize  R27     clusters from zero-suppressed digits: peaks in (pad, time), 3 x 3 centre of gravity
+//   orc_fit_physics / orc_tag_clusters  R28  refit with multiple-scattering process noise and outlier rejection;
+//                           per-cluster tags for a compression step
+//   orc_pair_sides  R29     pairing of the two TPC sides' collisions into (t, z_vertex)
+//   orc_set_arith, orc_decisions_begin/end   arithmetic contract switch and the follower's decision log (near-tie report)
 //
 // Every function exists for real_t = float (suffix _f32: reproduces the GPU's arithmetic: one IEEE
 // operation per written operation -- build with -ffp-contract=off -- where mad(a, b, c) is the IEEE
@@ -33,7 +40,9 @@
 //
 // Pins (-m "not gpu"): tests/test_oracle_pins.py (I1-I10 of SURVEY.md §8(c)), tests/test_oracle_r17.py (R17: the
 // wave test line by line, the wave loop, the three R17 modes measured against one another, configs[0] against the
-// stored summary), tests/test_oracle_beamline.py (R24), tests/test_oracle_collisions.py (R25).  Track count,
+// stored summary), tests/test_oracle_arith.py (the fused arithmetic term by term, one rounding against the other, the
+// near-tie report), tests/test_oracle_beamline.py (R24), tests/test_oracle_collisions.py (R25, R29),
+// tests/test_oracle_merge.py (R26), tests/test_oracle_clusterizer.py (R27), tests/test_oracle_physics.py (R28).  Track count,
 // efficiency and fake rate themselves are "parity unpinned" by the paper (it publishes no number
 // for any synthetic workload); they are fixed only by oracle == GPU.
 // =============================================================================================
