@@ -123,3 +123,24 @@ def test_cluster_tags(orc):
     tag = orc.tag_clusters(ct, qpt, ndf, nh, fh, hits, flag, qpt_max=10.0)
     assert tag.tolist() == [0, 1, 1 | 4, 1 | 2, 1 | 2, 1 | 2, 0, 1 | 2]
     assert orc.tag_clusters(ct, qpt, ndf, nh, fh, hits, None, qpt_max=20.0).tolist() == [0, 1, 1, 1, 1, 3, 0, 3]
+
+
+def test_tags_single_out_the_low_pt_loopers_of_a_pileup_event(orc):
+    """R28c against the generator's truth on a configs[3]-like event (10 % of the particles are loopers with
+    pT 0.05-0.2 GeV, A2): with qpt_max = 1 / (0.2 GeV) the clusters tagged "not used for physics" are, almost all of them,
+    clusters of true low-pT particles, and most attached clusters of such particles are tagged."""
+    from paper_2106_03636_b200.synth import config3
+    ev = config3(n_coll=1, n_tracks=1500)
+    o = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)
+    tag = orc.tag_clusters(o["cluster_track"], o["par"][4], o["ndf"], o["trk_nhits"], o["trk_first_hit"], o["trk_hits"], None,
+                           qpt_max=5.0)
+    tt = ev.true_track
+    pt_true = np.where(tt >= 0, 1.0 / np.abs(ev.trk["qpt"][np.maximum(tt, 0)]), np.inf)
+    attached = tag & 1 > 0
+    removable = tag & 2 > 0
+    low = (tt >= 0) & (pt_true < 0.2)
+    high = (tt >= 0) & (pt_true > 0.3)
+    assert low.sum() > 2000 and (attached & low).sum() > 500
+    assert (removable & low & attached).sum() >= 0.85 * (attached & low).sum(), "attached looper clusters that escape the tag"
+    assert (removable & high).sum() <= 0.01 * (attached & high).sum(), "clusters of physics tracks tagged for removal"
+    assert not (removable & ~attached).any()
