@@ -98,3 +98,23 @@ def test_binding_refuses_cpu_tensors():
     import torch
     with pytest.raises(binding.TpcError):
         binding._dp(torch.zeros(4))
+
+
+@pytest.mark.parametrize("name,mirror", [("tpc_result_t", "tpc_result_t"), ("tpc_merge_params_t", "tpc_merge_params_t"),
+                                         ("tpc_merged_t", "tpc_merged_t")])
+def test_other_struct_layouts_match_header(name, mirror):
+    """Field order of the ctypes mirrors == the header's typedefs (pointer structs: one pointer per member)."""
+    txt = open(HEADER).read()
+    body = re.search(r"typedef struct \{((?:(?!typedef struct).)*?)\} " + name + ";", txt, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if decl:
+            fields.append(decl.split()[-1].lstrip("*"))
+    cls = getattr(binding, mirror)
+    assert fields == [f[0] for f in cls._fields_]
+    if name != "tpc_merge_params_t":
+        assert C.sizeof(cls) == 8 * len(fields)
+    else:
+        assert C.sizeof(cls) == 16
