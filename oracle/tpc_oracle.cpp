@@ -23,8 +23,8 @@
 //   orc_merge_match / orc_merge_fit  R26  links between sector-local tracks (sector edges, central electrode, long
 //                           holes) by a 5-parameter chi2, reciprocal arg-mins; refit of the merged hit lists
 //   orc_clusterize  R27     clusters from zero-suppressed digits: peaks in (pad, time), 3 x 3 centre of gravity
-//   orc_fit_physics / orc_tag_clusters  R28  refit with multiple-scattering process noise and outlier rejection;
-//                           per-cluster tags for a compression step
+//   orc_fit_physics / orc_tag_clusters  R28  refit with multiple-scattering process noise, outlier rejection, mean
+//                           energy loss, angle- and drift-dependent cluster errors; per-cluster tags for a compression step
 //   orc_pair_sides  R29     pairing of the two TPC sides' collisions into (t, z_vertex)
 //   orc_set_arith, orc_decisions_begin/end   arithmetic contract switch and the follower's decision log (near-tie report)
 //
@@ -1434,12 +1434,25 @@ ORC_API int64_t orc_clusterize(const OrcParams* P, int64_t n, const int32_t* sr,
 //        x0inv = 0 (the synthetic events have no material) reproduces R22 bit for bit.
 //   R28b outlier rejection.  In the LAST pass a hit whose chi2 against the predicted state exceeds outlier_cut is not
 //        used: no update, hit_flag = 1, ndf loses 2.  outlier_cut <= 0 switches it off.
+//   R28d energy loss.  After every transport (after R28a) the momentum changes by the mean loss dedx (GeV / cm of path,
+//        beta = 1) over the path L:  dp/p = -dedx L / p = -dedx |arc| |q|  (p = sqrt(1 + tl^2) / |q|, L = |arc| sqrt(1 + tl^2)),
+//        to first order  dq = (dedx |arc| |q|) q;  a track is taken to fly outward, so the outward passes lose momentum,
+//        q' = q + dq, and the inward passes gain it back, q' = q - dq.  Straggling: C44 += (eloss_sigma dq)^2.
+//        dedx = 0 reproduces R28a bit for bit.
+//   R28e cluster errors.  At every hit, from the PREDICTED state (s, tl) and the hit's drift length d:
+//        sigma_y^2 = sy2 (1 + err_ang_y s^2 / (1 - s^2)) + err_drift_y d,   sigma_z^2 = sz2 (1 + err_ang_z tl^2) + err_drift_z d
+//        d = max(0, z_len - |z + side v_drift t0|) with the track's time offset t0 of R24 (R5: z_true = z + side v_d t);
+//        without trk_t0 (NULL, or a NaN entry) the drift terms are left out.  Used by the outlier test and the update alike.
+//        All four coefficients 0 reproduce R28a/b bit for bit.
 //   R28c cluster tags (what a compression step would drop): per cluster, bit 0 = attached to a track; bit 1 = that
 //        track is not used for physics: its refit failed (ndf < 0) or |q/pT| > qpt_max (low-pT loopers);
 //        bit 2 = the hit was rejected by R28b.  An unattached cluster has tag 0.
 // ---------------------------------------------------------------------------------------------
 struct OrcFitOptions {
   double x0inv, outlier_cut;
+  double dedx, eloss_sigma;
+  double err_ang_y, err_ang_z, err_drift_y, err_drift_z;
+  double v_drift, z_len;
 };
 
 template <class T>
@@ -1457,10 +1470,45 @@ void add_scattering(State<T>& st, T arc, T x0inv) {
   st.C[4][4] = st.C[4][4] + ((th2 * tl) * tl) * (q * q);
 }
 
-// fit_one (R21-R22) with the R28 options; hit_flag[n] receives 1 for hits rejected in the last pass
+// R28d: mean energy loss over |arc| (dir = +1 outward: momentum is lost; -1 inward: gained back) and its straggling
+template <class T>
+void add_energy_loss(State<T>& st, T arc, int dir, T dedx, T eloss_sigma) {
+  if (!(dedx > (T)0)) return;
+  const T q = st.p[4];
+  const T rel = (dedx * std::fabs(arc)) * std::fabs(q);
+  const T dq = rel * q;
+  st.p[4] = dir > 0 ? q + dq : q - dq;
+  st.C[4][4] = st.C[4][4] + (eloss_sigma * dq) * (eloss_sigma * dq);
+}
+
+// R28e: the two measurement variances at a hit of raw z, for the predicted state st; zs = side v_drift t0
+template <class T>
+void cluster_errors(const State<T>& st, const OrcFitOptions& O, T sy2, T sz2, bool have_d, T z_raw, T zs, T* sy2h, T* sz2h) {
+  T ey = sy2, ez = sz2;
+  if (O.err_ang_y > 0) {
+    const T s = st.p[2];
+    const T tan2 = (s * s) / ((T)1 - s * s);
+    ey = ey * ((T)1 + (T)O.err_ang_y * tan2);
+  }
+  if (O.err_ang_z > 0) {
+    const T tl = st.p[3];
+    ez = ez * ((T)1 + (T)O.err_ang_z * (tl * tl));
+  }
+  if (have_d) {
+    T d = (T)O.z_len - std::fabs(z_raw + zs);
+    if (d < (T)0) d = 0;
+    if (O.err_drift_y > 0) ey = ey + (T)O.err_drift_y * d;
+    if (O.err_drift_z > 0) ez = ez + (T)O.err_drift_z * d;
+  }
+  *sy2h = ey;
+  *sz2h = ez;
+}
+
+// fit_one (R21-R22) with the R28 options; hit_flag[n] receives 1 for hits rejected in the last pass; t0 = the track's
+// time offset (R24) or NaN
 template <class T>
 bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G, const Clusters<T>& cl, const int32_t* hits,
-                     int n, T* par, T* cov, T* xref, T* zref_out, T* chi2_out, int32_t* ndf, uint8_t* hit_flag) {
+                     int n, T t0, T* par, T* cov, T* xref, T* zref_out, T* chi2_out, int32_t* ndf, uint8_t* hit_flag) {
   const int32_t a = hits[0], b = hits[n / 2], c = hits[n - 1];
   const T x1 = G.X[cl.row(a)], y1 = cl.y[a], x2 = G.X[cl.row(b)], y2 = cl.y[b], x3 = G.X[cl.row(c)], y3 = cl.y[c];
   const T cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
@@ -1482,6 +1530,9 @@ bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G
   int at = 0, nrej = 0;
   bool ok = true;
   for (int i = 0; i < n; i++) hit_flag[i] = 0;
+  const bool have_d = t0 == t0;
+  const T side = cl.sector(a) < 18 ? (T)1 : (T)-1;
+  const T zs = have_d ? side * ((T)O.v_drift * t0) : (T)0;
   for (int pass = 0; pass < P.n_fit_passes && ok; pass++) {
     reset_cov(st, P);
     chi2 = 0;
@@ -1501,10 +1552,13 @@ bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G
         const T Lc = dxk * std::sqrt(mad(t, t, (T)1));
         const T arc = Lc * asin_ratio((kap * Lc) * (T)0.5);
         add_scattering(st, arc, (T)O.x0inv);
+        add_energy_loss(st, arc, dir, (T)O.dedx, (T)O.eloss_sigma);
         at = k;
       }
+      T sy2h, sz2h;
+      cluster_errors(st, O, G.sy2, G.sz2, have_d, cl.z[h], zs, &sy2h, &sz2h);
       if (last && O.outlier_cut > 0) {
-        const Innov<T> I = innovation(st, G.sy2, G.sz2);
+        const Innov<T> I = innovation(st, sy2h, sz2h);
         const T c2h = chi2_of(I, cl.y[h] - st.p[0], (cl.z[h] - zref) - st.p[1]);
         if (c2h > (T)O.outlier_cut) {
           hit_flag[k] = 1;
@@ -1512,7 +1566,7 @@ bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G
           continue;
         }
       }
-      chi2 += update(st, cl.y[h], cl.z[h] - zref, G.sy2, G.sz2);
+      chi2 += update(st, cl.y[h], cl.z[h] - zref, sy2h, sz2h);
     }
   }
   for (int i = 0; i < 5; i++) par[i] = st.p[i];
@@ -1527,14 +1581,15 @@ bool fit_one_physics(const OrcParams& P, const OrcFitOptions& O, const Geo<T>& G
 
 template <class T>
 void fit_physics_impl(const OrcParams* P, const OrcFitOptions* O, int64_t n, const T* y, const T* z, const int32_t* sr, int64_t K,
-                      const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, T* par, T* cov, T* xref,
-                      T* zref, T* chi2, int32_t* ndf, uint8_t* hit_flag) {
+                      const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits, const T* trk_t0, T* par,
+                      T* cov, T* xref, T* zref, T* chi2, int32_t* ndf, uint8_t* hit_flag) {
   OrcParams Pp = *P;
   Geo<T> G(Pp);
   Clusters<T> cl{n, y, z, sr, Pp.n_rows};
+  const T nan = std::nan("");
   for (int64_t k = 0; k < K; k++) {
     T p5[5], c15[15];
-    fit_one_physics(Pp, *O, G, cl, trk_hits + trk_first_hit[k], trk_nhits[k], p5, c15, xref + k, zref + k, chi2 + k, ndf + k,
+    fit_one_physics(Pp, *O, G, cl, trk_hits + trk_first_hit[k], trk_nhits[k], trk_t0 ? trk_t0[k] : nan, p5, c15, xref + k, zref + k, chi2 + k, ndf + k,
                     hit_flag + trk_first_hit[k]);
     for (int i = 0; i < 5; i++) par[i * K + k] = p5[i];
     for (int i = 0; i < 15; i++) cov[i * K + k] = c15[i];
@@ -1543,15 +1598,15 @@ void fit_physics_impl(const OrcParams* P, const OrcFitOptions* O, int64_t n, con
 
 ORC_API void orc_fit_physics_f32(const OrcParams* P, const OrcFitOptions* O, int64_t n, const float* y, const float* z,
                                  const int32_t* sr, int64_t K, const int32_t* trk_nhits, const int64_t* trk_first_hit,
-                                 const int32_t* trk_hits, float* par, float* cov, float* xref, float* zref, float* chi2,
-                                 int32_t* ndf, uint8_t* hit_flag) {
-  fit_physics_impl<float>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag);
+                                 const int32_t* trk_hits, const float* trk_t0, float* par, float* cov, float* xref, float* zref,
+                                 float* chi2, int32_t* ndf, uint8_t* hit_flag) {
+  fit_physics_impl<float>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, trk_t0, par, cov, xref, zref, chi2, ndf, hit_flag);
 }
 ORC_API void orc_fit_physics_f64(const OrcParams* P, const OrcFitOptions* O, int64_t n, const double* y, const double* z,
                                  const int32_t* sr, int64_t K, const int32_t* trk_nhits, const int64_t* trk_first_hit,
-                                 const int32_t* trk_hits, double* par, double* cov, double* xref, double* zref, double* chi2,
-                                 int32_t* ndf, uint8_t* hit_flag) {
-  fit_physics_impl<double>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag);
+                                 const int32_t* trk_hits, const double* trk_t0, double* par, double* cov, double* xref,
+                                 double* zref, double* chi2, int32_t* ndf, uint8_t* hit_flag) {
+  fit_physics_impl<double>(P, O, n, y, z, sr, K, trk_nhits, trk_first_hit, trk_hits, trk_t0, par, cov, xref, zref, chi2, ndf, hit_flag);
 }
 // R28c: tag[n] from cluster_track[n], the per-track q/pT (par row 4, leading dimension ldp) and ndf, and hit_flag in
 // hit-list order (may be NULL)

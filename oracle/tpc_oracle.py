@@ -404,16 +404,22 @@ def merge(p, y, z, sector_row, o, mp=None, precision="f32", want_pairs=False):
 
 
 class OrcFitOptions(C.Structure):
-    _fields_ = [("x0inv", C.c_double), ("outlier_cut", C.c_double)]
+    _fields_ = [(nm, C.c_double) for nm in ("x0inv", "outlier_cut", "dedx", "eloss_sigma", "err_ang_y", "err_ang_z",
+                                            "err_drift_y", "err_drift_z", "v_drift", "z_len")]
 
 
-def fit_physics(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, x0inv=0.0, outlier_cut=0.0, precision="f32"):
-    """R21-R22 with the R28 options (process noise per unit path, outlier rejection in the last pass):
+def fit_physics(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, x0inv=0.0, outlier_cut=0.0, precision="f32",
+                dedx=0.0, eloss_sigma=0.0, err_ang_y=0.0, err_ang_z=0.0, err_drift_y=0.0, err_drift_z=0.0, v_drift=0.0,
+                z_len=250.0, trk_t0=None):
+    """R21-R22 with the R28 options (a: scattering noise per unit path, b: outlier rejection in the last pass, d: mean
+    energy loss, e: angle- and drift-dependent cluster errors; trk_t0 = R24's time offsets for the drift length):
     dict(par, cov, xref, zref, chi2, ndf, hit_flag[n_hits])."""
     rt, sfx = _real(precision)
     P = make_params(p, precision)
     rnd = (lambda v: float(np.float32(v))) if precision == "f32" else float
-    O = OrcFitOptions(rnd(x0inv), rnd(outlier_cut))
+    O = OrcFitOptions(*[rnd(v) for v in (x0inv, outlier_cut, dedx, eloss_sigma, err_ang_y, err_ang_z, err_drift_y, err_drift_z,
+                                         v_drift, z_len)])
+    t0 = None if trk_t0 is None else np.ascontiguousarray(trk_t0, rt)
     y = np.ascontiguousarray(y, rt); z = np.ascontiguousarray(z, rt); sr = np.ascontiguousarray(sector_row, np.int32)
     nh = np.ascontiguousarray(trk_nhits, np.int32); fh = np.ascontiguousarray(trk_first_hit, np.int64)
     th = np.ascontiguousarray(trk_hits, np.int32)
@@ -423,8 +429,8 @@ def fit_physics(p, y, z, sector_row, trk_nhits, trk_first_hit, trk_hits, x0inv=0
     flag = np.zeros(max(th.size, 1), np.uint8)
     fn = getattr(lib(), f"orc_fit_physics_{sfx}")
     fn.restype = None
-    fn(C.byref(P), C.byref(O), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int64(K), _ptr(nh), _ptr(fh), _ptr(th), _ptr(par),
-       _ptr(cov), _ptr(xref), _ptr(zref), _ptr(chi2), _ptr(ndf), _ptr(flag))
+    fn(C.byref(P), C.byref(O), C.c_int64(y.size), _ptr(y), _ptr(z), _ptr(sr), C.c_int64(K), _ptr(nh), _ptr(fh), _ptr(th), _ptr(t0),
+       _ptr(par), _ptr(cov), _ptr(xref), _ptr(zref), _ptr(chi2), _ptr(ndf), _ptr(flag))
     return dict(par=par, cov=cov, xref=xref, zref=zref, chi2=chi2, ndf=ndf, hit_flag=flag[:th.size])
 
 
