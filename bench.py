@@ -425,6 +425,34 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                          "holes, merged hit lists refitted (DESIGN.md R26); not included in `value`"}
         binding.profile_collect(reset=True)
 
+    # ---- after the hot path: the refit with every R28 option on + the cluster tags a compression step would use --------
+    physics = None
+    if int(ev.params.n_sectors) > 1:
+        from paper_2106_03636_b200.synth import V_DRIFT
+        trk.track_time(V_DRIFT)                              # R24: the time offsets the drift lengths of R28e come from
+        popt = dict(x0inv=2e-4, outlier_cut=12.0, dedx=2e-6, eloss_sigma=0.3, err_ang_y=1.5, err_ang_z=0.8, err_drift_y=2e-4,
+                    err_drift_z=3e-4, v_drift=V_DRIFT, z_len=250.0)
+
+        def physics_step():
+            trk.fit_tracks_physics(trk_t0=trk.trk_t0, want_numpy=False, **popt)
+            return trk.tag_clusters(qpt_max=4.0, use_physics_fit=True, want_numpy=False)
+
+        physics_step()
+        torch.cuda.synchronize()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record()
+        for _ in range(3):
+            tag = physics_step()
+        p1.record()
+        torch.cuda.synchronize()
+        physics = {"ms": p0.elapsed_time(p1) / 3, "options": popt,
+                   "hits_rejected": int(trk._physics["hit_flag"][:n_hits].sum().item()),
+                   "clusters_tagged_for_removal": int(((tag[:n] & 2) != 0).sum().item()),
+                   "what": "tpc_fit_tracks_physics (scattering noise, energy loss, angle- and drift-dependent cluster errors, "
+                           "outlier rejection; DESIGN.md R28a-e) + tpc_tag_clusters; not included in `value`"}
+        del tag
+        binding.profile_collect(reset=True)
+
     # ---- in front of the hot path (not part of `value`): tpc_clusterize (R27) on the digits of a slab of the event ---
     cluster = None
     if world == 1 and not args.no_cpu_baseline:
@@ -544,7 +572,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "follower_work": work,
            "clocks": clocks, "gpu_launches": launches, "gpu_launches_per_step": launches / args.steps, "kernels": kern,
            "kernels_ms_sum": round(sum(v["ms_per_step"] for v in kern.values()), 3), "roofline": roofline,
-           "after_hot_path": {"merge": merge}, "before_hot_path": {"clusterizer": cluster}}
+           "after_hot_path": {"merge": merge, "physics_refit_and_tags": physics}, "before_hot_path": {"clusterizer": cluster}}
     if not args.no_e2e:
         out["e2e"] = {"value": tot_clusters / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d) * world,
                       "d2h_bytes_per_step": int(d2h) * world, "ms_per_step": t_e2e * 1e3,

@@ -284,21 +284,41 @@ int tpc_track_host(const tpc_params_t* params_host, int64_t n_clusters, int64_t 
 
 /* ---- physics options of the refit and cluster tags ("removal of hits of tracks
  * not used for physics"; R28) -------------------------------------------------------------------------
- * tpc_fit_tracks_physics: tpc_fit_tracks' self-contained path (hits gathered through y, z, sector_row, trk_hits;
- * no workspace) with two options: x0inv > 0 adds multiple-scattering process noise after every transport over a path
- * of L cm, theta0^2 = (0.0136 GeV)^2 (q/pT)^2 / (1 + tanl^2) L x0inv (x0inv = 1 / radiation length, per cm), to the
- * covariance of sinphi, tanlambda and q/pT (R28a); outlier_cut > 0 leaves out, in the last pass, every hit whose chi2
- * against the predicted state exceeds it: hit_flag = 1, ndf loses 2 (R28b).  hit_flag [n_clusters], in hit-list
- * order (same indexing as trk_hits), is always written (0 = used).  x0inv = 0 and outlier_cut <= 0 give
- * tpc_fit_tracks' results bit for bit.  TPC_EINVAL for x0inv < 0, NaN options or missing buffers.
+ * tpc_fit_tracks_physics: tpc_fit_tracks (same workspace rule: workspace != NULL streams the track-ordered hit records
+ * tpc_find_tracks left there and reads neither y, z nor trk_hits; workspace == NULL gathers through y, z, sector_row,
+ * trk_hits and ignores max_tracklets / ws_bytes; both bit-identical; sector_row is needed either way, for the TPC
+ * side) with the options of tpc_fit_options_t (host struct, read during the call):
+ *   R28a x0inv > 0: multiple-scattering process noise after every transport over a path of L cm,
+ *        theta0^2 = (0.0136 GeV)^2 (q/pT)^2 / (1 + tanl^2) L x0inv (x0inv = 1 / radiation length, per cm), added to the
+ *        covariance of sinphi, tanlambda and q/pT;
+ *   R28b outlier_cut > 0: in the last pass a hit whose chi2 against the predicted state exceeds it is left out:
+ *        hit_flag = 1, ndf loses 2;
+ *   R28d dedx > 0 (GeV per cm of path, beta = 1): after every transport q/pT changes by dq = (dedx |arc| |q/pT|) q/pT,
+ *        added in the outward passes (a track is taken to fly outward and lose momentum), subtracted in the inward
+ *        ones; C44 += (eloss_sigma dq)^2;
+ *   R28e cluster errors at the predicted state (s = sinphi, tl = tanlambda) and the hit's drift length d:
+ *        sigma_y^2 = sigma_y^2 (1 + err_ang_y s^2 / (1 - s^2)) + err_drift_y d,
+ *        sigma_z^2 = sigma_z^2 (1 + err_ang_z tl^2) + err_drift_z d,   d = max(0, z_len - |z + side v_drift t0|),
+ *        side = +1 for sectors < 18 else -1, t0 = trk_t0[track] (device, [max_tracks], the time offsets
+ *        tpc_track_time writes; NULL or a NaN entry: no drift terms).
+ * hit_flag [n_clusters], in hit-list order (same indexing as trk_hits), is always written (0 = used).  All options 0
+ * (outlier_cut <= 0) give tpc_fit_tracks' results bit for bit.  TPC_EINVAL for a NULL options pointer, a negative,
+ * infinite or NaN option (outlier_cut: NaN only), or missing buffers.
  * tpc_tag_clusters: tag [n_clusters] (uint8): bit 0 = attached to a track; bit 1 = that track is not used for
  * physics: ndf < 0 or |q/pT| = |par[4][track]| > qpt_max (low-pT loopers); bit 2 = rejected by R28b (hit_flag may be
  * NULL: bit 2 is then never set); 0 = unattached.  H = counters[TPC_CNT_HITS] is read on the device.  Enqueue only. */
-int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
+typedef struct {
+  float x0inv, outlier_cut;                              /* R28a, R28b */
+  float dedx, eloss_sigma;                               /* R28d */
+  float err_ang_y, err_ang_z, err_drift_y, err_drift_z;  /* R28e */
+  float v_drift, z_len;                                  /* cm/us, cm: drift length of R28e */
+} tpc_fit_options_t;
+int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets,
+                           void* workspace, size_t ws_bytes, const float* y, const float* z,
                            const int32_t* sector_row, const int32_t* counters, int64_t max_tracks,
                            const int32_t* trk_nhits, const int64_t* trk_first_hit, const int32_t* trk_hits,
-                           float x0inv, float outlier_cut, float* par, float* cov, float* xref, float* zref,
-                           float* chi2, int32_t* ndf, uint8_t* hit_flag, void* stream);
+                           const tpc_fit_options_t* options_host, const float* trk_t0, float* par, float* cov,
+                           float* xref, float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, void* stream);
 int tpc_tag_clusters(int64_t n_clusters, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
                      const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag,
                      double qpt_max, uint8_t* tag, void* stream);

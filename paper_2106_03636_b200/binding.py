@@ -58,6 +58,12 @@ class tpc_merge_params_t(C.Structure):
     _fields_ = [("chi2_cut", C.c_float), ("dz_max", C.c_float), ("ce_tol", C.c_float), ("max_rows", C.c_int32)]
 
 
+class tpc_fit_options_t(C.Structure):
+    """Mirror of tpc_fit_options_t (R28a, b, d, e)."""
+    _fields_ = [(nm, C.c_float) for nm in ("x0inv", "outlier_cut", "dedx", "eloss_sigma", "err_ang_y", "err_ang_z", "err_drift_y",
+                                           "err_drift_z", "v_drift", "z_len")]
+
+
 class tpc_merged_t(C.Structure):
     """Mirror of tpc_merged_t: device outputs of tpc_merge_tracks (R26)."""
     _fields_ = [(nm, C.c_void_p) for nm in ("trk_succ", "trk_pred", "trk_succ_chi2", "trk_global", "n_global", "g_head", "g_nseg",
@@ -304,6 +310,7 @@ class Tracker:
         _check(self.lib.tpc_track_time(C.byref(self.P), _dp(self.counters), C.c_int64(K), _dp(self.trk_sector), _dp(self.par),
                                        _dp(self.xref), _dp(self.zref), C.c_float(v_drift), _dp(out["phi0"]), _dp(out["z0"]),
                                        _dp(out["dca"]), _dp(out["t0"]), _stream()), "tpc_track_time")
+        self.trk_t0 = out["t0"]                           # device [max_tracks]: what fit_tracks_physics(trk_t0=...) takes
         k = int(self.counters[CNT_TRACKS].item())
         return {n: v[:k].cpu().numpy() for n, v in out.items()}
 
@@ -318,6 +325,7 @@ class Tracker:
         _check(self.lib.tpc_track_time(C.byref(self.P), _dp(self.counters), C.c_int64(K), _dp(self.trk_sector), _dp(self.par),
                                        _dp(self.xref), _dp(self.zref), C.c_float(v_drift), _dp(tt["phi0"]), _dp(tt["z0"]),
                                        _dp(tt["dca"]), _dp(tt["t0"]), _stream()), "tpc_track_time")
+        self.trk_t0 = tt["t0"]
         nb = int(math.ceil((t_hi - t_lo) / bin_width))
         wsb = C.c_size_t(0)
         _check(self.lib.tpc_collisions_workspace_bytes(C.c_int64(nb), C.c_int64(K), C.byref(wsb)), "tpc_collisions_workspace_bytes")
@@ -339,37 +347,53 @@ class Tracker:
         return dict(n_found=found, coll_time=ct[:n].cpu().numpy(), coll_ntracks=cn[:n].cpu().numpy(), coll_bin=cb[:n].cpu().numpy(),
                     trk_collision=tc[:k].cpu().numpy(), t0=tt["t0"][:k].cpu().numpy(), dca=tt["dca"][:k].cpu().numpy())
 
-    def fit_tracks_physics(self, x0inv: float = 0.0, outlier_cut: float = 0.0):
-        """tpc_fit_tracks_physics (R28a/b) on the hit lists of the last find: numpy dict(par, cov, xref, zref, chi2, ndf,
-        hit_flag); the Tracker's own fit outputs are left untouched.  Synchronises."""
+    def fit_tracks_physics(self, x0inv: float = 0.0, outlier_cut: float = 0.0, dedx: float = 0.0, eloss_sigma: float = 0.0,
+                           err_ang_y: float = 0.0, err_ang_z: float = 0.0, err_drift_y: float = 0.0, err_drift_z: float = 0.0,
+                           v_drift: float = 0.0, z_len: float = 250.0, trk_t0=None, want_numpy: bool = True,
+                           use_workspace: bool = True):
+        """tpc_fit_tracks_physics (R28a/b/d/e) on the hit lists of the last find: numpy dict(par, cov, xref, zref, chi2,
+        ndf, hit_flag); the Tracker's own fit outputs are left untouched.  trk_t0: device float32 [max_tracks] (the t0 of
+        track_time) or None.  use_workspace=False takes the self-contained gather path.  Synchronises unless want_numpy is False (then: the device tensors, enqueue only)."""
         t = self.torch
         K, dev = self.max_tracks, self.device
         y, z, sr = self._inputs
-        o = dict(par=t.empty((5, K), dtype=t.float32, device=dev), cov=t.empty((15, K), dtype=t.float32, device=dev),
-                 xref=t.empty(K, dtype=t.float32, device=dev), zref=t.empty(K, dtype=t.float32, device=dev),
-                 chi2=t.empty(K, dtype=t.float32, device=dev), ndf=t.empty(K, dtype=t.int32, device=dev),
-                 hit_flag=t.zeros(max(self.n, 1), dtype=t.uint8, device=dev))
-        _check(self.lib.tpc_fit_tracks_physics(C.byref(self.P), C.c_int64(self.n), _dp(y), _dp(z), _dp(sr), _dp(self.counters),
+        o = getattr(self, "_physics", None)
+        opt = tpc_fit_options_t(x0inv, outlier_cut, dedx, eloss_sigma, err_ang_y, err_ang_z, err_drift_y, err_drift_z, v_drift,
+                                z_len)
+        if trk_t0 is not None and (trk_t0.dtype != t.float32 or trk_t0.numel() < K or not trk_t0.is_cuda):
+            raise ValueError("trk_t0: device float32 [max_tracks]")
+        if o is None:
+            o = dict(par=t.empty((5, K), dtype=t.float32, device=dev), cov=t.empty((15, K), dtype=t.float32, device=dev),
+                     xref=t.empty(K, dtype=t.float32, device=dev), zref=t.empty(K, dtype=t.float32, device=dev),
+                     chi2=t.empty(K, dtype=t.float32, device=dev), ndf=t.empty(K, dtype=t.int32, device=dev),
+                     hit_flag=t.zeros(max(self.n, 1), dtype=t.uint8, device=dev))
+        _check(self.lib.tpc_fit_tracks_physics(C.byref(self.P), C.c_int64(self.n), C.c_int64(self.max_tracklets),
+                                               _dp(self.workspace) if use_workspace else C.c_void_p(0), C.c_size_t(self.ws_bytes),
+                                               _dp(y), _dp(z), _dp(sr), _dp(self.counters),
                                                C.c_int64(K), _dp(self.trk_nhits), _dp(self.trk_first_hit), _dp(self.trk_hits),
-                                               C.c_float(x0inv), C.c_float(outlier_cut), _dp(o["par"]), _dp(o["cov"]),
+                                               C.byref(opt), _dp(trk_t0), _dp(o["par"]), _dp(o["cov"]),
                                                _dp(o["xref"]), _dp(o["zref"]), _dp(o["chi2"]), _dp(o["ndf"]), _dp(o["hit_flag"]),
                                                _stream()), "tpc_fit_tracks_physics")
         self._physics = o
+        if not want_numpy:
+            return o
         cnt = self.counters.cpu().numpy()
         k, h = int(cnt[CNT_TRACKS]), int(cnt[CNT_HITS])
         return dict(par=o["par"][:, :k].cpu().numpy(), cov=o["cov"][:, :k].cpu().numpy(), xref=o["xref"][:k].cpu().numpy(),
                     zref=o["zref"][:k].cpu().numpy(), chi2=o["chi2"][:k].cpu().numpy(), ndf=o["ndf"][:k].cpu().numpy(),
                     hit_flag=o["hit_flag"][:h].cpu().numpy())
 
-    def tag_clusters(self, qpt_max: float = 10.0, use_physics_fit: bool = False):
+    def tag_clusters(self, qpt_max: float = 10.0, use_physics_fit: bool = False, want_numpy: bool = True):
         """tpc_tag_clusters (R28c): uint8 tag per cluster, from the Tracker's fit or from the last fit_tracks_physics."""
         t = self.torch
-        tag = t.empty(max(self.n, 1), dtype=t.uint8, device=self.device)
+        tag = getattr(self, "_tag", None)
+        if tag is None:
+            tag = self._tag = t.empty(max(self.n, 1), dtype=t.uint8, device=self.device)
         src = self._physics if use_physics_fit else dict(par=self.par, ndf=self.ndf, hit_flag=None)
         _check(self.lib.tpc_tag_clusters(C.c_int64(self.n), _dp(self.cluster_track), _dp(self.counters), C.c_int64(self.max_tracks),
                                          _dp(src["par"]), _dp(src["ndf"]), _dp(self.trk_hits), _dp(src["hit_flag"]),
                                          C.c_double(qpt_max), _dp(tag), _stream()), "tpc_tag_clusters")
-        return tag[:self.n].cpu().numpy()
+        return tag[:self.n].cpu().numpy() if want_numpy else tag
 
     def merge_alloc(self):
         """Workspace and device outputs of tpc_merge_tracks (allocated once per Tracker)."""

@@ -327,20 +327,31 @@ int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, cons
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 
-int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, const float* y, const float* z,
-                           const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
-                           const int64_t* trk_first_hit, const int32_t* trk_hits, float x0inv, float outlier_cut, float* par,
-                           float* cov, float* xref, float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, void* stream) {
-  tpc::Geo G;
-  int64_t nb = 0;
-  if (!make_geo(params_host, &G, &nb)) return TPC_EINVAL;
-  if (n_clusters < 0 || max_tracks < 1 || !(x0inv >= 0.0f) || outlier_cut != outlier_cut || !counters || !trk_nhits ||
-      !trk_first_hit || !par || !cov || !xref || !zref || !chi2 || !ndf)
+int tpc_fit_tracks_physics(const tpc_params_t* params_host, int64_t n_clusters, int64_t max_tracklets, void* workspace,
+                           size_t ws_bytes, const float* y, const float* z, const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
+                           const int64_t* trk_first_hit, const int32_t* trk_hits, const tpc_fit_options_t* options_host,
+                           const float* trk_t0, float* par, float* cov, float* xref, float* zref, float* chi2, int32_t* ndf,
+                           uint8_t* hit_flag, void* stream) {
+  Prep pr;
+  if (!options_host) return TPC_EINVAL;
+  if (workspace) {
+    const int rc = prepare(params_host, n_clusters, max_tracklets, workspace, ws_bytes, &pr);
+    if (rc != TPC_OK) return rc;
+  } else {
+    int64_t nb = 0;
+    if (!make_geo(params_host, &pr.G, &nb)) return TPC_EINVAL;
+  }
+  const tpc_fit_options_t o = *options_host;
+  // every option is a finite number; all but outlier_cut (<= 0 switches it off) are non-negative
+  const float nonneg[] = {o.x0inv, o.dedx, o.eloss_sigma, o.err_ang_y, o.err_ang_z, o.err_drift_y, o.err_drift_z, o.v_drift, o.z_len};
+  for (float v : nonneg)
+    if (!(v >= 0.0f) || v > 3.0e38f) return TPC_EINVAL;
+  if (o.outlier_cut != o.outlier_cut) return TPC_EINVAL;
+  if (n_clusters < 0 || max_tracks < 1 || !counters || !trk_nhits || !trk_first_hit || !par || !cov || !xref || !zref || !chi2 || !ndf)
     return TPC_EINVAL;
-  if (n_clusters > 0 && (!y || !z || !sector_row || !trk_hits || !hit_flag)) return TPC_EINVAL;
-  const cudaError_t e = tpc::launch_fit_physics(G, x0inv, outlier_cut, y, z, sector_row, counters, max_tracks, trk_nhits,
-                                                trk_first_hit, trk_hits, par, cov, xref, zref, chi2, ndf, hit_flag,
-                                                (cudaStream_t)stream);
+  if (n_clusters > 0 && (!sector_row || !hit_flag || (!workspace && (!y || !z || !trk_hits)))) return TPC_EINVAL;
+  const cudaError_t e = tpc::launch_fit_physics(pr.G, o, workspace ? &pr.W : nullptr, y, z, sector_row, counters, max_tracks, trk_nhits, trk_first_hit, trk_hits,
+                                                trk_t0, par, cov, xref, zref, chi2, ndf, hit_flag, (cudaStream_t)stream);
   return e == cudaSuccess ? TPC_OK : cuda_fail(e);
 }
 

@@ -247,10 +247,10 @@ cudaError_t launch_pair_sides(const int32_t* n_a, const float* t_a, const int32_
                               int32_t* n_pairs, cudaStream_t st);
 
 // tpc_fit.cu (R28)
-cudaError_t launch_fit_physics(const Geo& g, float x0inv, float outlier_cut, const float* y, const float* z,
+cudaError_t launch_fit_physics(const Geo& g, const tpc_fit_options_t& opt, const Ws* w, const float* y, const float* z,
                                const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
-                               const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
-                               float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st);
+                               const int64_t* trk_first_hit, const int32_t* trk_hits, const float* trk_t0, float* par, float* cov,
+                               float* xref, float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st);
 cudaError_t launch_tag_clusters(int64_t n, const int32_t* cluster_track, const int32_t* counters, int64_t max_tracks,
                                 const float* par, const int32_t* ndf, const int32_t* trk_hits, const uint8_t* hit_flag,
                                 double qpt_max, uint8_t* tag, cudaStream_t st);

@@ -108,12 +108,48 @@ __device__ __forceinline__ void add_scattering(KState& st, float arc, float x0in
   st.C[TPC_CI(4, 4)] = st.C[TPC_CI(4, 4)] + ((th2 * tl) * tl) * (q * q);
 }
 
+// R28d: mean energy loss over |arc| (dir > 0 outward: momentum is lost; inward: gained back) and its straggling
+__device__ __forceinline__ void add_energy_loss(KState& st, float arc, int dir, float dedx, float eloss_sigma) {
+  if (!(dedx > 0.0f)) return;
+  const float q = st.p[4];
+  const float rel = (dedx * fabsf(arc)) * fabsf(q);
+  const float dq = rel * q;
+  st.p[4] = dir > 0 ? q + dq : q - dq;
+  st.C[TPC_CI(4, 4)] = st.C[TPC_CI(4, 4)] + (eloss_sigma * dq) * (eloss_sigma * dq);
+}
+
+// R28e: the two measurement variances at a hit of raw z for the predicted state; zs = side v_drift t0
+__device__ __forceinline__ void cluster_errors(const KState& st, const tpc_fit_options_t& o, float sy2, float sz2, bool have_d,
+                                               float z_raw, float zs, float& ey, float& ez) {
+  ey = sy2;
+  ez = sz2;
+  if (o.err_ang_y > 0.0f) {
+    const float s = st.p[2];
+    const float tan2 = (s * s) / (1.0f - s * s);
+    ey = ey * (1.0f + o.err_ang_y * tan2);
+  }
+  if (o.err_ang_z > 0.0f) {
+    const float tl = st.p[3];
+    ez = ez * (1.0f + o.err_ang_z * (tl * tl));
+  }
+  if (have_d) {
+    float d = o.z_len - fabsf(z_raw + zs);
+    if (d < 0.0f) d = 0.0f;
+    if (o.err_drift_y > 0.0f) ey = ey + o.err_drift_y * d;
+    if (o.err_drift_z > 0.0f) ez = ez + o.err_drift_z * d;
+  }
+}
+
+// REC: hits streamed from the workspace's track-ordered records (y, z, row, orig) that tpc_find_tracks wrote (one
+// sequential 16-byte stream per track, as in k_fit); else gathered through y / z / sector_row and trk_hits.
+template <bool REC>
 __global__ void __launch_bounds__(kFitThreads)
-k_fit_physics(const __grid_constant__ Geo g, float x0inv, float outlier_cut, const float* __restrict__ y,
-              const float* __restrict__ z, const int32_t* __restrict__ sector_row, const int32_t* __restrict__ counters,
-              int64_t max_tracks, const int32_t* __restrict__ trk_nhits, const int64_t* __restrict__ trk_first_hit,
-              const int32_t* __restrict__ trk_hits, float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref,
-              float* __restrict__ zref_out, float* __restrict__ chi2_out, int32_t* __restrict__ ndf, uint8_t* __restrict__ hit_flag) {
+k_fit_physics(const __grid_constant__ Geo g, const __grid_constant__ tpc_fit_options_t opt, const float4* __restrict__ hit_rec,
+              const float* __restrict__ y, const float* __restrict__ z, const int32_t* __restrict__ sector_row,
+              const int32_t* __restrict__ counters, int64_t max_tracks, const int32_t* __restrict__ trk_nhits,
+              const int64_t* __restrict__ trk_first_hit, const int32_t* __restrict__ trk_hits, const float* __restrict__ trk_t0,
+              float* __restrict__ par, float* __restrict__ cov, float* __restrict__ xref, float* __restrict__ zref_out,
+              float* __restrict__ chi2_out, int32_t* __restrict__ ndf, uint8_t* __restrict__ hit_flag) {
   __shared__ float sX[kMaxRows];
   const Scalars& sc = g.s;
   const int nrows = sc.nrows;
@@ -125,32 +161,44 @@ k_fit_physics(const __grid_constant__ Geo g, float x0inv, float outlier_cut, con
   for (int64_t k = (int64_t)blockIdx.x * kFitThreads + threadIdx.x; k < K; k += (int64_t)gridDim.x * kFitThreads) {
     const int n = trk_nhits[k];
     const int64_t first = trk_first_hit[k];
-    const int32_t* hits = trk_hits + first;
-    auto rowx = [&](int h) { return sX[__ldg(sector_row + h) % nrows]; };
-    const int a = hits[0], b = hits[n / 2], c = hits[n - 1], h1 = hits[n > 1 ? 1 : 0];
-    const float x1 = rowx(a), y1 = __ldg(y + a), x2 = rowx(b), y2 = __ldg(y + b), x3 = rowx(c), y3 = __ldg(y + c);
+    // hit i of the list as (y, raw z, x of its row, original cluster index)
+    auto hit_at = [&](int i) {
+      if (REC) {
+        const float4 r = __ldg(hit_rec + first + i);
+        return make_float4(r.x, r.y, sX[__float_as_int(r.z)], r.w);
+      }
+      const int h = trk_hits[first + i];
+      return make_float4(__ldg(y + h), __ldg(z + h), sX[__ldg(sector_row + h) % nrows], __int_as_float(h));
+    };
+    const float4 ha = hit_at(0), hb = hit_at(n / 2), hc = hit_at(n - 1), hh1 = hit_at(n > 1 ? 1 : 0);
+    const float x1 = ha.z, y1 = ha.x, x2 = hb.z, y2 = hb.x, x3 = hc.z, y3 = hc.x;
     const float cross = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
     const float d12 = sqrtf((x2 - x1) * (x2 - x1) + (y2 - y1) * (y2 - y1));
     const float d23 = sqrtf((x3 - x2) * (x3 - x2) + (y3 - y2) * (y3 - y2));
     const float d13 = sqrtf((x3 - x1) * (x3 - x1) + (y3 - y1) * (y3 - y1));
     const float kappa = (2.0f * cross) / ((d12 * d23) * d13);
-    const float dx = rowx(h1) - x1, dy = __ldg(y + h1) - y1;
+    const float dx = hh1.z - x1, dy = hh1.x - y1;
     const float ch = sqrtf(dx * dx + dy * dy);
     float sphi = dy / ch - ((kappa * ch) * 0.5f) * (dx / ch);
     if (sphi > ms) sphi = ms;
     if (sphi < -ms) sphi = -ms;
-    const float zref = __ldg(z + a);
+    const float zref = ha.y;
     KState st;
     st.p[0] = y1;
     st.p[1] = 0.0f;
     st.p[2] = sphi;
-    st.p[3] = (__ldg(z + h1) - zref) / ch;
+    st.p[3] = (hh1.y - zref) / ch;
     st.p[4] = -(kappa / kB);
     float chi2 = 0.0f;
     float x_at = x1;
     int nrej = 0;
     bool ok = true;
     for (int i = 0; i < n; i++) hit_flag[first + i] = 0;
+    const float t0 = trk_t0 ? trk_t0[k] : 0.0f;
+    const bool have_d = trk_t0 && t0 == t0;
+    const float side = (__ldg(sector_row + __float_as_int(ha.w)) / nrows) < 18 ? 1.0f : -1.0f;
+    const float zs = have_d ? side * (opt.v_drift * t0) : 0.0f;
+    const float x0inv = opt.x0inv, outlier_cut = opt.outlier_cut;
     for (int pass = 0; pass < sc.n_fit_passes && ok; pass++) {
       reset_cov(st, sc.cov0);
       chi2 = 0.0f;
@@ -158,8 +206,8 @@ k_fit_physics(const __grid_constant__ Geo g, float x0inv, float outlier_cut, con
       const int dir = (pass & 1) ? -1 : 1;
       int i = dir > 0 ? 0 : n - 1;
       for (int cnt = 0; cnt < n; cnt++, i += dir) {
-        const int h = hits[i];
-        const float xh = rowx(h);
+        const float4 hit = hit_at(i);
+        const float xh = hit.z;
         if (cnt > 0) {  // the first hit of a pass is the one the state already sits at (no transport)
           const float dxk = xh - x_at;
           const float s1 = st.p[2], kap = -(kB * st.p[4]);
@@ -171,11 +219,16 @@ k_fit_physics(const __grid_constant__ Geo g, float x0inv, float outlier_cut, con
           const float c1 = sqrtf(mad(-s1, s1, 1.0f)), c2 = sqrtf(mad(-s2, s2, 1.0f));
           const float t = (s1 + s2) / (c1 + c2);
           const float Lc = dxk * sqrtf(mad(t, t, 1.0f));
-          add_scattering(st, Lc * asin_ratio((kap * Lc) * 0.5f), x0inv);
+          const float arc = Lc * asin_ratio((kap * Lc) * 0.5f);
+          add_scattering(st, arc, x0inv);
+          add_energy_loss(st, arc, dir, opt.dedx, opt.eloss_sigma);
           x_at = xh;
         }
-        const Innov I = innovation(st, sy2, sz2);
-        const float yh = __ldg(y + h), zh = __ldg(z + h) - zref;
+        const float zraw = hit.y;
+        float sy2h, sz2h;
+        cluster_errors(st, opt, sy2, sz2, have_d, zraw, zs, sy2h, sz2h);
+        const Innov I = innovation(st, sy2h, sz2h);
+        const float yh = hit.x, zh = zraw - zref;
         if (last && outlier_cut > 0.0f && chi2_of(I, yh - st.p[0], zh - st.p[1]) > outlier_cut) {
           hit_flag[first + i] = 1;
           nrej++;
@@ -423,17 +476,24 @@ cudaError_t launch_fit(const Geo& g, const Ws* w, int64_t n, const float* y, con
   return cudaGetLastError();
 }
 
-cudaError_t launch_fit_physics(const Geo& g, float x0inv, float outlier_cut, const float* y, const float* z,
+cudaError_t launch_fit_physics(const Geo& g, const tpc_fit_options_t& opt, const Ws* w, const float* y, const float* z,
                                const int32_t* sector_row, const int32_t* counters, int64_t max_tracks, const int32_t* trk_nhits,
-                               const int64_t* trk_first_hit, const int32_t* trk_hits, float* par, float* cov, float* xref,
-                               float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st) {
+                               const int64_t* trk_first_hit, const int32_t* trk_hits, const float* trk_t0, float* par, float* cov,
+                               float* xref, float* zref, float* chi2, int32_t* ndf, uint8_t* hit_flag, cudaStream_t st) {
   if (max_tracks <= 0) return cudaSuccess;
   int64_t blocks = (max_tracks + kFitThreads - 1) / kFitThreads;
   if (blocks > 148 * 16) blocks = 148 * 16;
-  TPC_LAUNCH(KID_FIT_PHYSICS, st,
-             (k_fit_physics<<<(unsigned)blocks, kFitThreads, 0, st>>>(g, x0inv, outlier_cut, y, z, sector_row, counters, max_tracks,
-                                                                     trk_nhits, trk_first_hit, trk_hits, par, cov, xref, zref, chi2,
-                                                                     ndf, hit_flag)));
+  if (w) {
+    TPC_LAUNCH(KID_FIT_PHYSICS, st,
+               (k_fit_physics<true><<<(unsigned)blocks, kFitThreads, 0, st>>>(g, opt, w->hit_rec, y, z, sector_row, counters, max_tracks,
+                                                                             trk_nhits, trk_first_hit, trk_hits, trk_t0, par, cov,
+                                                                             xref, zref, chi2, ndf, hit_flag)));
+  } else {
+    TPC_LAUNCH(KID_FIT_PHYSICS, st,
+               (k_fit_physics<false><<<(unsigned)blocks, kFitThreads, 0, st>>>(g, opt, nullptr, y, z, sector_row, counters, max_tracks,
+                                                                              trk_nhits, trk_first_hit, trk_hits, trk_t0, par, cov,
+                                                                              xref, zref, chi2, ndf, hit_flag)));
+  }
   return cudaGetLastError();
 }
 

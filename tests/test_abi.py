@@ -101,7 +101,7 @@ def test_binding_refuses_cpu_tensors():
 
 
 @pytest.mark.parametrize("name,mirror", [("tpc_result_t", "tpc_result_t"), ("tpc_merge_params_t", "tpc_merge_params_t"),
-                                         ("tpc_merged_t", "tpc_merged_t")])
+                                         ("tpc_merged_t", "tpc_merged_t"), ("tpc_fit_options_t", "tpc_fit_options_t")])
 def test_other_struct_layouts_match_header(name, mirror):
     """Field order of the ctypes mirrors == the header's typedefs (pointer structs: one pointer per member)."""
     txt = open(HEADER).read()
@@ -111,10 +111,12 @@ def test_other_struct_layouts_match_header(name, mirror):
     for decl in body.split(";"):
         decl = decl.strip()
         if decl:
-            fields.append(decl.split()[-1].lstrip("*"))
+            fields += [piece.split()[-1].lstrip("*") for piece in decl.split(",")]
     cls = getattr(binding, mirror)
     assert fields == [f[0] for f in cls._fields_]
-    if name != "tpc_merge_params_t":
-        assert C.sizeof(cls) == 8 * len(fields)
-    else:
+    if name == "tpc_merge_params_t":
         assert C.sizeof(cls) == 16
+    elif name == "tpc_fit_options_t":
+        assert C.sizeof(cls) == 4 * len(fields) and all(f[1] is C.c_float for f in cls._fields_)
+    else:
+        assert C.sizeof(cls) == 8 * len(fields)
