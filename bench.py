@@ -56,7 +56,8 @@ KERNEL_MODEL = {
     # recorded by the follower, hit = hit of an accepted track
     "k_bucket_hist": ("hbm", {"cluster": 12}, None),                # y, z, sector_row in
     "k_scan_*": ("hbm", {"cluster": 12, "tracklet": 24}, None),     # all scans of a step: 2 reads + 1 write per element
-    "k_bucket_scatter": ("hbm", {"cluster": 12 + 16}, None),        # inputs in, 16 B record out
+    "k_part_scatter": ("hbm", {"cluster": 12 + 16}, None),          # inputs in, 16 B record out (part order)
+    "k_bucket_scatter": ("hbm", {"cluster": 16 + 16}, None),        # record in, record out (bucket order)
     "k_bucket_sort": ("hbm", {"cluster": 16 + 16, "bin": 4}, None), # records in (second read from L2), records + bin_first out
     "k_neighbours": ("hbm", {"cluster": 16 + 8}, None),           # own record in, two links out (neighbours from L2)
     "k_clean": ("hbm", {"cluster": 8 + 8}, None),

@@ -23,7 +23,7 @@ struct Rec2 {
 };
 Rec2 g_rec[kMaxRec];
 int g_nrec = 0, g_nrec_created = 0;
-const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
+const char* const kKernelNames[KID_N] = {"k_bucket_hist", "k_scan_*", "k_part_scatter", "k_bucket_scatter", "k_bucket_sort", "k_neighbours", "k_clean",
                                          "k_compact_starts", "k_follow", "k_survivor_*", "k_follow", "k_push_keys", "k_count_kept", "k_write_tracks",
                                          "k_assign", "k_fit", "k_track_time", "k_t0_*", "k_merge_*", "k_digit_*", "k_fit_physics+k_tag_*", "k_export_*"};
 }  // namespace

@@ -129,7 +129,7 @@ inline Layout make_layout(int64_t n, int64_t scap, int64_t nb, int nrows, int64_
   L.off_rec = take(sizeof(Rec) * (size_t)(n + 1));
   L.off_key = take(sizeof(int32_t) * (size_t)(n + 1));      // start-hit flags and their scan (R10)
   L.off_bucket_first = take(sizeof(int32_t) * (size_t)(kMaxBuckets + 2));
-  L.off_bucket_cursor = take(sizeof(int32_t) * (size_t)(kMaxBuckets + 2));
+  L.off_bucket_cursor = take(sizeof(int32_t) * (size_t)(kMaxBuckets + 2 + 1024 + 2));  // + the part cursors of the grid build
   L.off_bin_first = take(sizeof(int32_t) * (size_t)(nb + 2));
   L.off_link_up = take(sizeof(int32_t) * (size_t)(n + 1));
   L.off_link_dn = take(sizeof(int32_t) * (size_t)(n + 1));

@@ -7,9 +7,12 @@
 //                     consecutive bins (a few thousand clusters).  Per-block shared-memory
 //                     histogram over the buckets, flushed with one atomic per non-empty bucket.
 //   scan              bucket offsets.
-//   k_bucket_scatter  cluster -> 16-byte record appended to its bucket's range of a temporary
-//                     array (warp-aggregated cursor atomics; the ~2e4 append frontiers are L2
-//                     resident, so DRAM sees whole lines).
+//   k_part_scatter    cluster -> 16-byte record moved into the range of its PART (~sqrt(#buckets)
+//                     consecutive buckets) of one temporary array; a tile of 4096 clusters is
+//                     ranked in shared memory, staged there in destination order and written out
+//                     as whole runs: one global atomic per (tile, part) instead of one per cluster.
+//   k_bucket_scatter  the same step inside the parts: records of a part -> their buckets' ranges of
+//                     the second temporary array.
 //   k_bucket_sort     one block per bucket: counts the bucket's bins in shared memory, scans them
 //                     (-> bin_first), places the records, and re-orders every bin holding >= 2
 //                     clusters by original index, which turns the arrival order of the atomics
@@ -17,7 +20,7 @@
 //                     run and equal to a stable sort by bin.  The bucket (~100 KB) stays in L2
 //                     between the passes.
 //
-// Roofline: HBM streaming, 72 B per cluster + 4 B per bin.
+// Roofline: HBM streaming, 104 B per cluster + 4 B per bin.
 // =============================================================================================
 #include "tpc_common.cuh"
 #include "tpc_scan.cuh"
@@ -28,7 +31,6 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int64_t kScatterCap = 148 * 1024;  // no grid-stride loop: measured 3.33 -> 3.12 ms on configs[4]
 constexpr int64_t kSortCap = kMaxBuckets;    // one block per bucket: measured 2.62 -> 2.37 ms
 constexpr int kHistThreads = 1024;  // the bucket histogram takes up to 192 KB of shared memory: one or two big blocks per SM
 constexpr int kUnroll = 4;  // independent loads in flight per thread in the streaming passes
@@ -114,56 +116,190 @@ k_bucket_hist(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nb
   if (__any_sync(kFull, bad) && (threadIdx.x & 31) == 0) atomicOr(ws_counters + WC_STATUS, TPC_ST_BAD_ROW);
 }
 
-__global__ void __launch_bounds__(kThreads)
-k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int nbuckets, const float* __restrict__ y,
-                 const float* __restrict__ z, const int32_t* __restrict__ sector_row, int32_t* __restrict__ cursor,
-                 Rec* __restrict__ tmp) {
-  __shared__ GridSmem sm;
-  load_grid_rows(sm, g);
-  __syncthreads();
+// ---- two-pass scatter: global cursor atomics replaced by shared-memory ranks ----------------------------------------
+// A PART is 2^part_shift consecutive buckets (about the square root of the bucket count).  k_part_scatter moves every
+// cluster, as a 16-byte record, into its part's range; k_bucket_scatter moves the records of a part into their
+// buckets' ranges.  Both rank the records of a 4096-element tile in shared memory and reserve one run per (tile,
+// destination) with a single global atomic, so the global atomics drop from one per cluster to one per ~20 clusters and
+// every run is written as consecutive records.  The order inside a bucket is arbitrary either way; k_bucket_sort's
+// re-ordering by original index makes the grid the stable sort R7 asks for.
+constexpr int kPartThreads = 512, kPartItems = 8, kPartTile = kPartThreads * kPartItems;
+constexpr int kMaxParts = 1024;   // parts of the first pass (+ 1 for the bad-row bucket)
+constexpr int kLocalCap = 2048;   // buckets a tile of the second pass can rank in shared memory (a tile straddling parts)
+
+__device__ __forceinline__ int part_of(int bk, int part_shift, int nbuckets, int nparts) {
+  return bk == nbuckets ? nparts : bk >> part_shift;
+}
+
+// shared-memory rank of a key inside the tile; a warp whose lanes all hold the same key (inputs ordered by row) takes
+// one atomic for all of them
+__device__ __forceinline__ int tile_rank(int32_t* cnt, int key, bool valid, int lane) {
+  const int k0 = __shfl_sync(kFull, key, 0);
+  if (__all_sync(kFull, valid && key == k0)) {
+    int base = 0;
+    if (lane == 0) base = atomicAdd(cnt + key, 32);
+    return __shfl_sync(kFull, base, 0) + lane;
+  }
+  return valid ? atomicAdd(cnt + key, 1) : 0;
+}
+
+__global__ void k_scan_cursors(int nbuckets, int part_shift, int nparts, const int32_t* __restrict__ bucket_first,
+                              int32_t* __restrict__ bucket_cursor, int32_t* __restrict__ part_cursor) {
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j <= nbuckets + 1; j += gridDim.x * blockDim.x) {
+    bucket_cursor[j] = bucket_first[j];
+    if (j <= nparts) {
+      const int64_t b = (int64_t)j << part_shift;
+      part_cursor[j] = bucket_first[b < nbuckets ? b : nbuckets];
+    }
+  }
+}
+
+// Shared state of one tile: counts per destination, their exclusive offsets inside the tile, and (global base of the
+// run - offset inside the tile) so that staged position p goes to delta[dest] + p.
+template <int NDEST>
+struct TileSmem {
+  GridSmem grid;
+  int32_t cnt[NDEST];
+  int32_t loc[NDEST];
+  int32_t delta[NDEST];
+  uint16_t dest[kPartTile];  // destination of every staged position
+  int32_t scan[kPartThreads / 32 + 1];
+};
+
+// counts -> offsets inside the tile, one global atomic per non-empty destination; ndest <= NDEST (a multiple of kPartThreads)
+template <int NDEST>
+__device__ __forceinline__ void tile_reserve(TileSmem<NDEST>& sm, int ndest, int32_t* __restrict__ cursor) {
+  constexpr int PER = NDEST / kPartThreads;
+  const int tid = threadIdx.x;
+  int c[PER], acc = 0;
+#pragma unroll
+  for (int k = 0; k < PER; k++) {
+    const int j = tid * PER + k;
+    c[k] = j < ndest ? sm.cnt[j] : 0;
+    acc += c[k];
+  }
+  int total;
+  int ex = block_excl_scan<int, kPartThreads>(acc, &total, sm.scan);
+#pragma unroll
+  for (int k = 0; k < PER; k++) {
+    const int j = tid * PER + k;
+    if (j < ndest) {
+      sm.loc[j] = ex;
+      if (c[k]) sm.delta[j] = atomicAdd(cursor + j, c[k]) - ex;
+      ex += c[k];
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kPartThreads, 2)
+k_part_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int part_shift, int nbuckets, int nparts,
+               const float* __restrict__ y, const float* __restrict__ z, const int32_t* __restrict__ sector_row,
+               int32_t* __restrict__ part_cursor, Rec* __restrict__ out) {
+  extern __shared__ float4 stage[];  // [kPartTile]: the tile's records in destination order
+  __shared__ TileSmem<kMaxParts + kPartThreads> sm;
+  load_grid_rows(sm.grid, g);
   const Scalars& sc = g.s;
   const int sr_end = sc.nsec * sc.nrows;
-  const int lane = threadIdx.x & 31;
-  const int64_t span = (int64_t)kThreads * kUnroll;
-  for (int64_t i0 = (int64_t)blockIdx.x * span + (int64_t)(threadIdx.x >> 5) * (32 * kUnroll); i0 < n;
-       i0 += (int64_t)gridDim.x * span) {
-    int srv[kUnroll];
-    float yv[kUnroll], zv[kUnroll];
+  const int tid = threadIdx.x, lane = tid & 31;
+  for (int64_t t0 = (int64_t)blockIdx.x * kPartTile; t0 < n; t0 += (int64_t)gridDim.x * kPartTile) {
+    for (int j = tid; j <= nparts; j += kPartThreads) sm.cnt[j] = 0;
+    __syncthreads();
+    int srv[kPartItems];
+    float yv[kPartItems], zv[kPartItems];
 #pragma unroll
-    for (int j = 0; j < kUnroll; j++) {
-      const int64_t i = i0 + j * 32 + lane;
+    for (int j = 0; j < kPartItems; j++) {
+      const int64_t i = t0 + j * kPartThreads + tid;
       srv[j] = i < n ? __ldcs(sector_row + i) : 0;
       yv[j] = i < n ? __ldcs(y + i) : 0.0f;
       zv[j] = i < n ? __ldcs(z + i) : 0.0f;
     }
+    int where[kPartItems];  // part << 13 | rank inside the tile (< 4096)
 #pragma unroll
-    for (int j = 0; j < kUnroll; j++) {
-      const int64_t i = i0 + j * 32 + lane;
-      int bk = -1;
-      if (i < n) {
+    for (int j = 0; j < kPartItems; j++) {
+      const bool valid = t0 + j * kPartThreads + tid < n;
+      int pt = 0;
+      if (valid) {
         if ((unsigned)srv[j] < (unsigned)sr_end) {
-          bk = bin_of(sm, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift;
+          pt = part_of(bin_of(sm.grid, sc, srv[j], yv[j], zv[j], nullptr) >> bucket_shift, part_shift, nbuckets, nparts);
         } else {  // no such (sector, row): parked behind the grid with an impossible sector_row (see k_bucket_hist)
-          bk = nbuckets;
+          pt = nparts;
           srv[j] = kBadRow;
         }
       }
-      // Warp-aggregated append.  match.any is slow when all 32 keys differ (shuffled input), and then there is
-      // nothing to aggregate: it is only used when some neighbouring lanes share a bucket (inputs ordered by row,
-      // where it turns up to 32 same-address atomics into one).
-      int slot;
-      if (__any_sync(kFull, bk == __shfl_xor_sync(kFull, bk, 1))) {
-        const unsigned peers = __match_any_sync(kFull, bk);
-        const int leader = __ffs(peers) - 1;
-        int base = 0;
-        if (bk >= 0 && lane == leader) base = atomicAdd(cursor + bk, __popc(peers));
-        base = __shfl_sync(kFull, base, leader);
-        slot = base + __popc(peers & ((1u << lane) - 1u));
-      } else {
-        slot = bk >= 0 ? atomicAdd(cursor + bk, 1) : 0;
-      }
-      if (bk >= 0) tmp[slot] = make_float4(yv[j], zv[j], __int_as_float((int)i), __int_as_float(srv[j]));
+      where[j] = (pt << 13) | tile_rank(sm.cnt, pt, valid, lane);
     }
+    __syncthreads();
+    tile_reserve(sm, nparts + 1, part_cursor);
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kPartItems; j++) {
+      const int64_t i = t0 + j * kPartThreads + tid;
+      if (i < n) {
+        const int pt = where[j] >> 13, p = sm.loc[pt] + (where[j] & 8191);
+        stage[p] = make_float4(yv[j], zv[j], __int_as_float((int)i), __int_as_float(srv[j]));
+        sm.dest[p] = (uint16_t)pt;
+      }
+    }
+    __syncthreads();
+    const int count = (int)(n - t0 < kPartTile ? n - t0 : kPartTile);
+    for (int p = tid; p < count; p += kPartThreads) out[sm.delta[sm.dest[p]] + p] = stage[p];  // consecutive lanes, consecutive records
+    __syncthreads();
+  }
+}
+
+// Second pass: the runs of a tile all lie inside one part (a few MB, a handful of pages), so they are written straight
+// from the registers (staging them as in the first pass was measured slower: 1.25 -> 1.45 ms).
+__global__ void __launch_bounds__(kPartThreads, 2)
+k_bucket_scatter(const __grid_constant__ Geo g, int64_t n, int bucket_shift, int part_shift, int nbuckets,
+                  const Rec* __restrict__ in, int32_t* __restrict__ cursor, Rec* __restrict__ out) {
+  __shared__ GridSmem sm;
+  __shared__ int32_t cnt[kLocalCap];
+  __shared__ int32_t s_min;
+  load_grid_rows(sm, g);
+  const Scalars& sc = g.s;
+  const int tid = threadIdx.x, lane = tid & 31;
+  for (int64_t t0 = (int64_t)blockIdx.x * kPartTile; t0 < n; t0 += (int64_t)gridDim.x * kPartTile) {
+    for (int j = tid; j < kLocalCap; j += kPartThreads) cnt[j] = 0;
+    if (tid == 0) s_min = 0x7fffffff;
+    __syncthreads();
+    Rec r[kPartItems];
+    int bk[kPartItems];
+    int mn = 0x7fffffff;
+#pragma unroll
+    for (int j = 0; j < kPartItems; j++) {
+      const int64_t i = t0 + j * kPartThreads + tid;
+      r[j] = in[i < n ? i : n - 1];
+    }
+#pragma unroll
+    for (int j = 0; j < kPartItems; j++) {
+      const int sr = rec_sr(r[j]);
+      bk[j] = sr == kBadRow ? nbuckets : bin_of(sm, sc, sr, r[j].x, r[j].y, nullptr) >> bucket_shift;
+      if (t0 + j * kPartThreads + tid < n && bk[j] < mn) mn = bk[j];
+    }
+    mn = __reduce_min_sync(kFull, mn);
+    if (lane == 0) atomicMin(&s_min, mn);
+    __syncthreads();
+    const int b0 = (s_min >> part_shift) << part_shift;  // the records are ordered by part: the tile starts in this one
+    int where[kPartItems];  // rank inside the tile; -1 - slot for a bucket beyond the tile's reach (a tile that straddles
+                            // many small parts): that record takes a cursor atomic of its own
+#pragma unroll
+    for (int j = 0; j < kPartItems; j++) {
+      const bool valid = t0 + j * kPartThreads + tid < n;
+      const int loc = bk[j] - b0;
+      const bool local = loc < kLocalCap;
+      const int rk = tile_rank(cnt, local ? loc : 0, valid && local, lane);
+      where[j] = (valid && !local) ? -1 - atomicAdd(cursor + bk[j], 1) : rk;
+    }
+    __syncthreads();
+    for (int j = tid; j < kLocalCap; j += kPartThreads) {
+      const int c = cnt[j];
+      if (c) cnt[j] = atomicAdd(cursor + b0 + j, c);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kPartItems; j++)
+      if (t0 + j * kPartThreads + tid < n) out[where[j] < 0 ? -1 - where[j] : cnt[bk[j] - b0] + where[j]] = r[j];
+    __syncthreads();
   }
 }
 
@@ -285,6 +421,7 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
     if ((e = cudaFuncSetAttribute(k_bucket_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (kMaxBuckets + 1) * 4)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_bucket_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (32768 + 1024 + 32) * 4)) != cudaSuccess)
       return e;
+    if ((e = cudaFuncSetAttribute(k_part_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, kPartTile * 16)) != cudaSuccess) return e;
     attr_done = true;
   }
   if ((e = cudaMemsetAsync(w.counters, 0, sizeof(int32_t) * WC_N, st)) != cudaSuccess) return e;
@@ -296,13 +433,22 @@ cudaError_t launch_grid_build(const Geo& g, const Ws& w, const float* y, const f
                    g, n, sh, nbuckets, y, z, sector_row, w.bucket_first, w.counters)));
   // nbuckets grid buckets + the bucket of clusters without a valid (sector, row) + the total
   if ((e = exclusive_scan<int32_t>(w.bucket_first, w.bucket_first, nbuckets + 2, (int32_t*)w.scan_tmp, st)) != cudaSuccess) return e;
-  if ((e = cudaMemcpyAsync(w.bucket_cursor, w.bucket_first, sizeof(int32_t) * (size_t)(nbuckets + 2), cudaMemcpyDeviceToDevice,
-                           st)) != cudaSuccess)
-    return e;
-  if (n > 0)
+  // parts of 2^ps buckets: about the square root of the bucket count, at most kMaxParts
+  int ps = 0;
+  while (((int64_t)1 << (2 * ps)) < nbuckets || ((nbuckets + (1 << ps) - 1) >> ps) > kMaxParts) ps++;
+  const int nparts = (nbuckets + (1 << ps) - 1) >> ps;
+  int32_t* part_cursor = w.bucket_cursor + kMaxBuckets + 2;
+  TPC_LAUNCH(KID_SCAN, st,
+             (k_scan_cursors<<<blocks_for(nbuckets + 2, 256, 64), 256, 0, st>>>(nbuckets, ps, nparts, w.bucket_first, w.bucket_cursor,
+                                                                                part_cursor)));
+  if (n > 0) {
+    TPC_LAUNCH(KID_PART_SCATTER, st,
+               (k_part_scatter<<<blocks_for(n, kPartTile, 148 * 64), kPartThreads, kPartTile * 16, st>>>(g, n, sh, ps, nbuckets, nparts, y, z, sector_row,
+                                                                                            part_cursor, w.rec)));
     TPC_LAUNCH(KID_BUCKET_SCATTER, st,
-               (k_bucket_scatter<<<blocks_for(n, kThreads * kUnroll, kScatterCap), kThreads, 0, st>>>(g, n, sh, nbuckets, y, z, sector_row, w.bucket_cursor,
-                                                                              (Rec*)w.hit_rec)));
+               (k_bucket_scatter<<<blocks_for(n, kPartTile, 148 * 64), kPartThreads, 0, st>>>(g, n, sh, ps, nbuckets, w.rec, w.bucket_cursor,
+                                                                                               (Rec*)w.hit_rec)));
+  }
   TPC_LAUNCH(KID_BUCKET_SORT, st,
              (k_bucket_sort<<<blocks_for(nbuckets, 1, kSortCap), kSortThreads, sort_smem, st>>>(
                  g, n, nb, sh, nbuckets, w.bucket_first, (const Rec*)w.hit_rec, w.rec, w.bin_first)));

@@ -18,6 +18,7 @@ namespace tpc {
 enum KernelId {
   KID_BUCKET_HIST = 0,
   KID_SCAN,
+  KID_PART_SCATTER,
   KID_BUCKET_SCATTER,
   KID_BUCKET_SORT,
   KID_NEIGHBOURS,
