@@ -72,6 +72,7 @@ bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
   tpc::Scalars& s = G->s;
   s.nsec = P->n_sectors;
   s.nrows = P->n_rows;
+  s.rows_magic = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)P->n_rows - 1) / (uint64_t)P->n_rows);
   const float zspan = (P->z_hi - P->z_lo) / P->cell_z;
   if (!(zspan < 2.0e9f)) return false;
   s.nz = (int)ceilf(zspan);

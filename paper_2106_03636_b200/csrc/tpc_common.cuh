@@ -39,6 +39,7 @@ struct CaGeo {
 // Scalars (R4, R6, R7, R9-R22).
 struct Scalars {
   int32_t nsec, nrows, nz, bins_per_sector;
+  uint32_t rows_magic;  // ceil(2^32 / nrows): sector = umulhi(sector_row, rows_magic), exact for sector_row < 2^24
   int32_t slab_w, nslab;  // tracklet ordering: z slabs of slab_w bins, nslab = ceil(nz / slab_w)
   float inv_cy, inv_cz, z_lo, z_hi;
   float kB, sy2, sz2, sig_y, sig_z;
@@ -280,6 +281,9 @@ __device__ __forceinline__ int clampbin(float v, int n) {
 __device__ __forceinline__ Rec ld_rec(const Rec* __restrict__ recs, int k) { return __ldg(recs + k); }
 __device__ __forceinline__ int rec_idx(const Rec& r) { return __float_as_int(r.z); }
 __device__ __forceinline__ int rec_sr(const Rec& r) { return __float_as_int(r.w) & (kStartBit - 1); }
+// sector of a VALID sector_row (0 <= sr < nsec * nrows <= 2^24): sr / nrows without the integer division
+// (rows_magic * nrows - 2^32 < nrows <= 152, so the quotient is exact while sr * 152 < 2^32)
+__device__ __forceinline__ int sector_of(const Scalars& sc, int sr) { return (int)__umulhi((unsigned)sr, sc.rows_magic); }
 __device__ __forceinline__ bool rec_is_start(const Rec& r) { return (__float_as_int(r.w) & kStartBit) != 0; }
 
 // R20 selection key (layout above)

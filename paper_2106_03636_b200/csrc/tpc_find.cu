@@ -129,9 +129,10 @@ k_neighbours(const __grid_constant__ Geo g, int64_t n, const Rec* __restrict__ r
   for (int64_t p = (int64_t)blockIdx.x * kThreads + tid; p < n; p += (int64_t)gridDim.x * kThreads) {
     const Rec h = ld_rec(rec, (int)p);
     const int sr = rec_sr(h);
-    const int s = sr / nrows, r = sr - s * nrows;
+    const bool on_grid = sr < sc.nsec * nrows;  // (a cluster parked behind the grid has an impossible sector_row)
+    const int s = on_grid ? sector_of(sc, sr) : 0, r = sr - s * nrows;
     int bu = -1, bd = -1;
-    if (s < sc.nsec && r >= 1 && r <= nrows - 2) {  // (a cluster parked behind the grid has an impossible sector)
+    if (on_grid && r >= 1 && r <= nrows - 2) {
       const float yh = h.x, zh = h.y;
       const float wu = ca.wu[r], iy = ca.iy[r], iz = ca.iz[r];
       const float wyu = ca.wyu[r], wzu = ca.wzu[r], wyd = ca.wyd[r], wzd = ca.wzd[r];

@@ -51,7 +51,7 @@ __device__ __forceinline__ void load_grid_rows(GridSmem& sm, const Geo& g) {
 
 // R7 bin id, fp32, one rounding per operation; *clamped is raised for zeta outside [z_lo, z_hi].
 __device__ __forceinline__ int bin_of(const GridSmem& sm, const Scalars& sc, int sr, float yy, float zz, bool* clamped) {
-  const int s = sr / sc.nrows, r = sr - s * sc.nrows;
+  const int s = sector_of(sc, sr), r = sr - s * sc.nrows;  // callers pass valid sector_rows only
   const float zeta = (s < 18) ? zz : -zz;  // R2/R7: mirrored drift coordinate
   const int yb = clampbin((yy + sm.ymax[r]) * sc.inv_cy, sm.ny[r]);
   const int zb = clampbin((zeta - sc.z_lo) * sc.inv_cz, sc.nz);
