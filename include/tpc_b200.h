@@ -54,7 +54,8 @@ typedef enum {
   TPC_OK = 0,
   TPC_EINVAL = -1,     /* NULL pointer, negative size, n_rows/n_sectors out of range, bins >= 2^31 */
   TPC_ENOMEM_WS = -2,  /* ws_bytes smaller than tpc_workspace_bytes() for these sizes */
-  TPC_ECUDA = -3       /* a CUDA runtime call failed at enqueue time (see tpc_last_cuda_error) */
+  TPC_ECUDA = -3,      /* a CUDA runtime call failed at enqueue time (see tpc_last_cuda_error) */
+  TPC_ELIMIT = -4      /* a size beyond the fixed scratch array of a *_static entry point (tpc_pair_sides_static) */
 } tpc_status_t;
 
 /* indices into the int32 counters[TPC_N_COUNTERS] device array written by tpc_find_tracks */
@@ -234,6 +235,39 @@ int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, cons
                    int64_t max_collisions, double dt_max, double sigma_t, double v_drift, void* workspace,
                    size_t ws_bytes, int32_t* pair_of_a, int32_t* pair_of_c, float* t, float* z_vertex,
                    int32_t* n_pairs, void* stream);
+
+/* tpc_pair_sides without a workspace, for callers that cannot allocate device memory.
+ * Who that is: code that runs where cudaMalloc is not allowed or not wanted -- a processing step inside a framework
+ * that hands out all GPU memory itself from one big pre-allocated block (the online processing keeps
+ * reusing one block of GPU memory for its consecutive processing steps, sized so that a whole Time Frame fits), a callback or a thread
+ * that must not take the allocator's device-wide lock or cause the implicit synchronisation a cudaMalloc / cudaFree
+ * brings, a process whose memory budget was handed out completely at start-up.  Such a caller has device buffers for
+ * its inputs and outputs but no spare block to pass as `workspace` and no way to get one.
+ * What it does: exactly tpc_pair_sides (same kernels, same arithmetic, same outputs bit for bit), with the two
+ * arg-min tables best_c / best_a -- the only scratch memory that operation needs -- placed in an array that is part of
+ * the library image: 2 x 65 792 bytes = 128.5 KiB of device memory on every GPU that loads the library, held until
+ * the process exits.  The caller passes inputs and outputs only; the call makes no cudaMalloc, cudaFree or any
+ * other allocating call (it does not create events either: its three launches are counted by tpc_profile_collect
+ * but never timed).
+ * Limit: max_collisions <= TPC_PAIR_SIDES_STATIC_MAX (16 384 collisions per side; a 128-orbit Time Frame at 50 kHz
+ * holds about 570).  A larger value returns TPC_ELIMIT and enqueues nothing; use tpc_pair_sides with a workspace of
+ * your own for that.  As for tpc_pair_sides, max_collisions must be at least the capacity the two
+ * tpc_find_collisions calls were given (the device-side counts n_collisions_a[1], n_collisions_c[1] are trusted
+ * not to exceed it).
+ * First call on a device: the library looks up the device address of the array once per device (with the
+ * caller's current device; cudaGetSymbolAddress, which may also make the CUDA runtime load the library's
+ * kernels on that device).  Make this first call during set-up, outside any stream capture; an easy way is one call
+ * with empty lists (n_collisions_*[1] = 0).  Later calls on that device only launch the three kernels on `stream`.
+ * Sharing: all calls on one GPU use the same array -- from every stream, every host thread and every library user in
+ * the process.  Nothing in it has to start at zero (each call overwrites the entries it later reads), so there is
+ * nothing to clear between calls; but two calls whose kernels can overlap on the GPU (different streams without an
+ * event between them) race on it and give wrong pairs.  Keep all calls on one stream, or order them with events.
+ * Errors: TPC_EINVAL as tpc_pair_sides; TPC_ELIMIT as above; TPC_ECUDA if the address look-up or a launch fails. */
+#define TPC_PAIR_SIDES_STATIC_MAX 16384
+int tpc_pair_sides_static(const int32_t* n_collisions_a, const float* coll_time_a, const int32_t* coll_ntracks_a,
+                          const int32_t* n_collisions_c, const float* coll_time_c, const int32_t* coll_ntracks_c,
+                          int64_t max_collisions, double dt_max, double sigma_t, double v_drift, int32_t* pair_of_a,
+                          int32_t* pair_of_c, float* t, float* z_vertex, int32_t* n_pairs, void* stream);
 
 /* ---- host-buffer entry points (bench.py `e2e`; a continuous stream of Time Frames through
  * reused GPU memory) ---------------------------------------------------------------------------------------------

@@ -30,7 +30,7 @@ SYMBOLS = ("tpc_strerror", "tpc_last_cuda_error", "tpc_version", "tpc_grid_bins"
            "tpc_grid_build", "tpc_grid_export", "tpc_find_tracks", "tpc_find_export", "tpc_fit_tracks",
            "tpc_track_time", "tpc_collisions_workspace_bytes", "tpc_find_collisions", "tpc_merge_workspace_bytes",
            "tpc_merge_tracks", "tpc_clusterize_workspace_bytes", "tpc_clusterize", "tpc_fit_tracks_physics",
-           "tpc_tag_clusters", "tpc_pair_sides_workspace_bytes", "tpc_pair_sides", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
+           "tpc_tag_clusters", "tpc_pair_sides_workspace_bytes", "tpc_pair_sides", "tpc_pair_sides_static", "tpc_track_host", "tpc_track_host_async", "tpc_track_host_fetch", "tpc_profile_enable", "tpc_profile_kernels", "tpc_profile_name", "tpc_profile_collect", "tpc_fp32_peak")
 
 
 class tpc_params_t(C.Structure):
@@ -206,6 +206,43 @@ def clusterize(params, sector_row, pad, time, adc, pad_width, time_width, peak_m
     res = {k: v[:written].cpu().numpy() for k, v in out.items()}
     res["n_found"] = found
     return res
+
+
+PAIR_SIDES_STATIC_MAX = 16384   # TPC_PAIR_SIDES_STATIC_MAX
+
+
+def pair_sides_static(n_a, t_a, c_a, n_c, t_c, c_c, max_collisions: int, dt_max: float = 15.5, sigma_t: float = 3.88,
+                      v_drift: float = 2.58, out=None):
+    """tpc_pair_sides_static: the R29 pairing for callers that cannot allocate device memory -- code running inside a
+    framework that owns all GPU memory, or anywhere a cudaMalloc (device-wide lock, implicit synchronisation) is not
+    acceptable.  The library keeps the two small arg-min tables the pairing needs in an array of its own device image
+    (128.5 KiB per GPU, up to PAIR_SIDES_STATIC_MAX = 16384 collisions per side; more raises TpcError "size beyond the
+    fixed scratch array").  The result is that of Tracker.pair_sides bit for bit.
+    Inputs: the device tensors two find_collisions calls left (n_collisions [2] int32, coll_time float32, coll_ntracks
+    int32, side A then side C).  out: optional dict of preallocated device tensors pair_of_a, pair_of_c (int32
+    [max_collisions]), t, z_vertex (float32 [max_collisions]), n_pairs (int32 [1]); with it this wrapper allocates
+    nothing on the device either and only enqueues (returns `out`).  Without it the outputs are torch tensors made here
+    and the numpy dict of Tracker.pair_sides comes back (synchronises).
+    The first call on a GPU looks up the array's address: make it before any stream capture.  All calls on a GPU share
+    the array: keep them on one stream (calls that overlap on the GPU race)."""
+    import torch as t
+    cap = int(max_collisions)
+    o = out
+    if o is None:
+        dev = t_a.device
+        o = dict(pair_of_a=t.empty(max(cap, 1), dtype=t.int32, device=dev), pair_of_c=t.empty(max(cap, 1), dtype=t.int32, device=dev),
+                 t=t.empty(max(cap, 1), dtype=t.float32, device=dev), z_vertex=t.empty(max(cap, 1), dtype=t.float32, device=dev),
+                 n_pairs=t.zeros(1, dtype=t.int32, device=dev))
+    _check(load().tpc_pair_sides_static(_dp(n_a), _dp(t_a), _dp(c_a), _dp(n_c), _dp(t_c), _dp(c_c), C.c_int64(cap),
+                                        C.c_double(dt_max), C.c_double(sigma_t), C.c_double(v_drift), _dp(o["pair_of_a"]),
+                                        _dp(o["pair_of_c"]), _dp(o["t"]), _dp(o["z_vertex"]), _dp(o["n_pairs"]), _stream()),
+           "tpc_pair_sides_static")
+    if out is not None:
+        return out
+    k = int(o["n_pairs"].item())
+    na, nc_ = int(n_a[1].item()), int(n_c[1].item())
+    return dict(pair_of_a=o["pair_of_a"][:na].cpu().numpy(), pair_of_c=o["pair_of_c"][:nc_].cpu().numpy(), t=o["t"][:k].cpu().numpy(),
+                z_vertex=o["z_vertex"][:k].cpu().numpy())
 
 
 def work_counts(counters) -> dict:
@@ -459,6 +496,12 @@ class Tracker:
         na, nc_ = int(a["n"][1].item()), int(c["n"][1].item())
         return dict(pair_of_a=pa[:na].cpu().numpy(), pair_of_c=pc[:nc_].cpu().numpy(), t=tt[:k].cpu().numpy(),
                     z_vertex=zv[:k].cpu().numpy())
+
+    def pair_sides_static(self, dt_max: float = 15.5, sigma_t: float = 3.88, v_drift: float = 2.58):
+        """pair_sides through tpc_pair_sides_static: same result, no workspace (see pair_sides_static below)."""
+        a, c = self._coll[1], self._coll[-1]
+        return pair_sides_static(a["n"], a["time"], a["ntracks"], c["n"], c["time"], c["ntracks"], min(a["cap"], c["cap"]),
+                                 dt_max, sigma_t, v_drift)
 
     def step(self, y, z, sector_row):
         """One pass of the whole hot path (a1..a6) on device-resident inputs; asynchronous."""

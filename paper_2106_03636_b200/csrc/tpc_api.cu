@@ -48,6 +48,8 @@ void prof_end(int id, cudaStream_t st) {
   cudaEventRecord(g_rec[g_nrec].b, st);
   g_nrec++;
 }
+
+void prof_count(int id) { g_launches[id]++; }
 }  // namespace tpc
 
 namespace {
@@ -58,6 +60,14 @@ int cuda_fail(cudaError_t e) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
   return TPC_ECUDA;
 }
+}  // namespace
+
+// cuda_fail for the entry points that live beside their kernels (tpc_pair_sides_static in tpc_collisions.cu).
+namespace tpc {
+int report_cuda_error(cudaError_t e) { return cuda_fail(e); }
+}  // namespace tpc
+
+namespace {
 
 // Builds the device geometry from the host POD.  Returns false if the parameters are unusable.
 bool make_geo(const tpc_params_t* P, tpc::Geo* G, int64_t* n_bins) {
@@ -167,6 +177,7 @@ const char* tpc_strerror(int status) {
     case TPC_EINVAL: return "invalid argument";
     case TPC_ENOMEM_WS: return "workspace too small";
     case TPC_ECUDA: return "CUDA runtime error";
+    case TPC_ELIMIT: return "size beyond the fixed scratch array of a *_static entry point";
     default: return "unknown status";
   }
 }

@@ -10,6 +10,8 @@
 //
 // Sizes are tiny next to the hot path (1.8e6 tracks, ~1e4 bins per Time Frame): clarity over speed.
 // =============================================================================================
+#include <mutex>
+
 #include "tpc_common.cuh"
 #include "tpc_prof.cuh"
 #include "tpc_scan.cuh"
@@ -224,3 +226,82 @@ cudaError_t launch_collisions(const int32_t* counters, int64_t max_tracks, const
 }
 
 }  // namespace tpc
+
+// =============================================================================================
+// tpc_pair_sides_static -- tpc_pair_sides for callers that cannot allocate device memory (include/tpc_b200.h has the
+// user's view: who such callers are, the limit, the first-call rule, the sharing rule).
+//
+// The two arg-min tables of R29 (best_c: side A's choice per side-A collision, best_a: side C's choice) are the only
+// scratch memory the pairing needs.  Here they live in a file-scope __device__ array, i.e. in the device image of
+// this library: the driver reserves it on a GPU when the library's module is loaded there and keeps it until the
+// process ends.  Nothing is allocated at call time.
+//
+// g_pair_scratch below is only a handle on the host side.  Host code cannot use `g_pair_scratch` as a pointer: that
+// expression is the address of a host shadow variable, and a kernel handed it would fault (or, on a system where the
+// GPU can read host memory, scribble over the shadow instead of the real array).  The device address is asked for once
+// per device with cudaGetSymbolAddress while that device is current, checked, cached in g_pair_scratch_dev[device], and
+// that pointer is what the kernels get -- the very kernels tpc_pair_sides runs, through the same launch sequence.
+// =============================================================================================
+namespace {
+
+constexpr size_t kPairStaticHalf = (sizeof(int32_t) * (size_t)(TPC_PAIR_SIDES_STATIC_MAX + 1) + 255) & ~(size_t)255;  // one table
+static __device__ __align__(256) unsigned char g_pair_scratch[2 * kPairStaticHalf];  // best_c | best_a, 131 584 bytes
+
+constexpr int kPairMaxDevices = 64;
+void* g_pair_scratch_dev[kPairMaxDevices] = {nullptr};  // device address of g_pair_scratch on device d; NULL = not looked up yet
+std::mutex g_pair_scratch_mutex;
+
+// Device address of the scratch array on the CURRENT device.  The first call per device does the look-up (and with it
+// whatever module loading the runtime still owes on that device); later calls read the cache.
+cudaError_t pair_scratch_address(void** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool cached = dev >= 0 && dev < kPairMaxDevices;
+  std::lock_guard<std::mutex> lock(g_pair_scratch_mutex);
+  if (cached && g_pair_scratch_dev[dev]) {
+    *out = g_pair_scratch_dev[dev];
+    return cudaSuccess;
+  }
+  void* p = nullptr;
+  e = cudaGetSymbolAddress(&p, g_pair_scratch);
+  if (e != cudaSuccess) return e;
+  if (!p || ((uintptr_t)p & 255) != 0) return cudaErrorInvalidSymbol;
+  if (cached) g_pair_scratch_dev[dev] = p;
+  *out = p;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int tpc_pair_sides_static(const int32_t* n_collisions_a, const float* coll_time_a, const int32_t* coll_ntracks_a,
+                                     const int32_t* n_collisions_c, const float* coll_time_c, const int32_t* coll_ntracks_c,
+                                     int64_t max_collisions, double dt_max, double sigma_t, double v_drift, int32_t* pair_of_a,
+                                     int32_t* pair_of_c, float* t, float* z_vertex, int32_t* n_pairs, void* stream) {
+  if (max_collisions < 1 || !(dt_max > 0.0) || !(sigma_t > 0.0) || !(v_drift > 0.0) || !n_collisions_a || !coll_time_a ||
+      !coll_ntracks_a || !n_collisions_c || !coll_time_c || !coll_ntracks_c || !pair_of_a || !pair_of_c || !t || !z_vertex ||
+      !n_pairs)
+    return TPC_EINVAL;
+  if (max_collisions > TPC_PAIR_SIDES_STATIC_MAX) return TPC_ELIMIT;  // the tables would not fit the fixed array
+  void* scratch = nullptr;
+  cudaError_t e = pair_scratch_address(&scratch);
+  if (e != cudaSuccess) return tpc::report_cuda_error(e);
+  // Same layout as launch_pair_sides gives a caller's workspace: best_c first, best_a one 256-byte-rounded table
+  // later.  max_collisions <= the static maximum, so both tables end inside the array.
+  int32_t* best_c = (int32_t*)scratch;
+  int32_t* best_a = (int32_t*)((char*)scratch + tpc::align256(sizeof(int32_t) * (size_t)(max_collisions + 1)));
+  cudaStream_t st = (cudaStream_t)stream;
+  const unsigned blocks = tpc::blocks_for(max_collisions, tpc::kThreads, 148 * 4);
+  // plain launches: counted, never bracketed by events (creating an event is an allocation)
+  tpc::prof_count(tpc::KID_COLLISIONS);
+  tpc::k_pair_best<<<blocks, tpc::kThreads, 0, st>>>(0, n_collisions_a, coll_time_a, coll_ntracks_a, n_collisions_c, coll_time_c,
+                                                     coll_ntracks_c, dt_max, sigma_t, best_c);
+  tpc::prof_count(tpc::KID_COLLISIONS);
+  tpc::k_pair_best<<<blocks, tpc::kThreads, 0, st>>>(1, n_collisions_a, coll_time_a, coll_ntracks_a, n_collisions_c, coll_time_c,
+                                                     coll_ntracks_c, dt_max, sigma_t, best_a);
+  tpc::prof_count(tpc::KID_COLLISIONS);
+  tpc::k_pair_emit<<<1, 1, 0, st>>>(n_collisions_a, coll_time_a, n_collisions_c, coll_time_c, best_c, best_a, v_drift, pair_of_a,
+                                    pair_of_c, t, z_vertex, n_pairs);
+  e = cudaGetLastError();
+  return e == cudaSuccess ? TPC_OK : tpc::report_cuda_error(e);
+}

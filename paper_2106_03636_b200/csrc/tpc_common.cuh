@@ -241,6 +241,9 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
                          int32_t* g_head, int32_t* g_nseg, int32_t* g_nhits, float* gpar, float* gcov, float* gxref,
                          float* gzref, float* gchi2, int32_t* gndf, cudaStream_t st);
 
+// tpc_api.cu: records the text of a failed CUDA call for tpc_last_cuda_error and returns TPC_ECUDA
+int report_cuda_error(cudaError_t e);
+
 size_t pair_sides_ws_bytes(int64_t max_collisions);
 cudaError_t launch_pair_sides(const int32_t* n_a, const float* t_a, const int32_t* c_a, const int32_t* n_c, const float* t_c,
                               const int32_t* c_c, int64_t max_collisions, double dt_max, double sigma_t, double v_drift,

@@ -43,6 +43,9 @@ enum KernelId {
 
 void prof_begin(int id, cudaStream_t st);
 void prof_end(int id, cudaStream_t st);
+// Counts one launch of kernel `id` and nothing else: no event is created or recorded, whatever tpc_profile_enable
+// says.  For entry points that promise to allocate nothing (tpc_pair_sides_static).
+void prof_count(int id);
 
 struct ProfScope {
   int id;
