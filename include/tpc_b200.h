@@ -228,7 +228,10 @@ int tpc_find_collisions(const int32_t* counters, int64_t max_tracks, const float
  * the reciprocal arg-mins (ties: the lower index).  Outputs (device): pair_of_a, pair_of_c [max_collisions] (partner
  * or -1), t, z_vertex [max_collisions] per pair in ascending side-A index (t = (t_a + t_c)/2, z_vertex =
  * v_drift (t_c - t_a)/2), n_pairs [1].  workspace: tpc_pair_sides_workspace_bytes(max_collisions), 256-byte aligned.
- * Enqueue only. */
+ * max_collisions is the capacity of every per-collision array passed here; a side whose list holds more
+ * (n_collisions[1] > max_collisions, e.g. tpc_find_collisions was given a larger capacity) is read up to its first
+ * max_collisions entries only -- the lists are in time order, so the later collisions stay unpaired -- and nothing is
+ * written beyond that capacity.  max_collisions <= 2147483000.  Enqueue only. */
 int tpc_pair_sides_workspace_bytes(int64_t max_collisions, size_t* bytes_host);
 int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, const int32_t* coll_ntracks_a,
                    const int32_t* n_collisions_c, const float* coll_time_c, const int32_t* coll_ntracks_c,
@@ -251,9 +254,8 @@ int tpc_pair_sides(const int32_t* n_collisions_a, const float* coll_time_a, cons
  * but never timed).
  * Limit: max_collisions <= TPC_PAIR_SIDES_STATIC_MAX (16 384 collisions per side; a 128-orbit Time Frame at 50 kHz
  * holds about 570).  A larger value returns TPC_ELIMIT and enqueues nothing; use tpc_pair_sides with a workspace of
- * your own for that.  As for tpc_pair_sides, max_collisions must be at least the capacity the two
- * tpc_find_collisions calls were given (the device-side counts n_collisions_a[1], n_collisions_c[1] are trusted
- * not to exceed it).
+ * your own for that.  As for tpc_pair_sides, a list longer than max_collisions is read up to its first
+ * max_collisions entries, so the array is never overrun whatever the device-side counts say.
  * First call on a device: the library looks up the device address of the array once per device (with the
  * caller's current device; cudaGetSymbolAddress, which may also make the CUDA runtime load the library's
  * kernels on that device).  Make this first call during set-up, outside any stream capture; an easy way is one call

@@ -118,9 +118,10 @@ k_t0_assign(const int32_t* __restrict__ counters, int64_t max_tracks, int64_t nb
 // order; ties go to the lower index (strict < while the partner index ascends).
 __global__ void __launch_bounds__(kThreads)
 k_pair_best(int which, const int32_t* __restrict__ n_a, const float* __restrict__ t_a, const int32_t* __restrict__ c_a,
-            const int32_t* __restrict__ n_c, const float* __restrict__ t_c, const int32_t* __restrict__ c_c, double dt_max,
-            double sigma_t, int32_t* __restrict__ best) {
-  const int nA = n_a[1], nC = n_c[1];
+            const int32_t* __restrict__ n_c, const float* __restrict__ t_c, const int32_t* __restrict__ c_c, int max_coll,
+            double dt_max, double sigma_t, int32_t* __restrict__ best) {
+  // the counts come from device memory: never beyond the capacity the tables and outputs were sized for
+  const int nA = min(max(n_a[1], 0), max_coll), nC = min(max(n_c[1], 0), max_coll);
   const int n_own = which == 0 ? nA : nC, n_oth = which == 0 ? nC : nA;
   for (int i = blockIdx.x * kThreads + threadIdx.x; i < n_own; i += gridDim.x * kThreads) {
     int b = -1;
@@ -143,9 +144,9 @@ k_pair_best(int which, const int32_t* __restrict__ n_a, const float* __restrict_
 // reciprocal pairs in ascending order of the side-A index (a Time Frame holds a few hundred collisions: one thread)
 __global__ void k_pair_emit(const int32_t* __restrict__ n_a, const float* __restrict__ t_a, const int32_t* __restrict__ n_c,
                             const float* __restrict__ t_c, const int32_t* __restrict__ best_c, const int32_t* __restrict__ best_a,
-                            double v_drift, int32_t* __restrict__ pair_of_a, int32_t* __restrict__ pair_of_c, float* __restrict__ t_out,
-                            float* __restrict__ zv_out, int32_t* __restrict__ n_pairs) {
-  const int nA = n_a[1], nC = n_c[1];
+                            int max_coll, double v_drift, int32_t* __restrict__ pair_of_a, int32_t* __restrict__ pair_of_c,
+                            float* __restrict__ t_out, float* __restrict__ zv_out, int32_t* __restrict__ n_pairs) {
+  const int nA = min(max(n_a[1], 0), max_coll), nC = min(max(n_c[1], 0), max_coll);
   for (int j = 0; j < nC; j++) pair_of_c[j] = -1;
   int np = 0;
   for (int i = 0; i < nA; i++) {
@@ -174,10 +175,11 @@ cudaError_t launch_pair_sides(const int32_t* n_a, const float* t_a, const int32_
   int32_t* best_c = (int32_t*)workspace;
   int32_t* best_a = (int32_t*)((char*)workspace + align256(sizeof(int32_t) * (size_t)(max_collisions + 1)));
   const unsigned blocks = blocks_for(max_collisions, kThreads, 148 * 4);
-  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(0, n_a, t_a, c_a, n_c, t_c, c_c, dt_max, sigma_t, best_c)));
-  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(1, n_a, t_a, c_a, n_c, t_c, c_c, dt_max, sigma_t, best_a)));
+  const int cap = (int)max_collisions;
+  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(0, n_a, t_a, c_a, n_c, t_c, c_c, cap, dt_max, sigma_t, best_c)));
+  TPC_LAUNCH(KID_COLLISIONS, st, (k_pair_best<<<blocks, kThreads, 0, st>>>(1, n_a, t_a, c_a, n_c, t_c, c_c, cap, dt_max, sigma_t, best_a)));
   TPC_LAUNCH(KID_COLLISIONS, st,
-             (k_pair_emit<<<1, 1, 0, st>>>(n_a, t_a, n_c, t_c, best_c, best_a, v_drift, pair_of_a, pair_of_c, t_out, zv_out, n_pairs)));
+             (k_pair_emit<<<1, 1, 0, st>>>(n_a, t_a, n_c, t_c, best_c, best_a, cap, v_drift, pair_of_a, pair_of_c, t_out, zv_out, n_pairs)));
   return cudaGetLastError();
 }
 
@@ -294,13 +296,14 @@ extern "C" int tpc_pair_sides_static(const int32_t* n_collisions_a, const float*
   const unsigned blocks = tpc::blocks_for(max_collisions, tpc::kThreads, 148 * 4);
   // plain launches: counted, never bracketed by events (creating an event is an allocation)
   tpc::prof_count(tpc::KID_COLLISIONS);
+  const int cap = (int)max_collisions;
   tpc::k_pair_best<<<blocks, tpc::kThreads, 0, st>>>(0, n_collisions_a, coll_time_a, coll_ntracks_a, n_collisions_c, coll_time_c,
-                                                     coll_ntracks_c, dt_max, sigma_t, best_c);
+                                                     coll_ntracks_c, cap, dt_max, sigma_t, best_c);
   tpc::prof_count(tpc::KID_COLLISIONS);
   tpc::k_pair_best<<<blocks, tpc::kThreads, 0, st>>>(1, n_collisions_a, coll_time_a, coll_ntracks_a, n_collisions_c, coll_time_c,
-                                                     coll_ntracks_c, dt_max, sigma_t, best_a);
+                                                     coll_ntracks_c, cap, dt_max, sigma_t, best_a);
   tpc::prof_count(tpc::KID_COLLISIONS);
-  tpc::k_pair_emit<<<1, 1, 0, st>>>(n_collisions_a, coll_time_a, n_collisions_c, coll_time_c, best_c, best_a, v_drift, pair_of_a,
+  tpc::k_pair_emit<<<1, 1, 0, st>>>(n_collisions_a, coll_time_a, n_collisions_c, coll_time_c, best_c, best_a, cap, v_drift, pair_of_a,
                                     pair_of_c, t, z_vertex, n_pairs);
   e = cudaGetLastError();
   return e == cudaSuccess ? TPC_OK : tpc::report_cuda_error(e);

@@ -96,3 +96,45 @@ def test_pair_sides_matches_oracle_and_truth(slice8, orc):
         d = np.abs(p["t"] - t)
         assert d.min() < 1.0, f"collision at {t:.1f} us has no pair (nearest {p['t'][d.argmin()]:.1f})"
         assert abs(p["z_vertex"][d.argmin()] - z) < 2.0
+
+
+def test_pair_sides_reads_no_more_than_its_capacity(orc):
+    """The per-side counts are read on the device.  A list longer than the max_collisions passed to tpc_pair_sides (the
+    collision finder was given a larger capacity) is paired on its first max_collisions entries only and nothing is
+    written beyond the capacity of the outputs or of the workspace."""
+    import ctypes as C
+    import torch
+    from paper_2106_03636_b200 import binding
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: -m gpu tests must run on the B200 box")
+    lib = binding.load()
+    rng = np.random.default_rng(29)
+    n, cap, guard = 600, 256, 64
+    t_true = np.sort(rng.uniform(0.0, 12000.0, n))
+    zv = rng.normal(0.0, 5.0, n)
+    tA, tC = np.sort(t_true - zv / V_DRIFT).astype(np.float32), np.sort(t_true + zv / V_DRIFT).astype(np.float32)
+    cA = rng.integers(10, 900, n).astype(np.int32)
+    cC = np.maximum(1, cA + rng.integers(-8, 9, n)).astype(np.int32)
+    dev = lambda a: torch.from_numpy(a).cuda()
+    nn = torch.tensor([n, n], dtype=torch.int32, device="cuda")
+    wsb = C.c_size_t(0)
+    assert lib.tpc_pair_sides_workspace_bytes(C.c_int64(cap), C.byref(wsb)) == 0
+    ws = torch.full((int(wsb.value) + 4 * guard,), 0x5A, dtype=torch.uint8, device="cuda")
+    mk = lambda dt, v: torch.full((cap + guard,), v, dtype=dt, device="cuda")
+    pa, pc, tt, zz = mk(torch.int32, -7), mk(torch.int32, -7), mk(torch.float32, -7.0), mk(torch.float32, -7.0)
+    npairs = torch.zeros(1, dtype=torch.int32, device="cuda")
+    p = lambda x: C.c_void_p(x.data_ptr())
+    dA, dcA, dC, dcC = dev(tA), dev(cA), dev(tC), dev(cC)
+    rc = lib.tpc_pair_sides(p(nn), p(dA), p(dcA), p(nn), p(dC), p(dcC), C.c_int64(cap), C.c_double(15.5), C.c_double(3.88),
+                            C.c_double(V_DRIFT), p(ws), C.c_size_t(int(wsb.value)), p(pa), p(pc), p(tt), p(zz), p(npairs),
+                            C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert rc == 0
+    torch.cuda.synchronize()
+    o = orc.pair_sides(tA[:cap], cA[:cap], tC[:cap], cC[:cap], v_drift=V_DRIFT)
+    k = int(npairs.item())
+    assert k == o["t"].size > 200
+    assert np.array_equal(pa[:cap].cpu().numpy(), o["pair_of_a"]) and np.array_equal(pc[:cap].cpu().numpy(), o["pair_of_c"])
+    assert np.array_equal(tt[:k].cpu().numpy(), o["t"]) and np.array_equal(zz[:k].cpu().numpy(), o["z_vertex"])
+    for out in (pa, pc, tt, zz):
+        assert bool((out[cap:] == -7).all()), "written beyond max_collisions"
+    assert bool((ws[int(wsb.value):] == 0x5A).all()), "workspace overrun"
