@@ -408,7 +408,10 @@ int tpc_clusterize(const tpc_params_t* params_host, int64_t n_digits, const int3
  *                                     keeps its tpc_fit_tracks result; chi2 = ndf = -1 if a transport ran into max_sinphi
  * K = counters[TPC_CNT_TRACKS] is read on the device.  Enqueue only.  TPC_EINVAL for missing buffers or parameters
  * out of range (chi2_cut, dz_max > 0, ce_tol >= 0, 1 <= max_rows <= 151, max_tracks <= 2^28), TPC_ENOMEM_WS for a short
- * workspace. */
+ * workspace.
+ * params->n_fit_passes must be even (TPC_EINVAL otherwise): the matching and the chain refit take the state of every
+ * sector-local track at its INNERMOST hit, which is where tpc_fit_tracks leaves it after an even number of passes
+ * (outward, inward, ...; the default is 2); after an odd number it sits at the outermost hit. */
 typedef struct {
   float chi2_cut;    /* 50  */
   float dz_max;      /* 64 cm */

@@ -396,6 +396,8 @@ def merge_fit(p, y, z, sector_row, fit, sector, trk_nhits, trk_first_hit, trk_hi
 def merge(p, y, z, sector_row, o, mp=None, precision="f32", want_pairs=False):
     """R26 on the output `o` of run(): matching + refit of the chains.  Returns the two dicts merged, plus the
     per-track (sector, row_first, row_last) it derived from the hit lists."""
+    if int(p.n_fit_passes) % 2 != 0:
+        raise ValueError("R26 takes every fitted state at the track's innermost hit: n_fit_passes must be even")
     sector, rf, rl = track_rows(int(p.n_rows), sector_row, o["trk_nhits"], o["trk_first_hit"], o["trk_hits"])
     m = merge_match(p, o["par"], o["cov"], o["zref"], sector, rf, rl, o["trk_seed"], mp, precision, want_pairs)
     f = merge_fit(p, y, z, sector_row, o, sector, o["trk_nhits"], o["trk_first_hit"], o["trk_hits"], m["succ"], m["pred"],

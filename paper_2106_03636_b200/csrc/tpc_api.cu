@@ -417,6 +417,10 @@ int tpc_merge_tracks(const tpc_params_t* params_host, const tpc_merge_params_t* 
   Prep pr;
   const int rc = prepare(params_host, n_clusters, max_tracklets, find_workspace, find_ws_bytes, &pr);
   if (rc != TPC_OK) return rc;
+  // R26 reads every fitted state at the track's innermost hit (end buckets, z windows, the transport to the outer end, the
+  // start of the chain refit).  R22 leaves it there only after an even number of passes (out, in, ...); after an odd
+  // number it sits at the outermost hit and all of that would be silently wrong.
+  if (params_host->n_fit_passes % 2 != 0) return TPC_EINVAL;
   if (!merge_host || !(merge_host->chi2_cut > 0.0f) || !(merge_host->dz_max > 0.0f) || !(merge_host->ce_tol >= 0.0f) ||
       merge_host->max_rows < 1 || merge_host->max_rows > 151)
     return TPC_EINVAL;

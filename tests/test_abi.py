@@ -120,3 +120,23 @@ def test_other_struct_layouts_match_header(name, mirror):
         assert C.sizeof(cls) == 4 * len(fields) and all(f[1] is C.c_float for f in cls._fields_)
     else:
         assert C.sizeof(cls) == 8 * len(fields)
+
+
+def test_merge_refuses_an_odd_number_of_fit_passes_without_a_gpu():
+    """R26 reads the fitted states at the innermost hit, where R22 leaves them after an even number of passes only.  With
+    every other argument valid an odd n_fit_passes is TPC_EINVAL; the same call with an even one gets as far as the last
+    host-side check (merge workspace too small: TPC_ENOMEM_WS).  Nothing is enqueued either way."""
+    lib = binding.load()
+    fake = 256 * 1000                       # aligned, never dereferenced
+    dev = binding.tpc_result_t(*[C.c_void_p(fake)] * len(binding.tpc_result_t._fields_))
+    out = binding.tpc_merged_t(*[C.c_void_p(fake)] * len(binding.tpc_merged_t._fields_))
+    M = binding.tpc_merge_params_t(50.0, 64.0, 1.0, 12)
+
+    def call(passes):
+        P = binding.make_params(TpcParams(n_fit_passes=passes))
+        return lib.tpc_merge_tracks(C.byref(P), C.byref(M), C.c_int64(10), C.c_int64(10), C.c_void_p(fake), C.c_size_t(1 << 40),
+                                    C.c_void_p(fake), C.c_int64(100), C.byref(dev), C.c_void_p(fake), C.c_size_t(0), C.byref(out),
+                                    C.c_void_p(0))
+
+    assert call(2) == -2 and call(4) == -2
+    assert call(1) == -1 and call(3) == -1

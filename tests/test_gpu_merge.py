@@ -85,3 +85,18 @@ def test_merge_argument_errors(torch_cuda):
         trk.merge_tracks(chi2_cut=0.0)
     with pytest.raises(binding.TpcError):
         trk.merge_tracks(max_rows=0)
+
+
+@pytest.mark.parametrize("passes", [1, 3])
+def test_merge_refuses_tracks_fitted_with_an_odd_number_of_passes(torch_cuda, passes):
+    """After an odd number of R22 passes the fitted state sits at the outermost hit; R26 needs it at the innermost one.
+    find + fit run as usual, tpc_merge_tracks returns TPC_EINVAL instead of linking from the wrong end."""
+    from paper_2106_03636_b200 import binding
+    ev = make_config(0)
+    t = torch_cuda
+    p = ev.params.with_(n_fit_passes=passes)
+    trk = binding.Tracker(p, ev.n)
+    res = trk.run(t.from_numpy(ev.y).cuda(), t.from_numpy(ev.z).cuda(), t.from_numpy(ev.sector_row).cuda())
+    assert res["trk_seed"].size > 50
+    with pytest.raises(binding.TpcError, match="invalid argument"):
+        trk.merge_tracks()
