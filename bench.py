@@ -10,7 +10,7 @@ One "step" = one pass of the whole hot path (tpc_grid_build -> tpc_find_tracks -
  value        clusters/s with the clusters resident in HBM (CUDA events around K steps, no per-kernel events inside;
               max over ranks)
  e2e          same metric through tpc_track_host_async / tpc_track_host_fetch: pinned host buffers, H2D of the inputs
-              and D2H of EVERY output inside the timed region, two Time Frames in flight
+              and D2H of EVERY output inside the timed region, four Time Frames in flight
  kernels      per-kernel CUDA-event times from a second, separately profiled loop (tpc_profile_*)
  roofline     the dominant kernel of that table; the FP32 roof is measured by the library (tpc_fp32_peak, FFMA chains),
               the HBM roof is MEASURED_PEAKS.json; `traffic` comes from profiles/*_ncu_traffic.csv and is null when
@@ -421,7 +421,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         m1.record()
         torch.cuda.synchronize()
         ng = trk._merge["out"]["n_global"].cpu().numpy()
-        merge = {"ms": m0.elapsed_time(m1) / 3, "global_tracks": int(ng[0]), "links": int(ng[1]),
+        if int(ng[3]) != 0:
+            raise RuntimeError(f"tpc_merge_tracks left {int(ng[3])} candidate pairs untested (pair list full): the merge figure is void")
+        merge = {"ms": m0.elapsed_time(m1) / 3, "global_tracks": int(ng[0]), "links": int(ng[1]), "pairs": int(ng[2]), "pairs_dropped": int(ng[3]),
                  "what": "tpc_merge_tracks: sector-local tracks linked across sector edges / the central electrode / long "
                          "holes, merged hit lists refitted (DESIGN.md R26); not included in `value`"}
         binding.profile_collect(reset=True)

@@ -398,7 +398,12 @@ int tpc_clusterize(const tpc_params_t* params_host, int64_t n_digits, const int3
  *   trk_succ_chi2 [max_tracks]      : chi2 of the best candidate successor (before reciprocity), -1 = none
  *   trk_global [max_tracks]         : global track of a sector-local track
  *   n_global [4]                    : global tracks M; links; pairs that passed the windows and the gate; pairs not
- *                                     tested because the pair list (4 max_tracks entries) was full (0 in practice)
+ *                                     tested because the pair list (4 max_tracks entries) was full.  n_global[3] is the
+ *                                     overflow word of this call, as TPC_CNT_STATUS is for tpc_find_tracks: it is 0 on
+ *                                     every workload seen so far (0.4 pairs per track on the bench Time Frame); when it is
+ *                                     not, which pairs were left out depends on arrival order, so the links are
+ *                                     incomplete and not reproducible -- treat it as an error and retry with a larger
+ *                                     max_tracks (the Python binding raises)
  *   g_head, g_nseg, g_nhits [max_tracks] : first (innermost) piece, pieces and hits of global track g < M, in
  *                                     ascending order of g_head
  *   gpar [5][max_tracks], gcov [15][max_tracks], gxref, gzref, gchi2, gndf [max_tracks] : refit of the merged hit

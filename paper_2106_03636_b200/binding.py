@@ -469,6 +469,9 @@ class Tracker:
         o = self._merge["out"]
         k = int(self.counters[CNT_TRACKS].item())
         m, links, pairs, dropped = (int(v) for v in o["n_global"].cpu().numpy())
+        if dropped:
+            raise TpcError(f"tpc_merge_tracks: {dropped} of {pairs} candidate pairs did not fit the pair list (4 x max_tracks "
+                           f"entries) and were not tested: links are incomplete and depend on arrival order; raise max_tracks")
         per_trk = ("trk_succ", "trk_pred", "trk_succ_chi2", "trk_global")
         res = {nm: o[nm][:k].cpu().numpy() for nm in per_trk}
         res.update({nm: (o[nm][:, :m] if o[nm].dim() == 2 else o[nm][:m]).cpu().numpy()

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 def torch_cuda():
     import torch
     if not torch.cuda.is_available():
-        pytest.skip("no CUDA device")
+        pytest.fail("no CUDA device: -m gpu tests must run on the B200 box")
     return torch
 
 

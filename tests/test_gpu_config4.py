@@ -76,6 +76,8 @@ def test_c4_merge_and_tags_invariants(c4_run):
     compared link for link on configs 0-3 in tests/test_gpu_merge.py): properties that hold at any size."""
     ev, res, _ = c4_run
     m, K = res["merge"], res["trk_seed"].size
+    assert m["n_pairs_dropped"] == 0, "pair list full: links would be incomplete and not reproducible"
+    assert m["n_links"] <= m["n_pairs"] <= 4 * K
     succ, pred = m["trk_succ"], m["trk_pred"]
     a = np.nonzero(succ >= 0)[0]
     assert np.array_equal(pred[succ[a]], a), "succ and pred must be inverse to one another"

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 def torch_cuda():
     import torch
     if not torch.cuda.is_available():
-        pytest.skip("no CUDA device")
+        pytest.fail("no CUDA device: -m gpu tests must run on the B200 box")
     return torch
 
 
@@ -35,6 +35,7 @@ def compare_merge(orc, ev, res, gm):
         b = seed_or_none(gm["trk_" + key][to_g], res["trk_seed"])
         assert np.array_equal(a, b), f"{key}: {np.count_nonzero(a != b)} of {a.size} links differ"
     assert np.array_equal(m["succ_chi2"], gm["trk_succ_chi2"][to_g]), "chi2 of the best successor differs"
+    assert gm["n_pairs_dropped"] == 0 and gm["n_pairs"] >= int((m["succ_chi2"] >= 0).sum())
     n_links = int((m["succ"] >= 0).sum())
     assert gm["n_links"] == n_links and gm["n_global"] == m["g_head"].size == o["trk_seed"].size - n_links
     # global tracks, matched by the seed of the head
