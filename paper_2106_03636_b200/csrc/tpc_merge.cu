@@ -403,15 +403,17 @@ k_merge_chains(const int32_t* __restrict__ counters, int64_t max_tracks, const i
   }
 }
 
-// R26 refit of one chain per thread.  The hits of a chain are walked piece by piece in the direction of the pass;
-// `piece` / `i` address the current hit, prev[] is rebuilt from succ[] on the way out (chains are a few pieces long).
-constexpr int kMaxPieces = 16;
+// R26 refit of one chain per thread.  The hits of a chain are walked piece by piece in the direction of the pass: `k` / `i`
+// address the current hit, succ[] leads to the next piece on the way out and pred[] on the way in, so a chain may have
+// any number of pieces (holes longer than max_gap inside one sector give one piece each; with a small min_hits that is
+// dozens).
 
 __global__ void __launch_bounds__(kThreads)
 k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_global, int64_t max_tracks,
               const int32_t* __restrict__ trk_sector, const int32_t* __restrict__ trk_nhits,
               const int64_t* __restrict__ trk_first_hit, const float4* __restrict__ hit_rec, const float* __restrict__ par,
-              const float* __restrict__ zref, const int32_t* __restrict__ succ, const int32_t* __restrict__ g_head,
+              const float* __restrict__ zref, const int32_t* __restrict__ succ, const int32_t* __restrict__ pred,
+              const int32_t* __restrict__ g_head,
               const int32_t* __restrict__ g_nseg, const int32_t* __restrict__ g_nhits, float* __restrict__ gpar,
               float* __restrict__ gcov, float* __restrict__ gxref, float* __restrict__ gzref, float* __restrict__ gchi2,
               int32_t* __restrict__ gndf, const int32_t* __restrict__ mlist) {
@@ -424,12 +426,10 @@ k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_globa
   const float kB = sc.kB, ms = sc.max_sinphi, sy2 = sc.sy2, sz2 = sc.sz2;
   for (int64_t li = (int64_t)blockIdx.x * kThreads + threadIdx.x; li < M; li += (int64_t)gridDim.x * kThreads) {
     const int gi = mlist[li];
-    const int nseg = g_nseg[gi];
     const int h = g_head[gi];
-    int seg[kMaxPieces];
-    int np = 0;
-    for (int k = h; k >= 0 && np < kMaxPieces; k = succ[k]) seg[np++] = k;
-    bool ok = nseg <= kMaxPieces;  // longer chains do not occur (a chain crosses a sector edge per piece); flagged if they do
+    int tail = h;
+    for (int k = succ[h]; k >= 0; k = succ[k]) tail = k;
+    bool ok = true;
     KState st;
 #pragma unroll
     for (int i = 0; i < 5; i++) st.p[i] = par[i * max_tracks + h];
@@ -446,10 +446,9 @@ k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_globa
       c2 = 0.0f;
       lost = 0;
       const int dir = (pass & 1) ? -1 : 1;
-      int piece = dir > 0 ? 0 : np - 1;
-      int i = dir > 0 ? 0 : trk_nhits[seg[piece]] - 1;
+      int k = dir > 0 ? h : tail;
+      int i = dir > 0 ? 0 : trk_nhits[k] - 1;
       for (int cnt = 0; cnt < N && ok; cnt++) {
-        const int k = seg[piece];
         const float4 hit = __ldg(hit_rec + trk_first_hit[k] + i);
         const int hs = trk_sector[k];
         const float xh = sX[__float_as_int(hit.z)];
@@ -482,8 +481,11 @@ k_merge_refit(const __grid_constant__ Geo g, const int32_t* __restrict__ n_globa
         // next hit in the direction of the pass
         i += dir;
         if (i < 0 || i >= trk_nhits[k]) {
-          piece += dir;
-          if (piece >= 0 && piece < np) i = dir > 0 ? 0 : trk_nhits[seg[piece]] - 1;
+          const int nk = dir > 0 ? succ[k] : pred[k];
+          if (nk >= 0) {
+            k = nk;
+            i = dir > 0 ? 0 : trk_nhits[k] - 1;
+          }
         }
       }
     }
@@ -619,7 +621,7 @@ cudaError_t launch_merge(const Geo& g, const Ws& fw, float chi2_cut, float dz_ma
                                                          gcov, gxref, gzref, gchi2, gndf, w.mlist, w.n_pairs, w.pair_cap)));
   TPC_LAUNCH(KID_MERGE, st,
              (k_merge_refit<<<blocks, kThreads, 0, st>>>(g, n_global, max_tracks, trk_sector, trk_nhits, trk_first_hit, fw.hit_rec,
-                                                        par, zref, trk_succ, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref,
+                                                        par, zref, trk_succ, trk_pred, g_head, g_nseg, g_nhits, gpar, gcov, gxref, gzref,
                                                         gchi2, gndf, w.mlist)));
   return cudaGetLastError();
 }

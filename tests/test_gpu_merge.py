@@ -19,9 +19,9 @@ def torch_cuda():
     return torch
 
 
-def compare_merge(orc, ev, res, gm):
+def compare_merge(orc, ev, res, gm, mp=None):
     o = orc.run(ev.params, ev.y, ev.z, ev.sector_row, "f32", True)
-    m = orc.merge(ev.params, ev.y, ev.z, ev.sector_row, o, None, "f32")
+    m = orc.merge(ev.params, ev.y, ev.z, ev.sector_row, o, mp, "f32")
     assert res["trk_seed"].size == o["trk_seed"].size
     g_of_seed = {int(s): i for i, s in enumerate(res["trk_seed"])}
     to_g = np.array([g_of_seed[int(s)] for s in o["trk_seed"]])            # oracle track -> cuda track
@@ -101,3 +101,34 @@ def test_merge_refuses_tracks_fitted_with_an_odd_number_of_passes(torch_cuda, pa
     assert res["trk_seed"].size > 50
     with pytest.raises(binding.TpcError, match="invalid argument"):
         trk.merge_tracks()
+
+
+
+def test_merge_refits_chains_of_more_than_16_pieces(torch_cuda, orc):
+    """Holes longer than max_gap inside one sector give one piece each, so the number of pieces of a chain is not
+    bounded by the sector crossings.  A 400-particle collision with two of every six pad rows removed, max_gap = 1 and
+    min_hits = 4 leaves pieces of four hits; with a wide chi2 cut they chain up to ~20 pieces, and every chain is refitted
+    (the refit kernel used to give up beyond 16 pieces while the oracle went on)."""
+    from types import SimpleNamespace
+    from paper_2106_03636_b200 import binding
+    full = make_config(1, n_tracks=400)
+    keep = (full.sector_row % full.params.n_rows) % 6 < 4
+    ev = SimpleNamespace(params=full.params.with_(max_gap=1, min_hits=4), y=full.y[keep], z=full.z[keep],
+                         sector_row=full.sector_row[keep], n=int(keep.sum()))
+    mp = dict(chi2_cut=500.0, dz_max=64.0, ce_tol=1.0, max_rows=12)
+    t = torch_cuda
+    dev = [t.from_numpy(a).cuda() for a in (ev.y, ev.z, ev.sector_row)]
+    # ~8300 four-hit pieces with ~15 candidate pairs each under this cut: the pair list of the default capacity
+    # (4 x max_tracks entries) overflows, and that is reported, not swallowed ...
+    small = binding.Tracker(ev.params, ev.n)
+    small.run(*dev)
+    with pytest.raises(binding.TpcError, match="pair list"):
+        small.merge_tracks(**mp)
+    # ... and with room for every pair the result is the oracle's
+    trk = binding.Tracker(ev.params, ev.n, max_tracklets=65536, max_tracks=262144)   # room for ~50 candidate pairs per piece
+    res = trk.run(*dev)
+    assert res["status"] == 0
+    gm = trk.merge_tracks(**mp)
+    compare_merge(orc, ev, res, gm, mp)
+    long_chain = gm["g_nseg"] > 16
+    assert long_chain.sum() >= 10 and (gm["gndf"][long_chain] > 0).sum() >= 10
