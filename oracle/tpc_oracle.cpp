@@ -1352,7 +1352,8 @@ ORC_API int64_t orc_merge_fit_f64(const OrcParams* P, int64_t n, const double* y
 
 // ---------------------------------------------------------------------------------------------
 // R27 (the TPC clusterizer is the step that feeds the tracker).
-// Input: zero-suppressed digits (sector_row, pad, time bin, ADC), any order; two digits of the same cell add up.
+// Input: zero-suppressed digits (sector_row, pad, time bin, ADC), any order; two digits of the same cell add up.  A
+// digit of ADC <= 0 is not a zero-suppressed digit and is ignored (so every cell holds a positive sum and S > 0).
 // The paper gives no algorithm; this is the textbook reading:
 //   peak    : a digit of ADC a >= peak_min that beats its 8 neighbours in (pad, time) -- strictly the four "earlier"
 //             ones (time - 1 at any pad, and pad - 1 at the same time), at least equal to the four "later" ones, so a
@@ -1369,9 +1370,11 @@ ORC_API int64_t orc_clusterize(const OrcParams* P, int64_t n, const int32_t* sr,
                                const int32_t* adc, double pad_width, double time_width, int32_t peak_min, int64_t cap,
                                float* y, float* z, float* q, int32_t* out_sr, int32_t* out_pad, int32_t* out_time) {
   Geo<float> G(*P);
-  std::vector<std::pair<uint64_t, int64_t>> cells((size_t)n);
+  std::vector<std::pair<uint64_t, int64_t>> cells;
+  cells.reserve((size_t)n);
   auto key = [](int64_t s, int64_t t, int64_t p) { return ((uint64_t)s << 40) | ((uint64_t)t << 16) | (uint64_t)p; };
-  for (int64_t i = 0; i < n; i++) cells[(size_t)i] = {key(sr[i], tim[i], pad[i]), (int64_t)adc[i]};
+  for (int64_t i = 0; i < n; i++)
+    if (adc[i] > 0) cells.push_back({key(sr[i], tim[i], pad[i]), (int64_t)adc[i]});
   std::sort(cells.begin(), cells.end());
   size_t m = 0;   // cells of the same key add up
   for (size_t i = 0; i < cells.size(); i++) {

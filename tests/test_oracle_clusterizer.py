@@ -3,7 +3,7 @@ oracle only.  PAPER.md names the step (l.35, l.98) and gives no algorithm; what 
   * the definition written a second time, densely, in numpy (arrays + shifts instead of sorted cells + look-ups),
     compared cluster for cluster and bit for bit
   * hand-made cases: a plateau gives exactly one peak (the earlier cell), a missing neighbour counts as zero, two
-    digits of one cell add up, peak_min
+    digits of one cell add up, peak_min; digits of ADC <= 0 change nothing, wherever they sit
   * an isolated Gaussian deposit comes back where it was put (closed form of the response: the 3-cell centre of
     gravity of a sampled Gaussian), translation by whole cells moves the clusters by whole cells
   * end to end: digits of configs[0] -> clusters -> the tracker finds the tracks it finds on the true clusters
@@ -24,7 +24,9 @@ def dense_reference(p, sr, pad, time, adc, pw, tw, peak_min):
     f = np.float32
     X = np.asarray(p.row_x, np.float32)
     for s in np.unique(sr):
-        m = sr == s
+        m = (sr == s) & (adc > 0)
+        if not m.any():
+            continue
         P, T = int(pad[m].max()) + 3, int(time[m].max()) + 3
         a = np.zeros((T + 2, P + 2), np.int64)                 # one cell of zeros all around
         np.add.at(a, (time[m] + 1, pad[m] + 1), adc[m])
@@ -99,6 +101,40 @@ def test_plateau_missing_neighbours_duplicates_and_peak_min(orc):
     assert c["n_found"] == 1
     assert c["y"][0] == pytest.approx((4.5 + 6 / 18) * PW - float(ymax), abs=1e-5)
     assert c["z"][0] == pytest.approx((4.5 + 2 / 18) * TW + P1.z_lo, abs=1e-5)
+
+
+def test_digits_without_charge_are_ignored(orc):
+    """R27: a digit of ADC <= 0 is not a zero-suppressed digit.  By hand: a peak of 6 between two digits of -3 would have
+    S = 0 (centre of gravity 0/0); with the rule it is the lone digit of the third case above.  On a digitised event:
+    zero and negative digits sprinkled on empty cells, on cells next to peaks and on occupied cells leave every cluster as
+    it was."""
+    s = 5
+    ymax = np.float32(np.float32(P1.row_x[s]) * np.float32(P1.tan_half))
+    sr, pad, tim, adc = digits_of([(s, 10, 20, 6), (s, 9, 20, -3), (s, 11, 20, -3), (s, 10, 21, 0)])
+    c = orc.clusterize(P1, sr, pad, tim, adc, PW, TW, peak_min=6)
+    assert c["n_found"] == 1 and as_tuples(c)[0][:4] == (s, 20, 10, 6)
+    assert c["y"][0] == np.float32(np.float32(10.5) * np.float32(PW)) - ymax
+    assert c["z"][0] == np.float32(np.float32(20.5) * np.float32(TW)) + np.float32(P1.z_lo)
+    # a negative digit on an occupied cell does not lower it: 4 + (-2) stays a peak of 4 (= peak_min), 7 + (-5) one of 7
+    sr, pad, tim, adc = digits_of([(s, 3, 3, 4), (s, 3, 3, -2), (s, 30, 30, 7), (s, 30, 30, -5)])
+    c = orc.clusterize(P1, sr, pad, tim, adc, PW, TW, peak_min=4)
+    assert c["n_found"] == 2 and sorted(c["q"].tolist()) == [4.0, 7.0]
+    ev = config0()
+    d = digitize(ev)
+    base = orc.clusterize(ev.params, d.sector_row, d.pad, d.time, d.adc, d.pad_width, d.time_width)
+    rng = np.random.default_rng(27)
+    k = rng.integers(0, d.sector_row.size, 5000)
+    extra_sr = d.sector_row[k]
+    extra_pad = np.clip(d.pad[k] + rng.integers(-1, 2, k.size), 0, 65535).astype(np.int32)
+    extra_time = np.clip(d.time[k] + rng.integers(-1, 2, k.size), 0, None).astype(np.int32)
+    extra_adc = rng.integers(-40, 1, k.size).astype(np.int32)
+    cat = lambda a, b: np.concatenate([a, b]).astype(np.int32)
+    more = orc.clusterize(ev.params, cat(d.sector_row, extra_sr), cat(d.pad, extra_pad), cat(d.time, extra_time),
+                          cat(d.adc, extra_adc), d.pad_width, d.time_width)
+    assert more["n_found"] == base["n_found"] > 1000
+    for key in ("y", "z", "q", "sector_row", "pad", "time"):
+        assert np.array_equal(more[key], base[key]), key
+    assert np.isfinite(more["y"]).all() and np.isfinite(more["z"]).all()
 
 
 def test_isolated_deposit_comes_back_and_whole_cell_shifts(orc):
