@@ -362,13 +362,15 @@ int tpc_tag_clusters(int64_t n_clusters, const int32_t* cluster_track, const int
 /* ---- clusterizer (the step that feeds the tracker; R27) --------
  * Clusters from zero-suppressed digits (sector_row, pad, time_bin, adc), any order; two digits of one cell add up;
  * a digit with sector_row outside [0, n_sectors*n_rows), pad outside [0, 65535] or time_bin outside [0, 2^24) is
- * ignored.  A cell of ADC >= peak_min is a peak iff it is strictly above its four earlier neighbours (time_bin - 1 at
+ * ignored, and so is one with adc <= 0 (not a zero-suppressed digit; every cell sum and S stay positive).  A cell of ADC >= peak_min is a peak iff it is strictly above its four earlier neighbours (time_bin - 1 at
  * pad - 1, pad, pad + 1; pad - 1 at the same time) and at least equal to the four later ones (missing = 0).  A peak
  * gives one cluster from the integer sums over its 3 x 3 cells, S = sum a, Sp = sum a dpad, St = sum a dtime:
  *   y = ((pad + 0.5) + Sp/S) pad_width - ymax_row,  zeta = ((time_bin + 0.5) + St/S) time_width + z_lo,
  *   z = zeta on side A (sectors < 18), -zeta on side C;  q = S           (fp32, one rounding per operation)
- * Outputs (device, [max_clusters]; the order is unspecified): y, z, q and sector_row -- what tpc_grid_build takes --
- * plus the peak cell out_pad / out_time; n_clusters [2] (device): clusters found; clusters written
+ * Outputs (device, [max_clusters]): y, z, q and sector_row -- what tpc_grid_build takes -- plus the peak cell out_pad /
+ * out_time.  The SET of clusters is deterministic; their ORDER is the order in which the peaks were found and changes
+ * from run to run.  tpc_find_tracks breaks exact ties by input index, so a caller that needs tracks reproducible to the
+ * last tie orders the clusters by (sector_row, out_time, out_pad) -- unique per cluster -- before tpc_grid_build; n_clusters [2] (device): clusters found; clusters written
  * (= min(found, max_clusters)).  workspace: tpc_clusterize_workspace_bytes(n_digits) bytes, 256-byte aligned,
  * caller-owned.  Enqueue only.  TPC_EINVAL for missing buffers, n_digits > 2^31, pad_width / time_width <= 0,
  * peak_min < 1; TPC_ENOMEM_WS for a short workspace. */

@@ -43,6 +43,7 @@ k_digit_insert(int64_t n, int sr_end, const int32_t* __restrict__ sr, const int3
   for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) {
     const int s = sr[i], p = pad[i], t = tim[i];
     if ((unsigned)s >= (unsigned)sr_end || (unsigned)p > 65535u || (unsigned)t >= (1u << 24)) continue;  // no such cell
+    if (adc[i] <= 0) continue;  // R27: not a zero-suppressed digit (keeps every cell sum, and so S at a peak, positive)
     const unsigned long long k = cell_key(s, t, p);
     unsigned long long h = mix64(k) & mask;
     for (;;) {
