@@ -112,6 +112,54 @@ def test_noiseless_helix_across_the_central_electrode(orc):
     assert (zb - z_a_at_xb) / (2 * gen.V_DRIFT) == pytest.approx(t_us, abs=1e-3)
 
 
+@pytest.mark.parametrize("t_us", [40.0, 5000.0])
+def test_electrode_link_at_the_collision_times_of_a_time_frame(orc, t_us):
+    """The two sides measure z_true -+ v_d t, so across the electrode the z window is on z_A + z_B (= 2 z_true, small
+    near the electrode), never on z_B - z_A (= 2 v_d t: 206 cm at 40 us, 258 m at 5000 us -- the collision times of a
+    Time Frame run up to 1.1e4 us, R3).  Same helix as above at such times: linked, refit as before, 2 v_d t read back."""
+    assert 2 * gen.V_DRIFT * t_us > 3 * 64.0, "the jump must be far outside dz_max for this to pin the sign"
+    ev = tracks_event(one(1.2, 15.0, -0.35, 60.0), t_us=[t_us])
+    o, m = run_merge(orc, ev)
+    ch = chains(m)
+    assert len(ch) == 1 and len(ch[0]) == o["trk_seed"].size >= 2
+    sides = m["trk_sector"][ch[0]] < 18
+    k = int(np.nonzero(np.diff(sides.astype(int)))[0][0])
+    a, b = ch[0][k], ch[0][k + 1]
+    assert m["g_nhits"][0] == ev.n and m["gndf"][0] == 2 * ev.n - 6
+    assert m["gpar"][4, 0] == pytest.approx(1.2, rel=1e-5) and m["gpar"][3, 0] == pytest.approx(-0.35, rel=1e-5)
+    zb = o["zref"][b] + o["par"][1, b]
+    dxs = gen.default_row_x()[m["row_first"][b]] - gen.default_row_x()[m["row_first"][a]]
+    st = orc.propagate(ev.params, o["par"][:, a], o["cov"][:, a], float(dxs), "f64")
+    assert st[0]
+    assert (zb - (o["zref"][a] + st[1][1])) / (2 * gen.V_DRIFT) == pytest.approx(t_us, rel=1e-6, abs=1e-3)
+
+
+def test_same_side_pieces_with_mirrored_z_are_not_linked(orc):
+    """Inside one side the window is on z_B - z_A.  Two particles on the same circle in the bending plane, flat in z
+    (tan lambda = 0.01), one measured at z = +40 cm and one -- a later collision -- at z = -40 cm on the same side; the
+    first keeps its clusters below row 70, the second those above row 75.  Every test of R26 but the z window would pass
+    (same sector, 7 rows apart, same tan lambda and q/pT, same y and direction): z_B + z_A = 0 but z_B - z_A = -80 cm,
+    beyond dz_max = 64 -- not compared.  Control: the second particle at z = +40 as well -- linked."""
+    from types import SimpleNamespace
+    t_shift = 80.0 / gen.V_DRIFT                          # side A measures z_true - v_d t
+    for z2, linked in ((-40.0, False), (40.0, True)):
+        t = dict(qpt=[0.3, 0.3], phi=[math.radians(10.0)] * 2, tanl=[0.01, 0.01], vx=[0.0, 0.0], vy=[0.0, 0.0], vz=[40.0, 40.0])
+        full = tracks_event(t, t_us=[0.0, t_shift if z2 < 0 else 0.0])
+        row = full.sector_row % NR
+        assert np.all(full.sector_row // NR == 0)
+        keep = ((full.true_track == 0) & (row < 70)) | ((full.true_track == 1) & (row > 75))
+        ev = SimpleNamespace(params=full.params, y=full.y[keep], z=full.z[keep], sector_row=full.sector_row[keep])
+        assert abs(float(np.median(ev.z[row[keep] > 75])) - z2) < 3.0      # 40 cm + 0.01 x path, shifted
+        o, m = run_merge(orc, ev)
+        assert o["trk_seed"].size == 2
+        a, b = np.argsort(m["row_first"])
+        assert m["row_last"][a] == 69 and m["row_first"][b] == 76
+        if linked:
+            assert m["succ"][a] == b and m["pred"][b] == a and 0.0 <= m["pair_chi2"][a, b] < 1e-6
+        else:
+            assert m["succ"][a] == -1 and m["pred"][b] == -1 and m["pair_chi2"][a, b] == -1.0
+
+
 def test_different_tracks_at_the_same_edge_are_not_linked(orc):
     """Two particles of the SAME curvature and dip leave a sector through the same edge, 0.6 degrees and 7 cm in z
     apart: the piece of one in the first sector and the piece of the other in the second pass every window and the

@@ -209,6 +209,25 @@ def test_R17_clean_fragments(orc):
         assert list(res[mode][3].keys()) == [11] and len(res[mode][3][11]) == n
 
 
+def test_R16_leg_bridges_max_gap_missing_rows_and_no_more(orc):
+    """R16: a leg goes on over rows without a hit and stops after max_gap + 1 of them in a row -- max_gap is the longest
+    hole that is bridged.  Mode 0 (every start hit followed in full, nothing absorbed), a straight line in two
+    fragments: with exactly max_gap missing rows the lower tracklet's upward leg (and the upper one's downward leg)
+    crosses the hole and both record every cluster; with max_gap + 1 both stop at the hole and each keeps its own
+    fragment.  (The wave test has its own pin at the same boundary; this is the leg that does the bridging.)"""
+    for g, bridged in ((MAX_GAP - 1, True), (MAX_GAP, True), (MAX_GAP + 1, False), (MAX_GAP + 2, False)):
+        y, z, sr, r_up = two_fragments(g)
+        n_lo, n_up = 41, 25
+        assert y.size == n_lo + n_up
+        rows, ran, n_hits, tracks, o = run_modes(orc, P1, y, z, sr)[orc.R17_NAIVE]
+        assert rows == [11, r_up] and ran == [1, 1]
+        assert n_hits == ([n_lo + n_up] * 2 if bridged else [n_lo, n_up]), f"{g} missing rows"
+        if bridged:
+            assert list(tracks.keys()) == [11] and len(tracks[11]) == n_lo + n_up
+        else:
+            assert tracks == {11: set(range(n_lo)), r_up: set(range(n_lo, n_lo + n_up))}
+
+
 def stub_below(row_top, dy):
     """A 16-cluster chain whose top sits on row `row_top`, `dy` cm beside the default line through (row 60, 0, 100),
     and which runs off at a very different angle (slope + 0.6): a plausible-looking predecessor that is none."""
