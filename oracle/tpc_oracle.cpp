@@ -843,6 +843,12 @@ inline int sector_relation(int sa, int sb) {
 
 // Rotation of a state at x into the frame turned by D (cd = cos D, sd = sin D).  Returns false if the track does not
 // point into the +x half of the new frame (cosphi' <= 0) or |sinphi'| > max_sinphi.
+// Covariance: the rotated state is a state at the FIXED plane x' = xn of the new frame.  A shift dy along the old plane
+// moves the point to (xn + dy sd, yn + dy cd); brought back to x' = xn along the track (slope sn / cn) that is
+// dy' = dy (cd - sd sn / cn) = dy c / cn, and a change ds at the same point turns the direction by ds' = ds cn / c: the
+// diagonal J below.  The same step back over dx' = -dy sd also changes z by -dy sd tanl / cn and sinphi by -dy sd kappa
+// (kappa = -kB q/pT): these two cross terms (dz'/dy, dsinphi'/dy) are DROPPED -- R26 keeps the diagonal form, an
+// approximation stated in DESIGN.md R26 and measured by the pin (at 20 degrees: |dz'/dy| = 0.34 |tanl| / cn).
 template <class T>
 bool rotate_state(State<T>& st, T& x, T cd, T sd, T max_sinphi) {
   const T y = st.p[0], s = st.p[2];
@@ -1185,6 +1191,28 @@ ORC_API int orc_propagate_f32(const OrcParams* P, float* p5, float* c15, float d
 }
 ORC_API int orc_propagate_f64(const OrcParams* P, double* p5, double* c15, double dx, double* F25) {
   return propagate_impl<double>(P, p5, c15, dx, F25);
+}
+// R26 rotation primitive, exported for its pin (tests/test_oracle_merge.py: every entry of J against finite differences
+// of the exact map built from the pinned R12).  p5 / c15 (lower triangle, row-major) / x are updated in place.
+template <class T>
+int rotate_impl(const OrcParams* P, T* p5, T* c15, T* x, T cd, T sd) {
+  State<T> st;
+  for (int i = 0; i < 5; i++) st.p[i] = p5[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++, m++) st.C[i][j] = st.C[j][i] = c15[m];
+  T xx = *x;
+  if (!rotate_state(st, xx, cd, sd, (T)P->max_sinphi)) return 0;
+  for (int i = 0; i < 5; i++) p5[i] = st.p[i];
+  for (int i = 0, m = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++, m++) c15[m] = st.C[i][j];
+  *x = xx;
+  return 1;
+}
+ORC_API int orc_rotate_f32(const OrcParams* P, float* p5, float* c15, float* x, float cd, float sd) {
+  return rotate_impl<float>(P, p5, c15, x, cd, sd);
+}
+ORC_API int orc_rotate_f64(const OrcParams* P, double* p5, double* c15, double* x, double cd, double sd) {
+  return rotate_impl<double>(P, p5, c15, x, cd, sd);
 }
 ORC_API float orc_update_f32(const OrcParams* P, float* p5, float* c15, float ym, float zm) {
   return update_impl<float>(P, p5, c15, ym, zm);

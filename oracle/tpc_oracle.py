@@ -493,6 +493,18 @@ def propagate(p, par5, cov15, dx, precision="f64"):
     return bool(ok), a, c, F.reshape(5, 5)
 
 
+def rotate(p, par5, cov15, x, delta, precision="f64"):
+    """R26 rotation primitive: the state (par5, cov15) at x, expressed in the frame turned by `delta` rad.
+    Returns (ok, par5', cov15', x')."""
+    rt, sfx = _real(precision)
+    P = make_params(p, precision)
+    a = np.array(par5, rt); c = np.array(cov15, rt)
+    ct = C.c_float if sfx == "f32" else C.c_double
+    xx = ct(float(x))
+    ok = getattr(lib(), f"orc_rotate_{sfx}")(C.byref(P), _ptr(a), _ptr(c), C.byref(xx), ct(math.cos(delta)), ct(math.sin(delta)))
+    return bool(ok), a, c, float(xx.value)
+
+
 def update(p, par5, cov15, ym, zm, precision="f64"):
     """R13 primitive: returns (chi2, par5', cov15')."""
     rt, sfx = _real(precision)

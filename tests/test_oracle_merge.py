@@ -160,6 +160,64 @@ def test_same_side_pieces_with_mirrored_z_are_not_linked(orc):
             assert m["succ"][a] == -1 and m["pred"][b] == -1 and m["pair_chi2"][a, b] == -1.0
 
 
+# ------------------------------------------------------------------------------------------------------------
+# the rotation primitive
+# ------------------------------------------------------------------------------------------------------------
+def exact_rotation_map(orc, p, v, x0, delta, x_fixed):
+    """The map R26's rotation stands for, built from plane geometry and the pinned R12 only: the state v = (y, z, sinphi,
+    tanlambda, q/pT) at the plane x0 of the old frame -> the state of the same helix at the FIXED plane x_fixed of the frame
+    turned by delta."""
+    y, z, s, tl, q = v
+    cd, sd = math.cos(delta), math.sin(delta)
+    xr, yr = x0 * cd + y * sd, y * cd - x0 * sd
+    sr = s * cd - math.sqrt(1.0 - s * s) * sd
+    ok, par, _, _ = orc.propagate(p, [yr, z, sr, tl, q], np.zeros(15), x_fixed - xr, "f64")
+    assert ok
+    return par
+
+
+@pytest.mark.parametrize("delta_deg", [20.0, -20.0])
+@pytest.mark.parametrize("v,x0", [((38.0, 12.0, 0.25, 0.6, 1.5), 150.0), ((-25.0, -40.0, -0.3, -1.1, -2.5), 110.0),
+                                  ((5.0, 100.0, 0.05, 0.2, 0.2), 220.0)])
+def test_rotation_jacobian_against_finite_differences(orc, v, x0, delta_deg):
+    """orc.rotate: (i) point and direction are the plane rotation; (ii) the covariance is D C D with D the DIAGONAL of the
+    Jacobian of the exact map -- taken here from central differences, not from a formula -- entry by entry; (iii) the exact
+    map has two more non-zero entries, dz'/dy = -sin(delta) tanl / cosphi' and dsinphi'/dy = -sin(delta) kappa, which R26
+    drops (R26 says so): their size is measured here so that the approximation is a stated number."""
+    p = TpcParams()
+    delta = math.radians(delta_deg)
+    v = np.array(v, float)
+    rng = np.random.default_rng(26)
+    A = rng.normal(size=(5, 5)) * np.array([0.1, 0.1, 0.01, 0.01, 0.05])[:, None]
+    Cm = A @ A.T + np.diag([1e-3, 1e-3, 1e-5, 1e-5, 1e-4])
+    c15 = np.array([Cm[i, j] for i in range(5) for j in range(i + 1)])
+    ok, par, cov, xn = orc.rotate(p, v, c15, x0, delta, "f64")
+    assert ok
+    cd, sd = math.cos(delta), math.sin(delta)
+    assert xn == pytest.approx(x0 * cd + v[0] * sd, rel=1e-14)
+    want = exact_rotation_map(orc, p, v, x0, delta, xn)
+    assert np.allclose(par, want, rtol=0, atol=1e-12), "(i) the rotated state is the helix at the plane x' = xn"
+    J = np.zeros((5, 5))
+    for j, h in enumerate([1e-4, 1e-4, 1e-6, 1e-6, 1e-6]):
+        e = np.zeros(5); e[j] = h
+        J[:, j] = (exact_rotation_map(orc, p, v + e, x0, delta, xn) - exact_rotation_map(orc, p, v - e, x0, delta, xn)) / (2 * h)
+    D = np.diag(J)
+    Cn = np.zeros((5, 5))
+    for i in range(5):
+        for j in range(i + 1):
+            Cn[i, j] = Cn[j, i] = cov[i * (i + 1) // 2 + j]
+    assert np.allclose(Cn, D[:, None] * Cm * D[None, :], rtol=2e-7, atol=0), "(ii) C' = D C D, D = diag of the exact Jacobian"
+    assert abs(D[0] - 1) > 0.01 and abs(D[2] - 1) > 0.01 and np.allclose(D[[1, 3, 4]], 1.0, atol=1e-9)
+    # (iii) what the diagonal form leaves out
+    cn = math.sqrt(1.0 - par[2] ** 2)
+    kappa = -KB_TRK * v[4]
+    off = J - np.diag(D)
+    assert off[1, 0] == pytest.approx(-sd * v[3] / cn, rel=1e-6)
+    assert off[2, 0] == pytest.approx(-sd * kappa, rel=1e-5, abs=1e-10)
+    off[1, 0] = off[2, 0] = 0.0
+    assert np.abs(off).max() < 1e-7, "no other entry"
+
+
 def test_different_tracks_at_the_same_edge_are_not_linked(orc):
     """Two particles of the SAME curvature and dip leave a sector through the same edge, 0.6 degrees and 7 cm in z
     apart: the piece of one in the first sector and the piece of the other in the second pass every window and the
